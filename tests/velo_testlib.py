@@ -1,0 +1,97 @@
+"""Shared helpers for the tests: canonical ordering, comparison rule
+(O-17), hand-made events. Holds no method arithmetic of either side."""
+from __future__ import annotations
+
+import numpy as np
+
+from paper_2412_05041_b200 import datagen
+
+MODULE_Z = datagen.MODULE_Z.astype(np.float32)
+M = MODULE_Z.shape[0]
+
+
+def split_tracks(res: dict, event: int):
+    """List of (hit-index tuple, state vector[13]) of one event."""
+    eto, tho, th, st = res["event_track_offsets"], res["track_hit_offsets"], res["track_hits"], res["states"]
+    out = []
+    for t in range(int(eto[event]), int(eto[event + 1])):
+        hits = tuple(int(v) for v in th[int(tho[t]):int(tho[t + 1])])
+        out.append((hits, np.array(st[:, t], dtype=np.float32)))
+    return out
+
+
+def canonical_order(res: dict) -> np.ndarray:
+    """Permutation of track ids putting every event's tracks in canonical order (O-16): by hit list,
+    lexicographic. The first two hits (h0, centre h1) are unique per candidate (O-8: one seed per
+    centre hit), so (event, hits[0], hits[1]) is a total order equal to the lexicographic one."""
+    eto = np.asarray(res["event_track_offsets"], dtype=np.int64)
+    tho = np.asarray(res["track_hit_offsets"], dtype=np.int64)
+    th = np.asarray(res["track_hits"], dtype=np.int64)
+    nt = int(eto[-1])
+    if nt == 0:
+        return np.zeros(0, dtype=np.int64)
+    ev = np.repeat(np.arange(eto.shape[0] - 1), np.diff(eto))
+    h0 = th[tho[:nt]]
+    h1 = th[tho[:nt] + 1]
+    return np.lexsort((h1, h0, ev))
+
+
+def canonical(res: dict) -> dict:
+    """Canonically ordered copy: event_track_offsets, per-track n, flattened hits, states."""
+    eto = np.asarray(res["event_track_offsets"], dtype=np.int64)
+    tho = np.asarray(res["track_hit_offsets"], dtype=np.int64)
+    th = np.asarray(res["track_hits"])
+    nt = int(eto[-1])
+    order = canonical_order(res)
+    n = (tho[1:nt + 1] - tho[:nt])[order]
+    starts = tho[:nt][order]
+    new_off = np.zeros(nt + 1, dtype=np.int64)
+    np.cumsum(n, out=new_off[1:])
+    idx = np.repeat(starts - new_off[:-1], n) + np.arange(int(new_off[-1]))
+    hits = th[idx] if nt else th[:0]
+    st = np.asarray(res["states"])[:, :nt][:, order]
+    return {"event_track_offsets": eto, "n": n, "track_hit_offsets": new_off, "track_hits": hits, "states": st}
+
+
+def assert_same_result(got: dict, want: dict, rel: float = 1e-5):
+    """O-17: hit lists, offsets, n_hits bit-exact; states |g-o| <= rel*|o| with 0 == 0 passing."""
+    a, b = canonical(got), canonical(want)
+    np.testing.assert_array_equal(a["event_track_offsets"], b["event_track_offsets"])
+    np.testing.assert_array_equal(a["n"], b["n"])
+    np.testing.assert_array_equal(a["track_hits"], b["track_hits"])
+    ga, wa = a["states"], b["states"]
+    # last plane: n_hits as u32 bits, exact
+    np.testing.assert_array_equal(ga[12].view(np.uint32), wa[12].view(np.uint32))
+    np.testing.assert_array_equal(ga[12].view(np.uint32).astype(np.int64), a["n"])
+    g = ga[:12].astype(np.float64)
+    w = wa[:12].astype(np.float64)
+    bad = np.abs(g - w) > rel * np.abs(w)
+    assert not bad.any(), f"{int(bad.sum())} state words beyond {rel} relative; first at {np.argwhere(bad)[:5]}"
+    return {"bit_identical_states": bool(np.array_equal(ga.view(np.uint32), wa.view(np.uint32)))}
+
+
+def line_event(modules, tx=0.1, ty=0.0, x0=0.0, y0=0.0, extra=()):
+    """Hits of the line x = x0 + tx z, y = y0 + ty z on the given modules (fp32-rounded), plus
+    extra (x, y, module) hits. Returns x, y, z, module arrays."""
+    xs, ys, zs, ms = [], [], [], []
+    for m in modules:
+        z = float(MODULE_Z[m])
+        xs.append(x0 + tx * z); ys.append(y0 + ty * z); zs.append(z); ms.append(m)
+    for (x, y, m) in extra:
+        xs.append(x); ys.append(y); zs.append(float(MODULE_Z[m])); ms.append(m)
+    return (np.array(xs, np.float32), np.array(ys, np.float32), np.array(zs, np.float32),
+            np.array(ms, np.uint8))
+
+
+def batch_of(events):
+    """Concatenate per-event (x, y, z, module) tuples into batch arrays + offsets."""
+    off = np.zeros(len(events) + 1, np.uint32)
+    for i, e in enumerate(events):
+        off[i + 1] = off[i] + e[0].shape[0]
+    cat = lambda k, dt: (np.concatenate([e[k] for e in events]).astype(dt) if events else np.zeros(0, dt))
+    return cat(0, np.float32), cat(1, np.float32), cat(2, np.float32), cat(3, np.uint8), off
+
+
+def track_modules(res, module, event=0):
+    """Sorted tuple of module-id tuples of the event's tracks."""
+    return sorted(tuple(int(module[h]) for h in hits) for hits, _ in split_tracks(res, event))
