@@ -1,0 +1,160 @@
+/* velo.h — C-ABI of libvelo: B200-native (sm_100a) VELO pixel-detector track reconstruction.
+ *
+ * What the library computes. The data-parallel core of the GPU first-stage trigger (HLT1) of
+ * arxiv/paper_2412_05041: reconstruction of "VELO tracks", the objects that the paper's forward
+ * tracking and seeding-matching consume (§5), over batches of independent events
+ * (30 MHz event stream, §3). The paper says only that HLT1 uses "a more simplified
+ * pattern recognition algorithm" and "simplified track fitting" (§5); the steps
+ * (per-module phi sort, search-by-triplet seeding, forwarding, ghost/clone filter, straight-line
+ * least-squares fit to the state at closest approach to the beamline) are named by
+ * BASELINE.json:north_star and made precise in SURVEY.md §8(c) items O-1 ... O-17, restated in
+ * DESIGN.md §3. Coordinates: origin at the nominal interaction point, z along the beam, y up
+ * (§2); lengths in mm.
+ *
+ * Conventions.
+ *  - Every function returns VELO_OK (0) or a negative error code; nothing throws or aborts.
+ *  - "DEVICE" pointers are CUDA device pointers of the current device; "HOST" pointers are plain
+ *    host pointers. The caller owns every buffer it passes. The library allocates device memory
+ *    only inside velo_scheduler_create.
+ *  - velo_reconstruct is asynchronous on `stream`: no allocation, no host synchronisation, no
+ *    use of the default stream. Its return value reports synchronous failures only (bad
+ *    arguments, workspace too small, launch error). Data-dependent failures are written to
+ *    out->summary[2] on the device (see velo_tracks_t).
+ *  - Concurrent calls on different streams with different workspaces and outputs are allowed.
+ *  - Inputs must be finite; NaN/Inf coordinates are undefined behaviour.
+ *  - There is no CPU fallback: without a CUDA device every compute entry point returns
+ *    VELO_ERR_CUDA.
+ */
+#ifndef VELO_H_
+#define VELO_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  VELO_OK = 0,
+  VELO_ERR_ARG = -1,       /* null pointer, zero capacity, inconsistent sizes                   */
+  VELO_ERR_GEOMETRY = -2,  /* n_modules outside 3..32, module_z not strictly increasing          */
+  VELO_ERR_WORKSPACE = -3, /* workspace_bytes < velo_workspace_bytes(...)                        */
+  VELO_ERR_CUDA = -4,      /* a CUDA runtime call or a kernel launch failed                      */
+  VELO_ERR_CAPACITY = -5,  /* (device status) tracks or track-hits exceed the output capacities  */
+  VELO_ERR_INPUT = -6      /* (device status) module id >= n_modules, non-monotone offsets, or   */
+                           /* an event with more than VELO_MAX_EVENT_HITS hits                   */
+};
+
+#define VELO_MAX_MODULES 32
+#define VELO_MAX_EVENT_HITS 65535u /* event-local hit indices are 16-bit inside the kernels     */
+#define VELO_N_STATE 13            /* words per track state, see velo_tracks_t.states           */
+
+/* ---- geometry (BASELINE.json:configs[0], configs[3]) ---------------- */
+typedef struct velo_geometry velo_geometry_t; /* opaque, host-resident, immutable after load    */
+
+typedef struct {           /* HOST POD, copied by velo_geometry_load                             */
+  uint32_t n_modules;      /* 26 in the paper's detector; must be 3..VELO_MAX_MODULES            */
+  const float* module_z;   /* HOST, n_modules, strictly increasing (mm)                          */
+  float r_in, r_out;       /* active annulus 5.1 .. 42.0 mm (informational)                      */
+  float pitch;             /* pixel pitch 0.055 mm; sets the default sigma_hit = pitch/sqrt(12)  */
+  float half_shift_x;      /* 0 closed; 24.5 = the 2023 49 mm opening (§2)           */
+} velo_geometry_desc_t;
+
+/* Validates and copies the description. *out is set to a new handle (free it with
+ * velo_geometry_free) or left untouched on error. Needs no CUDA device. */
+int velo_geometry_load(const velo_geometry_desc_t* desc, velo_geometry_t** out);
+void velo_geometry_free(velo_geometry_t* g);
+uint32_t velo_geometry_n_modules(const velo_geometry_t* g);
+
+/* ---- parameters (SURVEY.md §8(c) O-3, O-4, O-7, O-8, O-10 ... O-13; defaults A5 ... A13) ---- */
+typedef struct {           /* HOST POD                                                           */
+  int32_t phi_window_seed; /* O-8 window half-width, phi16 units (1 unit = pi/32768 rad); 300    */
+  int32_t phi_window_fwd;  /* O-7 window half-width; 300                                         */
+  float max_scatter_seed;  /* O-8 accept sc <= this (mm^2); 0.1                                  */
+  float max_scatter_fwd;   /* O-7; 0.1                                                           */
+  float max_scatter_weak;  /* O-10: 3-hit tracks need seed scatter <= this; 0.05                 */
+  uint32_t max_skipped;    /* O-7: consecutive missed modules a track survives; 1                */
+  float sigma_hit;         /* O-11: (float)(pitch/sqrt(12)) = 0x1.042186p-6 for 55 um pixels     */
+  float max_chi2_ndof;     /* O-12; 100                                                          */
+  uint32_t clone_num, clone_den; /* O-13: killed iff lost*den > n*num; 1, 3                      */
+} velo_params_t;
+
+/* Fills *p with the defaults above (sigma_hit from the geometry's pitch). */
+void velo_params_default(const velo_geometry_t* g, velo_params_t* p);
+
+/* ---- input: hits of a batch of events, structure of arrays ------ */
+typedef struct {
+  const float *x, *y, *z;        /* global-frame hit coordinates (mm). Indexed by ABSOLUTE hit    */
+                                 /* index, i.e. the same index space as event_offsets.            */
+  const uint8_t* module;         /* module id of each hit, 0 .. n_modules-1 (by increasing z)     */
+  const uint32_t* event_offsets; /* n_events+1, non-decreasing. Event e owns hits                 */
+                                 /* [event_offsets[e], event_offsets[e+1]). event_offsets[0] may  */
+                                 /* be non-zero: a batch is a slice of a larger array.            */
+  uint32_t n_events;
+  uint32_t n_hits;               /* = event_offsets[n_events] - event_offsets[0] (host knowledge) */
+} velo_hits_t;
+/* Hit order inside an event is arbitrary; there is no alignment or padding requirement. An event
+ * holds at most VELO_MAX_EVENT_HITS hits. Empty events and empty modules are legal (A15). */
+
+/* ---- output: VELO tracks = hit lists + beamline states (§5; O-11, O-14) --------- */
+typedef struct {
+  uint32_t* event_track_offsets; /* n_events+1. Tracks of event e are                             */
+                                 /* [event_track_offsets[e], event_track_offsets[e+1]).           */
+  uint32_t* track_hit_offsets;   /* cap_tracks+1; [n_tracks] = n_track_hits                       */
+  uint32_t* track_hits;          /* cap_track_hits; ABSOLUTE hit indices (same index space as     */
+                                 /* hits.x), in discovery order = decreasing module               */
+  float* states;                 /* VELO_N_STATE planes of cap_tracks words (plane stride =       */
+                                 /* cap_tracks): x, y, tx, ty, z at the point of closest approach */
+                                 /* to the z axis; cxx, cxtx, ctxtx, cyy, cyty, ctyty; chi2; and  */
+                                 /* n_hits stored as the bit pattern of a uint32                  */
+  uint32_t cap_tracks, cap_track_hits;
+  uint32_t* summary;             /* u32[4]: n_tracks, n_track_hits, status (VELO_OK or a negative */
+                                 /* code as two's complement), n_candidates                       */
+} velo_tracks_t;
+/* If the batch needs more than cap_tracks tracks or cap_track_hits track-hits, summary[2] =
+ * VELO_ERR_CAPACITY, summary[0..1] hold the REQUIRED sizes and the other output arrays are
+ * unspecified: results are never silently truncated. On VELO_ERR_INPUT the offending events
+ * contribute zero tracks. cap_tracks = n_hits and cap_track_hits = n_modules * n_hits can never
+ * overflow; cap_tracks = n_hits/4 + n_events and cap_track_hits = 2*n_hits is ample for the
+ * BASELINE.json workloads. Tracks of an event are emitted in creation order: seeding step
+ * (centre module) descending, then sorted position of the seed's centre hit. */
+
+/* Bytes of DEVICE workspace velo_reconstruct needs for a batch of this shape. */
+size_t velo_workspace_bytes(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks,
+                            uint32_t cap_track_hits);
+
+/* Reconstructs one batch. hits/out hold DEVICE pointers; geometry, params and the two structs
+ * themselves are HOST memory read before the call returns. workspace: DEVICE, 256-byte aligned,
+ * used until the work enqueued on `stream` completes. `stream` is a cudaStream_t passed as
+ * void* so that this header needs no CUDA include. */
+int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- event-batch scheduler on streams (§3) ------------------ */
+/* Owns n_streams CUDA streams, each with device input, output and workspace buffers for batches
+ * of up to max_batch_events events / max_batch_hits hits, and pinned staging for the summaries. */
+typedef struct velo_scheduler velo_scheduler_t;
+int velo_scheduler_create(const velo_geometry_t* g, uint32_t n_streams, uint32_t max_batch_events,
+                          uint32_t max_batch_hits, velo_scheduler_t** out);
+void velo_scheduler_free(velo_scheduler_t* s);
+
+/* End-to-end path over HOST buffers. hits holds HOST pointers (pinned memory makes the copies
+ * asynchronous). Events are cut into n_batches contiguous batches at batch_begin[0..n_batches]
+ * (event indices, batch_begin[0] = 0, batch_begin[n_batches] = hits->n_events); batch b runs on
+ * stream b % n_streams: host->device copy of its slice, velo_reconstruct, device->host copy of
+ * exactly the produced tracks into out[b] (HOST pointers, capacities per batch; summary is a
+ * HOST u32[4]). Offsets in out[b] are batch-local; track_hits are absolute hit indices.
+ * Returns after every copy has completed. A batch larger than the scheduler's limits or an
+ * output capacity below cap_tracks = n_hits/4 + n_events, cap_track_hits = 2*n_hits of the
+ * device buffers is reported per batch through out[b].summary[2]. */
+int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, const velo_hits_t* hits,
+                            const uint32_t* batch_begin, uint32_t n_batches, velo_tracks_t* out);
+
+/* Library version string, e.g. "velo-b200 0.1 (sm_100a)". */
+const char* velo_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VELO_H_ */

@@ -1,0 +1,86 @@
+// velo_api.cu — the C-ABI of libvelo (include/velo.h): argument checks, workspace carving, kernel
+// launches and the event-batch scheduler on streams. No reconstruction arithmetic lives here.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "velo_internal.h"
+
+struct velo_geometry {
+  uint32_t n_modules;
+  float module_z[VELO_MAX_MODULES];
+  float r_in, r_out, pitch, half_shift_x;
+};
+
+extern "C" {
+
+const char* velo_version(void) { return "velo-b200 0.1 (sm_100a)"; }
+
+int velo_geometry_load(const velo_geometry_desc_t* desc, velo_geometry_t** out) {
+  if (!desc || !out || !desc->module_z) return VELO_ERR_ARG;
+  if (desc->n_modules < 3 || desc->n_modules > VELO_MAX_MODULES) return VELO_ERR_GEOMETRY;
+  for (uint32_t m = 0; m < desc->n_modules; ++m) {
+    if (!isfinite(desc->module_z[m])) return VELO_ERR_GEOMETRY;
+    if (m && !(desc->module_z[m] > desc->module_z[m - 1])) return VELO_ERR_GEOMETRY;
+  }
+  if (!(desc->pitch > 0.0f) || !isfinite(desc->pitch)) return VELO_ERR_GEOMETRY;
+  velo_geometry* g = new (std::nothrow) velo_geometry();
+  if (!g) return VELO_ERR_ARG;
+  g->n_modules = desc->n_modules;
+  memcpy(g->module_z, desc->module_z, sizeof(float) * desc->n_modules);
+  g->r_in = desc->r_in; g->r_out = desc->r_out; g->pitch = desc->pitch; g->half_shift_x = desc->half_shift_x;
+  *out = g;
+  return VELO_OK;
+}
+
+void velo_geometry_free(velo_geometry_t* g) { delete g; }
+
+uint32_t velo_geometry_n_modules(const velo_geometry_t* g) { return g ? g->n_modules : 0; }
+
+void velo_params_default(const velo_geometry_t* g, velo_params_t* p) {
+  if (!p) return;
+  const double pitch = g ? (double)g->pitch : 0.055;
+  p->phi_window_seed = 300; p->phi_window_fwd = 300;
+  p->max_scatter_seed = 0.1f; p->max_scatter_fwd = 0.1f; p->max_scatter_weak = 0.05f;
+  p->max_skipped = 1;
+  p->sigma_hit = (float)(pitch / sqrt(12.0));
+  p->max_chi2_ndof = 100.0f;
+  p->clone_num = 1; p->clone_den = 3;
+}
+
+size_t velo_workspace_bytes(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits) {
+  (void)n_hits;
+  return velo::carve_workspace(nullptr, n_events, cap_tracks, cap_track_hits, velo::default_n_slabs()).bytes;
+}
+
+int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!g || !hits || !params || !out || !workspace) return VELO_ERR_ARG;
+  if (!hits->event_offsets || !out->event_track_offsets || !out->track_hit_offsets || !out->summary)
+    return VELO_ERR_ARG;
+  if (hits->n_hits && (!hits->x || !hits->y || !hits->z || !hits->module)) return VELO_ERR_ARG;
+  if (!out->track_hits || !out->states || out->cap_tracks == 0 || out->cap_track_hits == 0) return VELO_ERR_ARG;
+  if (((uintptr_t)workspace & 255u) != 0) return VELO_ERR_ARG;
+  if (params->clone_den == 0) return VELO_ERR_ARG;
+  const size_t need = velo_workspace_bytes(hits->n_events, hits->n_hits, out->cap_tracks, out->cap_track_hits);
+  if (workspace_bytes < need) return VELO_ERR_WORKSPACE;
+
+  velo::KernelArgs a{};
+  a.x = hits->x; a.y = hits->y; a.z = hits->z; a.module = hits->module;
+  a.event_offsets = hits->event_offsets;
+  a.n_events = hits->n_events; a.n_modules = g->n_modules;
+  a.P = *params;
+  if (a.P.max_skipped > 200u) a.P.max_skipped = 200u;  // more misses than modules is all the same
+  a.event_track_offsets = out->event_track_offsets; a.track_hit_offsets = out->track_hit_offsets;
+  a.track_hits = out->track_hits; a.states = out->states;
+  a.cap_tracks = out->cap_tracks; a.cap_track_hits = out->cap_track_hits; a.summary = out->summary;
+  a.ws = velo::carve_workspace(workspace, hits->n_events, out->cap_tracks, out->cap_track_hits,
+                               velo::default_n_slabs());
+  const int err = velo::launch_reconstruct(a, (cudaStream_t)stream);
+  return err == 0 ? VELO_OK : VELO_ERR_CUDA;
+}
+
+}  // extern "C"

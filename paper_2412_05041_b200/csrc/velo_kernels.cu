@@ -1,0 +1,437 @@
+// velo_kernels.cu — sm_100a kernels of the VELO hot path (SURVEY.md §8(a) S0 ... S7).
+//
+// One CTA reconstructs one event at a time: S0 decode (phi16, bucket key), S1 phi sort, the
+// 24-step module loop with S3 forwarding and S2 search-by-triplet seeding, S4 ghost filter, S5
+// straight-line fit, S6 clone filter, then writes its surviving tracks into a temp block
+// allocated with one atomic per event. A scan kernel turns the per-event counts into
+// offsets and a copy kernel moves the temp blocks into event order (S7).
+// Step semantics: SURVEY.md §8(c) O-1 ... O-14 (restated in DESIGN.md §3); the paper itself
+// (§5) names the objects but gives no step.
+#include "velo_device.cuh"
+#include "velo_internal.h"
+
+namespace velo {
+
+namespace {
+
+constexpr int kThreads = 256;            // CTA size of the event kernel
+constexpr unsigned kInactive = 255u;     // tmiss value of a track that stopped forwarding
+
+// Per-event arrays (sorted-hit order) and the candidate-track table. The pointers address either
+// shared memory (small events) or the CTA's slab in global memory (large events).
+struct Ev {
+  float *sx, *sy, *sz;       // sorted hit coordinates
+  int16_t* phi;              // sorted phi16
+  uint16_t* perm;            // sorted position -> original event-local index
+  uint8_t* flag;             // O-5 flag[h]
+  unsigned long long* owner; // O-13 owner[h]
+  uint32_t *stash, *tmp;     // sort scratch
+  uint16_t* th;              // candidate hits, th[k * tcap + t] = k-th hit of track t (sorted idx)
+  uint8_t *tn, *tmiss;       // hits on the track; consecutive misses (kInactive = stopped)
+  uint16_t* tcentre;         // sorted index of the seed's centre hit
+  float* tseed;              // seed scatter
+  unsigned long long* tkey;  // O-13 key
+  uint8_t* tpass;            // 0 dropped by O-10/O-12, 1 passed, 2 survives O-13
+  uint32_t tcap;             // capacity of the track table
+};
+
+struct Shared {
+  uint32_t binoff[kMaxBins + 1];      // histogram, then exclusive offsets of the phi buckets
+  unsigned long long warp_sums[33];
+  uint32_t mod_off[VELO_MAX_MODULES + 1];
+  uint32_t ticket, bad, ntracks, tbase, hbase;
+};
+
+// Visits, in ascending sorted index, every hit j of module m with |int16(phi[j] - c)| <= W (O-3).
+template <class F>
+__device__ __forceinline__ void for_window(const Ev& ev, const uint32_t* binoff, int m, int c, int W, F&& f) {
+  if (W < 0) return;
+  const uint32_t* bo = binoff + m * kBinsPerModule;
+  if (2 * (long long)W + 1 >= 65536) {
+    for (uint32_t j = bo[0]; j < bo[kBinsPerModule]; ++j) f(j);
+    return;
+  }
+  const int lo = c + 32768 - W, hi = c + 32768 + W;  // unsigned-phi interval, may leave [0, 65535]
+  auto seg = [&](int a, int b) {
+    const uint32_t j1 = bo[(b >> kBinShift) + 1];
+    for (uint32_t j = bo[a >> kBinShift]; j < j1; ++j) {
+      const int pu = (int)ev.phi[j] + 32768;
+      if (pu >= a && pu <= b) f(j);
+    }
+  };
+  if (lo < 0) { seg(0, hi); seg(lo + 65536, 65535); }
+  else if (hi > 65535) { seg(0, hi - 65536); seg(lo, 65535); }
+  else seg(lo, hi);
+}
+
+// O-11 straight-line fit of the hits of candidate t; writes the 13 state words to st[].
+__device__ __forceinline__ void fit_track(const Ev& ev, uint32_t t, uint32_t n, float sig2, float inv_s2,
+                                          float* st) {
+  float sz = 0.0f, sx = 0.0f, sy = 0.0f;
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t h = ev.th[i * ev.tcap + t];
+    sz = __fadd_rn(sz, ev.sz[h]); sx = __fadd_rn(sx, ev.sx[h]); sy = __fadd_rn(sy, ev.sy[h]);
+  }
+  const float nf = (float)n;
+  const float zb = __fdiv_rn(sz, nf), xb = __fdiv_rn(sx, nf), yb = __fdiv_rn(sy, nf);
+  float sdd = 0.0f, sdx = 0.0f, sdy = 0.0f;
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t h = ev.th[i * ev.tcap + t];
+    const float d = __fsub_rn(ev.sz[h], zb);
+    sdd = __fadd_rn(sdd, __fmul_rn(d, d));
+    sdx = __fadd_rn(sdx, __fmul_rn(d, __fsub_rn(ev.sx[h], xb)));
+    sdy = __fadd_rn(sdy, __fmul_rn(d, __fsub_rn(ev.sy[h], yb)));
+  }
+  const float tx = __fdiv_rn(sdx, sdd), ty = __fdiv_rn(sdy, sdd);
+  float c = 0.0f;
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t h = ev.th[i * ev.tcap + t];
+    const float d = __fsub_rn(ev.sz[h], zb);
+    const float rx = __fsub_rn(__fsub_rn(ev.sx[h], xb), __fmul_rn(tx, d));
+    const float ry = __fsub_rn(__fsub_rn(ev.sy[h], yb), __fmul_rn(ty, d));
+    c = __fadd_rn(c, __fmul_rn(rx, rx));
+    c = __fadd_rn(c, __fmul_rn(ry, ry));
+  }
+  const float chi2 = __fmul_rn(c, inv_s2);
+  const float s2 = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
+  float dzb;
+  if (s2 < 1e-12f) dzb = 0.0f;
+  else dzb = -__fdiv_rn(__fadd_rn(__fmul_rn(xb, tx), __fmul_rn(yb, ty)), s2);
+  const float vt = __fdiv_rn(sig2, sdd);
+  const float cxtx = __fmul_rn(dzb, vt);
+  const float cxx = __fadd_rn(__fdiv_rn(sig2, nf), __fmul_rn(__fmul_rn(dzb, dzb), vt));
+  st[0] = __fadd_rn(xb, __fmul_rn(tx, dzb));
+  st[1] = __fadd_rn(yb, __fmul_rn(ty, dzb));
+  st[2] = tx; st[3] = ty;
+  st[4] = __fadd_rn(zb, dzb);
+  st[5] = cxx; st[6] = cxtx; st[7] = vt;
+  st[8] = cxx; st[9] = cxtx; st[10] = vt;
+  st[11] = chi2;
+  st[12] = __uint_as_float(n);
+}
+
+__device__ __forceinline__ void set_status(uint32_t* counters, int code) {
+  // first error wins; VELO_OK is 0
+  atomicCAS(&counters[kCtrStatus], 0u, (uint32_t)code);
+}
+
+// Reconstructs event e with the CTA's arrays `ev`. Called by all threads of the CTA.
+__device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uint32_t e) {
+  const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+  const uint32_t M = a.n_modules;
+  const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
+  const uint32_t nbins = M * kBinsPerModule;
+  const velo_params_t& P = a.P;
+
+  // ---- input checks (VELO_ERR_INPUT): the event then contributes zero tracks -------------------
+  if (o1 < o0 || o1 - o0 > VELO_MAX_EVENT_HITS) {
+    if (tid == 0) { set_status(a.ws.counters, VELO_ERR_INPUT); a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); }
+    return;
+  }
+  const uint32_t n = o1 - o0;
+  const float* gx = a.x + o0; const float* gy = a.y + o0; const float* gz = a.z + o0;
+  const uint8_t* gm = a.module + o0;
+
+  // ---- S0 decode: phi16 and bucket histogram (O-1) ---------------------------------------------
+  for (uint32_t b = tid; b <= nbins; b += nthr) sh.binoff[b] = 0;
+  if (tid == 0) { sh.bad = 0; sh.ntracks = 0; }
+  __syncthreads();
+  for (uint32_t i = tid; i < n; i += nthr) {
+    const uint32_t m = gm[i];
+    if (m >= M) { sh.bad = 1; continue; }
+    const uint32_t pu = (uint32_t)(phi16(gx[i], gy[i]) + 32768);
+    const uint32_t slot = atomicAdd(&sh.binoff[m * kBinsPerModule + (pu >> kBinShift)], 1u);
+    ev.stash[i] = (pu << 16) | slot;
+  }
+  __syncthreads();
+  if (sh.bad) {
+    if (tid == 0) { set_status(a.ws.counters, VELO_ERR_INPUT); a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); }
+    __syncthreads();
+    return;
+  }
+  // exclusive scan of the histogram -> bucket offsets; binoff[nbins] = n
+  {
+    const uint32_t per = (nbins + nthr - 1) / nthr;
+    const uint32_t b0 = tid * per, b1 = min(b0 + per, nbins);
+    uint32_t s = 0;
+    for (uint32_t b = b0; b < b1; ++b) s += sh.binoff[b];
+    unsigned long long tot;
+    uint32_t run = (uint32_t)block_scan_excl(s, sh.warp_sums, &tot);
+    for (uint32_t b = b0; b < b1; ++b) { const uint32_t c = sh.binoff[b]; sh.binoff[b] = run; run += c; }
+    if (tid == 0) sh.binoff[nbins] = n;
+  }
+  __syncthreads();
+  for (uint32_t m = tid; m <= M; m += nthr) sh.mod_off[m] = sh.binoff[m * kBinsPerModule];
+
+  // ---- S1 phi sort (O-2): group by bucket, then rank inside the bucket by (phi16, index) -------
+  for (uint32_t i = tid; i < n; i += nthr) {
+    const uint32_t st = ev.stash[i], pu = st >> 16;
+    const uint32_t bin = (uint32_t)gm[i] * kBinsPerModule + (pu >> kBinShift);
+    ev.tmp[sh.binoff[bin] + (st & 0xffffu)] = (pu << 16) | i;
+  }
+  __syncthreads();
+  for (uint32_t i = tid; i < n; i += nthr) {
+    const uint32_t pu = ev.stash[i] >> 16;
+    const uint32_t bin = (uint32_t)gm[i] * kBinsPerModule + (pu >> kBinShift);
+    const uint32_t item = (pu << 16) | i;
+    const uint32_t lo = sh.binoff[bin], hi = sh.binoff[bin + 1];
+    uint32_t r = lo;
+    for (uint32_t j = lo; j < hi; ++j) r += (ev.tmp[j] < item) ? 1u : 0u;
+    ev.sx[r] = gx[i]; ev.sy[r] = gy[i]; ev.sz[r] = gz[i];
+    ev.phi[r] = (int16_t)((int)pu - 32768);
+    ev.perm[r] = (uint16_t)i;
+    ev.flag[r] = 0;
+    ev.owner[r] = ~0ull;
+  }
+  __syncthreads();
+
+  // ---- O-6 module loop --------------------------------------------------------------------------
+  for (uint32_t s = M - 2; s >= 1; --s) {
+    const uint32_t u = s - 1;
+    // (A) O-7 forwarding into module u of every track active at the start of the step
+    const uint32_t nt0 = sh.ntracks;
+    for (uint32_t t = tid; t < nt0; t += nthr) {
+      const uint32_t miss = ev.tmiss[t];
+      if (miss == kInactive) continue;
+      const uint32_t nh = ev.tn[t];
+      const uint32_t ha = ev.th[(nh - 2) * ev.tcap + t], hb = ev.th[(nh - 1) * ev.tcap + t];
+      const float x1 = ev.sx[hb], y1 = ev.sy[hb], z1 = ev.sz[hb];
+      const float dx = __fsub_rn(x1, ev.sx[ha]), dy = __fsub_rn(y1, ev.sy[ha]), dz = __fsub_rn(z1, ev.sz[ha]);
+      bool found = false; uint32_t best = 0; float best_sc = 0.0f;
+      for_window(ev, sh.binoff, (int)u, (int)ev.phi[hb], P.phi_window_fwd, [&](uint32_t c) {
+        const float sc = scatter(dx, dy, dz, x1, y1, z1, ev.sx[c], ev.sy[c], ev.sz[c]);
+        if (sc <= P.max_scatter_fwd && (!found || sc < best_sc)) { found = true; best = c; best_sc = sc; }
+      });
+      if (found) {
+        ev.th[nh * ev.tcap + t] = (uint16_t)best;
+        ev.tn[t] = (uint8_t)(nh + 1);
+        ev.tmiss[t] = 0;
+        if (nh + 1 == 4) { for (uint32_t i = 0; i < 3; ++i) ev.flag[ev.th[i * ev.tcap + t]] = 1; }
+        if (nh + 1 >= 4) ev.flag[best] = 1;   // (B): forwarding never reads flags, so set them now
+      } else {
+        ev.tmiss[t] = (miss + 1 > P.max_skipped) ? (uint8_t)kInactive : (uint8_t)(miss + 1);
+      }
+    }
+    __syncthreads();
+    // (C) O-8 seeding with centre module s; one thread per centre hit, tracks numbered by a scan
+    const uint32_t c_begin = sh.mod_off[s], c_end = sh.mod_off[s + 1];
+    for (uint32_t c0 = c_begin; c0 < c_end; c0 += nthr) {
+      const uint32_t h1 = c0 + tid;
+      bool found = false; uint32_t b0 = 0, b2 = 0; float best_sc = 0.0f;
+      if (h1 < c_end && !ev.flag[h1]) {
+        const float x1 = ev.sx[h1], y1 = ev.sy[h1], z1 = ev.sz[h1];
+        const int c = (int)ev.phi[h1];
+        for_window(ev, sh.binoff, (int)s + 1, c, P.phi_window_seed, [&](uint32_t h0) {
+          if (ev.flag[h0]) return;
+          const float dx = __fsub_rn(x1, ev.sx[h0]), dy = __fsub_rn(y1, ev.sy[h0]), dz = __fsub_rn(z1, ev.sz[h0]);
+          for_window(ev, sh.binoff, (int)s - 1, c, P.phi_window_seed, [&](uint32_t h2) {
+            if (ev.flag[h2]) return;
+            const float sc = scatter(dx, dy, dz, x1, y1, z1, ev.sx[h2], ev.sy[h2], ev.sz[h2]);
+            if (sc <= P.max_scatter_seed && (!found || sc < best_sc)) { found = true; b0 = h0; b2 = h2; best_sc = sc; }
+          });
+        });
+      }
+      unsigned long long tot;
+      const uint32_t slot = sh.ntracks + (uint32_t)block_scan_excl(found ? 1ull : 0ull, sh.warp_sums, &tot);
+      if (found && slot < ev.tcap) {
+        ev.th[0 * ev.tcap + slot] = (uint16_t)b0;
+        ev.th[1 * ev.tcap + slot] = (uint16_t)h1;
+        ev.th[2 * ev.tcap + slot] = (uint16_t)b2;
+        ev.tn[slot] = 3; ev.tmiss[slot] = 0;
+        ev.tseed[slot] = best_sc; ev.tcentre[slot] = (uint16_t)h1;
+      }
+      __syncthreads();
+      if (tid == 0) sh.ntracks += (uint32_t)tot;
+      __syncthreads();
+    }
+    __syncthreads();
+  }
+  const uint32_t nt = sh.ntracks;  // candidates never exceed the centre hits, hence never tcap (slab)
+
+  // ---- O-10 ghost filter, O-11 fit, O-12 chi2 cut, O-13 owners ----------------------------------
+  const float sig2 = __fmul_rn(P.sigma_hit, P.sigma_hit);
+  const float inv_s2 = __fdiv_rn(1.0f, sig2);
+  for (uint32_t t = tid; t < nt; t += nthr) {
+    const uint32_t nh = ev.tn[t];
+    bool pass = true;
+    if (nh == 3) {
+      if (ev.flag[ev.th[t]] || ev.flag[ev.th[ev.tcap + t]] || ev.flag[ev.th[2 * ev.tcap + t]]) pass = false;
+      if (!(ev.tseed[t] <= P.max_scatter_weak)) pass = false;
+    }
+    unsigned long long key = 0;
+    if (pass) {
+      float st[VELO_N_STATE];
+      fit_track(ev, t, nh, sig2, inv_s2, st);
+      const float lim = __fmul_rn(P.max_chi2_ndof, (float)(2 * (int)nh - 4));
+      if (st[11] > lim) pass = false;
+      key = ((unsigned long long)(255u - nh) << 56) | ((unsigned long long)__float_as_uint(st[11]) << 24) |
+            (unsigned long long)ev.tcentre[t];
+    }
+    ev.tpass[t] = pass ? 1 : 0;
+    ev.tkey[t] = key;
+    if (pass) for (uint32_t i = 0; i < nh; ++i) atomicMin(&ev.owner[ev.th[i * ev.tcap + t]], key);
+  }
+  __syncthreads();
+  // ---- O-13 clone filter; per-thread totals of survivors --------------------------------------
+  uint32_t my_t = 0, my_h = 0;
+  for (uint32_t t = tid; t < nt; t += nthr) {
+    if (!ev.tpass[t]) continue;
+    const uint32_t nh = ev.tn[t];
+    const unsigned long long key = ev.tkey[t];
+    uint32_t lost = 0;
+    for (uint32_t i = 0; i < nh; ++i) lost += (ev.owner[ev.th[i * ev.tcap + t]] != key) ? 1u : 0u;
+    if (!((unsigned long long)lost * P.clone_den > (unsigned long long)nh * P.clone_num)) {
+      ev.tpass[t] = 2; my_t += 1; my_h += nh;
+    }
+  }
+  // ---- S7 part 1: allocate the event's temp block, write survivors in creation order -----------
+  unsigned long long tot;
+  block_scan_excl(((unsigned long long)my_h << 32) | my_t, sh.warp_sums, &tot);
+  const uint32_t ev_nt = (uint32_t)(tot & 0xffffffffu), ev_nh = (uint32_t)(tot >> 32);
+  if (tid == 0) {
+    sh.tbase = atomicAdd(&a.ws.counters[kCtrTracks], ev_nt);
+    sh.hbase = atomicAdd(&a.ws.counters[kCtrHits], ev_nh);
+    atomicAdd(&a.ws.counters[kCtrCand], nt);
+    a.ws.ev_rec[e] = make_uint4(sh.tbase, sh.hbase, ev_nt, ev_nh);
+  }
+  __syncthreads();
+  const uint32_t tbase = sh.tbase, hbase = sh.hbase;
+  const bool fits = (unsigned long long)tbase + ev_nt <= a.cap_tracks &&
+                    (unsigned long long)hbase + ev_nh <= a.cap_track_hits;
+  unsigned long long run = 0;  // (hits << 32 | tracks) written so far
+  for (uint32_t t0 = 0; t0 < nt; t0 += nthr) {
+    const uint32_t t = t0 + tid;
+    const bool surv = t < nt && ev.tpass[t] == 2;
+    const uint32_t nh = surv ? ev.tn[t] : 0;
+    unsigned long long ctot;
+    const unsigned long long pre = run + block_scan_excl(surv ? (((unsigned long long)nh << 32) | 1ull) : 0ull,
+                                                         sh.warp_sums, &ctot);
+    run += ctot;
+    if (surv && fits) {
+      const uint32_t lt = (uint32_t)(pre & 0xffffffffu), lh = (uint32_t)(pre >> 32);
+      float st[VELO_N_STATE];
+      fit_track(ev, t, nh, sig2, inv_s2, st);
+#pragma unroll
+      for (int k = 0; k < VELO_N_STATE; ++k) a.ws.tmp_states[(size_t)k * a.cap_tracks + tbase + lt] = st[k];
+      a.ws.tmp_loff[tbase + lt] = lh;
+      for (uint32_t i = 0; i < nh; ++i) a.ws.tmp_hits[hbase + lh + i] = o0 + ev.perm[ev.th[i * ev.tcap + t]];
+    }
+  }
+  __syncthreads();
+}
+
+// ---- event kernel, slab variant: persistent CTAs pull events from a ticket counter -------------
+__global__ void __launch_bounds__(kThreads) velo_event_slab_kernel(const KernelArgs a) {
+  __shared__ Shared sh;
+  const SlabLayout L = slab_layout();
+  unsigned char* slab = a.ws.slabs + (size_t)blockIdx.x * L.bytes;
+  Ev ev;
+  ev.sx = (float*)(slab + L.sx); ev.sy = (float*)(slab + L.sy); ev.sz = (float*)(slab + L.sz);
+  ev.phi = (int16_t*)(slab + L.phi); ev.perm = (uint16_t*)(slab + L.perm); ev.flag = slab + L.flag;
+  ev.owner = (unsigned long long*)(slab + L.owner);
+  ev.stash = (uint32_t*)(slab + L.stash); ev.tmp = (uint32_t*)(slab + L.tmp);
+  ev.th = (uint16_t*)(slab + L.th); ev.tn = slab + L.tn; ev.tmiss = slab + L.tmiss;
+  ev.tcentre = (uint16_t*)(slab + L.tcentre); ev.tseed = (float*)(slab + L.tseed);
+  ev.tkey = (unsigned long long*)(slab + L.tkey); ev.tpass = slab + L.tpass;
+  ev.tcap = kSlabHits;
+  for (;;) {
+    if (threadIdx.x == 0) sh.ticket = atomicAdd(&a.ws.counters[kCtrTicket], 1u);
+    __syncthreads();
+    const uint32_t e = sh.ticket;
+    __syncthreads();
+    if (e >= a.n_events) break;
+    process_event(a, ev, sh, e);
+  }
+}
+
+// ---- S7 part 2: exclusive scans of the per-event counts (one CTA) ------------------------------
+__global__ void __launch_bounds__(1024) velo_offsets_kernel(const KernelArgs a) {
+  __shared__ unsigned long long warp_sums[33];
+  const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;
+  const uint32_t per = (ne + nthr - 1) / nthr;
+  const uint32_t e0 = min(tid * per, ne), e1 = min(e0 + per, ne);
+  unsigned long long s = 0;
+  for (uint32_t e = e0; e < e1; ++e) { const uint4 r = a.ws.ev_rec[e]; s += ((unsigned long long)r.w << 32) | r.z; }
+  unsigned long long tot;
+  unsigned long long run = block_scan_excl(s, warp_sums, &tot);
+  const uint32_t n_tracks = (uint32_t)(tot & 0xffffffffu), n_hits = (uint32_t)(tot >> 32);
+  for (uint32_t e = e0; e < e1; ++e) {
+    const uint4 r = a.ws.ev_rec[e];
+    a.event_track_offsets[e] = (uint32_t)(run & 0xffffffffu);
+    a.ws.ev_hit_base[e] = (uint32_t)(run >> 32);
+    run += ((unsigned long long)r.w << 32) | r.z;
+  }
+  if (tid == 0) {
+    a.event_track_offsets[ne] = n_tracks;
+    a.ws.ev_hit_base[ne] = n_hits;
+    uint32_t status = a.ws.counters[kCtrStatus];
+    const bool over = n_tracks > a.cap_tracks || n_hits > a.cap_track_hits;
+    if (status == 0 && over) status = (uint32_t)VELO_ERR_CAPACITY;
+    if (!over) a.track_hit_offsets[n_tracks] = n_hits;
+    a.summary[0] = n_tracks; a.summary[1] = n_hits; a.summary[2] = status;
+    a.summary[3] = a.ws.counters[kCtrCand];
+  }
+}
+
+// ---- S7 part 3: move every event's temp block to its place in event order ----------------------
+// One warp per event keeps the copies coalesced (tracks of an event are contiguous on both sides).
+__global__ void __launch_bounds__(256) velo_compact_kernel(const KernelArgs a) {
+  const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t tot_t = a.event_track_offsets[a.n_events], tot_h = a.ws.ev_hit_base[a.n_events];
+  if (tot_t > a.cap_tracks || tot_h > a.cap_track_hits) return;  // VELO_ERR_CAPACITY: nothing valid
+  for (uint32_t e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; e < a.n_events; e += warps) {
+    const uint4 r = a.ws.ev_rec[e];
+    const uint32_t dst_t = a.event_track_offsets[e], dst_h = a.ws.ev_hit_base[e];
+    for (uint32_t k = lane; k < r.z; k += 32) {
+      a.track_hit_offsets[dst_t + k] = dst_h + a.ws.tmp_loff[r.x + k];
+#pragma unroll
+      for (int p = 0; p < VELO_N_STATE; ++p)
+        a.states[(size_t)p * a.cap_tracks + dst_t + k] = a.ws.tmp_states[(size_t)p * a.cap_tracks + r.x + k];
+    }
+    for (uint32_t k = lane; k < r.w; k += 32) a.track_hits[dst_h + k] = a.ws.tmp_hits[r.y + k];
+  }
+}
+
+}  // namespace
+
+// ---- host side -----------------------------------------------------------------------------------
+uint32_t default_n_slabs() { return 148u * 2u; }
+
+Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, uint32_t cap_track_hits,
+                          uint32_t n_slabs) {
+  Workspace w{};
+  size_t o = 0;
+  unsigned char* b = (unsigned char*)base;
+  auto take = [&](size_t bytes) { size_t r = o; o += ((bytes + 255) / 256) * 256; return b + r; };
+  w.counters = (uint32_t*)take(sizeof(uint32_t) * kNumCounters);
+  w.ev_rec = (uint4*)take(sizeof(uint4) * ((size_t)n_events + 1));
+  w.ev_hit_base = (uint32_t*)take(4 * ((size_t)n_events + 1));
+  w.large_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
+  w.tmp_loff = (uint32_t*)take(4 * ((size_t)cap_tracks + 1));
+  w.tmp_hits = (uint32_t*)take(4 * ((size_t)cap_track_hits + 1));
+  w.tmp_states = (float*)take(4 * (size_t)VELO_N_STATE * ((size_t)cap_tracks + 1));
+  w.n_slabs = n_slabs;
+  w.slabs = take((size_t)n_slabs * slab_layout().bytes);
+  w.bytes = o;
+  return w;
+}
+
+int launch_reconstruct(const KernelArgs& a, cudaStream_t stream) {
+  cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);
+  if (err != cudaSuccess) return (int)err;
+  if (a.n_events > 0) {
+    const uint32_t grid = a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events;
+    velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a);
+  }
+  velo_offsets_kernel<<<1, 1024, 0, stream>>>(a);
+  if (a.n_events > 0) {
+    const uint32_t warps_per_cta = 256 / 32;
+    uint32_t grid = (a.n_events + warps_per_cta - 1) / warps_per_cta;
+    if (grid > 148u * 8u) grid = 148u * 8u;
+    velo_compact_kernel<<<grid, 256, 0, stream>>>(a);
+  }
+  return (int)cudaGetLastError();
+}
+
+}  // namespace velo
