@@ -131,6 +131,24 @@ size_t velo_workspace_bytes(uint32_t n_events, uint32_t n_hits, uint32_t cap_tra
 int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
                      velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Same call with launch options, for measurement and tuning. opts may be NULL (= velo_reconstruct).
+ * event_kernel_start/stop: cudaEvent_t handles (or NULL) recorded on `stream` immediately before
+ * and after the event kernel (the kernel that carries S0 ... S6), so that a benchmark can time the
+ * dominant kernel of a batch on the stream it runs on. ctas_per_sm: persistent CTAs per SM of the
+ * event kernel, 0 = library default; the workspace must have been sized for the default or for
+ * velo_workspace_bytes_opts with the same value. */
+typedef struct {
+  void* event_kernel_start;
+  void* event_kernel_stop;
+  uint32_t ctas_per_sm;
+  uint32_t reserved;
+} velo_launch_options_t;
+size_t velo_workspace_bytes_opts(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks,
+                                 uint32_t cap_track_hits, const velo_launch_options_t* opts);
+int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                          velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
+                          const velo_launch_options_t* opts);
+
 /* ---- event-batch scheduler on streams (§3) ------------------ */
 /* Owns n_streams CUDA streams, each with device input, output and workspace buffers for batches
  * of up to max_batch_events events / max_batch_hits hits, and pinned staging for the summaries. */

@@ -51,13 +51,24 @@ void velo_params_default(const velo_geometry_t* g, velo_params_t* p) {
   p->clone_num = 1; p->clone_den = 3;
 }
 
-size_t velo_workspace_bytes(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits) {
-  (void)n_hits;
-  return velo::carve_workspace(nullptr, n_events, cap_tracks, cap_track_hits, velo::default_n_slabs()).bytes;
+static uint32_t n_slabs_for(const velo_launch_options_t* opts) {
+  const uint32_t per_sm = (opts && opts->ctas_per_sm) ? opts->ctas_per_sm : 0;
+  return per_sm ? velo::num_sms() * (per_sm > 16 ? 16 : per_sm) : velo::default_n_slabs();
 }
 
-int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
-                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream) {
+size_t velo_workspace_bytes_opts(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits,
+                                 const velo_launch_options_t* opts) {
+  (void)n_hits;
+  return velo::carve_workspace(nullptr, n_events, cap_tracks, cap_track_hits, n_slabs_for(opts)).bytes;
+}
+
+size_t velo_workspace_bytes(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits) {
+  return velo_workspace_bytes_opts(n_events, n_hits, cap_tracks, cap_track_hits, nullptr);
+}
+
+int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                          velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
+                          const velo_launch_options_t* opts) {
   if (!g || !hits || !params || !out || !workspace) return VELO_ERR_ARG;
   if (!hits->event_offsets || !out->event_track_offsets || !out->track_hit_offsets || !out->summary)
     return VELO_ERR_ARG;
@@ -65,7 +76,7 @@ int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const ve
   if (!out->track_hits || !out->states || out->cap_tracks == 0 || out->cap_track_hits == 0) return VELO_ERR_ARG;
   if (((uintptr_t)workspace & 255u) != 0) return VELO_ERR_ARG;
   if (params->clone_den == 0) return VELO_ERR_ARG;
-  const size_t need = velo_workspace_bytes(hits->n_events, hits->n_hits, out->cap_tracks, out->cap_track_hits);
+  const size_t need = velo_workspace_bytes_opts(hits->n_events, hits->n_hits, out->cap_tracks, out->cap_track_hits, opts);
   if (workspace_bytes < need) return VELO_ERR_WORKSPACE;
 
   velo::KernelArgs a{};
@@ -77,10 +88,15 @@ int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const ve
   a.event_track_offsets = out->event_track_offsets; a.track_hit_offsets = out->track_hit_offsets;
   a.track_hits = out->track_hits; a.states = out->states;
   a.cap_tracks = out->cap_tracks; a.cap_track_hits = out->cap_track_hits; a.summary = out->summary;
-  a.ws = velo::carve_workspace(workspace, hits->n_events, out->cap_tracks, out->cap_track_hits,
-                               velo::default_n_slabs());
-  const int err = velo::launch_reconstruct(a, (cudaStream_t)stream);
+  a.ws = velo::carve_workspace(workspace, hits->n_events, out->cap_tracks, out->cap_track_hits, n_slabs_for(opts));
+  const int err = velo::launch_reconstruct(a, (cudaStream_t)stream, opts ? (cudaEvent_t)opts->event_kernel_start : nullptr,
+                                           opts ? (cudaEvent_t)opts->event_kernel_stop : nullptr);
   return err == 0 ? VELO_OK : VELO_ERR_CUDA;
+}
+
+int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream) {
+  return velo_reconstruct_opts(g, hits, params, out, workspace, workspace_bytes, stream, nullptr);
 }
 
 }  // extern "C"

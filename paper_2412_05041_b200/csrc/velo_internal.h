@@ -58,6 +58,7 @@ struct Workspace {
 Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, uint32_t cap_track_hits,
                           uint32_t n_slabs);
 uint32_t default_n_slabs();
+uint32_t num_sms();  // SM count of the current device (148 on B200); 148 if no device is present
 
 struct KernelArgs {
   // input
@@ -77,6 +78,6 @@ struct KernelArgs {
 };
 
 // Enqueues the whole path for one batch on `stream`. Returns a cudaError_t as int.
-int launch_reconstruct(const KernelArgs& a, cudaStream_t stream);
+int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop);
 
 }  // namespace velo

@@ -396,7 +396,20 @@ __global__ void __launch_bounds__(256) velo_compact_kernel(const KernelArgs a) {
 }  // namespace
 
 // ---- host side -----------------------------------------------------------------------------------
-uint32_t default_n_slabs() { return 148u * 2u; }
+uint32_t num_sms() {
+  static const uint32_t n = [] {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+      cudaGetLastError();
+      return 148u;
+    }
+    return (uint32_t)sms;
+  }();
+  return n;
+}
+
+uint32_t default_n_slabs() { return num_sms() * 4u; }
 
 Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, uint32_t cap_track_hits,
                           uint32_t n_slabs) {
@@ -417,13 +430,15 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, ui
   return w;
 }
 
-int launch_reconstruct(const KernelArgs& a, cudaStream_t stream) {
+int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop) {
   cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);
   if (err != cudaSuccess) return (int)err;
+  if (ev_start) cudaEventRecord(ev_start, stream);
   if (a.n_events > 0) {
     const uint32_t grid = a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events;
     velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a);
   }
+  if (ev_stop) cudaEventRecord(ev_stop, stream);
   velo_offsets_kernel<<<1, 1024, 0, stream>>>(a);
   if (a.n_events > 0) {
     const uint32_t warps_per_cta = 256 / 32;

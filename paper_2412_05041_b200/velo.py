@@ -1,0 +1,257 @@
+"""Thin ctypes binding of libvelo (include/velo.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C-ABI; PyTorch supplies device
+memory and streams. There is no CPU fallback: if libvelo.so is missing or no CUDA device is
+present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_float, c_int, c_int32, c_size_t, c_uint32, c_void_p
+
+import numpy as np
+
+from . import build as _build
+
+VELO_OK, VELO_ERR_ARG, VELO_ERR_GEOMETRY, VELO_ERR_WORKSPACE = 0, -1, -2, -3
+VELO_ERR_CUDA, VELO_ERR_CAPACITY, VELO_ERR_INPUT = -4, -5, -6
+VELO_MAX_MODULES, VELO_MAX_EVENT_HITS, VELO_N_STATE = 32, 65535, 13
+STATE_NAMES = ("x", "y", "tx", "ty", "z", "cxx", "cxtx", "ctxtx", "cyy", "cyty", "ctyty", "chi2", "n_hits")
+ERROR_NAMES = {0: "VELO_OK", -1: "VELO_ERR_ARG", -2: "VELO_ERR_GEOMETRY", -3: "VELO_ERR_WORKSPACE",
+               -4: "VELO_ERR_CUDA", -5: "VELO_ERR_CAPACITY", -6: "VELO_ERR_INPUT"}
+
+# every symbol include/velo.h declares
+EXPORTS = ("velo_version", "velo_geometry_load", "velo_geometry_free", "velo_geometry_n_modules",
+           "velo_params_default", "velo_workspace_bytes", "velo_workspace_bytes_opts", "velo_reconstruct",
+           "velo_reconstruct_opts", "velo_scheduler_create",
+           "velo_scheduler_free", "velo_scheduler_run_host")
+
+
+class VeloError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        super().__init__(f"{where}: {ERROR_NAMES.get(code, code)}")
+        self.code = code
+
+
+class GeometryDesc(ctypes.Structure):
+    _fields_ = [("n_modules", c_uint32), ("module_z", POINTER(c_float)), ("r_in", c_float),
+                ("r_out", c_float), ("pitch", c_float), ("half_shift_x", c_float)]
+
+
+class Params(ctypes.Structure):
+    _fields_ = [("phi_window_seed", c_int32), ("phi_window_fwd", c_int32),
+                ("max_scatter_seed", c_float), ("max_scatter_fwd", c_float), ("max_scatter_weak", c_float),
+                ("max_skipped", c_uint32), ("sigma_hit", c_float), ("max_chi2_ndof", c_float),
+                ("clone_num", c_uint32), ("clone_den", c_uint32)]
+
+
+class Hits(ctypes.Structure):
+    _fields_ = [("x", c_void_p), ("y", c_void_p), ("z", c_void_p), ("module", c_void_p),
+                ("event_offsets", c_void_p), ("n_events", c_uint32), ("n_hits", c_uint32)]
+
+
+class Tracks(ctypes.Structure):
+    _fields_ = [("event_track_offsets", c_void_p), ("track_hit_offsets", c_void_p), ("track_hits", c_void_p),
+                ("states", c_void_p), ("cap_tracks", c_uint32), ("cap_track_hits", c_uint32),
+                ("summary", c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libvelo.so (built in-tree by paper_2412_05041_b200.build). Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(f"{path} is missing: run `python -m paper_2412_05041_b200.build` "
+                               "(there is no fallback path)")
+        L = ctypes.CDLL(path)
+        L.velo_version.restype = ctypes.c_char_p
+        L.velo_geometry_load.argtypes = [POINTER(GeometryDesc), POINTER(c_void_p)]
+        L.velo_geometry_load.restype = c_int
+        L.velo_geometry_free.argtypes = [c_void_p]
+        L.velo_geometry_free.restype = None
+        L.velo_geometry_n_modules.argtypes = [c_void_p]
+        L.velo_geometry_n_modules.restype = c_uint32
+        L.velo_params_default.argtypes = [c_void_p, POINTER(Params)]
+        L.velo_params_default.restype = None
+        L.velo_workspace_bytes.argtypes = [c_uint32, c_uint32, c_uint32, c_uint32]
+        L.velo_workspace_bytes.restype = c_size_t
+        L.velo_reconstruct.argtypes = [c_void_p, POINTER(Hits), POINTER(Params), POINTER(Tracks), c_void_p,
+                                       c_size_t, c_void_p]
+        L.velo_reconstruct.restype = c_int
+        L.velo_scheduler_create.argtypes = [c_void_p, c_uint32, c_uint32, c_uint32, POINTER(c_void_p)]
+        L.velo_scheduler_create.restype = c_int
+        L.velo_scheduler_free.argtypes = [c_void_p]
+        L.velo_scheduler_free.restype = None
+        L.velo_scheduler_run_host.argtypes = [c_void_p, POINTER(Params), POINTER(Hits), c_void_p, c_uint32,
+                                              POINTER(Tracks)]
+        L.velo_scheduler_run_host.restype = c_int
+        _lib = L
+    return _lib
+
+
+def velo_version() -> str:
+    return lib().velo_version().decode()
+
+
+class Geometry:
+    """Owns a velo_geometry_t handle."""
+
+    def __init__(self, module_z, r_in=5.1, r_out=42.0, pitch=0.055, half_shift_x=0.0):
+        z = np.ascontiguousarray(module_z, dtype=np.float32)
+        desc = GeometryDesc(n_modules=z.shape[0], module_z=z.ctypes.data_as(POINTER(c_float)),
+                            r_in=r_in, r_out=r_out, pitch=pitch, half_shift_x=half_shift_x)
+        h = c_void_p()
+        rc = lib().velo_geometry_load(byref(desc), byref(h))
+        if rc != VELO_OK:
+            raise VeloError(rc, "velo_geometry_load")
+        self.handle = h
+        self.n_modules = int(lib().velo_geometry_n_modules(h))
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h and _lib is not None:
+            _lib.velo_geometry_free(h)
+
+
+def velo_geometry_load(module_z, **kw) -> Geometry:
+    return Geometry(module_z, **kw)
+
+
+def velo_params_default(geometry: Geometry | None = None) -> Params:
+    p = Params()
+    lib().velo_params_default(geometry.handle if geometry is not None else None, byref(p))
+    return p
+
+
+def velo_workspace_bytes(n_events: int, n_hits: int, cap_tracks: int, cap_track_hits: int) -> int:
+    return int(lib().velo_workspace_bytes(n_events, n_hits, cap_tracks, cap_track_hits))
+
+
+# ---- device-side helpers (PyTorch = device memory and streams only) -----------------------------
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("libvelo needs a CUDA device (there is no CPU path)")
+    return torch
+
+
+def default_capacities(n_events: int, n_hits: int) -> tuple[int, int]:
+    """Practical output sizing of include/velo.h: cap_tracks = n_hits/4 + n_events,
+    cap_track_hits = 2*n_hits (+1 so that an empty batch still has non-zero capacities)."""
+    return n_hits // 4 + n_events + 1, 2 * n_hits + 1
+
+
+class DeviceHits:
+    """Hits of a batch resident in HBM: x, y, z (f32), module (u8), event_offsets (u32 stored in an
+    int32 tensor: torch has no unsigned 32-bit arithmetic, the bits are what the library reads)."""
+
+    def __init__(self, x, y, z, module, event_offsets, device="cuda"):
+        torch = _torch()
+        f = lambda a, dt: torch.as_tensor(np.ascontiguousarray(a, dtype=dt)).to(device, non_blocking=False)
+        self.x, self.y, self.z = f(x, np.float32), f(y, np.float32), f(z, np.float32)
+        self.module = f(module, np.uint8)
+        off = np.ascontiguousarray(event_offsets, dtype=np.uint32)
+        self.event_offsets = torch.as_tensor(off.view(np.int32)).to(device)
+        self.n_events = off.shape[0] - 1
+        self.n_hits = int(off[-1]) - int(off[0]) if off.shape[0] else 0
+        self.first_hit = int(off[0]) if off.shape[0] else 0
+
+    def slice_struct(self, e0: int = 0, e1: int | None = None, n_hits: int | None = None) -> Hits:
+        """velo_hits_t for events [e0, e1): same hit arrays, a slice of the offsets."""
+        e1 = self.n_events if e1 is None else e1
+        return Hits(x=self.x.data_ptr(), y=self.y.data_ptr(), z=self.z.data_ptr(), module=self.module.data_ptr(),
+                    event_offsets=self.event_offsets.data_ptr() + 4 * e0, n_events=e1 - e0,
+                    n_hits=self.n_hits if n_hits is None else n_hits)
+
+
+class DeviceTracks:
+    """Caller-allocated output buffers of one batch (velo_tracks_t) plus its workspace."""
+
+    def __init__(self, n_events: int, n_hits: int, cap_tracks: int | None = None, cap_track_hits: int | None = None,
+                 device="cuda"):
+        torch = _torch()
+        ct, ch = default_capacities(n_events, n_hits)
+        self.cap_tracks = int(cap_tracks if cap_tracks is not None else ct)
+        self.cap_track_hits = int(cap_track_hits if cap_track_hits is not None else ch)
+        self.n_events = n_events
+        i32 = dict(dtype=torch.int32, device=device)
+        self.event_track_offsets = torch.empty(n_events + 1, **i32)
+        self.track_hit_offsets = torch.empty(self.cap_tracks + 1, **i32)
+        self.track_hits = torch.empty(self.cap_track_hits, **i32)
+        self.states = torch.empty((VELO_N_STATE, self.cap_tracks), dtype=torch.float32, device=device)
+        self.summary = torch.zeros(4, **i32)
+        self.workspace_bytes = velo_workspace_bytes(n_events, n_hits, self.cap_tracks, self.cap_track_hits)
+        self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=device)
+        self.workspace_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+
+    def struct(self) -> Tracks:
+        return Tracks(event_track_offsets=self.event_track_offsets.data_ptr(),
+                      track_hit_offsets=self.track_hit_offsets.data_ptr(), track_hits=self.track_hits.data_ptr(),
+                      states=self.states.data_ptr(), cap_tracks=self.cap_tracks, cap_track_hits=self.cap_track_hits,
+                      summary=self.summary.data_ptr())
+
+    def to_host(self) -> dict:
+        """Synchronises and returns the result as numpy arrays (same keys as the test oracle's
+        result dict). Raises VeloError on a device-side status."""
+        s = self.summary.cpu().numpy().view(np.uint32)
+        nt, nh, status = int(s[0]), int(s[1]), int(np.int32(s[2]))
+        if status != VELO_OK:
+            raise VeloError(status, f"velo_reconstruct (device status; required tracks={nt}, track_hits={nh})")
+        u = lambda t: t.cpu().numpy().view(np.uint32)
+        return {"event_track_offsets": u(self.event_track_offsets), "track_hit_offsets": u(self.track_hit_offsets[:nt + 1]),
+                "track_hits": u(self.track_hits[:nh]), "states": self.states[:, :nt].cpu().numpy(),
+                "n_tracks": nt, "n_track_hits": nh, "status": status, "n_candidates": int(s[3])}
+
+
+def velo_reconstruct(geometry: Geometry, hits: Hits, params: Params, out: DeviceTracks, stream=None) -> None:
+    """Enqueues one batch on `stream` (a torch.cuda.Stream; default: the current stream)."""
+    torch = _torch()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    tr = out.struct()
+    rc = lib().velo_reconstruct(geometry.handle, byref(hits), byref(params), byref(tr), c_void_p(out.workspace_ptr),
+                                c_size_t(out.workspace_bytes), c_void_p(st.cuda_stream))
+    if rc != VELO_OK:
+        raise VeloError(rc, "velo_reconstruct")
+
+
+def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None = None, n_batches: int = 1,
+                cap_tracks: int | None = None, cap_track_hits: int | None = None, **geom_kw) -> dict:
+    """Convenience for tests and examples: upload host arrays, run n_batches streamed batches,
+    download, and stitch the batch results into one result dict (offsets made global)."""
+    torch = _torch()
+    g = Geometry(module_z, **geom_kw)
+    P = params if params is not None else velo_params_default(g)
+    dh = DeviceHits(x, y, z, module, event_offsets)
+    off = np.ascontiguousarray(event_offsets, dtype=np.uint32).astype(np.int64)
+    cuts = [dh.n_events * b // n_batches for b in range(n_batches + 1)]
+    streams = [torch.cuda.Stream() for _ in range(n_batches)]
+    outs = []
+    torch.cuda.synchronize()
+    for b in range(n_batches):
+        e0, e1 = cuts[b], cuts[b + 1]
+        nh = int(off[e1] - off[e0])
+        o = DeviceTracks(e1 - e0, nh, cap_tracks, cap_track_hits)
+        velo_reconstruct(g, dh.slice_struct(e0, e1, nh), P, o, streams[b])
+        outs.append(o)
+    torch.cuda.synchronize()
+    return stitch([o.to_host() for o in outs])
+
+
+def stitch(parts: list[dict]) -> dict:
+    """Concatenates per-batch results (batch-local offsets) into one result."""
+    eto, tho, th, st = [np.zeros(1, np.uint32)], [np.zeros(1, np.uint32)], [], []
+    nt = nh = nc = 0
+    for p in parts:
+        eto.append(p["event_track_offsets"][1:] + np.uint32(nt))
+        tho.append(p["track_hit_offsets"][1:] + np.uint32(nh))
+        th.append(p["track_hits"]); st.append(p["states"])
+        nt += p["n_tracks"]; nh += p["n_track_hits"]; nc += p["n_candidates"]
+    return {"event_track_offsets": np.concatenate(eto), "track_hit_offsets": np.concatenate(tho),
+            "track_hits": np.concatenate(th) if th else np.zeros(0, np.uint32),
+            "states": np.concatenate(st, axis=1) if st else np.zeros((VELO_N_STATE, 0), np.float32),
+            "n_tracks": nt, "n_track_hits": nh, "status": 0, "n_candidates": nc}

@@ -1,0 +1,216 @@
+"""GPU-vs-oracle parity (BASELINE.json:north_star): the CUDA path,
+called through the C-ABI, against the CPU oracle on the same seeded inputs. Hit lists, offsets and
+n_hits bit-exact after canonical ordering; states within 1e-5 relative (in fact bit-identical,
+because the kernels follow O-11 operator by operator without FMA contraction)."""
+import numpy as np
+import pytest
+
+from paper_2412_05041_b200 import datagen
+from tests import velo_testlib as T
+
+pytestmark = pytest.mark.gpu
+
+M = 26
+
+
+@pytest.fixture(scope="module")
+def velo():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2412_05041_b200 import build as vbuild
+    from paper_2412_05041_b200 import velo as v
+    vbuild.build()
+    v.lib()  # fails loudly if the extension is missing
+    return v
+
+
+def gpu(velo, d, **kw):
+    return velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], datagen.MODULE_Z, **kw)
+
+
+def cpu(d, params=None, workers=None):
+    return T.oracle_parallel(d, M, params, workers)
+
+
+def check(got, want):
+    info = T.assert_same_result(got, want)
+    assert got["n_tracks"] == want["n_tracks"] and got["n_track_hits"] == want["n_track_hits"]
+    return info
+
+
+# ---- BASELINE.json:configs[0]: everything, element by element -----------------------------------
+def test_config0_full(velo):
+    d = datagen.generate_config(0)
+    got, want = gpu(velo, d), cpu(d)
+    info = check(got, want)
+    assert info["bit_identical_states"]
+    assert got["n_candidates"] == want["n_candidates"]
+    assert want["n_tracks"] > 15000          # 100 events x ~190 tracks: the comparison is not vacuous
+
+
+def test_config0_emits_oracle_order(velo):
+    """Tracks come out in creation order (include/velo.h), which is also the oracle's order."""
+    d = datagen.generate_config(0, n_events=20)
+    got, want = gpu(velo, d), cpu(d, workers=1)
+    np.testing.assert_array_equal(got["track_hit_offsets"], want["track_hit_offsets"])
+    np.testing.assert_array_equal(got["track_hits"], want["track_hits"])
+    np.testing.assert_array_equal(got["states"].view(np.uint32), want["states"].view(np.uint32))
+
+
+def test_streamed_batches_equal_single_batch(velo):
+    d = datagen.generate_config(1, n_events=403)     # ragged: 403 events in 4 batches
+    a, b = gpu(velo, d), gpu(velo, d, n_batches=4)
+    for k in ("event_track_offsets", "track_hit_offsets", "track_hits"):
+        np.testing.assert_array_equal(a[k], b[k])
+    np.testing.assert_array_equal(a["states"].view(np.uint32), b["states"].view(np.uint32))
+    check(b, cpu(d))
+
+
+def test_run_to_run_determinism(velo):
+    d = datagen.generate_config(0, n_events=60)
+    ref = gpu(velo, d)
+    for _ in range(5):
+        r = gpu(velo, d)
+        for k in ("event_track_offsets", "track_hit_offsets", "track_hits"):
+            np.testing.assert_array_equal(ref[k], r[k])
+        np.testing.assert_array_equal(ref["states"].view(np.uint32), r["states"].view(np.uint32))
+
+
+# ---- the other workloads ------------------------------------------------------------------------
+def test_config1_10k_events(velo):
+    d = datagen.generate_config(1)
+    got = gpu(velo, d)
+    want = cpu(d)
+    check(got, want)
+
+
+def test_config3_open_velo(velo):
+    d = datagen.generate_config(3, n_events=20000)
+    check(gpu(velo, d, n_batches=4), cpu(d))
+
+
+def test_config4_ion_like(velo):
+    d = datagen.generate_config(4, n_events=160)
+    nh = np.diff(d["event_offsets"].astype(np.int64))
+    assert nh.max() > 20000                  # the large-event path is exercised
+    check(gpu(velo, d), cpu(d))
+
+
+# ---- hand-made and degenerate inputs (SURVEY.md §8(c) whole-path pins, A14, A15) -----------------
+def _run_events(velo, events, params=None):
+    x, y, z, m, off = T.batch_of(events)
+    d = {"x": x, "y": y, "z": z, "module": m, "event_offsets": off, "n_events": len(events)}
+    got = velo.reconstruct(x, y, z, m, off, datagen.MODULE_Z, params=params)
+    import oracle
+    want = oracle.reconstruct(x, y, z, m, off, M, None if params is None else _oracle_params(params))
+    return got, want, d
+
+
+def _oracle_params(p):
+    import oracle
+    q = oracle.Params()
+    for name, _ in q._fields_:
+        setattr(q, name, getattr(p, name))
+    return q
+
+
+def test_hand_events_and_empty_events(velo):
+    empty = (np.zeros(0, np.float32),) * 3 + (np.zeros(0, np.uint8),)
+    events = [
+        T.line_event([10, 11, 12, 13]),
+        empty,
+        T.line_event([10, 11, 12, 13, 14, 15]),
+        T.line_event([10, 11, 13, 14, 15]),                      # one miss bridged
+        T.line_event([13, 14, 15, 10]),                          # weak 3-hit track + lone hit
+        T.line_event([9, 10, 11, 14, 15, 16]),                   # two consecutive misses: two tracks
+        T.line_event([10, 12, 13]),                              # no three consecutive modules
+        T.line_event([10, 11, 12, 13], extra=[(7.6 + 0.07, 0.05, 11), (10.1 + 0.07, 0.05, 12)]),
+        empty,
+        T.line_event(list(range(26)), tx=0.02, ty=-0.03),        # crosses every module
+        T.line_event([3, 4, 5, 6], tx=0.05, ty=0.0),             # x < 0, y = 0: phi16 = -32768
+        tuple(np.concatenate(p) for p in zip(T.line_event([3, 4, 5, 6], tx=0.05, ty=2e-4),     # two tracks on
+                                             T.line_event([3, 4, 5, 6], tx=0.05, ty=-2e-4))),  # either side of the wrap
+    ]
+    got, want, d = _run_events(velo, events)
+    check(got, want)
+    assert [len(T.split_tracks(got, e)) for e in range(len(events))] == [1, 0, 1, 1, 1, 2, 0, 1, 0, 2, 1, 2]
+    assert T.track_modules(got, d["module"], 3) == [(15, 14, 13, 11, 10)]
+
+
+def test_zero_events_and_all_empty(velo):
+    z = np.zeros(0, np.float32)
+    r = velo.reconstruct(z, z, z, np.zeros(0, np.uint8), np.zeros(1, np.uint32), datagen.MODULE_Z)
+    assert r["n_tracks"] == 0 and r["event_track_offsets"].tolist() == [0]
+    r = velo.reconstruct(z, z, z, np.zeros(0, np.uint8), np.zeros(6, np.uint32), datagen.MODULE_Z)
+    assert r["n_tracks"] == 0 and r["event_track_offsets"].tolist() == [0] * 6
+
+
+def test_duplicate_hits_and_ties(velo):
+    """A14: identical coordinates are legal; ties resolve by index on both sides alike."""
+    e = T.line_event([10, 11, 12, 13, 14])
+    dup = tuple(np.concatenate([a, a]) for a in e)
+    got, want, _ = _run_events(velo, [dup, e, dup])
+    check(got, want)
+
+
+def test_parameter_variants(velo):
+    d = datagen.generate_config(0, n_events=30)
+    g = velo.velo_geometry_load(datagen.MODULE_Z)
+    for change in ({"phi_window_seed": 40000, "phi_window_fwd": 40000},      # whole-module windows
+                   {"phi_window_seed": 0, "phi_window_fwd": 5},
+                   {"max_skipped": 0}, {"max_skipped": 3},
+                   {"clone_num": 0, "clone_den": 1}, {"clone_num": 1, "clone_den": 1},
+                   {"max_chi2_ndof": 2.0}, {"max_scatter_seed": 0.5, "max_scatter_fwd": 0.02, "max_scatter_weak": 0.5}):
+        p = velo.velo_params_default(g)
+        for k, v in change.items():
+            setattr(p, k, v)
+        got = velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], datagen.MODULE_Z, params=p)
+        check(got, cpu(d, _oracle_params(p), workers=4))
+
+
+def test_status_codes(velo):
+    d = datagen.generate_config(0, n_events=10)
+    # capacity overflow: required sizes are reported, nothing is silently truncated
+    full = gpu(velo, d)
+    with pytest.raises(velo.VeloError) as e:
+        gpu(velo, d, cap_tracks=full["n_tracks"] - 1)
+    assert e.value.code == velo.VELO_ERR_CAPACITY and f"tracks={full['n_tracks']}" in str(e.value)
+    with pytest.raises(velo.VeloError) as e:
+        gpu(velo, d, cap_track_hits=full["n_track_hits"] - 1)
+    assert e.value.code == velo.VELO_ERR_CAPACITY
+    exact = gpu(velo, d, cap_tracks=full["n_tracks"], cap_track_hits=full["n_track_hits"])
+    np.testing.assert_array_equal(exact["track_hits"], full["track_hits"])
+    # bad module id
+    bad = dict(d); bad["module"] = d["module"].copy(); bad["module"][5] = 26
+    with pytest.raises(velo.VeloError) as e:
+        gpu(velo, bad)
+    assert e.value.code == velo.VELO_ERR_INPUT
+    # non-monotone offsets
+    bad = dict(d); bad["event_offsets"] = d["event_offsets"].copy(); bad["event_offsets"][3] = bad["event_offsets"][5] + 7
+    with pytest.raises(velo.VeloError) as e:
+        gpu(velo, bad)
+    assert e.value.code == velo.VELO_ERR_INPUT
+
+
+# ---- full size, in the launch configuration bench.py times: sampled events -----------------------
+@pytest.mark.parametrize("config", [2, 3])
+def test_full_size_sampled_events(velo, config):
+    d = datagen.generate_config(config)
+    got = gpu(velo, d, n_batches=4)
+    rng = np.random.default_rng(7)
+    nh = np.diff(d["event_offsets"].astype(np.int64))
+    ids = np.unique(np.concatenate([rng.integers(0, d["n_events"], 400), np.argsort(nh)[-8:], np.argsort(nh)[:8],
+                                    [0, 24999, 25000, 49999, 50000, 99999]]))
+    sub = T.gather_events(d, ids)
+    check(T.select_events(got, d, ids), cpu(sub))
+    # properties that hold at any size
+    eto = got["event_track_offsets"].astype(np.int64); tho = got["track_hit_offsets"].astype(np.int64)
+    assert (np.diff(eto) >= 0).all() and (np.diff(tho) >= 3).all() and tho[-1] == got["n_track_hits"]
+    ev_of_track = np.repeat(np.arange(d["n_events"]), np.diff(eto))
+    ev_of_hit = np.repeat(ev_of_track, np.diff(tho))
+    off = d["event_offsets"].astype(np.int64)
+    th = got["track_hits"].astype(np.int64)
+    assert ((th >= off[ev_of_hit]) & (th < off[ev_of_hit + 1])).all()        # hits belong to their event
+    mod = d["module"][th].astype(np.int64)
+    same_track = np.ones(th.shape[0] - 1, bool); same_track[tho[1:-1] - 1] = False
+    assert (np.diff(mod)[same_track] < 0).all()                              # decreasing module order

@@ -95,3 +95,80 @@ def batch_of(events):
 def track_modules(res, module, event=0):
     """Sorted tuple of module-id tuples of the event's tracks."""
     return sorted(tuple(int(module[h]) for h in hits) for hits, _ in split_tracks(res, event))
+
+
+def gather_events(d: dict, ids) -> dict:
+    """Sub-batch made of the selected events of a generated batch (inputs only)."""
+    off = d["event_offsets"].astype(np.int64)
+    ids = np.asarray(ids, dtype=np.int64)
+    n = off[ids + 1] - off[ids]
+    new_off = np.zeros(ids.shape[0] + 1, np.int64)
+    np.cumsum(n, out=new_off[1:])
+    idx = np.repeat(off[ids] - new_off[:-1], n) + np.arange(int(new_off[-1]))
+    return {"x": d["x"][idx], "y": d["y"][idx], "z": d["z"][idx], "module": d["module"][idx],
+            "event_offsets": new_off.astype(np.uint32), "n_events": ids.shape[0], "n_hits": int(new_off[-1])}
+
+
+def select_events(res: dict, d: dict, ids) -> dict:
+    """The part of a full-batch result that belongs to the selected events, re-indexed as if the
+    sub-batch of gather_events(d, ids) had been reconstructed on its own."""
+    off = d["event_offsets"].astype(np.int64)
+    ids = np.asarray(ids, dtype=np.int64)
+    eto = np.asarray(res["event_track_offsets"]).astype(np.int64)
+    tho = np.asarray(res["track_hit_offsets"]).astype(np.int64)
+    th = np.asarray(res["track_hits"]).astype(np.int64)
+    new_hoff = np.concatenate([[0], np.cumsum(off[ids + 1] - off[ids])])
+    nt = eto[ids + 1] - eto[ids]
+    new_eto = np.concatenate([[0], np.cumsum(nt)])
+    tids = np.repeat(eto[ids] - new_eto[:-1], nt) + np.arange(int(new_eto[-1]))
+    shift = np.repeat(new_hoff[:-1] - off[ids], nt)          # per selected track: hit index shift
+    n = tho[tids + 1] - tho[tids]
+    new_tho = np.concatenate([[0], np.cumsum(n)])
+    hidx = np.repeat(tho[tids] - new_tho[:-1], n) + np.arange(int(new_tho[-1]))
+    hits = th[hidx] + np.repeat(shift, n)
+    return {"event_track_offsets": new_eto.astype(np.uint32), "track_hit_offsets": new_tho.astype(np.uint32),
+            "track_hits": hits.astype(np.uint32), "states": np.asarray(res["states"])[:, tids],
+            "n_tracks": int(new_eto[-1]), "n_track_hits": int(new_tho[-1])}
+
+
+def oracle_parallel(d: dict, n_modules: int, params=None, workers: int | None = None) -> dict:
+    """The oracle over a batch, forked over contiguous event ranges (events are independent), and
+    the per-range results stitched. Each worker is the single-threaded oracle as it stands."""
+    import multiprocessing as mp
+    import os
+    ne = int(d["n_events"])
+    workers = workers or min(os.cpu_count() or 1, 32)
+    workers = max(1, min(workers, ne // 8 or 1))
+    off = d["event_offsets"].astype(np.int64)
+    tot = int(off[-1] - off[0])
+    # cut so that every range holds about the same number of hits
+    cuts = [0] + [int(np.searchsorted(off - off[0], tot * k / workers)) for k in range(1, workers)] + [ne]
+    cuts = sorted(set(min(max(c, 0), ne) for c in cuts))
+    jobs = [(d, n_modules, params, cuts[i], cuts[i + 1]) for i in range(len(cuts) - 1)]
+    if len(jobs) == 1:
+        parts = [_oracle_range(jobs[0])]
+    else:
+        with mp.get_context("fork").Pool(len(jobs)) as pool:
+            parts = pool.map(_oracle_range, jobs)
+    eto, tho, th, st = [np.zeros(1, np.int64)], [np.zeros(1, np.int64)], [], []
+    nt = nh = nc = 0
+    for p in parts:
+        eto.append(p["event_track_offsets"][1:].astype(np.int64) + nt)
+        tho.append(p["track_hit_offsets"][1:].astype(np.int64) + nh)
+        th.append(p["track_hits"]); st.append(p["states"])
+        nt += p["n_tracks"]; nh += p["n_track_hits"]; nc += p["n_candidates"]
+    return {"event_track_offsets": np.concatenate(eto).astype(np.uint32),
+            "track_hit_offsets": np.concatenate(tho).astype(np.uint32),
+            "track_hits": np.concatenate(th), "states": np.concatenate(st, axis=1), "n_tracks": nt,
+            "n_track_hits": nh, "status": max((p["status"] for p in parts), key=abs), "n_candidates": nc}
+
+
+def _oracle_range(job):
+    import oracle
+    d, n_modules, params, e0, e1 = job
+    off = d["event_offsets"]
+    h0, h1 = int(off[e0]), int(off[e1])
+    r = oracle.reconstruct(d["x"][h0:h1], d["y"][h0:h1], d["z"][h0:h1], d["module"][h0:h1],
+                           (off[e0:e1 + 1].astype(np.int64) - h0).astype(np.uint32), n_modules, params)
+    r["track_hits"] = r["track_hits"] + np.uint32(h0)
+    return r
