@@ -57,6 +57,11 @@ class Tracks(ctypes.Structure):
                 ("summary", c_void_p)]
 
 
+class LaunchOptions(ctypes.Structure):
+    _fields_ = [("event_kernel_start", c_void_p), ("event_kernel_stop", c_void_p), ("ctas_per_sm", c_uint32),
+                ("reserved", c_uint32)]
+
+
 _lib = None
 
 
@@ -83,6 +88,11 @@ def lib():
         L.velo_reconstruct.argtypes = [c_void_p, POINTER(Hits), POINTER(Params), POINTER(Tracks), c_void_p,
                                        c_size_t, c_void_p]
         L.velo_reconstruct.restype = c_int
+        L.velo_workspace_bytes_opts.argtypes = [c_uint32, c_uint32, c_uint32, c_uint32, POINTER(LaunchOptions)]
+        L.velo_workspace_bytes_opts.restype = c_size_t
+        L.velo_reconstruct_opts.argtypes = [c_void_p, POINTER(Hits), POINTER(Params), POINTER(Tracks), c_void_p,
+                                            c_size_t, c_void_p, POINTER(LaunchOptions)]
+        L.velo_reconstruct_opts.restype = c_int
         L.velo_scheduler_create.argtypes = [c_void_p, c_uint32, c_uint32, c_uint32, POINTER(c_void_p)]
         L.velo_scheduler_create.restype = c_int
         L.velo_scheduler_free.argtypes = [c_void_p]
@@ -132,6 +142,12 @@ def velo_workspace_bytes(n_events: int, n_hits: int, cap_tracks: int, cap_track_
     return int(lib().velo_workspace_bytes(n_events, n_hits, cap_tracks, cap_track_hits))
 
 
+def velo_workspace_bytes_opts(n_events: int, n_hits: int, cap_tracks: int, cap_track_hits: int,
+                              opts: LaunchOptions | None) -> int:
+    return int(lib().velo_workspace_bytes_opts(n_events, n_hits, cap_tracks, cap_track_hits,
+                                               byref(opts) if opts is not None else None))
+
+
 # ---- device-side helpers (PyTorch = device memory and streams only) -----------------------------
 def _torch():
     import torch
@@ -173,7 +189,7 @@ class DeviceTracks:
     """Caller-allocated output buffers of one batch (velo_tracks_t) plus its workspace."""
 
     def __init__(self, n_events: int, n_hits: int, cap_tracks: int | None = None, cap_track_hits: int | None = None,
-                 device="cuda"):
+                 device="cuda", opts: LaunchOptions | None = None):
         torch = _torch()
         ct, ch = default_capacities(n_events, n_hits)
         self.cap_tracks = int(cap_tracks if cap_tracks is not None else ct)
@@ -185,7 +201,7 @@ class DeviceTracks:
         self.track_hits = torch.empty(self.cap_track_hits, **i32)
         self.states = torch.empty((VELO_N_STATE, self.cap_tracks), dtype=torch.float32, device=device)
         self.summary = torch.zeros(4, **i32)
-        self.workspace_bytes = velo_workspace_bytes(n_events, n_hits, self.cap_tracks, self.cap_track_hits)
+        self.workspace_bytes = velo_workspace_bytes_opts(n_events, n_hits, self.cap_tracks, self.cap_track_hits, opts)
         self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=device)
         self.workspace_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
 
@@ -208,15 +224,21 @@ class DeviceTracks:
                 "n_tracks": nt, "n_track_hits": nh, "status": status, "n_candidates": int(s[3])}
 
 
-def velo_reconstruct(geometry: Geometry, hits: Hits, params: Params, out: DeviceTracks, stream=None) -> None:
-    """Enqueues one batch on `stream` (a torch.cuda.Stream; default: the current stream)."""
+def velo_reconstruct(geometry: Geometry, hits: Hits, params: Params, out: DeviceTracks, stream=None,
+                     opts: LaunchOptions | None = None) -> None:
+    """Enqueues one batch on `stream` (a torch.cuda.Stream; default: the current stream). With
+    `opts` the call goes through velo_reconstruct_opts."""
     torch = _torch()
     st = stream if stream is not None else torch.cuda.current_stream()
     tr = out.struct()
-    rc = lib().velo_reconstruct(geometry.handle, byref(hits), byref(params), byref(tr), c_void_p(out.workspace_ptr),
-                                c_size_t(out.workspace_bytes), c_void_p(st.cuda_stream))
+    rc = lib().velo_reconstruct_opts(geometry.handle, byref(hits), byref(params), byref(tr),
+                                     c_void_p(out.workspace_ptr), c_size_t(out.workspace_bytes),
+                                     c_void_p(st.cuda_stream), byref(opts) if opts is not None else None)
     if rc != VELO_OK:
         raise VeloError(rc, "velo_reconstruct")
+
+
+velo_reconstruct_opts = velo_reconstruct
 
 
 def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None = None, n_batches: int = 1,
@@ -255,3 +277,70 @@ def stitch(parts: list[dict]) -> dict:
             "track_hits": np.concatenate(th) if th else np.zeros(0, np.uint32),
             "states": np.concatenate(st, axis=1) if st else np.zeros((VELO_N_STATE, 0), np.float32),
             "n_tracks": nt, "n_track_hits": nh, "status": 0, "n_candidates": nc}
+
+
+# ---- end-to-end path over host buffers: the event-batch scheduler -------------------------------
+class HostTracks:
+    """Host output buffers of one batch (pinned when torch can pin), velo_tracks_t with HOST pointers."""
+
+    def __init__(self, n_events: int, n_hits: int, pinned: bool = True):
+        import torch
+        self.cap_tracks, self.cap_track_hits = default_capacities(n_events, n_hits)
+        pin = pinned and torch.cuda.is_available()
+        mk = lambda n, dt: torch.empty(n, dtype=dt, pin_memory=pin)
+        self.event_track_offsets = mk(n_events + 1, torch.int32)
+        self.track_hit_offsets = mk(self.cap_tracks + 1, torch.int32)
+        self.track_hits = mk(self.cap_track_hits, torch.int32)
+        self.states = mk(VELO_N_STATE * self.cap_tracks, torch.float32).view(VELO_N_STATE, self.cap_tracks)
+        self.summary = torch.zeros(4, dtype=torch.int32)
+
+    def struct(self) -> Tracks:
+        return Tracks(event_track_offsets=self.event_track_offsets.data_ptr(),
+                      track_hit_offsets=self.track_hit_offsets.data_ptr(), track_hits=self.track_hits.data_ptr(),
+                      states=self.states.data_ptr(), cap_tracks=self.cap_tracks, cap_track_hits=self.cap_track_hits,
+                      summary=self.summary.data_ptr())
+
+    def result(self) -> dict:
+        s = self.summary.numpy().view(np.uint32)
+        nt, nh, status = int(s[0]), int(s[1]), int(np.int32(s[2]))
+        if status != VELO_OK:
+            raise VeloError(status, f"velo_scheduler_run_host (batch status; tracks={nt}, track_hits={nh})")
+        u = lambda t: t.numpy().view(np.uint32)
+        return {"event_track_offsets": u(self.event_track_offsets), "track_hit_offsets": u(self.track_hit_offsets)[:nt + 1],
+                "track_hits": u(self.track_hits)[:nh], "states": self.states.numpy()[:, :nt], "n_tracks": nt,
+                "n_track_hits": nh, "status": status, "n_candidates": int(s[3])}
+
+
+class Scheduler:
+    """velo_scheduler_t: n_streams streams with device buffers for batches of the given size."""
+
+    def __init__(self, geometry: Geometry, n_streams: int, max_batch_events: int, max_batch_hits: int):
+        _torch()
+        self.geometry = geometry
+        h = c_void_p()
+        rc = lib().velo_scheduler_create(geometry.handle, n_streams, max_batch_events, max_batch_hits, byref(h))
+        if rc != VELO_OK:
+            raise VeloError(rc, "velo_scheduler_create")
+        self.handle = h
+
+    def run_host(self, params: Params, x, y, z, module, event_offsets, batch_begin, outs: list) -> None:
+        """x, y, z, module, event_offsets: HOST numpy arrays or CPU torch tensors (pinned memory makes
+        the copies asynchronous); outs: one HostTracks per batch. Returns when all copies are done."""
+        ptr = lambda a: a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+        n_events = int(event_offsets.shape[0]) - 1
+        bb = np.ascontiguousarray(batch_begin, dtype=np.uint32)
+        first, last = int(event_offsets[0]), int(event_offsets[n_events])
+        hits = Hits(x=ptr(x), y=ptr(y), z=ptr(z), module=ptr(module), event_offsets=ptr(event_offsets),
+                    n_events=n_events, n_hits=(last - first) & 0xffffffff)
+        arr = (Tracks * len(outs))(*[o.struct() for o in outs])
+        rc = lib().velo_scheduler_run_host(self.handle, byref(params), byref(hits), c_void_p(bb.ctypes.data),
+                                           len(outs), arr)
+        if rc != VELO_OK:
+            raise VeloError(rc, "velo_scheduler_run_host")
+
+    def close(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h and _lib is not None:
+            _lib.velo_scheduler_free(h)
+
+    __del__ = close
