@@ -40,7 +40,9 @@ def parse_args():
     ap.add_argument("--impl", default="velo", choices=["velo", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json:configs index (default 2)")
     ap.add_argument("--events", type=int, default=None, help="override the number of events (debugging)")
-    ap.add_argument("--ctas-per-sm", type=int, default=0, help="launch option (0 = library default)")
+    ap.add_argument("--ctas-per-sm", type=int, default=0, help="slab-kernel launch option (0 = library default)")
+    ap.add_argument("--teams", type=int, default=0, help="teams per CTA of the team kernel (0 = library default)")
+    ap.add_argument("--path", type=int, default=0, help="0 = team kernel + slab for deferred events, 1 = slab only")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -201,7 +203,8 @@ def run_velo(args):
     g = velo.velo_geometry_load(datagen.MODULE_Z, half_shift_x=cfg.half_shift_x)
     P = velo.velo_params_default(g)
     dh = velo.DeviceHits(d["x"], d["y"], d["z"], d["module"], off)
-    opts0 = velo.LaunchOptions(ctas_per_sm=args.ctas_per_sm)
+    opts0 = velo.LaunchOptions(ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams)
+    launches_per_batch = 3 if args.path == 1 else 4   # [team kernel,] slab kernel, offsets, compaction
     streams = [torch.cuda.Stream() for _ in range(n_batches)]
     main = torch.cuda.current_stream()
     outs, hstructs = [], []
@@ -223,7 +226,7 @@ def run_velo(args):
             ks, ke = kev[i][b]
             ks.record(streams[b]); ke.record(streams[b])
             o = velo.LaunchOptions(event_kernel_start=ks.cuda_event, event_kernel_stop=ke.cuda_event,
-                                   ctas_per_sm=args.ctas_per_sm)
+                                   ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams)
             velo.velo_reconstruct(g, hstructs[b], P, outs[b], streams[b], o)
             joins[b].record(streams[b])
             main.wait_event(joins[b])
@@ -252,6 +255,7 @@ def run_velo(args):
     # -- results of the last step: sizes for the byte counts, status for validity --
     res = [o.to_host() for o in outs]          # raises on any device-side status
     n_tracks = sum(r["n_tracks"] for r in res); n_thits = sum(r["n_track_hits"] for r in res)
+    n_deferred = sum(r["n_deferred"] for r in res)
     alg_batch = [algorithmic_bytes(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]]),
                                    res[b]["n_tracks"], res[b]["n_track_hits"]) for b in range(n_batches)]
     kern_ms = [kev[i][b][0].elapsed_time(kev[i][b][1]) for i in range(args.warmup, n_steps_total)
@@ -269,16 +273,18 @@ def run_velo(args):
         "hits_per_s": world * n_hits / (ms_step * 1e-3),
         "config": {"workload": workload_name(args.config, n_events, n_batches), "events_per_gpu": n_events,
                    "hits_per_gpu": n_hits, "tracks": n_tracks, "track_hits": n_thits, "streams": n_batches,
+                   "events_deferred_to_slab_kernel": n_deferred,
+                   "event_kernels": "slab only" if args.path == 1 else "shared-memory teams + slab for deferred events",
                    "cache": "inputs larger than L2 (%.2f GB per step)" % (13 * n_hits / 1e9),
                    "parallelism": f"events sharded over {world} GPU(s), no collective"},
-        "roofline": {"bound": "hbm", "kernel": "velo_event_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": "velo_event_slab_kernel" if args.path == 1 else "velo_event_team_kernel (+ slab kernel for deferred events)", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": float(np.mean(alg_batch)), "kernel_ms_per_launch": avg_kern_ms,
                      "kernel_share_of_step": avg_kern_ms * n_batches / ms_step,
                      "step_achieved": step_gbs, "step_frac": step_gbs / peak,
                      "frac_of_nominal_8TBs": step_gbs / 8000.0},
         "clocks": clocks,
-        "gpu_launches": 3 * n_batches * args.steps,
+        "gpu_launches": launches_per_batch * n_batches * (args.steps + args.warmup),
     }
 
     # -- end to end through the host-buffer C-ABI call (velo_scheduler_run_host): pinned host
@@ -311,7 +317,7 @@ def run_velo(args):
         line["e2e"] = {"value": world * n_events / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s, "steps": e2e_steps,
                        "api": "velo_scheduler_run_host (pinned host buffers, %d streams)" % n_batches}
-        line["gpu_launches"] += 3 * n_batches * (e2e_steps + 1)
+        line["gpu_launches"] += 4 * n_batches * (e2e_steps + 1)
         sched.close()
 
     # -- the oracle on this box's host cores (rank 0, N=1 only): a baseline, not the target --

@@ -49,6 +49,7 @@ enum {
 #define VELO_MAX_MODULES 32
 #define VELO_MAX_EVENT_HITS 65535u /* event-local hit indices are 16-bit inside the kernels     */
 #define VELO_N_STATE 13            /* words per track state, see velo_tracks_t.states           */
+#define VELO_N_SUMMARY 8           /* words of velo_tracks_t.summary                            */
 
 /* ---- geometry (BASELINE.json:configs[0], configs[3]) ---------------- */
 typedef struct velo_geometry velo_geometry_t; /* opaque, host-resident, immutable after load    */
@@ -109,8 +110,10 @@ typedef struct {
                                  /* to the z axis; cxx, cxtx, ctxtx, cyy, cyty, ctyty; chi2; and  */
                                  /* n_hits stored as the bit pattern of a uint32                  */
   uint32_t cap_tracks, cap_track_hits;
-  uint32_t* summary;             /* u32[4]: n_tracks, n_track_hits, status (VELO_OK or a negative */
-                                 /* code as two's complement), n_candidates                       */
+  uint32_t* summary;             /* u32[VELO_N_SUMMARY]: n_tracks, n_track_hits, status (VELO_OK  */
+                                 /* or a negative code as two's complement), n_candidates (before */
+                                 /* the filters), n_deferred (events the team kernel handed to    */
+                                 /* the general slab kernel), then three reserved zeros           */
 } velo_tracks_t;
 /* If the batch needs more than cap_tracks tracks or cap_track_hits track-hits, summary[2] =
  * VELO_ERR_CAPACITY, summary[0..1] hold the REQUIRED sizes and the other output arrays are
@@ -133,14 +136,21 @@ int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const ve
 
 /* Same call with launch options, for measurement and tuning. opts may be NULL (= velo_reconstruct).
  * event_kernel_start/stop: cudaEvent_t handles (or NULL) recorded on `stream` immediately before
- * and after the event kernel (the kernel that carries S0 ... S6), so that a benchmark can time the
- * dominant kernel of a batch on the stream it runs on. ctas_per_sm: persistent CTAs per SM of the
- * event kernel, 0 = library default; the workspace must have been sized for the default or for
- * velo_workspace_bytes_opts with the same value. */
+ * and after the event kernels (the kernels that carry S0 ... S6), so that a benchmark can time the
+ * dominant part of a batch on the stream it runs on.
+ * path: VELO_PATH_DEFAULT = the shared-memory team kernel, with the general slab kernel for the
+ * events it defers (hits off their module plane, events too large for one SM's shared memory);
+ * VELO_PATH_SLAB_ONLY = the general slab kernel for every event. Both give identical results.
+ * teams_per_cta: teams of 128 threads per persistent CTA of the team kernel (4 ... 8), 0 = default.
+ * ctas_per_sm: persistent CTAs per SM of the slab kernel, 0 = library default; the workspace must
+ * have been sized for the default or for velo_workspace_bytes_opts with the same value. */
+enum { VELO_PATH_DEFAULT = 0, VELO_PATH_SLAB_ONLY = 1 };
 typedef struct {
   void* event_kernel_start;
   void* event_kernel_stop;
   uint32_t ctas_per_sm;
+  uint32_t path;
+  uint32_t teams_per_cta;
   uint32_t reserved;
 } velo_launch_options_t;
 size_t velo_workspace_bytes_opts(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks,

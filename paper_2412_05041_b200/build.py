@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libvelo.so")
-SOURCES = ["velo_api.cu", "velo_kernels.cu", "velo_scheduler.cu"]
+SOURCES = ["velo_api.cu", "velo_kernels.cu", "velo_event_smem.cu", "velo_scheduler.cu"]
 HEADERS = ["velo_device.cuh", "velo_internal.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-shared"]

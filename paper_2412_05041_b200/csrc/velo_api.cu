@@ -83,6 +83,7 @@ int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, con
   a.x = hits->x; a.y = hits->y; a.z = hits->z; a.module = hits->module;
   a.event_offsets = hits->event_offsets;
   a.n_events = hits->n_events; a.n_modules = g->n_modules;
+  for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
   a.P = *params;
   if (a.P.max_skipped > 200u) a.P.max_skipped = 200u;  // more misses than modules is all the same
   a.event_track_offsets = out->event_track_offsets; a.track_hit_offsets = out->track_hit_offsets;
@@ -90,7 +91,8 @@ int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, con
   a.cap_tracks = out->cap_tracks; a.cap_track_hits = out->cap_track_hits; a.summary = out->summary;
   a.ws = velo::carve_workspace(workspace, hits->n_events, out->cap_tracks, out->cap_track_hits, n_slabs_for(opts));
   const int err = velo::launch_reconstruct(a, (cudaStream_t)stream, opts ? (cudaEvent_t)opts->event_kernel_start : nullptr,
-                                           opts ? (cudaEvent_t)opts->event_kernel_stop : nullptr);
+                                           opts ? (cudaEvent_t)opts->event_kernel_stop : nullptr,
+                                           opts ? opts->path : 0u, opts ? opts->teams_per_cta : 0u);
   return err == 0 ? VELO_OK : VELO_ERR_CUDA;
 }
 

@@ -1,0 +1,726 @@
+// velo_event_smem.cu — the shared-memory event kernel of the VELO hot path (sm_100a).
+//
+// One persistent CTA per SM owns the SM's shared memory as a pool of 4 KB units. The CTA is cut
+// into teams of 128 threads; a team takes the next event from a global ticket, allocates from the
+// pool exactly what that event needs (events span 0 ... ~6 k hits at mu = 5, so a fixed slot per
+// event would waste more than half of the SM), and runs the whole per-event path there: S0 decode
+// (phi16), S1 phi sort, the module loop with S3 forwarding and S2 search-by-triplet seeding, S4
+// ghost filter, S5 fit, S6 clone filter, and the staging of its tracks for S7. Teams synchronise
+// with named barriers (bar.sync id, 128), never with the whole CTA, so ~5 independent events are
+// in flight per SM and hide each other's shared-memory and barrier latency.
+//
+// The team path keeps only 12 bytes per hit (x, y, one packed word) because it requires every hit
+// to lie on its module plane, z[i] == module_z[module[i]] bit for bit (true for the detector:
+// the geometry is what velo_geometry_load was given). Then z is a per-module constant and the
+// z-ratio of O-4 is computed once per track and step instead of once per candidate. Events that
+// break this, or that do not fit the pool, its 15-bit local indices or its candidate table, are
+// appended to ws.large_list and reconstructed by the general slab kernel (velo_kernels.cu).
+//
+// Step semantics: SURVEY.md §8(c) O-1 ... O-14 (restated in DESIGN.md §3). Every float operation
+// is a round-to-nearest intrinsic in the written order (no FMA contraction), so hit lists and
+// states are bit-identical to the oracle's.
+#include "velo_device.cuh"
+#include "velo_internal.h"
+
+namespace velo {
+
+namespace {
+
+constexpr int kTeamThreads = 128;
+constexpr int kTeamWarps = kTeamThreads / 32;
+constexpr uint32_t kUnitBytes = 4096;       // pool allocation unit
+constexpr uint32_t kPoolUnits = 54;         // 216 KB of pool + 8 KB of control = 224 KB per CTA
+constexpr uint32_t kCtlBytes = 2 * kUnitBytes;
+constexpr uint32_t kClChunk = 256;          // centre hits per seeding chunk (2 per thread)
+constexpr uint32_t kMaxTeams = 8;
+constexpr uint32_t kMaxTeamHits = 32767;    // local original index is stored in 15 bits
+constexpr uint32_t kMaxBinSlot = 2047;      // slot inside a phi bucket is stashed in 11 bits
+constexpr uint32_t kFlagBit = 0x8000u;      // O-5 flag[h] inside the packed hit word
+constexpr uint32_t kNoOwner = 0xffffu;
+constexpr int kRegTracks = 3;               // fitted states of the first 3 tracks per thread stay in registers
+
+// Per-team control block (fixed place in the CTA's control unit).
+struct TeamShared {
+  uint32_t wsum[2][kTeamWarps];   // team_scan scratch, parity-toggled
+  uint32_t wsum2[2][kTeamWarps];
+  uint32_t event, n, o0;          // the team's current event: index, hits, first hit
+  uint32_t pool_off;              // byte offset of its block inside the pool
+  uint32_t units, first_unit;
+  uint32_t defer;                 // != 0: the event goes to the slab path (or, bit 31, is bad input)
+  uint32_t tbase, hbase;          // temp-block bases from the global counters
+  uint32_t nt;                    // candidates so far (slot counter)
+  uint32_t nact[2];               // lengths of the two active-track lists
+  uint32_t ncl[2];                // length of cl[], double-buffered by chunk parity
+  uint32_t sstart[VELO_MAX_MODULES + 1];   // sstart[s] = candidates created before step s seeds
+  uint16_t cl[kClChunk];          // unflagged centre hits of the current chunk
+};
+
+struct Control {
+  unsigned long long bitmap;      // 1 = unit in use
+  uint32_t alloc_next, alloc_serving;   // FIFO ticket lock around the allocator: no starvation
+  float module_z[VELO_MAX_MODULES];
+  TeamShared team[kMaxTeams];
+};
+static_assert(sizeof(Control) <= kCtlBytes, "control block must fit its units");
+
+// Phase timing for tuning builds (-DVELO_PHASE_CLOCKS): the team leader adds the SM clocks spent
+// since the previous mark to ws.phase_clk[i]. Compiled out of the product library.
+#ifdef VELO_PHASE_CLOCKS
+#define VELO_PHASE(i)                                                                  \
+  do {                                                                                 \
+    if (tid == 0) {                                                                    \
+      const long long now_ = clock64();                                                \
+      atomicAdd(&a.ws.phase_clk[i], (unsigned long long)(now_ - ph_last));             \
+      ph_last = now_;                                                                  \
+    }                                                                                  \
+  } while (0)
+#else
+#define VELO_PHASE(i) do { } while (0)
+#endif
+
+__device__ __forceinline__ void team_sync(uint32_t team) {
+  asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(kTeamThreads) : "memory");
+}
+
+// Exclusive scan of one u32 per thread over the team (and of a second value in the same pass).
+// `parity` alternates the scratch buffer so that one barrier per call suffices.
+__device__ __forceinline__ uint32_t team_scan2(uint32_t v, uint32_t v2, TeamShared& ts, uint32_t team, uint32_t& parity,
+                                               uint32_t* total, uint32_t* prefix2, uint32_t* total2) {
+  const uint32_t lane = threadIdx.x & 31u, wid = (threadIdx.x & (kTeamThreads - 1)) >> 5;
+  uint32_t inc = v, inc2 = v2;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t o = __shfl_up_sync(0xffffffffu, inc, d), o2 = __shfl_up_sync(0xffffffffu, inc2, d);
+    if (lane >= (uint32_t)d) { inc += o; inc2 += o2; }
+  }
+  const uint32_t p = parity & 1u;
+  parity ^= 1u;
+  if (lane == 31) { ts.wsum[p][wid] = inc; ts.wsum2[p][wid] = inc2; }
+  team_sync(team);
+  uint32_t base = 0, base2 = 0, tot = 0, tot2 = 0;
+#pragma unroll
+  for (uint32_t k = 0; k < (uint32_t)kTeamWarps; ++k) {
+    const uint32_t s = ts.wsum[p][k], s2 = ts.wsum2[p][k];
+    if (k < wid) { base += s; base2 += s2; }
+    tot += s; tot2 += s2;
+  }
+  *total = tot; *total2 = tot2; *prefix2 = base2 + inc2 - v2;
+  return base + inc - v;
+}
+
+// Byte layout of one event's block in the pool.
+struct Layout {
+  uint32_t xy, w, bins, u;   // offsets: float2[n], u32[n], packed u16 bucket table, union region
+  uint32_t tcap;             // candidate-table capacity
+  uint32_t bytes;
+};
+__device__ __forceinline__ uint32_t align16(uint32_t v) { return (v + 15u) & ~15u; }
+__device__ __forceinline__ uint32_t track_bytes(uint32_t tcap, uint32_t M) { return tcap * (2u * M + 20u); }
+__device__ __forceinline__ Layout event_layout(uint32_t n, uint32_t M) {
+  Layout L;
+  uint32_t o = 0;
+  L.xy = o; o += align16(8u * n);
+  L.w = o; o += align16(4u * n);
+  L.bins = o; o += align16(2u * (M * kBinsPerModule + 2u));
+  L.u = o;
+  L.tcap = ((n >> 3) + 32u + 15u) & ~15u;   // candidates ~0.106/hit (max seen 0.157): n/8 + 32, else deferred
+  const uint32_t sortb = 8u * n, trkb = track_bytes(L.tcap, M);
+  o += align16(sortb > trkb ? sortb : trkb);
+  L.bytes = o;
+  return L;
+}
+
+// The arrays of one event, all in shared memory.
+struct Ev {
+  float2* xy;            // sorted hit coordinates
+  uint32_t* w;           // packed: (phi16 + 32768) << 16 | flag << 15 | original local index;
+                         // after the module loop the upper half becomes the O-13 owner (track id)
+  const uint16_t* bo;    // bucket offsets, bo[m * 64 + b], bo[M * 64] = n
+  // sort scratch (dead after S1), aliased by the candidate table
+  uint32_t *stash, *tmp;
+  // candidate table, column t of row-major arrays
+  uint16_t* th;          // th[k * tcap + t] = k-th hit (sorted index)
+  uint32_t* tmask;       // modules of the track's hits, bit m
+  uint32_t* tl;          // last two hits: older << 16 | latest         } reused as the
+  float* tseed;          // seed scatter                                  } 64-bit tkey[t]
+  uint16_t* tcentre;     // sorted index of the seed's centre hit
+  uint8_t *tn, *tmiss;   // hits on the track; consecutive misses; after the loop: pass state
+  uint16_t* act;         // two lists of tcap active-track ids; after the loop: order[] (creation order)
+  uint32_t tcap;
+};
+
+// ---- O-3 window of module m around unsigned phi `c`: at most two runs of sorted indices, in
+// ascending order, and a modular test ((pu - lo) & 0xffff) <= span for the hits inside them.
+struct Window { uint32_t b0, e0, b1, e1, lo, span; };
+__device__ __forceinline__ Window make_window(const uint16_t* bo_m, uint32_t c, int W) {
+  Window q;
+  q.b1 = q.e1 = 0;
+  if (W < 0) { q.b0 = q.e0 = 0; q.lo = 0; q.span = 0; return q; }
+  if (2 * (long long)W + 1 >= 65536) { q.b0 = bo_m[0]; q.e0 = bo_m[kBinsPerModule]; q.lo = 0; q.span = 0xffffu; return q; }
+  const uint32_t lo = (c - (uint32_t)W) & 0xffffu, hi = (c + (uint32_t)W) & 0xffffu;
+  q.lo = lo; q.span = 2u * (uint32_t)W;
+  if (lo <= hi) { q.b0 = bo_m[lo >> kBinShift]; q.e0 = bo_m[(hi >> kBinShift) + 1]; }
+  else if ((lo >> kBinShift) <= (hi >> kBinShift)) {  // wraps and the two runs would overlap: whole module
+    q.b0 = bo_m[0]; q.e0 = bo_m[kBinsPerModule];
+  } else {  // wraps: the low-phi run has the lower sorted indices and is visited first
+    q.b0 = bo_m[0]; q.e0 = bo_m[(hi >> kBinShift) + 1];
+    q.b1 = bo_m[lo >> kBinShift]; q.e1 = bo_m[kBinsPerModule];
+  }
+  return q;
+}
+__device__ __forceinline__ bool in_window(const Window& q, uint32_t wj) { return (((wj >> 16) - q.lo) & 0xffffu) <= q.span; }
+
+// ---- O-11 straight-line fit of candidate t with z taken from the module planes ---------------
+// s9 = x, y, tx, ty, z, cxx, cxtx, vt, chi2 (the 13 state words repeat cxx, cxtx, vt for y and add n).
+// Hits are visited in discovery order = decreasing module = the set bits of `mask` from the top.
+__device__ __forceinline__ void fit_track(const Ev& ev, const float* mz, uint32_t t, uint32_t n, uint32_t mask,
+                                          float sig2, float inv_s2, float* s9) {
+  float sz = 0.0f, sx = 0.0f, sy = 0.0f;
+  uint32_t mk = mask;
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
+    const float2 p = ev.xy[ev.th[i * ev.tcap + t]];
+    sz = __fadd_rn(sz, mz[m]); sx = __fadd_rn(sx, p.x); sy = __fadd_rn(sy, p.y);
+  }
+  const float nf = (float)n;
+  const float zb = __fdiv_rn(sz, nf), xb = __fdiv_rn(sx, nf), yb = __fdiv_rn(sy, nf);
+  float sdd = 0.0f, sdx = 0.0f, sdy = 0.0f;
+  mk = mask;
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
+    const float2 p = ev.xy[ev.th[i * ev.tcap + t]];
+    const float d = __fsub_rn(mz[m], zb);
+    sdd = __fadd_rn(sdd, __fmul_rn(d, d));
+    sdx = __fadd_rn(sdx, __fmul_rn(d, __fsub_rn(p.x, xb)));
+    sdy = __fadd_rn(sdy, __fmul_rn(d, __fsub_rn(p.y, yb)));
+  }
+  const float tx = __fdiv_rn(sdx, sdd), ty = __fdiv_rn(sdy, sdd);
+  float c = 0.0f;
+  mk = mask;
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
+    const float2 p = ev.xy[ev.th[i * ev.tcap + t]];
+    const float d = __fsub_rn(mz[m], zb);
+    const float rx = __fsub_rn(__fsub_rn(p.x, xb), __fmul_rn(tx, d));
+    const float ry = __fsub_rn(__fsub_rn(p.y, yb), __fmul_rn(ty, d));
+    c = __fadd_rn(c, __fmul_rn(rx, rx));
+    c = __fadd_rn(c, __fmul_rn(ry, ry));
+  }
+  const float s2 = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
+  float dzb;
+  if (s2 < 1e-12f) dzb = 0.0f;
+  else dzb = -__fdiv_rn(__fadd_rn(__fmul_rn(xb, tx), __fmul_rn(yb, ty)), s2);
+  const float vt = __fdiv_rn(sig2, sdd);
+  s9[0] = __fadd_rn(xb, __fmul_rn(tx, dzb));
+  s9[1] = __fadd_rn(yb, __fmul_rn(ty, dzb));
+  s9[2] = tx; s9[3] = ty;
+  s9[4] = __fadd_rn(zb, dzb);
+  s9[5] = __fadd_rn(__fdiv_rn(sig2, nf), __fmul_rn(__fmul_rn(dzb, dzb), vt));
+  s9[6] = __fmul_rn(dzb, vt);
+  s9[7] = vt;
+  s9[8] = __fmul_rn(c, inv_s2);
+}
+
+__device__ __forceinline__ void set_status(uint32_t* counters, int code) {
+  atomicCAS(&counters[kCtrStatus], 0u, (uint32_t)code);   // first error wins
+}
+
+__device__ __forceinline__ void defer_to_slab(const KernelArgs& a, uint32_t e) {
+  a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+}
+
+// ---- pool allocator (called by a team's leader thread only) ------------------------------------
+__device__ __forceinline__ uint32_t pool_alloc(Control& ctl, uint32_t units) {
+  const uint32_t my = atomicAdd(&ctl.alloc_next, 1u);
+  volatile uint32_t* serving = &ctl.alloc_serving;
+  while (*serving != my) __nanosleep(400);
+  volatile unsigned long long* bm = &ctl.bitmap;
+  const unsigned long long all = (1ull << kPoolUnits) - 1ull;
+  uint32_t first;
+  unsigned long long seen = ~0ull;
+  for (;;) {
+    const unsigned long long used = *bm;
+    if (used == seen) { __nanosleep(400); continue; }   // nothing was freed since the last failed try
+    unsigned long long r = ~used & all;          // bit p: unit p free
+    for (uint32_t i = 1; i < units && r; ++i) r &= (r >> 1);   // bit p: units p .. p+i free
+    if (r) {
+      first = (uint32_t)__ffsll((long long)r) - 1u;
+      const unsigned long long claim = ((units >= 64u ? ~0ull : ((1ull << units) - 1ull)) << first);
+      if (atomicCAS(&ctl.bitmap, used, used | claim) == used) break;
+    } else {
+      seen = used;
+    }
+  }
+  __threadfence_block();
+  *serving = my + 1u;
+  return first;
+}
+__device__ __forceinline__ void pool_free(Control& ctl, uint32_t first, uint32_t units) {
+  const unsigned long long claim = ((units >= 64u ? ~0ull : ((1ull << units) - 1ull)) << first);
+  atomicAnd(&ctl.bitmap, ~claim);
+}
+
+// Leader: take the next event and a pool block for it. ts.defer != 0 means "nothing to do here".
+__device__ void leader_fetch(const KernelArgs& a, Control& ctl, TeamShared& ts) {
+  const uint32_t e = atomicAdd(&a.ws.counters[kCtrTicket], 1u);
+  ts.event = e; ts.units = 0; ts.defer = 1; ts.n = 0;
+  if (e >= a.n_events) return;
+  const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
+  if (o1 < o0 || o1 - o0 > VELO_MAX_EVENT_HITS) {
+    set_status(a.ws.counters, VELO_ERR_INPUT); a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); return;
+  }
+  const uint32_t n = o1 - o0;
+  if (n == 0) { a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); return; }
+  if (n > kMaxTeamHits) { defer_to_slab(a, e); return; }
+  const Layout L = event_layout(n, a.n_modules);
+  const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;
+  if (units > kPoolUnits) { defer_to_slab(a, e); return; }
+  const uint32_t first = pool_alloc(ctl, units);
+  ts.n = n; ts.o0 = o0; ts.units = units; ts.first_unit = first; ts.pool_off = first * kUnitBytes; ts.defer = 0;
+}
+
+// ---- one event, by one team. Returns false if the event was deferred to the slab path ----------
+__device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, unsigned char* pool, uint32_t team,
+                           uint32_t tid, uint32_t& parity, long long& ph_last) {
+  (void)ph_last;
+  const uint32_t lane = tid & 31u, wid = tid >> 5;
+  const uint32_t M = a.n_modules, nbins = M * kBinsPerModule;
+  const velo_params_t& P = a.P;
+  const uint32_t e = ts.event, n = ts.n, o0 = ts.o0;
+  const float* mz = ctl.module_z;
+  const Layout L = event_layout(n, M);
+  unsigned char* blk = pool + ts.pool_off;
+  Ev ev;
+  ev.xy = (float2*)(blk + L.xy); ev.w = (uint32_t*)(blk + L.w);
+  uint32_t* binsw = (uint32_t*)(blk + L.bins);
+  uint16_t* bins16 = (uint16_t*)binsw;
+  ev.bo = bins16;
+  ev.stash = (uint32_t*)(blk + L.u); ev.tmp = ev.stash + n;
+  const uint32_t T = L.tcap;
+  ev.tcap = T;
+  {
+    unsigned char* q = blk + L.u;
+    ev.th = (uint16_t*)q; q += 2u * M * T;
+    ev.tmask = (uint32_t*)q; q += 4u * T;
+    ev.tl = (uint32_t*)q; q += 4u * T;
+    ev.tseed = (float*)q; q += 4u * T;
+    ev.tcentre = (uint16_t*)q; q += 2u * T;
+    ev.act = (uint16_t*)q; q += 4u * T;
+    ev.tn = q; q += T;
+    ev.tmiss = q;
+  }
+  unsigned long long* tkey = (unsigned long long*)ev.tl;   // 8 bytes per track over (tl, tseed), used after O-10
+  const float* gx = a.x + o0; const float* gy = a.y + o0; const float* gz = a.z + o0;
+  const uint8_t* gm = a.module + o0;
+
+  // ---- S0 decode: phi16, bucket histogram (O-1); the plane check of the team path ---------------
+  const uint32_t nwords = nbins / 2u;
+  for (uint32_t b = tid; b <= nwords; b += kTeamThreads) binsw[b] = 0;
+  team_sync(team);
+  {
+    uint32_t trouble = 0;
+    for (uint32_t i = tid; i < n; i += kTeamThreads) {
+      const uint32_t m = gm[i];
+      const float x = gx[i], y = gy[i], z = gz[i];
+      if (m >= M) { trouble |= 0x80000000u; continue; }
+      if (__float_as_uint(z) != __float_as_uint(mz[m])) trouble |= 1u;
+      const uint32_t pu = (uint32_t)(phi16(x, y) + 32768);
+      const uint32_t bin = m * kBinsPerModule + (pu >> kBinShift);
+      const uint32_t sh = (bin & 1u) * 16u;
+      const uint32_t slot = (atomicAdd(&binsw[bin >> 1], 1u << sh) >> sh) & 0xffffu;
+      if (slot > kMaxBinSlot) trouble |= 1u;
+      ev.stash[i] = (m << 27) | (pu << 11) | (slot & kMaxBinSlot);
+    }
+    if (trouble) atomicOr(&ts.defer, trouble);
+  }
+  team_sync(team);
+  VELO_PHASE(1);   // S0 decode
+  if (ts.defer) {
+    if (tid == 0) {
+      if (ts.defer & 0x80000000u) { set_status(a.ws.counters, VELO_ERR_INPUT); a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); }
+      else defer_to_slab(a, e);
+    }
+    return;
+  }
+  // exclusive scan of the packed histogram -> bucket offsets; bo[nbins] = n
+  {
+    const uint32_t per = (nwords + kTeamThreads - 1) / kTeamThreads;
+    const uint32_t w0 = min(tid * per, nwords), w1 = min(w0 + per, nwords);
+    uint32_t s = 0;
+    for (uint32_t k = w0; k < w1; ++k) { const uint32_t v = binsw[k]; s += (v & 0xffffu) + (v >> 16); }
+    uint32_t tot, p2, t2;
+    uint32_t run = team_scan2(s, 0u, ts, team, parity, &tot, &p2, &t2);
+    for (uint32_t k = w0; k < w1; ++k) {
+      const uint32_t v = binsw[k], c0 = v & 0xffffu, c1 = v >> 16;
+      binsw[k] = run | ((run + c0) << 16);
+      run += c0 + c1;
+    }
+    if (tid == 0) bins16[nbins] = (uint16_t)n;
+  }
+  team_sync(team);
+  VELO_PHASE(2);   // bucket scan
+  // ---- S1 phi sort (O-2): group by bucket, then rank inside the bucket by (phi16, index) --------
+  for (uint32_t i = tid; i < n; i += kTeamThreads) {
+    const uint32_t st = ev.stash[i], pu = (st >> 11) & 0xffffu;
+    const uint32_t bin = (st >> 27) * kBinsPerModule + (pu >> kBinShift);
+    ev.tmp[(uint32_t)bins16[bin] + (st & kMaxBinSlot)] = (pu << 16) | i;
+  }
+  team_sync(team);
+  for (uint32_t i = tid; i < n; i += kTeamThreads) {
+    const uint32_t st = ev.stash[i], pu = (st >> 11) & 0xffffu;
+    const uint32_t bin = (st >> 27) * kBinsPerModule + (pu >> kBinShift);
+    const uint32_t item = (pu << 16) | i;
+    const uint32_t lo = bins16[bin], hi = bins16[bin + 1];
+    uint32_t r = lo;
+    for (uint32_t j = lo; j < hi; ++j) r += (ev.tmp[j] < item) ? 1u : 0u;
+    ev.xy[r] = make_float2(gx[i], gy[i]);
+    ev.w[r] = item;
+  }
+  team_sync(team);   // the sort scratch is dead from here on: the candidate table takes its place
+  VELO_PHASE(3);   // S1 sort
+
+  // ---- O-6 module loop ---------------------------------------------------------------------------
+  // Dense work lists keep the lanes busy: act[] = the tracks still forwarding (order irrelevant:
+  // every decision of a phase reads only state from before the phase), cl[] = the unflagged
+  // centre hits of a chunk. Slots of new candidates come from an atomic counter, so the table
+  // order is arbitrary; the creation order is restored once, after the loop (sstart[], order[]).
+  if (tid == 0) { ts.nt = 0; ts.nact[0] = ts.nact[1] = 0; ts.ncl[0] = ts.ncl[1] = 0; ts.sstart[M - 1] = 0; }
+  uint32_t cur = 0, cpar = 0;
+  team_sync(team);
+  for (uint32_t s = M - 2; s >= 1; --s) {
+    const uint32_t u = s - 1, nxt = cur ^ 1u;
+    // (A) O-7 forwarding into module u of every track active at the start of the step
+    {
+      const uint32_t nact = ts.nact[cur];
+      const float z2 = mz[u];
+      const uint16_t* bo_u = ev.bo + u * kBinsPerModule;
+      const uint16_t* act = ev.act + cur * T;
+      uint16_t* act_next = ev.act + nxt * T;
+      for (uint32_t k0 = wid * 32u; k0 < nact; k0 += kTeamThreads) {
+        const uint32_t k = k0 + lane;
+        bool alive = false;
+        uint32_t t = 0;
+        if (k < nact) {
+          t = act[k];
+          const uint32_t l = ev.tl[t], ha = l >> 16, hb = l & 0xffffu;
+          const uint32_t mask = ev.tmask[t];
+          const uint32_t mb = __ffs(mask) - 1u, ma = __ffs(mask & (mask - 1u)) - 1u;
+          const float2 p1 = ev.xy[hb], p0 = ev.xy[ha];
+          const uint32_t c = ev.w[hb] >> 16;
+          const float z1 = mz[mb], z0 = mz[ma];
+          const float tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0));
+          const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
+          const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
+          const Window q = make_window(bo_u, c, P.phi_window_fwd);
+          bool found = false; uint32_t best = 0; float best_sc = 0.0f;
+          auto visit = [&](uint32_t j) {
+            if (!in_window(q, ev.w[j])) return;
+            const float2 p2 = ev.xy[j];
+            const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
+            const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+            if (sc <= P.max_scatter_fwd && (!found || sc < best_sc)) { found = true; best = j; best_sc = sc; }
+          };
+          for (uint32_t j = q.b0; j < q.e0; ++j) visit(j);
+          for (uint32_t j = q.b1; j < q.e1; ++j) visit(j);
+          if (found) {
+            const uint32_t nh = ev.tn[t];
+            ev.th[nh * T + t] = (uint16_t)best;
+            ev.tn[t] = (uint8_t)(nh + 1);
+            ev.tmiss[t] = 0;
+            ev.tl[t] = (hb << 16) | best;
+            ev.tmask[t] = mask | (1u << u);
+            // (B): forwarding never reads flags, so they can be set right away
+            if (nh + 1 == 4) { for (uint32_t i = 0; i < 3; ++i) ev.w[ev.th[i * T + t]] |= kFlagBit; }
+            if (nh + 1 >= 4) ev.w[best] |= kFlagBit;
+            alive = true;
+          } else {
+            const uint32_t miss = (uint32_t)ev.tmiss[t] + 1u;
+            ev.tmiss[t] = (uint8_t)miss;
+            alive = miss <= P.max_skipped;
+          }
+        }
+        const uint32_t ballot = __ballot_sync(0xffffffffu, alive);
+        if (ballot) {
+          uint32_t base = 0;
+          if (lane == 0) base = atomicAdd(&ts.nact[nxt], (uint32_t)__popc(ballot));
+          base = __shfl_sync(0xffffffffu, base, 0);
+          if (alive) act_next[base + __popc(ballot & ((1u << lane) - 1u))] = (uint16_t)t;
+        }
+      }
+    }
+    team_sync(team);
+    VELO_PHASE(4);   // (A) forwarding
+    if (tid == 0) { ts.nact[cur] = 0; ts.sstart[s] = ts.nt; }   // nact[cur] was read by everyone before the barrier
+    // (C) O-8 seeding with centre module s, in chunks of 2 x 128 centre hits
+    {
+      const uint32_t c_begin = ev.bo[s * kBinsPerModule], c_end = ev.bo[(s + 1) * kBinsPerModule];
+      const float z0 = mz[s + 1], z1 = mz[s], z2 = mz[u];
+      const float tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0));
+      const uint16_t* bo_0 = ev.bo + (s + 1) * kBinsPerModule;
+      const uint16_t* bo_2 = ev.bo + u * kBinsPerModule;
+      uint16_t* act_next = ev.act + nxt * T;
+      for (uint32_t c0 = c_begin; c0 < c_end; c0 += kClChunk) {
+        // (C1) the chunk's unflagged centre hits -> cl[] (flags are final for this step: (A) is done)
+#pragma unroll
+        for (uint32_t r = 0; r < kClChunk / kTeamThreads; ++r) {
+          const uint32_t h1 = c0 + r * kTeamThreads + tid;
+          const bool open = h1 < c_end && !(ev.w[h1] & kFlagBit);
+          const uint32_t ballot = __ballot_sync(0xffffffffu, open);
+          if (ballot) {
+            uint32_t base = 0;
+            if (lane == 0) base = atomicAdd(&ts.ncl[cpar], (uint32_t)__popc(ballot));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (open) ts.cl[base + __popc(ballot & ((1u << lane) - 1u))] = (uint16_t)h1;
+          }
+        }
+        team_sync(team);
+        VELO_PHASE(5);   // (C1) unflagged centre hits
+        const uint32_t ncl = ts.ncl[cpar];
+        if (tid == 0) ts.ncl[cpar ^ 1u] = 0;   // the other counter: last read before the barrier above
+        cpar ^= 1u;
+        // (C2) one thread per unflagged centre hit: best (h0, h2) under (scatter, h0, h2)
+        for (uint32_t k = tid; k < ncl; k += kTeamThreads) {
+          const uint32_t h1 = ts.cl[k];
+          const uint32_t w1 = ev.w[h1];
+          const float2 p1 = ev.xy[h1];
+          const Window q0 = make_window(bo_0, w1 >> 16, P.phi_window_seed);
+          const Window q2 = make_window(bo_2, w1 >> 16, P.phi_window_seed);
+          bool found = false; uint32_t b0 = 0, b2 = 0; float best_sc = 0.0f;
+          auto visit0 = [&](uint32_t h0) {
+            const uint32_t w0 = ev.w[h0];
+            if ((w0 & kFlagBit) || !in_window(q0, w0)) return;
+            const float2 p0 = ev.xy[h0];
+            const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
+            const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
+            auto visit2 = [&](uint32_t h2) {
+              const uint32_t w2 = ev.w[h2];
+              if ((w2 & kFlagBit) || !in_window(q2, w2)) return;
+              const float2 p2 = ev.xy[h2];
+              const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
+              const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+              // h0 ascending outside, h2 ascending inside: strict < keeps the lexicographic minimum
+              if (sc <= P.max_scatter_seed && (!found || sc < best_sc)) { found = true; b0 = h0; b2 = h2; best_sc = sc; }
+            };
+            for (uint32_t j = q2.b0; j < q2.e0; ++j) visit2(j);
+            for (uint32_t j = q2.b1; j < q2.e1; ++j) visit2(j);
+          };
+          for (uint32_t j = q0.b0; j < q0.e0; ++j) visit0(j);
+          for (uint32_t j = q0.b1; j < q0.e1; ++j) visit0(j);
+          if (found) {
+            const uint32_t slot = atomicAdd(&ts.nt, 1u);
+            if (slot < T) {
+              ev.th[slot] = (uint16_t)b0; ev.th[T + slot] = (uint16_t)h1; ev.th[2 * T + slot] = (uint16_t)b2;
+              ev.tn[slot] = 3; ev.tmiss[slot] = 0;
+              ev.tl[slot] = (h1 << 16) | b2;
+              ev.tmask[slot] = 7u << u;
+              ev.tseed[slot] = best_sc; ev.tcentre[slot] = (uint16_t)h1;
+              act_next[atomicAdd(&ts.nact[nxt], 1u)] = (uint16_t)slot;
+            }
+          }
+        }
+        team_sync(team);   // cl[] may be refilled; after the last chunk: the new tracks are visible
+        VELO_PHASE(6);   // (C2) seeding
+      }
+      if (c_begin >= c_end) team_sync(team);   // no chunk ran: still order this step's resets before the next step
+    }
+    if (ts.nt > T) {   // candidate table too small for this event: the general path takes it
+      if (tid == 0) defer_to_slab(a, e);
+      return;
+    }
+    cur = nxt;
+  }
+  const uint32_t nt = ts.nt;
+  // creation order (O-8: step descending, then sorted index of the centre hit) of the table entries
+  uint16_t* order = ev.act;   // the work lists are dead
+  if (tid == 0) ts.sstart[0] = nt;
+  team_sync(team);
+  for (uint32_t t = tid; t < nt; t += kTeamThreads) {
+    const uint32_t sc = 30u - __clz(ev.tmask[t]);            // centre module = step of creation
+    const uint32_t a0 = ts.sstart[sc], a1 = ts.sstart[sc - 1];
+    const uint32_t centre = ev.tcentre[t];
+    uint32_t r = a0;
+    for (uint32_t j = a0; j < a1; ++j) r += (ev.tcentre[j] < centre) ? 1u : 0u;
+    order[r] = (uint16_t)t;
+  }
+  // (visible to the scan below after the barriers of the phases in between)
+  VELO_PHASE(7);   // creation order
+
+  // ---- O-10 ghost filter part 1 (reads the final flags); tmiss[t] becomes the pass state ---------
+  for (uint32_t t = tid; t < nt; t += kTeamThreads) {
+    bool pass = true;
+    if (ev.tn[t] == 3) {
+      const uint32_t f = ev.w[ev.th[t]] | ev.w[ev.th[T + t]] | ev.w[ev.th[2 * T + t]];
+      if ((f & kFlagBit) || !(ev.tseed[t] <= P.max_scatter_weak)) pass = false;
+    }
+    ev.tmiss[t] = pass ? 1 : 0;
+  }
+  team_sync(team);
+  // ---- O-11 fit, O-12 chi2 cut, O-13 key; the packed words' upper halves become "no owner" -------
+  for (uint32_t i = tid; i < n; i += kTeamThreads) ev.w[i] |= 0xffff0000u;
+  const float sig2 = __fmul_rn(P.sigma_hit, P.sigma_hit);
+  const float inv_s2 = __fdiv_rn(1.0f, sig2);
+  float sreg[kRegTracks][9];
+  auto fit_and_key = [&](uint32_t t, float* s9) {
+    const uint32_t nh = ev.tn[t];
+    const uint32_t centre = ev.tcentre[t];
+    fit_track(ev, mz, t, nh, ev.tmask[t], sig2, inv_s2, s9);
+    const float lim = __fmul_rn(P.max_chi2_ndof, (float)(2 * (int)nh - 4));
+    if (s9[8] > lim) { ev.tmiss[t] = 0; return; }
+    tkey[t] = ((unsigned long long)(255u - nh) << 56) | ((unsigned long long)__float_as_uint(s9[8]) << 24) |
+              (unsigned long long)centre;
+  };
+  // tkey[t] overlays tl/tseed of tracks 2t, 2t+1: every thread must have read its seeds (above) first
+#pragma unroll
+  for (int k = 0; k < kRegTracks; ++k) {
+    const uint32_t t = tid + (uint32_t)k * kTeamThreads;
+    if (t < nt && ev.tmiss[t]) fit_and_key(t, sreg[k]);
+  }
+  for (uint32_t t = tid + kRegTracks * kTeamThreads; t < nt; t += kTeamThreads) {
+    float s9[9];
+    if (ev.tmiss[t]) fit_and_key(t, s9);
+  }
+  team_sync(team);
+  VELO_PHASE(8);   // O-10, fit, keys
+  // ---- O-13 owners: owner[h] = the candidate with the smallest key among those that contain h ----
+  for (uint32_t t = tid; t < nt; t += kTeamThreads) {
+    if (!ev.tmiss[t]) continue;
+    const uint32_t nh = ev.tn[t];
+    const unsigned long long key = tkey[t];
+    for (uint32_t i = 0; i < nh; ++i) {
+      uint32_t* wp = &ev.w[ev.th[i * T + t]];
+      uint32_t old = *(volatile uint32_t*)wp;
+      for (;;) {
+        const uint32_t cur = old >> 16;
+        if (cur != kNoOwner && tkey[cur] < key) break;
+        const uint32_t seen = atomicCAS(wp, old, (t << 16) | (old & 0xffffu));
+        if (seen == old) break;
+        old = seen;
+      }
+    }
+  }
+  team_sync(team);
+  VELO_PHASE(9);   // owners
+  // ---- O-13 clone filter, then the event's survivors in creation order (exclusive scans) ---------
+  uint32_t* pl = ev.tl;                 // per-track output position inside the event: track index and
+  uint32_t* ph = (uint32_t*)ev.tseed;   // hit offset (tkey, which overlays both, is dead after the owners phase)
+  uint32_t run_t = 0, run_h = 0;
+  for (uint32_t k0 = 0; k0 < nt; k0 += kTeamThreads) {
+    const uint32_t k = k0 + tid;
+    const uint32_t t = k < nt ? order[k] : 0u;   // the k-th candidate in creation order
+    uint32_t nh = 0, surv = 0;
+    if (k < nt && ev.tmiss[t]) {
+      nh = ev.tn[t];
+      uint32_t lost = 0;
+      for (uint32_t i = 0; i < nh; ++i) lost += ((ev.w[ev.th[i * T + t]] >> 16) != t) ? 1u : 0u;
+      surv = !((unsigned long long)lost * P.clone_den > (unsigned long long)nh * P.clone_num) ? 1u : 0u;
+      if (!surv) nh = 0;
+    }
+    uint32_t tot_h, pre_t, tot_t;
+    const uint32_t pre_h = team_scan2(nh, surv, ts, team, parity, &tot_h, &pre_t, &tot_t);
+    if (k < nt) { ev.tmiss[t] = (uint8_t)(surv ? 2 : 0); pl[t] = run_t + pre_t; ph[t] = run_h + pre_h; }
+    run_t += tot_t; run_h += tot_h;
+  }
+  const uint32_t ev_nt = run_t, ev_nh = run_h;
+  VELO_PHASE(10);  // clone filter + scans
+  // ---- S7 part 1: allocate the event's temp block; stage the hit lists; coalesced copy out -------
+  if (tid == 0) {
+    ts.tbase = atomicAdd(&a.ws.counters[kCtrTracks], ev_nt);
+    ts.hbase = atomicAdd(&a.ws.counters[kCtrHits], ev_nh);
+    atomicAdd(&a.ws.counters[kCtrCand], nt);
+    a.ws.ev_rec[e] = make_uint4(ts.tbase, ts.hbase, ev_nt, ev_nh);
+  }
+  team_sync(team);
+  const uint32_t tbase = ts.tbase, hbase = ts.hbase;
+  const bool fits = (unsigned long long)tbase + ev_nt <= a.cap_tracks &&
+                    (unsigned long long)hbase + ev_nh <= a.cap_track_hits;
+  if (!fits) return;   // VELO_ERR_CAPACITY is raised by the offsets kernel; nothing valid to write
+  uint32_t* stage = (uint32_t*)ev.xy;          // coordinates are dead after the fit: 2n words
+  const bool staged = ev_nh <= 2u * n && nt <= (uint32_t)kRegTracks * kTeamThreads;   // a re-fit below still reads xy
+  auto emit = [&](uint32_t t, const float* s9) {
+    const uint32_t nh = ev.tn[t], lt = pl[t], lh = ph[t];
+    float* st = a.ws.tmp_states + tbase + lt;
+    const size_t cs = a.cap_tracks;
+    st[0] = s9[0]; st[cs] = s9[1]; st[2 * cs] = s9[2]; st[3 * cs] = s9[3]; st[4 * cs] = s9[4];
+    st[5 * cs] = s9[5]; st[6 * cs] = s9[6]; st[7 * cs] = s9[7];
+    st[8 * cs] = s9[5]; st[9 * cs] = s9[6]; st[10 * cs] = s9[7];
+    st[11 * cs] = s9[8]; st[12 * cs] = __uint_as_float(nh);
+    a.ws.tmp_loff[tbase + lt] = lh;
+    if (staged) { for (uint32_t i = 0; i < nh; ++i) stage[lh + i] = o0 + (ev.w[ev.th[i * T + t]] & 0x7fffu); }
+    else { for (uint32_t i = 0; i < nh; ++i) a.ws.tmp_hits[hbase + lh + i] = o0 + (ev.w[ev.th[i * T + t]] & 0x7fffu); }
+  };
+#pragma unroll
+  for (int k = 0; k < kRegTracks; ++k) {
+    const uint32_t t = tid + (uint32_t)k * kTeamThreads;
+    if (t < nt && ev.tmiss[t] == 2) emit(t, sreg[k]);
+  }
+  for (uint32_t t = tid + kRegTracks * kTeamThreads; t < nt; t += kTeamThreads) {
+    if (ev.tmiss[t] != 2) continue;
+    float s9[9];
+    fit_track(ev, mz, t, ev.tn[t], ev.tmask[t], sig2, inv_s2, s9);   // rare: > 384 candidates in one event
+    emit(t, s9);
+  }
+  if (staged) {
+    team_sync(team);
+    for (uint32_t j = tid; j < ev_nh; j += kTeamThreads) a.ws.tmp_hits[hbase + j] = stage[j];
+  }
+  VELO_PHASE(11);  // output
+}
+
+// ---- the kernel: one CTA per SM, kTeams teams, events by ticket ---------------------------------
+template <int kTeams>
+__global__ void __launch_bounds__(kTeams* kTeamThreads, 1) velo_event_team_kernel(const KernelArgs a) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  Control& ctl = *reinterpret_cast<Control*>(smem);
+  unsigned char* pool = smem + kCtlBytes;
+  const uint32_t team = threadIdx.x / kTeamThreads, tid = threadIdx.x % kTeamThreads;
+  if (threadIdx.x == 0) { ctl.bitmap = 0ull; ctl.alloc_next = 0; ctl.alloc_serving = 0; }
+  if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
+  __syncthreads();
+  TeamShared& ts = ctl.team[team];
+  uint32_t parity = 0;
+  long long ph_last = clock64();
+  (void)ph_last;
+  for (;;) {
+    if (tid == 0) leader_fetch(a, ctl, ts);
+    team_sync(team);
+    if (ts.event >= a.n_events) break;
+    VELO_PHASE(0);   // ticket + pool allocation (waiting for shared memory)
+    if (!ts.defer) team_event(a, ctl, ts, pool, team, tid, parity, ph_last);
+    team_sync(team);   // every thread is done with the block and with ts before the leader reuses them
+    if (tid == 0 && ts.units) pool_free(ctl, ts.first_unit, ts.units);
+    VELO_PHASE(12);  // last barrier + free
+  }
+}
+
+template <int kTeams>
+int launch_teams(const KernelArgs& a, cudaStream_t stream) {
+  static_assert(kTeams <= (int)kMaxTeams && kTeams <= 15, "named barriers 1..15");
+  const uint32_t smem = kCtlBytes + kPoolUnits * kUnitBytes;
+  static bool configured = false;   // per process; the attribute is sticky per function and device
+  if (!configured) {
+    cudaError_t err = cudaFuncSetAttribute(velo_event_team_kernel<kTeams>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return (int)err;
+    configured = true;
+  }
+  const uint32_t sms = num_sms();
+  const uint32_t want = (a.n_events + kTeams - 1) / kTeams;
+  const uint32_t grid = want < sms ? (want ? want : 1u) : sms;
+  velo_event_team_kernel<kTeams><<<grid, kTeams * kTeamThreads, smem, stream>>>(a);
+  return (int)cudaGetLastError();
+}
+
+}  // namespace
+
+int launch_event_smem(const KernelArgs& a, cudaStream_t stream, uint32_t teams) {
+  switch (teams) {
+    case 4: return launch_teams<4>(a, stream);
+    case 5: return launch_teams<5>(a, stream);
+    case 8: return launch_teams<8>(a, stream);
+    case 7: return launch_teams<7>(a, stream);
+    case 0:
+    case 6:
+    default: return launch_teams<6>(a, stream);
+  }
+}
+
+}  // namespace velo

@@ -41,10 +41,11 @@ __host__ __device__ inline SlabLayout slab_layout() {
 // counters: u32[16]: 0 tracks allocated, 1 track-hits allocated, 2 status, 3 candidates,
 //           4 event ticket, 5 large-event list length, 6 large-event ticket
 enum { kCtrTracks = 0, kCtrHits = 1, kCtrStatus = 2, kCtrCand = 3, kCtrTicket = 4, kCtrLargeN = 5,
-       kCtrLargeTicket = 6, kNumCounters = 16 };
+       kCtrLargeTicket = 6, kNumCounters = 16, kNumPhaseClocks = 16 };
 
 struct Workspace {
   uint32_t* counters;     // kNumCounters
+  unsigned long long* phase_clk;  // kNumPhaseClocks SM-clock accumulators (written only by -DVELO_PHASE_CLOCKS builds)
   uint4* ev_rec;          // n_events: {temp track base, temp hit base, n_tracks, n_track_hits}
   uint32_t* ev_hit_base;  // n_events+1: exclusive scan of n_track_hits over events
   uint32_t* large_list;   // n_events: events deferred to the slab path
@@ -66,6 +67,7 @@ struct KernelArgs {
   const uint8_t* module;
   const uint32_t* event_offsets;
   uint32_t n_events, n_modules;
+  float module_z[VELO_MAX_MODULES];  // geometry: the shared-memory path requires z[i] == module_z[module[i]]
   velo_params_t P;
   // output
   uint32_t* event_track_offsets;
@@ -77,7 +79,16 @@ struct KernelArgs {
   Workspace ws;
 };
 
+// Which event kernel(s) a batch runs through (velo_launch_options_t.path).
+enum { kPathDefault = 0,   // shared-memory team kernel, slab kernel for the events it defers
+       kPathSlabOnly = 1 };  // slab kernel for every event (the general path on its own)
+
 // Enqueues the whole path for one batch on `stream`. Returns a cudaError_t as int.
-int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop);
+int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop,
+                       uint32_t path, uint32_t teams);
+
+// velo_event_smem.cu: the shared-memory event kernel (persistent, one CTA per SM, `teams` teams of
+// 128 threads). Events it cannot hold are appended to ws.large_list. Returns a cudaError_t as int.
+int launch_event_smem(const KernelArgs& a, cudaStream_t stream, uint32_t teams);
 
 }  // namespace velo

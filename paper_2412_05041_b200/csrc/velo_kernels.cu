@@ -321,7 +321,8 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
 }
 
 // ---- event kernel, slab variant: persistent CTAs pull events from a ticket counter -------------
-__global__ void __launch_bounds__(kThreads) velo_event_slab_kernel(const KernelArgs a) {
+// from_list = 0: every event of the batch; 1: the events the shared-memory kernel deferred (ws.large_list).
+__global__ void __launch_bounds__(kThreads) velo_event_slab_kernel(const KernelArgs a, const int from_list) {
   __shared__ Shared sh;
   const SlabLayout L = slab_layout();
   unsigned char* slab = a.ws.slabs + (size_t)blockIdx.x * L.bytes;
@@ -334,13 +335,14 @@ __global__ void __launch_bounds__(kThreads) velo_event_slab_kernel(const KernelA
   ev.tcentre = (uint16_t*)(slab + L.tcentre); ev.tseed = (float*)(slab + L.tseed);
   ev.tkey = (unsigned long long*)(slab + L.tkey); ev.tpass = slab + L.tpass;
   ev.tcap = kSlabHits;
+  const uint32_t limit = from_list ? a.ws.counters[kCtrLargeN] : a.n_events;
   for (;;) {
-    if (threadIdx.x == 0) sh.ticket = atomicAdd(&a.ws.counters[kCtrTicket], 1u);
+    if (threadIdx.x == 0) sh.ticket = atomicAdd(&a.ws.counters[from_list ? kCtrLargeTicket : kCtrTicket], 1u);
     __syncthreads();
-    const uint32_t e = sh.ticket;
+    const uint32_t k = sh.ticket;
     __syncthreads();
-    if (e >= a.n_events) break;
-    process_event(a, ev, sh, e);
+    if (k >= limit) break;
+    process_event(a, ev, sh, from_list ? a.ws.large_list[k] : k);
   }
 }
 
@@ -370,6 +372,8 @@ __global__ void __launch_bounds__(1024) velo_offsets_kernel(const KernelArgs a) 
     if (!over) a.track_hit_offsets[n_tracks] = n_hits;
     a.summary[0] = n_tracks; a.summary[1] = n_hits; a.summary[2] = status;
     a.summary[3] = a.ws.counters[kCtrCand];
+    a.summary[4] = a.ws.counters[kCtrLargeN];
+    a.summary[5] = a.summary[6] = a.summary[7] = 0;
   }
 }
 
@@ -417,7 +421,8 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, ui
   size_t o = 0;
   unsigned char* b = (unsigned char*)base;
   auto take = [&](size_t bytes) { size_t r = o; o += ((bytes + 255) / 256) * 256; return b + r; };
-  w.counters = (uint32_t*)take(sizeof(uint32_t) * kNumCounters);
+  w.counters = (uint32_t*)take(sizeof(uint32_t) * kNumCounters);                 // offset 0
+  w.phase_clk = (unsigned long long*)take(sizeof(unsigned long long) * kNumPhaseClocks);   // offset 256
   w.ev_rec = (uint4*)take(sizeof(uint4) * ((size_t)n_events + 1));
   w.ev_hit_base = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.large_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
@@ -430,13 +435,20 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, ui
   return w;
 }
 
-int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop) {
-  cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);
+int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop,
+                       uint32_t path, uint32_t teams) {
+  cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);   // phase_clk accumulates
   if (err != cudaSuccess) return (int)err;
   if (ev_start) cudaEventRecord(ev_start, stream);
   if (a.n_events > 0) {
     const uint32_t grid = a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events;
-    velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a);
+    if (path == kPathSlabOnly) {
+      velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a, 0);
+    } else {
+      const int rc = launch_event_smem(a, stream, teams);
+      if (rc != 0) return rc;
+      velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a, 1);   // the deferred events, usually none
+    }
   }
   if (ev_stop) cudaEventRecord(ev_stop, stream);
   velo_offsets_kernel<<<1, 1024, 0, stream>>>(a);

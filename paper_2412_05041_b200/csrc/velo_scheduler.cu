@@ -20,7 +20,7 @@ struct Lane {                 // one stream with its device buffers
   velo_tracks_t out{};        // device output buffers
   void* workspace = nullptr;
   size_t workspace_bytes = 0;
-  uint32_t* summary_host = nullptr;  // pinned u32[4]
+  uint32_t* summary_host = nullptr;  // pinned u32[VELO_N_SUMMARY]
   // batch in flight
   bool busy = false;
   uint32_t batch = 0;
@@ -56,7 +56,8 @@ int finish_lane(Lane& l, velo_tracks_t* outs) {
   const uint32_t nt = l.summary_host[0], nh = l.summary_host[1];
   int status = (int)l.summary_host[2];
   if (status == VELO_OK && (nt > o.cap_tracks || nh > o.cap_track_hits)) status = VELO_ERR_CAPACITY;
-  o.summary[0] = nt; o.summary[1] = nh; o.summary[2] = (uint32_t)status; o.summary[3] = l.summary_host[3];
+  for (int k = 0; k < VELO_N_SUMMARY; ++k) o.summary[k] = l.summary_host[k];
+  o.summary[2] = (uint32_t)status;
   if (status == VELO_ERR_CAPACITY) return VELO_OK;  // reported per batch; nothing valid to copy
   bool good = true;
   if (nt) {
@@ -104,10 +105,10 @@ int velo_scheduler_create(const velo_geometry_t* g, uint32_t n_streams, uint32_t
     good &= ok(cudaMalloc(&l.out.track_hit_offsets, 4 * ((size_t)s->cap_tracks + 1)));
     good &= ok(cudaMalloc(&l.out.track_hits, 4 * (size_t)s->cap_track_hits));
     good &= ok(cudaMalloc(&l.out.states, 4 * (size_t)VELO_N_STATE * s->cap_tracks));
-    good &= ok(cudaMalloc(&l.out.summary, 16));
+    good &= ok(cudaMalloc(&l.out.summary, 4 * VELO_N_SUMMARY));
     l.workspace_bytes = velo_workspace_bytes(max_batch_events, max_batch_hits, s->cap_tracks, s->cap_track_hits);
     good &= ok(cudaMalloc(&l.workspace, l.workspace_bytes));
-    good &= ok(cudaMallocHost(&l.summary_host, 16));
+    good &= ok(cudaMallocHost(&l.summary_host, 4 * VELO_N_SUMMARY));
     if (!good) break;
   }
   if (!good) { cudaGetLastError(); velo_scheduler_free(s); return VELO_ERR_CUDA; }
@@ -132,7 +133,8 @@ int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, co
     const uint32_t ne = e1 - e0;
     const uint32_t h0 = hits->event_offsets[e0], h1 = hits->event_offsets[e1];
     if (h1 < h0 || ne > s->max_events || h1 - h0 > s->max_hits) {
-      o.summary[0] = o.summary[1] = o.summary[3] = 0; o.summary[2] = (uint32_t)VELO_ERR_CAPACITY;
+      for (int k = 0; k < VELO_N_SUMMARY; ++k) o.summary[k] = 0;
+      o.summary[2] = (uint32_t)VELO_ERR_CAPACITY;
       continue;
     }
     const uint32_t nh = h1 - h0;
@@ -153,7 +155,7 @@ int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, co
     dh.event_offsets = l.offsets; dh.n_events = ne; dh.n_hits = nh;
     rc = velo_reconstruct(s->g, &dh, params, &l.out, l.workspace, l.workspace_bytes, (void*)l.stream);
     if (rc != VELO_OK) break;
-    good &= ok(cudaMemcpyAsync(l.summary_host, l.out.summary, 16, cudaMemcpyDeviceToHost, l.stream));
+    good &= ok(cudaMemcpyAsync(l.summary_host, l.out.summary, 4 * VELO_N_SUMMARY, cudaMemcpyDeviceToHost, l.stream));
     good &= ok(cudaMemcpyAsync(o.event_track_offsets, l.out.event_track_offsets, 4 * ((size_t)ne + 1),
                                cudaMemcpyDeviceToHost, l.stream));
     if (!good) { rc = VELO_ERR_CUDA; break; }

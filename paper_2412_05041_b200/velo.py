@@ -17,6 +17,8 @@ from . import build as _build
 VELO_OK, VELO_ERR_ARG, VELO_ERR_GEOMETRY, VELO_ERR_WORKSPACE = 0, -1, -2, -3
 VELO_ERR_CUDA, VELO_ERR_CAPACITY, VELO_ERR_INPUT = -4, -5, -6
 VELO_MAX_MODULES, VELO_MAX_EVENT_HITS, VELO_N_STATE = 32, 65535, 13
+VELO_PATH_DEFAULT, VELO_PATH_SLAB_ONLY = 0, 1
+VELO_N_SUMMARY = 8
 STATE_NAMES = ("x", "y", "tx", "ty", "z", "cxx", "cxtx", "ctxtx", "cyy", "cyty", "ctyty", "chi2", "n_hits")
 ERROR_NAMES = {0: "VELO_OK", -1: "VELO_ERR_ARG", -2: "VELO_ERR_GEOMETRY", -3: "VELO_ERR_WORKSPACE",
                -4: "VELO_ERR_CUDA", -5: "VELO_ERR_CAPACITY", -6: "VELO_ERR_INPUT"}
@@ -59,7 +61,7 @@ class Tracks(ctypes.Structure):
 
 class LaunchOptions(ctypes.Structure):
     _fields_ = [("event_kernel_start", c_void_p), ("event_kernel_stop", c_void_p), ("ctas_per_sm", c_uint32),
-                ("reserved", c_uint32)]
+                ("path", c_uint32), ("teams_per_cta", c_uint32), ("reserved", c_uint32)]
 
 
 _lib = None
@@ -200,7 +202,7 @@ class DeviceTracks:
         self.track_hit_offsets = torch.empty(self.cap_tracks + 1, **i32)
         self.track_hits = torch.empty(self.cap_track_hits, **i32)
         self.states = torch.empty((VELO_N_STATE, self.cap_tracks), dtype=torch.float32, device=device)
-        self.summary = torch.zeros(4, **i32)
+        self.summary = torch.zeros(VELO_N_SUMMARY, **i32)
         self.workspace_bytes = velo_workspace_bytes_opts(n_events, n_hits, self.cap_tracks, self.cap_track_hits, opts)
         self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=device)
         self.workspace_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
@@ -221,7 +223,7 @@ class DeviceTracks:
         u = lambda t: t.cpu().numpy().view(np.uint32)
         return {"event_track_offsets": u(self.event_track_offsets), "track_hit_offsets": u(self.track_hit_offsets[:nt + 1]),
                 "track_hits": u(self.track_hits[:nh]), "states": self.states[:, :nt].cpu().numpy(),
-                "n_tracks": nt, "n_track_hits": nh, "status": status, "n_candidates": int(s[3])}
+                "n_tracks": nt, "n_track_hits": nh, "status": status, "n_candidates": int(s[3]), "n_deferred": int(s[4])}
 
 
 def velo_reconstruct(geometry: Geometry, hits: Hits, params: Params, out: DeviceTracks, stream=None,
@@ -242,7 +244,8 @@ velo_reconstruct_opts = velo_reconstruct
 
 
 def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None = None, n_batches: int = 1,
-                cap_tracks: int | None = None, cap_track_hits: int | None = None, **geom_kw) -> dict:
+                cap_tracks: int | None = None, cap_track_hits: int | None = None,
+                opts: LaunchOptions | None = None, **geom_kw) -> dict:
     """Convenience for tests and examples: upload host arrays, run n_batches streamed batches,
     download, and stitch the batch results into one result dict (offsets made global)."""
     torch = _torch()
@@ -257,8 +260,8 @@ def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None 
     for b in range(n_batches):
         e0, e1 = cuts[b], cuts[b + 1]
         nh = int(off[e1] - off[e0])
-        o = DeviceTracks(e1 - e0, nh, cap_tracks, cap_track_hits)
-        velo_reconstruct(g, dh.slice_struct(e0, e1, nh), P, o, streams[b])
+        o = DeviceTracks(e1 - e0, nh, cap_tracks, cap_track_hits, opts=opts)
+        velo_reconstruct(g, dh.slice_struct(e0, e1, nh), P, o, streams[b], opts)
         outs.append(o)
     torch.cuda.synchronize()
     return stitch([o.to_host() for o in outs])
@@ -267,8 +270,9 @@ def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None 
 def stitch(parts: list[dict]) -> dict:
     """Concatenates per-batch results (batch-local offsets) into one result."""
     eto, tho, th, st = [np.zeros(1, np.uint32)], [np.zeros(1, np.uint32)], [], []
-    nt = nh = nc = 0
+    nt = nh = nc = nd = 0
     for p in parts:
+        nd += p.get("n_deferred", 0)
         eto.append(p["event_track_offsets"][1:] + np.uint32(nt))
         tho.append(p["track_hit_offsets"][1:] + np.uint32(nh))
         th.append(p["track_hits"]); st.append(p["states"])
@@ -276,7 +280,7 @@ def stitch(parts: list[dict]) -> dict:
     return {"event_track_offsets": np.concatenate(eto), "track_hit_offsets": np.concatenate(tho),
             "track_hits": np.concatenate(th) if th else np.zeros(0, np.uint32),
             "states": np.concatenate(st, axis=1) if st else np.zeros((VELO_N_STATE, 0), np.float32),
-            "n_tracks": nt, "n_track_hits": nh, "status": 0, "n_candidates": nc}
+            "n_tracks": nt, "n_track_hits": nh, "status": 0, "n_candidates": nc, "n_deferred": nd}
 
 
 # ---- end-to-end path over host buffers: the event-batch scheduler -------------------------------
@@ -292,7 +296,7 @@ class HostTracks:
         self.track_hit_offsets = mk(self.cap_tracks + 1, torch.int32)
         self.track_hits = mk(self.cap_track_hits, torch.int32)
         self.states = mk(VELO_N_STATE * self.cap_tracks, torch.float32).view(VELO_N_STATE, self.cap_tracks)
-        self.summary = torch.zeros(4, dtype=torch.int32)
+        self.summary = torch.zeros(VELO_N_SUMMARY, dtype=torch.int32)
 
     def struct(self) -> Tracks:
         return Tracks(event_track_offsets=self.event_track_offsets.data_ptr(),
@@ -308,7 +312,7 @@ class HostTracks:
         u = lambda t: t.numpy().view(np.uint32)
         return {"event_track_offsets": u(self.event_track_offsets), "track_hit_offsets": u(self.track_hit_offsets)[:nt + 1],
                 "track_hits": u(self.track_hits)[:nh], "states": self.states.numpy()[:, :nt], "n_tracks": nt,
-                "n_track_hits": nh, "status": status, "n_candidates": int(s[3])}
+                "n_track_hits": nh, "status": status, "n_candidates": int(s[3]), "n_deferred": int(s[4])}
 
 
 class Scheduler:

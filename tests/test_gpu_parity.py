@@ -45,6 +45,7 @@ def test_config0_full(velo):
     info = check(got, want)
     assert info["bit_identical_states"]
     assert got["n_candidates"] == want["n_candidates"]
+    assert got["n_deferred"] == 0            # every event ran in the shared-memory team kernel
     assert want["n_tracks"] > 15000          # 100 events x ~190 tracks: the comparison is not vacuous
 
 
@@ -76,6 +77,56 @@ def test_run_to_run_determinism(velo):
         np.testing.assert_array_equal(ref["states"].view(np.uint32), r["states"].view(np.uint32))
 
 
+# ---- the two event kernels: shared-memory teams (default) and the general slab kernel -----------
+def test_team_and_slab_paths_agree(velo):
+    d = datagen.generate_config(0)
+    want = cpu(d)
+    for kw in ({"path": velo.VELO_PATH_SLAB_ONLY}, {"teams_per_cta": 4}, {"teams_per_cta": 5}, {"teams_per_cta": 7},
+               {"teams_per_cta": 8}):
+        got = gpu(velo, d, opts=velo.LaunchOptions(**kw))
+        info = check(got, want)
+        assert info["bit_identical_states"], kw
+        np.testing.assert_array_equal(got["track_hits"], want["track_hits"])    # emitted in the oracle's order
+
+
+def test_hits_off_their_module_plane_are_deferred_to_the_general_kernel(velo):
+    """The team kernel requires z == module_z[module]; events that break it take the slab kernel
+    inside the same call, and the batch result is still the oracle's."""
+    d = datagen.generate_config(0, n_events=40)
+    z = d["z"].copy()
+    off = d["event_offsets"].astype(np.int64)
+    rng = np.random.default_rng(3)
+    for e in (0, 3, 4, 17, 39):
+        idx = rng.integers(off[e], off[e + 1], 25)
+        z[idx] += rng.normal(0, 0.2, idx.shape[0]).astype(np.float32)
+    d2 = dict(d); d2["z"] = z
+    got = gpu(velo, d2)
+    assert got["n_deferred"] == 5
+    check(got, cpu(d2))
+    z3 = d["z"].copy(); z3[z3 == 1.0] = np.float32(1.0) + np.float32(2.0 ** -20)   # every event, one module
+    d3 = dict(d); d3["z"] = z3
+    got = gpu(velo, d3)
+    assert got["n_deferred"] >= 25      # every event with a hit on that module
+    check(got, cpu(d3))
+
+
+@pytest.mark.parametrize("n_modules", [3, 4, 17, 32])
+def test_other_module_counts(velo, n_modules):
+    import oracle
+    from dataclasses import replace
+    mz = tuple(np.linspace(-50.0, 700.0, n_modules).round(0).tolist())
+    cfg = replace(datagen.GenConfig(), module_z=mz)
+    d = datagen.generate(cfg, 0, 24)
+    got = velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], np.array(mz))
+    want = oracle.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], n_modules)
+    check(got, want)
+    slab = velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], np.array(mz),
+                            opts=velo.LaunchOptions(path=velo.VELO_PATH_SLAB_ONLY))
+    check(slab, want)
+    if n_modules >= 4:
+        assert want["n_tracks"] > 0
+
+
 # ---- the other workloads ------------------------------------------------------------------------
 def test_config1_10k_events(velo):
     d = datagen.generate_config(1)
@@ -93,7 +144,9 @@ def test_config4_ion_like(velo):
     d = datagen.generate_config(4, n_events=160)
     nh = np.diff(d["event_offsets"].astype(np.int64))
     assert nh.max() > 20000                  # the large-event path is exercised
-    check(gpu(velo, d), cpu(d))
+    got = gpu(velo, d)
+    assert 0 < got["n_deferred"] < 160       # both kernels took part
+    check(got, cpu(d))
 
 
 # ---- hand-made and degenerate inputs (SURVEY.md §8(c) whole-path pins, A14, A15) -----------------
