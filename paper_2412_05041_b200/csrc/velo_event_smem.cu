@@ -9,7 +9,13 @@
 // with named barriers (bar.sync id, 128), never with the whole CTA, so ~5 independent events are
 // in flight per SM and hide each other's shared-memory and barrier latency.
 //
-// The team path keeps only 12 bytes per hit (x, y, one packed word) because it requires every hit
+// Shared memory holds what the module loop touches at random: 12 bytes per hit (x, y, one packed
+// word), the phi-bucket table and 22 bytes per candidate track. The candidates' hit lists (written
+// once per appended hit, read back only after the loop) and fitted states live in a per-team
+// scratch in global memory that stays L2-resident. Smaller blocks = more events in flight per SM,
+// and events in flight are what hides the latency of the 24 dependent, barrier-separated steps.
+//
+// The team path keeps only 12 bytes per hit because it requires every hit
 // to lie on its module plane, z[i] == module_z[module[i]] bit for bit (true for the detector:
 // the geometry is what velo_geometry_load was given). Then z is a per-module constant and the
 // z-ratio of O-4 is computed once per track and step instead of once per candidate. Events that
@@ -32,12 +38,11 @@ constexpr uint32_t kUnitBytes = 4096;       // pool allocation unit
 constexpr uint32_t kPoolUnits = 54;         // 216 KB of pool + 8 KB of control = 224 KB per CTA
 constexpr uint32_t kCtlBytes = 2 * kUnitBytes;
 constexpr uint32_t kClChunk = 256;          // centre hits per seeding chunk (2 per thread)
-constexpr uint32_t kMaxTeams = 8;
-constexpr uint32_t kMaxTeamHits = 32767;    // local original index is stored in 15 bits
+constexpr uint32_t kMaxTeams = kTeamsPerCtaMax;
+constexpr uint32_t kMaxTeamHits = kTeamMaxHits;   // <= 32767: the local original index is stored in 15 bits
 constexpr uint32_t kMaxBinSlot = 2047;      // slot inside a phi bucket is stashed in 11 bits
 constexpr uint32_t kFlagBit = 0x8000u;      // O-5 flag[h] inside the packed hit word
 constexpr uint32_t kNoOwner = 0xffffu;
-constexpr int kRegTracks = 3;               // fitted states of the first 3 tracks per thread stay in registers
 
 // Per-team control block (fixed place in the CTA's control unit).
 struct TeamShared {
@@ -74,8 +79,14 @@ static_assert(sizeof(Control) <= kCtlBytes, "control block must fit its units");
       ph_last = now_;                                                                  \
     }                                                                                  \
   } while (0)
+#ifdef VELO_PHASE_COUNTS
+#define VELO_COUNT(i, v) atomicAdd(&a.ws.phase_clk[i], (unsigned long long)(v))
+#else
+#define VELO_COUNT(i, v) do { } while (0)
+#endif
 #else
 #define VELO_PHASE(i) do { } while (0)
+#define VELO_COUNT(i, v) do { } while (0)
 #endif
 
 __device__ __forceinline__ void team_sync(uint32_t team) {
@@ -115,7 +126,7 @@ struct Layout {
   uint32_t bytes;
 };
 __device__ __forceinline__ uint32_t align16(uint32_t v) { return (v + 15u) & ~15u; }
-__device__ __forceinline__ uint32_t track_bytes(uint32_t tcap, uint32_t M) { return tcap * (2u * M + 20u); }
+constexpr uint32_t kTrackBytes = 22;   // shared-memory bytes per candidate slot (see Ev)
 __device__ __forceinline__ Layout event_layout(uint32_t n, uint32_t M) {
   Layout L;
   uint32_t o = 0;
@@ -124,29 +135,32 @@ __device__ __forceinline__ Layout event_layout(uint32_t n, uint32_t M) {
   L.bins = o; o += align16(2u * (M * kBinsPerModule + 2u));
   L.u = o;
   L.tcap = ((n >> 3) + 32u + 15u) & ~15u;   // candidates ~0.106/hit (max seen 0.157): n/8 + 32, else deferred
-  const uint32_t sortb = 8u * n, trkb = track_bytes(L.tcap, M);
+  const uint32_t sortb = 4u * n, trkb = kTrackBytes * L.tcap;
   o += align16(sortb > trkb ? sortb : trkb);
   L.bytes = o;
   return L;
 }
+static_assert(kTeamMaxHits / 8 + 48 <= kTeamMaxTracks, "team scratch rows must cover the candidate table");
 
-// The arrays of one event, all in shared memory.
+// The arrays of one event.
 struct Ev {
+  // shared memory
   float2* xy;            // sorted hit coordinates
   uint32_t* w;           // packed: (phi16 + 32768) << 16 | flag << 15 | original local index;
                          // after the module loop the upper half becomes the O-13 owner (track id)
   const uint16_t* bo;    // bucket offsets, bo[m * 64 + b], bo[M * 64] = n
-  // sort scratch (dead after S1), aliased by the candidate table
-  uint32_t *stash, *tmp;
-  // candidate table, column t of row-major arrays
-  uint16_t* th;          // th[k * tcap + t] = k-th hit (sorted index)
+  uint32_t* stash;       // sort scratch (dead after S1), aliased by the candidate table:
   uint32_t* tmask;       // modules of the track's hits, bit m
   uint32_t* tl;          // last two hits: older << 16 | latest         } reused as the
   float* tseed;          // seed scatter                                  } 64-bit tkey[t]
   uint16_t* tcentre;     // sorted index of the seed's centre hit
-  uint8_t *tn, *tmiss;   // hits on the track; consecutive misses; after the loop: pass state
+  uint16_t* th0;         // the seed's first hit (row[0]); with tl it flags a track that reaches 4 hits
   uint16_t* act;         // two lists of tcap active-track ids; after the loop: order[] (creation order)
+  uint8_t *tn, *tmiss;   // hits on the track; consecutive misses; after the loop: pass state
   uint32_t tcap;
+  // per-team scratch in global memory (L2-resident)
+  uint16_t* rows;        // rows[t * 32 + k] = k-th hit (sorted index) of candidate t
+  float* st;             // st[k * kTeamMaxTracks + t], k < 9: fitted state of candidate t
 };
 
 // ---- O-3 window of module m around unsigned phi `c`: at most two runs of sorted indices, in
@@ -170,6 +184,21 @@ __device__ __forceinline__ Window make_window(const uint16_t* bo_m, uint32_t c, 
 }
 __device__ __forceinline__ bool in_window(const Window& q, uint32_t wj) { return (((wj >> 16) - q.lo) & 0xffffu) <= q.span; }
 
+// Calls f(i, h) for the hits h (sorted indices) of candidate t in discovery order, i = 0 .. n-1.
+// One 16-byte load per 8 hits from the team's row scratch.
+template <class F>
+__device__ __forceinline__ void for_hits(const Ev& ev, uint32_t t, uint32_t n, F&& f) {
+  const uint4* row = reinterpret_cast<const uint4*>(ev.rows + t * 32u);
+  for (uint32_t g = 0; g * 8u < n; ++g) {
+    const uint4 v = row[g];
+    const uint32_t q[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (uint32_t j = 0; j < 8; ++j) {
+      if (g * 8u + j < n) f(g * 8u + j, (q[j >> 1] >> ((j & 1u) * 16u)) & 0xffffu);
+    }
+  }
+}
+
 // ---- O-11 straight-line fit of candidate t with z taken from the module planes ---------------
 // s9 = x, y, tx, ty, z, cxx, cxtx, vt, chi2 (the 13 state words repeat cxx, cxtx, vt for y and add n).
 // Hits are visited in discovery order = decreasing module = the set bits of `mask` from the top.
@@ -177,35 +206,35 @@ __device__ __forceinline__ void fit_track(const Ev& ev, const float* mz, uint32_
                                           float sig2, float inv_s2, float* s9) {
   float sz = 0.0f, sx = 0.0f, sy = 0.0f;
   uint32_t mk = mask;
-  for (uint32_t i = 0; i < n; ++i) {
+  for_hits(ev, t, n, [&](uint32_t, uint32_t h) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float2 p = ev.xy[ev.th[i * ev.tcap + t]];
+    const float2 p = ev.xy[h];
     sz = __fadd_rn(sz, mz[m]); sx = __fadd_rn(sx, p.x); sy = __fadd_rn(sy, p.y);
-  }
+  });
   const float nf = (float)n;
   const float zb = __fdiv_rn(sz, nf), xb = __fdiv_rn(sx, nf), yb = __fdiv_rn(sy, nf);
   float sdd = 0.0f, sdx = 0.0f, sdy = 0.0f;
   mk = mask;
-  for (uint32_t i = 0; i < n; ++i) {
+  for_hits(ev, t, n, [&](uint32_t, uint32_t h) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float2 p = ev.xy[ev.th[i * ev.tcap + t]];
+    const float2 p = ev.xy[h];
     const float d = __fsub_rn(mz[m], zb);
     sdd = __fadd_rn(sdd, __fmul_rn(d, d));
     sdx = __fadd_rn(sdx, __fmul_rn(d, __fsub_rn(p.x, xb)));
     sdy = __fadd_rn(sdy, __fmul_rn(d, __fsub_rn(p.y, yb)));
-  }
+  });
   const float tx = __fdiv_rn(sdx, sdd), ty = __fdiv_rn(sdy, sdd);
   float c = 0.0f;
   mk = mask;
-  for (uint32_t i = 0; i < n; ++i) {
+  for_hits(ev, t, n, [&](uint32_t, uint32_t h) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float2 p = ev.xy[ev.th[i * ev.tcap + t]];
+    const float2 p = ev.xy[h];
     const float d = __fsub_rn(mz[m], zb);
     const float rx = __fsub_rn(__fsub_rn(p.x, xb), __fmul_rn(tx, d));
     const float ry = __fsub_rn(__fsub_rn(p.y, yb), __fmul_rn(ty, d));
     c = __fadd_rn(c, __fmul_rn(rx, rx));
     c = __fadd_rn(c, __fmul_rn(ry, ry));
-  }
+  });
   const float s2 = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
   float dzb;
   if (s2 < 1e-12f) dzb = 0.0f;
@@ -279,9 +308,9 @@ __device__ void leader_fetch(const KernelArgs& a, Control& ctl, TeamShared& ts) 
   ts.n = n; ts.o0 = o0; ts.units = units; ts.first_unit = first; ts.pool_off = first * kUnitBytes; ts.defer = 0;
 }
 
-// ---- one event, by one team. Returns false if the event was deferred to the slab path ----------
-__device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, unsigned char* pool, uint32_t team,
-                           uint32_t tid, uint32_t& parity, long long& ph_last) {
+// ---- one event, by one team -----------------------------------------------------------------------
+__device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, unsigned char* pool,
+                           unsigned char* scratch, uint32_t team, uint32_t tid, uint32_t& parity, long long& ph_last) {
   (void)ph_last;
   const uint32_t lane = tid & 31u, wid = tid >> 5;
   const uint32_t M = a.n_modules, nbins = M * kBinsPerModule;
@@ -295,20 +324,22 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   uint32_t* binsw = (uint32_t*)(blk + L.bins);
   uint16_t* bins16 = (uint16_t*)binsw;
   ev.bo = bins16;
-  ev.stash = (uint32_t*)(blk + L.u); ev.tmp = ev.stash + n;
+  ev.stash = (uint32_t*)(blk + L.u);
   const uint32_t T = L.tcap;
   ev.tcap = T;
   {
     unsigned char* q = blk + L.u;
-    ev.th = (uint16_t*)q; q += 2u * M * T;
     ev.tmask = (uint32_t*)q; q += 4u * T;
     ev.tl = (uint32_t*)q; q += 4u * T;
     ev.tseed = (float*)q; q += 4u * T;
     ev.tcentre = (uint16_t*)q; q += 2u * T;
+    ev.th0 = (uint16_t*)q; q += 2u * T;
     ev.act = (uint16_t*)q; q += 4u * T;
     ev.tn = q; q += T;
     ev.tmiss = q;
   }
+  ev.rows = (uint16_t*)scratch;
+  ev.st = (float*)(scratch + (size_t)kTeamMaxTracks * 64u);
   unsigned long long* tkey = (unsigned long long*)ev.tl;   // 8 bytes per track over (tl, tseed), used after O-10
   const float* gx = a.x + o0; const float* gy = a.y + o0; const float* gz = a.z + o0;
   const uint8_t* gm = a.module + o0;
@@ -319,17 +350,28 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   team_sync(team);
   {
     uint32_t trouble = 0;
-    for (uint32_t i = tid; i < n; i += kTeamThreads) {
-      const uint32_t m = gm[i];
-      const float x = gx[i], y = gy[i], z = gz[i];
-      if (m >= M) { trouble |= 0x80000000u; continue; }
-      if (__float_as_uint(z) != __float_as_uint(mz[m])) trouble |= 1u;
-      const uint32_t pu = (uint32_t)(phi16(x, y) + 32768);
-      const uint32_t bin = m * kBinsPerModule + (pu >> kBinShift);
-      const uint32_t sh = (bin & 1u) * 16u;
-      const uint32_t slot = (atomicAdd(&binsw[bin >> 1], 1u << sh) >> sh) & 0xffffu;
-      if (slot > kMaxBinSlot) trouble |= 1u;
-      ev.stash[i] = (m << 27) | (pu << 11) | (slot & kMaxBinSlot);
+    constexpr uint32_t U = 4;   // hits in flight per thread: the loads of a group are issued together
+    for (uint32_t i0 = tid; i0 < n; i0 += U * kTeamThreads) {
+      float x[U], y[U], z[U]; uint32_t m[U];
+#pragma unroll
+      for (uint32_t k = 0; k < U; ++k) {
+        const uint32_t i = i0 + k * kTeamThreads;
+        const bool ok = i < n;
+        x[k] = ok ? gx[i] : 1.0f; y[k] = ok ? gy[i] : 0.0f; z[k] = ok ? gz[i] : 0.0f; m[k] = ok ? (uint32_t)gm[i] : 0xffffffffu;
+      }
+#pragma unroll
+      for (uint32_t k = 0; k < U; ++k) {
+        const uint32_t i = i0 + k * kTeamThreads;
+        if (i >= n) continue;
+        if (m[k] >= M) { trouble |= 0x80000000u; continue; }
+        if (__float_as_uint(z[k]) != __float_as_uint(mz[m[k]])) trouble |= 1u;
+        const uint32_t pu = (uint32_t)(phi16(x[k], y[k]) + 32768);
+        const uint32_t bin = m[k] * kBinsPerModule + (pu >> kBinShift);
+        const uint32_t sh = (bin & 1u) * 16u;
+        const uint32_t slot = (atomicAdd(&binsw[bin >> 1], 1u << sh) >> sh) & 0xffffu;
+        if (slot > kMaxBinSlot) trouble |= 1u;
+        ev.stash[i] = (m[k] << 27) | (pu << 11) | (slot & kMaxBinSlot);
+      }
     }
     if (trouble) atomicOr(&ts.defer, trouble);
   }
@@ -359,11 +401,11 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   }
   team_sync(team);
   VELO_PHASE(2);   // bucket scan
-  // ---- S1 phi sort (O-2): group by bucket, then rank inside the bucket by (phi16, index) --------
+  // ---- S1 phi sort (O-2): group by bucket in w[], rank inside the bucket by (phi16, index), place ---
   for (uint32_t i = tid; i < n; i += kTeamThreads) {
     const uint32_t st = ev.stash[i], pu = (st >> 11) & 0xffffu;
     const uint32_t bin = (st >> 27) * kBinsPerModule + (pu >> kBinShift);
-    ev.tmp[(uint32_t)bins16[bin] + (st & kMaxBinSlot)] = (pu << 16) | i;
+    ev.w[(uint32_t)bins16[bin] + (st & kMaxBinSlot)] = (pu << 16) | i;
   }
   team_sync(team);
   for (uint32_t i = tid; i < n; i += kTeamThreads) {
@@ -372,9 +414,28 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     const uint32_t item = (pu << 16) | i;
     const uint32_t lo = bins16[bin], hi = bins16[bin + 1];
     uint32_t r = lo;
-    for (uint32_t j = lo; j < hi; ++j) r += (ev.tmp[j] < item) ? 1u : 0u;
-    ev.xy[r] = make_float2(gx[i], gy[i]);
-    ev.w[r] = item;
+    for (uint32_t j = lo; j < hi; ++j) r += (ev.w[j] < item) ? 1u : 0u;
+    ev.stash[i] = (pu << 16) | r;   // r <= 32767
+  }
+  team_sync(team);   // every rank is known: w[] can take its final content
+  {
+    constexpr uint32_t U = 4;
+    for (uint32_t i0 = tid; i0 < n; i0 += U * kTeamThreads) {
+      float x[U], y[U];
+#pragma unroll
+      for (uint32_t k = 0; k < U; ++k) {
+        const uint32_t i = i0 + k * kTeamThreads;
+        x[k] = i < n ? gx[i] : 0.0f; y[k] = i < n ? gy[i] : 0.0f;   // second read of x, y: L2
+      }
+#pragma unroll
+      for (uint32_t k = 0; k < U; ++k) {
+        const uint32_t i = i0 + k * kTeamThreads;
+        if (i >= n) continue;
+        const uint32_t st = ev.stash[i], r = st & 0xffffu;
+        ev.xy[r] = make_float2(x[k], y[k]);
+        ev.w[r] = (st & 0xffff0000u) | i;
+      }
+    }
   }
   team_sync(team);   // the sort scratch is dead from here on: the candidate table takes its place
   VELO_PHASE(3);   // S1 sort
@@ -393,6 +454,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     {
       const uint32_t nact = ts.nact[cur];
       const float z2 = mz[u];
+      const float max_fwd = P.max_scatter_fwd;
       const uint16_t* bo_u = ev.bo + u * kBinsPerModule;
       const uint16_t* act = ev.act + cur * T;
       uint16_t* act_next = ev.act + nxt * T;
@@ -412,25 +474,28 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
           const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
           const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
           const Window q = make_window(bo_u, c, P.phi_window_fwd);
+          // branch-free visits (the loops are latency-bound: a taken branch costs more than the math)
           bool found = false; uint32_t best = 0; float best_sc = 0.0f;
-          auto visit = [&](uint32_t j) {
-            if (!in_window(q, ev.w[j])) return;
+          const uint32_t jend = q.e0 + (q.e1 - q.b1);
+          for (uint32_t jj = q.b0; jj < jend; ++jj) {
+            const uint32_t j = jj < q.e0 ? jj : jj - q.e0 + q.b1;
+            const uint32_t wj = ev.w[j];
             const float2 p2 = ev.xy[j];
             const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
             const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-            if (sc <= P.max_scatter_fwd && (!found || sc < best_sc)) { found = true; best = j; best_sc = sc; }
-          };
-          for (uint32_t j = q.b0; j < q.e0; ++j) visit(j);
-          for (uint32_t j = q.b1; j < q.e1; ++j) visit(j);
+            const bool better = in_window(q, wj) & (sc <= max_fwd) & (!found | (sc < best_sc));
+            found |= better; best = better ? j : best; best_sc = better ? sc : best_sc;
+          }
+          VELO_COUNT(16, 1); VELO_COUNT(17, jend - q.b0);
           if (found) {
             const uint32_t nh = ev.tn[t];
-            ev.th[nh * T + t] = (uint16_t)best;
+            ev.rows[t * 32u + nh] = (uint16_t)best;
             ev.tn[t] = (uint8_t)(nh + 1);
             ev.tmiss[t] = 0;
             ev.tl[t] = (hb << 16) | best;
             ev.tmask[t] = mask | (1u << u);
             // (B): forwarding never reads flags, so they can be set right away
-            if (nh + 1 == 4) { for (uint32_t i = 0; i < 3; ++i) ev.w[ev.th[i * T + t]] |= kFlagBit; }
+            if (nh + 1 == 4) { ev.w[ev.th0[t]] |= kFlagBit; ev.w[ha] |= kFlagBit; ev.w[hb] |= kFlagBit; }
             if (nh + 1 >= 4) ev.w[best] |= kFlagBit;
             alive = true;
           } else {
@@ -456,6 +521,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
       const uint32_t c_begin = ev.bo[s * kBinsPerModule], c_end = ev.bo[(s + 1) * kBinsPerModule];
       const float z0 = mz[s + 1], z1 = mz[s], z2 = mz[u];
       const float tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0));
+      const float max_seed = P.max_scatter_seed;
       const uint16_t* bo_0 = ev.bo + (s + 1) * kBinsPerModule;
       const uint16_t* bo_2 = ev.bo + u * kBinsPerModule;
       uint16_t* act_next = ev.act + nxt * T;
@@ -478,38 +544,52 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
         const uint32_t ncl = ts.ncl[cpar];
         if (tid == 0) ts.ncl[cpar ^ 1u] = 0;   // the other counter: last read before the barrier above
         cpar ^= 1u;
-        // (C2) one thread per unflagged centre hit: best (h0, h2) under (scatter, h0, h2)
-        for (uint32_t k = tid; k < ncl; k += kTeamThreads) {
-          const uint32_t h1 = ts.cl[k];
-          const uint32_t w1 = ev.w[h1];
-          const float2 p1 = ev.xy[h1];
-          const Window q0 = make_window(bo_0, w1 >> 16, P.phi_window_seed);
-          const Window q2 = make_window(bo_2, w1 >> 16, P.phi_window_seed);
-          bool found = false; uint32_t b0 = 0, b2 = 0; float best_sc = 0.0f;
-          auto visit0 = [&](uint32_t h0) {
-            const uint32_t w0 = ev.w[h0];
-            if ((w0 & kFlagBit) || !in_window(q0, w0)) return;
-            const float2 p0 = ev.xy[h0];
-            const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
-            const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
-            auto visit2 = [&](uint32_t h2) {
-              const uint32_t w2 = ev.w[h2];
-              if ((w2 & kFlagBit) || !in_window(q2, w2)) return;
-              const float2 p2 = ev.xy[h2];
-              const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
-              const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-              // h0 ascending outside, h2 ascending inside: strict < keeps the lexicographic minimum
-              if (sc <= P.max_scatter_seed && (!found || sc < best_sc)) { found = true; b0 = h0; b2 = h2; best_sc = sc; }
-            };
-            for (uint32_t j = q2.b0; j < q2.e0; ++j) visit2(j);
-            for (uint32_t j = q2.b1; j < q2.e1; ++j) visit2(j);
-          };
-          for (uint32_t j = q0.b0; j < q0.e0; ++j) visit0(j);
-          for (uint32_t j = q0.b1; j < q0.e1; ++j) visit0(j);
-          if (found) {
+        // (C2) four lanes per unflagged centre hit: lane `sub` takes every 4th h0 of the window; the
+        // quad's best (h0, h2) under (scatter, h0, h2) is reduced with shuffles
+        for (uint32_t k0 = 0; k0 < ncl; k0 += kTeamThreads / 4) {
+          const uint32_t k = k0 + (tid >> 2), sub = tid & 3u;
+          bool found = false; uint32_t b0 = 0, b2 = 0, h1 = 0; float best_sc = 0.0f;
+          if (k < ncl) {
+            h1 = ts.cl[k];
+            const uint32_t w1 = ev.w[h1];
+            const float2 p1 = ev.xy[h1];
+            const Window q0 = make_window(bo_0, w1 >> 16, P.phi_window_seed);
+            const Window q2 = make_window(bo_2, w1 >> 16, P.phi_window_seed);
+            const uint32_t end0 = q0.e0 + (q0.e1 - q0.b1), end2 = q2.e0 + (q2.e1 - q2.b1);
+            VELO_COUNT(18, 1); VELO_COUNT(19, end0 - q0.b0);
+            for (uint32_t jo = q0.b0 + sub; jo < end0; jo += 4) {
+              const uint32_t h0 = jo < q0.e0 ? jo : jo - q0.e0 + q0.b1;
+              const uint32_t w0 = ev.w[h0];
+              if ((w0 & kFlagBit) || !in_window(q0, w0)) continue;
+              VELO_COUNT(20, 1); VELO_COUNT(21, end2 - q2.b0);
+              const float2 p0 = ev.xy[h0];
+              const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
+              const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
+              // h0 and h2 ascending: strict < keeps this lane's lexicographic minimum; branch-free body
+              for (uint32_t ji = q2.b0; ji < end2; ++ji) {
+                const uint32_t h2 = ji < q2.e0 ? ji : ji - q2.e0 + q2.b1;
+                const uint32_t w2 = ev.w[h2];
+                const float2 p2 = ev.xy[h2];
+                const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
+                const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+                const bool better = !(w2 & kFlagBit) & in_window(q2, w2) & (sc <= max_seed) & (!found | (sc < best_sc));
+                found |= better; b0 = better ? h0 : b0; b2 = better ? h2 : b2; best_sc = better ? sc : best_sc;
+              }
+            }
+          }
+#pragma unroll
+          for (uint32_t d = 1; d <= 2; d <<= 1) {   // minimum over the quad, ties: lowest h0, then lowest h2
+            const bool of = __shfl_xor_sync(0xffffffffu, (int)found, d) != 0;
+            const float osc = __shfl_xor_sync(0xffffffffu, best_sc, d);
+            const uint32_t ob0 = __shfl_xor_sync(0xffffffffu, b0, d), ob2 = __shfl_xor_sync(0xffffffffu, b2, d);
+            const bool take = of & (!found | (osc < best_sc) | ((osc == best_sc) & ((ob0 < b0) | ((ob0 == b0) & (ob2 < b2)))));
+            found |= of; b0 = take ? ob0 : b0; b2 = take ? ob2 : b2; best_sc = take ? osc : best_sc;
+          }
+          if (found && sub == 0) {
             const uint32_t slot = atomicAdd(&ts.nt, 1u);
             if (slot < T) {
-              ev.th[slot] = (uint16_t)b0; ev.th[T + slot] = (uint16_t)h1; ev.th[2 * T + slot] = (uint16_t)b2;
+              *reinterpret_cast<uint2*>(ev.rows + slot * 32u) = make_uint2(b0 | (h1 << 16), b2);
+              ev.th0[slot] = (uint16_t)b0;
               ev.tn[slot] = 3; ev.tmiss[slot] = 0;
               ev.tl[slot] = (h1 << 16) | b2;
               ev.tmask[slot] = 7u << u;
@@ -520,6 +600,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
         }
         team_sync(team);   // cl[] may be refilled; after the last chunk: the new tracks are visible
         VELO_PHASE(6);   // (C2) seeding
+        if (tid == 0) { VELO_COUNT(22, 1); }
       }
       if (c_begin >= c_end) team_sync(team);   // no chunk ran: still order this step's resets before the next step
     }
@@ -549,45 +630,39 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   for (uint32_t t = tid; t < nt; t += kTeamThreads) {
     bool pass = true;
     if (ev.tn[t] == 3) {
-      const uint32_t f = ev.w[ev.th[t]] | ev.w[ev.th[T + t]] | ev.w[ev.th[2 * T + t]];
+      const uint32_t l = ev.tl[t];   // never extended: still (centre, third hit)
+      const uint32_t f = ev.w[ev.th0[t]] | ev.w[l >> 16] | ev.w[l & 0xffffu];
       if ((f & kFlagBit) || !(ev.tseed[t] <= P.max_scatter_weak)) pass = false;
     }
     ev.tmiss[t] = pass ? 1 : 0;
   }
   team_sync(team);
   // ---- O-11 fit, O-12 chi2 cut, O-13 key; the packed words' upper halves become "no owner" -------
+  // (tkey[t] overlays tl/tseed of other tracks: every thread has read those above)
   for (uint32_t i = tid; i < n; i += kTeamThreads) ev.w[i] |= 0xffff0000u;
   const float sig2 = __fmul_rn(P.sigma_hit, P.sigma_hit);
   const float inv_s2 = __fdiv_rn(1.0f, sig2);
-  float sreg[kRegTracks][9];
-  auto fit_and_key = [&](uint32_t t, float* s9) {
+  for (uint32_t t = tid; t < nt; t += kTeamThreads) {
+    if (!ev.tmiss[t]) continue;
     const uint32_t nh = ev.tn[t];
     const uint32_t centre = ev.tcentre[t];
+    float s9[9];
     fit_track(ev, mz, t, nh, ev.tmask[t], sig2, inv_s2, s9);
     const float lim = __fmul_rn(P.max_chi2_ndof, (float)(2 * (int)nh - 4));
-    if (s9[8] > lim) { ev.tmiss[t] = 0; return; }
+    if (s9[8] > lim) { ev.tmiss[t] = 0; continue; }
     tkey[t] = ((unsigned long long)(255u - nh) << 56) | ((unsigned long long)__float_as_uint(s9[8]) << 24) |
               (unsigned long long)centre;
-  };
-  // tkey[t] overlays tl/tseed of tracks 2t, 2t+1: every thread must have read its seeds (above) first
 #pragma unroll
-  for (int k = 0; k < kRegTracks; ++k) {
-    const uint32_t t = tid + (uint32_t)k * kTeamThreads;
-    if (t < nt && ev.tmiss[t]) fit_and_key(t, sreg[k]);
-  }
-  for (uint32_t t = tid + kRegTracks * kTeamThreads; t < nt; t += kTeamThreads) {
-    float s9[9];
-    if (ev.tmiss[t]) fit_and_key(t, s9);
+    for (uint32_t k = 0; k < 9; ++k) ev.st[k * kTeamMaxTracks + t] = s9[k];
   }
   team_sync(team);
   VELO_PHASE(8);   // O-10, fit, keys
   // ---- O-13 owners: owner[h] = the candidate with the smallest key among those that contain h ----
   for (uint32_t t = tid; t < nt; t += kTeamThreads) {
     if (!ev.tmiss[t]) continue;
-    const uint32_t nh = ev.tn[t];
     const unsigned long long key = tkey[t];
-    for (uint32_t i = 0; i < nh; ++i) {
-      uint32_t* wp = &ev.w[ev.th[i * T + t]];
+    for_hits(ev, t, ev.tn[t], [&](uint32_t, uint32_t h) {
+      uint32_t* wp = &ev.w[h];
       uint32_t old = *(volatile uint32_t*)wp;
       for (;;) {
         const uint32_t cur = old >> 16;
@@ -596,7 +671,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
         if (seen == old) break;
         old = seen;
       }
-    }
+    });
   }
   team_sync(team);
   VELO_PHASE(9);   // owners
@@ -611,7 +686,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     if (k < nt && ev.tmiss[t]) {
       nh = ev.tn[t];
       uint32_t lost = 0;
-      for (uint32_t i = 0; i < nh; ++i) lost += ((ev.w[ev.th[i * T + t]] >> 16) != t) ? 1u : 0u;
+      for_hits(ev, t, nh, [&](uint32_t, uint32_t h) { lost += ((ev.w[h] >> 16) != t) ? 1u : 0u; });
       surv = !((unsigned long long)lost * P.clone_den > (unsigned long long)nh * P.clone_num) ? 1u : 0u;
       if (!surv) nh = 0;
     }
@@ -635,9 +710,13 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
                     (unsigned long long)hbase + ev_nh <= a.cap_track_hits;
   if (!fits) return;   // VELO_ERR_CAPACITY is raised by the offsets kernel; nothing valid to write
   uint32_t* stage = (uint32_t*)ev.xy;          // coordinates are dead after the fit: 2n words
-  const bool staged = ev_nh <= 2u * n && nt <= (uint32_t)kRegTracks * kTeamThreads;   // a re-fit below still reads xy
-  auto emit = [&](uint32_t t, const float* s9) {
+  const bool staged = ev_nh <= 2u * n;
+  for (uint32_t t = tid; t < nt; t += kTeamThreads) {
+    if (ev.tmiss[t] != 2) continue;
     const uint32_t nh = ev.tn[t], lt = pl[t], lh = ph[t];
+    float s9[9];
+#pragma unroll
+    for (uint32_t k = 0; k < 9; ++k) s9[k] = ev.st[k * kTeamMaxTracks + t];
     float* st = a.ws.tmp_states + tbase + lt;
     const size_t cs = a.cap_tracks;
     st[0] = s9[0]; st[cs] = s9[1]; st[2 * cs] = s9[2]; st[3 * cs] = s9[3]; st[4 * cs] = s9[4];
@@ -645,19 +724,8 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     st[8 * cs] = s9[5]; st[9 * cs] = s9[6]; st[10 * cs] = s9[7];
     st[11 * cs] = s9[8]; st[12 * cs] = __uint_as_float(nh);
     a.ws.tmp_loff[tbase + lt] = lh;
-    if (staged) { for (uint32_t i = 0; i < nh; ++i) stage[lh + i] = o0 + (ev.w[ev.th[i * T + t]] & 0x7fffu); }
-    else { for (uint32_t i = 0; i < nh; ++i) a.ws.tmp_hits[hbase + lh + i] = o0 + (ev.w[ev.th[i * T + t]] & 0x7fffu); }
-  };
-#pragma unroll
-  for (int k = 0; k < kRegTracks; ++k) {
-    const uint32_t t = tid + (uint32_t)k * kTeamThreads;
-    if (t < nt && ev.tmiss[t] == 2) emit(t, sreg[k]);
-  }
-  for (uint32_t t = tid + kRegTracks * kTeamThreads; t < nt; t += kTeamThreads) {
-    if (ev.tmiss[t] != 2) continue;
-    float s9[9];
-    fit_track(ev, mz, t, ev.tn[t], ev.tmask[t], sig2, inv_s2, s9);   // rare: > 384 candidates in one event
-    emit(t, s9);
+    uint32_t* dst = staged ? stage + lh : a.ws.tmp_hits + hbase + lh;
+    for_hits(ev, t, nh, [&](uint32_t i, uint32_t h) { dst[i] = o0 + (ev.w[h] & 0x7fffu); });
   }
   if (staged) {
     team_sync(team);
@@ -677,6 +745,7 @@ __global__ void __launch_bounds__(kTeams* kTeamThreads, 1) velo_event_team_kerne
   if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
   __syncthreads();
   TeamShared& ts = ctl.team[team];
+  unsigned char* scratch = a.ws.team_scratch + ((size_t)blockIdx.x * kMaxTeams + team) * kTeamScratchBytes;
   uint32_t parity = 0;
   long long ph_last = clock64();
   (void)ph_last;
@@ -685,7 +754,7 @@ __global__ void __launch_bounds__(kTeams* kTeamThreads, 1) velo_event_team_kerne
     team_sync(team);
     if (ts.event >= a.n_events) break;
     VELO_PHASE(0);   // ticket + pool allocation (waiting for shared memory)
-    if (!ts.defer) team_event(a, ctl, ts, pool, team, tid, parity, ph_last);
+    if (!ts.defer) team_event(a, ctl, ts, pool, scratch, team, tid, parity, ph_last);
     team_sync(team);   // every thread is done with the block and with ts before the leader reuses them
     if (tid == 0 && ts.units) pool_free(ctl, ts.first_unit, ts.units);
     VELO_PHASE(12);  // last barrier + free

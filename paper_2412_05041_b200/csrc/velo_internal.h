@@ -37,11 +37,19 @@ __host__ __device__ inline SlabLayout slab_layout() {
   return L;
 }
 
+// ---- per-team scratch of the shared-memory team kernel (velo_event_smem.cu) --------------------
+// The candidates' hit lists (32 x u16 per candidate) and fitted states (9 x f32) of the event a
+// team is working on. Rewritten for every event, so it stays L2-resident.
+constexpr uint32_t kTeamMaxHits = 13312;                       // largest event the team path takes
+constexpr uint32_t kTeamMaxTracks = kTeamMaxHits / 8 + 64;     // >= its candidate-table capacity
+constexpr uint32_t kTeamScratchBytes = kTeamMaxTracks * (64 + 36);
+constexpr uint32_t kTeamsPerCtaMax = 8;
+
 // ---- workspace layout (device) ---------------------------------------------------------------
 // counters: u32[16]: 0 tracks allocated, 1 track-hits allocated, 2 status, 3 candidates,
 //           4 event ticket, 5 large-event list length, 6 large-event ticket
 enum { kCtrTracks = 0, kCtrHits = 1, kCtrStatus = 2, kCtrCand = 3, kCtrTicket = 4, kCtrLargeN = 5,
-       kCtrLargeTicket = 6, kNumCounters = 16, kNumPhaseClocks = 16 };
+       kCtrLargeTicket = 6, kNumCounters = 16, kNumPhaseClocks = 32 };
 
 struct Workspace {
   uint32_t* counters;     // kNumCounters
@@ -52,6 +60,7 @@ struct Workspace {
   uint32_t* tmp_loff;     // cap_tracks: hit offset of a track inside its event's hit block
   uint32_t* tmp_hits;     // cap_track_hits
   float* tmp_states;      // VELO_N_STATE * cap_tracks
+  unsigned char* team_scratch;  // num_sms * kTeamsPerCtaMax * kTeamScratchBytes
   unsigned char* slabs;   // n_slabs * slab bytes
   uint32_t n_slabs;
   size_t bytes;

@@ -429,6 +429,7 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, ui
   w.tmp_loff = (uint32_t*)take(4 * ((size_t)cap_tracks + 1));
   w.tmp_hits = (uint32_t*)take(4 * ((size_t)cap_track_hits + 1));
   w.tmp_states = (float*)take(4 * (size_t)VELO_N_STATE * ((size_t)cap_tracks + 1));
+  w.team_scratch = take((size_t)num_sms() * kTeamsPerCtaMax * kTeamScratchBytes);
   w.n_slabs = n_slabs;
   w.slabs = take((size_t)n_slabs * slab_layout().bytes);
   w.bytes = o;
