@@ -42,7 +42,6 @@ constexpr uint32_t kMaxTeams = kTeamsPerCtaMax;
 constexpr uint32_t kMaxTeamHits = kTeamMaxHits;   // <= 32767: the local original index is stored in 15 bits
 constexpr uint32_t kMaxBinSlot = 2047;      // slot inside a phi bucket is stashed in 11 bits
 constexpr uint32_t kFlagBit = 0x8000u;      // O-5 flag[h] inside the packed hit word
-constexpr uint32_t kNoOwner = 0xffffu;
 
 // Per-team control block (fixed place in the CTA's control unit).
 struct TeamShared {
@@ -165,14 +164,16 @@ struct Ev {
 
 // ---- O-3 window of module m around unsigned phi `c`: at most two runs of sorted indices, in
 // ascending order, and a modular test ((pu - lo) & 0xffff) <= span for the hits inside them.
-struct Window { uint32_t b0, e0, b1, e1, lo, span; };
+// lo and span are kept shifted to the phi field of the packed hit word: lo16 = lo << 16,
+// lim = span << 16 | 0xffff, so that the test is one subtract and one compare on the whole word.
+struct Window { uint32_t b0, e0, b1, e1, lo16, lim; };
 __device__ __forceinline__ Window make_window(const uint16_t* bo_m, uint32_t c, int W) {
   Window q;
   q.b1 = q.e1 = 0;
-  if (W < 0) { q.b0 = q.e0 = 0; q.lo = 0; q.span = 0; return q; }
-  if (2 * (long long)W + 1 >= 65536) { q.b0 = bo_m[0]; q.e0 = bo_m[kBinsPerModule]; q.lo = 0; q.span = 0xffffu; return q; }
+  if (W < 0) { q.b0 = q.e0 = 0; q.lo16 = 0; q.lim = 0; return q; }
+  if (2 * (long long)W + 1 >= 65536) { q.b0 = bo_m[0]; q.e0 = bo_m[kBinsPerModule]; q.lo16 = 0; q.lim = 0xffffffffu; return q; }
   const uint32_t lo = (c - (uint32_t)W) & 0xffffu, hi = (c + (uint32_t)W) & 0xffffu;
-  q.lo = lo; q.span = 2u * (uint32_t)W;
+  q.lo16 = lo << 16; q.lim = (2u * (uint32_t)W) << 16 | 0xffffu;
   if (lo <= hi) { q.b0 = bo_m[lo >> kBinShift]; q.e0 = bo_m[(hi >> kBinShift) + 1]; }
   else if ((lo >> kBinShift) <= (hi >> kBinShift)) {  // wraps and the two runs would overlap: whole module
     q.b0 = bo_m[0]; q.e0 = bo_m[kBinsPerModule];
@@ -182,7 +183,7 @@ __device__ __forceinline__ Window make_window(const uint16_t* bo_m, uint32_t c, 
   }
   return q;
 }
-__device__ __forceinline__ bool in_window(const Window& q, uint32_t wj) { return (((wj >> 16) - q.lo) & 0xffffu) <= q.span; }
+__device__ __forceinline__ bool in_window(const Window& q, uint32_t wj) { return wj - q.lo16 <= q.lim; }
 
 // Calls f(i, h) for the hits h (sorted indices) of candidate t in discovery order, i = 0 .. n-1.
 // One 16-byte load per 8 hits from the team's row scratch.
@@ -476,17 +477,17 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
           const Window q = make_window(bo_u, c, P.phi_window_fwd);
           // branch-free visits (the loops are latency-bound: a taken branch costs more than the math)
           bool found = false; uint32_t best = 0; float best_sc = 0.0f;
-          const uint32_t jend = q.e0 + (q.e1 - q.b1);
-          for (uint32_t jj = q.b0; jj < jend; ++jj) {
-            const uint32_t j = jj < q.e0 ? jj : jj - q.e0 + q.b1;
+          auto visit = [&](uint32_t j) {
             const uint32_t wj = ev.w[j];
             const float2 p2 = ev.xy[j];
             const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
             const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
             const bool better = in_window(q, wj) & (sc <= max_fwd) & (!found | (sc < best_sc));
             found |= better; best = better ? j : best; best_sc = better ? sc : best_sc;
-          }
-          VELO_COUNT(16, 1); VELO_COUNT(17, jend - q.b0);
+          };
+          for (uint32_t j = q.b0; j < q.e0; ++j) visit(j);
+          for (uint32_t j = q.b1; j < q.e1; ++j) visit(j);   // second run: only for a window across +-pi
+          VELO_COUNT(16, 1); VELO_COUNT(17, (q.e0 - q.b0) + (q.e1 - q.b1));
           if (found) {
             const uint32_t nh = ev.tn[t];
             ev.rows[t * 32u + nh] = (uint16_t)best;
@@ -555,26 +556,27 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
             const float2 p1 = ev.xy[h1];
             const Window q0 = make_window(bo_0, w1 >> 16, P.phi_window_seed);
             const Window q2 = make_window(bo_2, w1 >> 16, P.phi_window_seed);
-            const uint32_t end0 = q0.e0 + (q0.e1 - q0.b1), end2 = q2.e0 + (q2.e1 - q2.b1);
+            const uint32_t end0 = q0.e0 + (q0.e1 - q0.b1);
             VELO_COUNT(18, 1); VELO_COUNT(19, end0 - q0.b0);
             for (uint32_t jo = q0.b0 + sub; jo < end0; jo += 4) {
               const uint32_t h0 = jo < q0.e0 ? jo : jo - q0.e0 + q0.b1;
               const uint32_t w0 = ev.w[h0];
               if ((w0 & kFlagBit) || !in_window(q0, w0)) continue;
-              VELO_COUNT(20, 1); VELO_COUNT(21, end2 - q2.b0);
+              VELO_COUNT(20, 1); VELO_COUNT(21, (q2.e0 - q2.b0) + (q2.e1 - q2.b1));
               const float2 p0 = ev.xy[h0];
               const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
               const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
               // h0 and h2 ascending: strict < keeps this lane's lexicographic minimum; branch-free body
-              for (uint32_t ji = q2.b0; ji < end2; ++ji) {
-                const uint32_t h2 = ji < q2.e0 ? ji : ji - q2.e0 + q2.b1;
+              auto visit2 = [&](uint32_t h2) {
                 const uint32_t w2 = ev.w[h2];
                 const float2 p2 = ev.xy[h2];
                 const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
                 const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
                 const bool better = !(w2 & kFlagBit) & in_window(q2, w2) & (sc <= max_seed) & (!found | (sc < best_sc));
                 found |= better; b0 = better ? h0 : b0; b2 = better ? h2 : b2; best_sc = better ? sc : best_sc;
-              }
+              };
+              for (uint32_t j = q2.b0; j < q2.e0; ++j) visit2(j);
+              for (uint32_t j = q2.b1; j < q2.e1; ++j) visit2(j);
             }
           }
 #pragma unroll
@@ -637,9 +639,8 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     ev.tmiss[t] = pass ? 1 : 0;
   }
   team_sync(team);
-  // ---- O-11 fit, O-12 chi2 cut, O-13 key; the packed words' upper halves become "no owner" -------
+  // ---- O-11 fit, O-12 chi2 cut, O-13 key --------------------------------------------------------
   // (tkey[t] overlays tl/tseed of other tracks: every thread has read those above)
-  for (uint32_t i = tid; i < n; i += kTeamThreads) ev.w[i] |= 0xffff0000u;
   const float sig2 = __fmul_rn(P.sigma_hit, P.sigma_hit);
   const float inv_s2 = __fdiv_rn(1.0f, sig2);
   for (uint32_t t = tid; t < nt; t += kTeamThreads) {
@@ -658,20 +659,30 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   team_sync(team);
   VELO_PHASE(8);   // O-10, fit, keys
   // ---- O-13 owners: owner[h] = the candidate with the smallest key among those that contain h ----
-  for (uint32_t t = tid; t < nt; t += kTeamThreads) {
-    if (!ev.tmiss[t]) continue;
-    const unsigned long long key = tkey[t];
-    for_hits(ev, t, ev.tn[t], [&](uint32_t, uint32_t h) {
-      uint32_t* wp = &ev.w[h];
-      uint32_t old = *(volatile uint32_t*)wp;
-      for (;;) {
-        const uint32_t cur = old >> 16;
-        if (cur != kNoOwner && tkey[cur] < key) break;
-        const uint32_t seen = atomicCAS(wp, old, (t << 16) | (old & 0xffffu));
-        if (seen == old) break;
-        old = seen;
-      }
-    });
+  // Step 1: every passing candidate writes its id on its hits (plain 16-bit stores: where several
+  // candidates share a hit, any one of them lands). Step 2: a candidate that finds another id on
+  // one of its hits settles it with a compare-and-swap on the 64-bit keys. Hits are shared rarely,
+  // so the common path has no atomics and no dependent chain.
+  {
+    uint16_t* own = reinterpret_cast<uint16_t*>(ev.w);   // own[2h + 1] = upper half of w[h]
+    for (uint32_t t = tid; t < nt; t += kTeamThreads) {
+      if (!ev.tmiss[t]) continue;
+      for_hits(ev, t, ev.tn[t], [&](uint32_t, uint32_t h) { own[2u * h + 1u] = (uint16_t)t; });
+    }
+    team_sync(team);
+    for (uint32_t t = tid; t < nt; t += kTeamThreads) {
+      if (!ev.tmiss[t]) continue;
+      const unsigned long long key = tkey[t];
+      for_hits(ev, t, ev.tn[t], [&](uint32_t, uint32_t h) {
+        uint32_t* wp = &ev.w[h];
+        uint32_t old = *(volatile uint32_t*)wp;
+        while ((old >> 16) != t && key < tkey[old >> 16]) {
+          const uint32_t seen = atomicCAS(wp, old, (t << 16) | (old & 0xffffu));
+          if (seen == old) break;
+          old = seen;
+        }
+      });
+    }
   }
   team_sync(team);
   VELO_PHASE(9);   // owners
@@ -783,12 +794,12 @@ int launch_teams(const KernelArgs& a, cudaStream_t stream) {
 int launch_event_smem(const KernelArgs& a, cudaStream_t stream, uint32_t teams) {
   switch (teams) {
     case 4: return launch_teams<4>(a, stream);
-    case 5: return launch_teams<5>(a, stream);
-    case 8: return launch_teams<8>(a, stream);
+    case 6: return launch_teams<6>(a, stream);
     case 7: return launch_teams<7>(a, stream);
-    case 0:
-    case 6:
-    default: return launch_teams<6>(a, stream);
+    case 8: return launch_teams<8>(a, stream);
+    case 0:   // default: the pool holds about five mean mu = 5 events, more teams only wait for memory
+    case 5:
+    default: return launch_teams<5>(a, stream);
   }
 }
 
