@@ -263,14 +263,14 @@ __device__ __forceinline__ void defer_to_slab(const KernelArgs& a, uint32_t e) {
 __device__ __forceinline__ uint32_t pool_alloc(Control& ctl, uint32_t units) {
   const uint32_t my = atomicAdd(&ctl.alloc_next, 1u);
   volatile uint32_t* serving = &ctl.alloc_serving;
-  while (*serving != my) __nanosleep(400);
+  while (*serving != my) __nanosleep(1500);
   volatile unsigned long long* bm = &ctl.bitmap;
   const unsigned long long all = (1ull << kPoolUnits) - 1ull;
   uint32_t first;
   unsigned long long seen = ~0ull;
   for (;;) {
     const unsigned long long used = *bm;
-    if (used == seen) { __nanosleep(400); continue; }   // nothing was freed since the last failed try
+    if (used == seen) { __nanosleep(1500); continue; }   // nothing was freed since the last failed try
     unsigned long long r = ~used & all;          // bit p: unit p free
     for (uint32_t i = 1; i < units && r; ++i) r &= (r >> 1);   // bit p: units p .. p+i free
     if (r) {
@@ -792,12 +792,19 @@ int launch_teams(const KernelArgs& a, cudaStream_t stream) {
 }  // namespace
 
 int launch_event_smem(const KernelArgs& a, cudaStream_t stream, uint32_t teams) {
+  if (teams == 0) {
+    // Default: as many teams as mean-sized events fit the pool (about 16 bytes per hit + 5 KB per
+    // event), less one because blocks of unequal size never pack perfectly: 5 for mu = 5 events of
+    // 1.9 k hits, 8 for the 0.3 k-hit events of the open VELO. More teams would only wait for memory.
+    const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
+    const uint32_t fit = (kPoolUnits * kUnitBytes) / (16u * mean + 5120u);
+    teams = fit <= 5u ? 5u : (fit - 1u > kMaxTeams ? kMaxTeams : fit - 1u);
+  }
   switch (teams) {
     case 4: return launch_teams<4>(a, stream);
     case 6: return launch_teams<6>(a, stream);
     case 7: return launch_teams<7>(a, stream);
     case 8: return launch_teams<8>(a, stream);
-    case 0:   // default: the pool holds about five mean mu = 5 events, more teams only wait for memory
     case 5:
     default: return launch_teams<5>(a, stream);
   }

@@ -76,6 +76,7 @@ struct KernelArgs {
   const uint8_t* module;
   const uint32_t* event_offsets;
   uint32_t n_events, n_modules;
+  uint32_t n_hits;                   // host knowledge of the batch size: only steers launch heuristics
   float module_z[VELO_MAX_MODULES];  // geometry: the shared-memory path requires z[i] == module_z[module[i]]
   velo_params_t P;
   // output
