@@ -379,7 +379,10 @@ __global__ void __launch_bounds__(1024) velo_offsets_kernel(const KernelArgs a) 
 
 // ---- S7 part 3: move every event's temp block to its place in event order ----------------------
 // One warp per event keeps the copies coalesced (tracks of an event are contiguous on both sides).
-__global__ void __launch_bounds__(256) velo_compact_kernel(const KernelArgs a) {
+// CTAs of 128 threads and at most 32 registers: they fit beside the persistent CTA of the team
+// kernel of another stream's batch (which leaves about 6 k registers per SM free), so the copy of
+// one batch overlaps the event kernel of the next.
+__global__ void __launch_bounds__(128, 8) velo_compact_kernel(const KernelArgs a) {
   const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t tot_t = a.event_track_offsets[a.n_events], tot_h = a.ws.ev_hit_base[a.n_events];
@@ -454,10 +457,10 @@ int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_
   if (ev_stop) cudaEventRecord(ev_stop, stream);
   velo_offsets_kernel<<<1, 1024, 0, stream>>>(a);
   if (a.n_events > 0) {
-    const uint32_t warps_per_cta = 256 / 32;
+    const uint32_t warps_per_cta = 128 / 32;
     uint32_t grid = (a.n_events + warps_per_cta - 1) / warps_per_cta;
-    if (grid > 148u * 8u) grid = 148u * 8u;
-    velo_compact_kernel<<<grid, 256, 0, stream>>>(a);
+    if (grid > num_sms() * 16u) grid = num_sms() * 16u;
+    velo_compact_kernel<<<grid, 128, 0, stream>>>(a);
   }
   return (int)cudaGetLastError();
 }
