@@ -32,7 +32,10 @@ namespace velo {
 
 namespace {
 
-constexpr int kTeamThreads = 128;
+#ifndef VELO_TEAM_THREADS
+#define VELO_TEAM_THREADS 128
+#endif
+constexpr int kTeamThreads = VELO_TEAM_THREADS;   // tuning builds may try 64 or 256
 constexpr int kTeamWarps = kTeamThreads / 32;
 constexpr uint32_t kUnitBytes = 4096;       // pool allocation unit
 constexpr uint32_t kPoolUnits = 54;         // 216 KB of pool + 8 KB of control = 224 KB per CTA
@@ -83,9 +86,21 @@ static_assert(sizeof(Control) <= kCtlBytes, "control block must fit its units");
 #else
 #define VELO_COUNT(i, v) do { } while (0)
 #endif
+// finer marks inside a phase (leader only): clocks since the previous VELO_SUB / VELO_SUB_START
+#define VELO_SUB_START() long long sub_last_ = clock64()
+#define VELO_SUB(i)                                                                    \
+  do {                                                                                 \
+    if (tid == 0) {                                                                    \
+      const long long now_ = clock64();                                                \
+      atomicAdd(&a.ws.phase_clk[i], (unsigned long long)(now_ - sub_last_));           \
+      sub_last_ = now_;                                                                \
+    }                                                                                  \
+  } while (0)
 #else
 #define VELO_PHASE(i) do { } while (0)
 #define VELO_COUNT(i, v) do { } while (0)
+#define VELO_SUB_START() do { } while (0)
+#define VELO_SUB(i) do { } while (0)
 #endif
 
 __device__ __forceinline__ void team_sync(uint32_t team) {
@@ -184,6 +199,21 @@ __device__ __forceinline__ Window make_window(const uint16_t* bo_m, uint32_t c, 
   return q;
 }
 __device__ __forceinline__ bool in_window(const Window& q, uint32_t wj) { return wj - q.lo16 <= q.lim; }
+
+// Visits the sorted indices [b, e) in ascending order, four per trip: the eight shared-memory
+// loads of a trip are issued before any of its arithmetic, so a trip costs one load latency
+// instead of four (the scans are latency-bound, not bandwidth-bound). f(j, w, xy, valid) must be
+// branch-free; for the padding lanes of the last trip valid is false and j repeats e - 1.
+template <class F>
+__device__ __forceinline__ void scan4(const Ev& ev, uint32_t b, uint32_t e, F&& f) {
+  for (uint32_t j = b; j < e; j += 4u) {
+    uint32_t jj[4], wj[4]; float2 pj[4];
+#pragma unroll
+    for (uint32_t k = 0; k < 4; ++k) { jj[k] = min(j + k, e - 1u); wj[k] = ev.w[jj[k]]; pj[k] = ev.xy[jj[k]]; }
+#pragma unroll
+    for (uint32_t k = 0; k < 4; ++k) f(jj[k], wj[k], pj[k], j + k < e);
+  }
+}
 
 // Calls f(i, h) for the hits h (sorted indices) of candidate t in discovery order, i = 0 .. n-1.
 // One 16-byte load per 8 hits from the team's row scratch.
@@ -451,6 +481,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   team_sync(team);
   for (uint32_t s = M - 2; s >= 1; --s) {
     const uint32_t u = s - 1, nxt = cur ^ 1u;
+    VELO_SUB_START();
     // (A) O-7 forwarding into module u of every track active at the start of the step
     {
       const uint32_t nact = ts.nact[cur];
@@ -471,22 +502,23 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
           const float2 p1 = ev.xy[hb], p0 = ev.xy[ha];
           const uint32_t c = ev.w[hb] >> 16;
           const float z1 = mz[mb], z0 = mz[ma];
+          VELO_SUB(24);   // list entry, track words, hit words
           const float tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0));
           const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
           const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
           const Window q = make_window(bo_u, c, P.phi_window_fwd);
+          VELO_SUB(25);   // prediction, window
           // branch-free visits (the loops are latency-bound: a taken branch costs more than the math)
           bool found = false; uint32_t best = 0; float best_sc = 0.0f;
-          auto visit = [&](uint32_t j) {
-            const uint32_t wj = ev.w[j];
-            const float2 p2 = ev.xy[j];
+          auto visit = [&](uint32_t j, uint32_t wj, float2 p2, bool valid) {
             const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
             const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-            const bool better = in_window(q, wj) & (sc <= max_fwd) & (!found | (sc < best_sc));
+            const bool better = valid & in_window(q, wj) & (sc <= max_fwd) & (!found | (sc < best_sc));
             found |= better; best = better ? j : best; best_sc = better ? sc : best_sc;
           };
-          for (uint32_t j = q.b0; j < q.e0; ++j) visit(j);
-          for (uint32_t j = q.b1; j < q.e1; ++j) visit(j);   // second run: only for a window across +-pi
+          scan4(ev, q.b0, q.e0, visit);
+          scan4(ev, q.b1, q.e1, visit);   // second run: only for a window across +-pi
+          VELO_SUB(26);   // visits
           VELO_COUNT(16, 1); VELO_COUNT(17, (q.e0 - q.b0) + (q.e1 - q.b1));
           if (found) {
             const uint32_t nh = ev.tn[t];
@@ -505,6 +537,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
             alive = miss <= P.max_skipped;
           }
         }
+        VELO_SUB(27);   // track update, flags
         const uint32_t ballot = __ballot_sync(0xffffffffu, alive);
         if (ballot) {
           uint32_t base = 0;
@@ -514,7 +547,9 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
         }
       }
     }
+    VELO_SUB(28);   // list append
     team_sync(team);
+    VELO_SUB(29);   // barrier
     VELO_PHASE(4);   // (A) forwarding
     if (tid == 0) { ts.nact[cur] = 0; ts.sstart[s] = ts.nt; }   // nact[cur] was read by everyone before the barrier
     // (C) O-8 seeding with centre module s, in chunks of 2 x 128 centre hits
@@ -567,16 +602,14 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
               const float px = __fadd_rn(p1.x, __fmul_rn(__fsub_rn(p1.x, p0.x), tz));
               const float py = __fadd_rn(p1.y, __fmul_rn(__fsub_rn(p1.y, p0.y), tz));
               // h0 and h2 ascending: strict < keeps this lane's lexicographic minimum; branch-free body
-              auto visit2 = [&](uint32_t h2) {
-                const uint32_t w2 = ev.w[h2];
-                const float2 p2 = ev.xy[h2];
+              auto visit2 = [&](uint32_t h2, uint32_t w2, float2 p2, bool valid) {
                 const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
                 const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-                const bool better = !(w2 & kFlagBit) & in_window(q2, w2) & (sc <= max_seed) & (!found | (sc < best_sc));
+                const bool better = valid & !(w2 & kFlagBit) & in_window(q2, w2) & (sc <= max_seed) & (!found | (sc < best_sc));
                 found |= better; b0 = better ? h0 : b0; b2 = better ? h2 : b2; best_sc = better ? sc : best_sc;
               };
-              for (uint32_t j = q2.b0; j < q2.e0; ++j) visit2(j);
-              for (uint32_t j = q2.b1; j < q2.e1; ++j) visit2(j);
+              scan4(ev, q2.b0, q2.e0, visit2);
+              scan4(ev, q2.b1, q2.e1, visit2);
             }
           }
 #pragma unroll
@@ -775,6 +808,9 @@ __global__ void __launch_bounds__(kTeams* kTeamThreads, 1) velo_event_team_kerne
 template <int kTeams>
 int launch_teams(const KernelArgs& a, cudaStream_t stream) {
   static_assert(kTeams <= (int)kMaxTeams && kTeams <= 15, "named barriers 1..15");
+  if constexpr (kTeams * kTeamThreads > 1024) {
+    return launch_teams<1024 / kTeamThreads>(a, stream);
+  } else {
   const uint32_t smem = kCtlBytes + kPoolUnits * kUnitBytes;
   static bool configured = false;   // per process; the attribute is sticky per function and device
   if (!configured) {
@@ -787,6 +823,7 @@ int launch_teams(const KernelArgs& a, cudaStream_t stream) {
   const uint32_t grid = want < sms ? (want ? want : 1u) : sms;
   velo_event_team_kernel<kTeams><<<grid, kTeams * kTeamThreads, smem, stream>>>(a);
   return (int)cudaGetLastError();
+  }
 }
 
 }  // namespace
@@ -801,6 +838,9 @@ int launch_event_smem(const KernelArgs& a, cudaStream_t stream, uint32_t teams) 
     teams = fit <= 5u ? 5u : (fit - 1u > kMaxTeams ? kMaxTeams : fit - 1u);
   }
   switch (teams) {
+    case 1: return launch_teams<1>(a, stream);
+    case 2: return launch_teams<2>(a, stream);
+    case 3: return launch_teams<3>(a, stream);
     case 4: return launch_teams<4>(a, stream);
     case 6: return launch_teams<6>(a, stream);
     case 7: return launch_teams<7>(a, stream);
