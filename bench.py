@@ -209,7 +209,7 @@ def run_velo(args):
     P = velo.velo_params_default(g)
     dh = velo.DeviceHits(d["x"], d["y"], d["z"], d["module"], off)
     opts0 = velo.LaunchOptions(ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams)
-    launches_per_batch = 3 if args.path == 1 else 4   # [team kernel,] slab kernel, offsets, compaction
+    launches_per_batch = 3 if args.path == 1 else 5   # [order, team kernel,] slab kernel, offsets, compaction
     streams = [torch.cuda.Stream() for _ in range(n_batches)]
     main = torch.cuda.current_stream()
     outs, hstructs = [], []
@@ -331,7 +331,7 @@ def run_velo(args):
         line["e2e"] = {"value": world * n_events / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s, "steps": e2e_steps,
                        "api": "velo_scheduler_run_host (pinned host buffers, %d streams)" % n_batches}
-        line["gpu_launches"] += 4 * n_batches * (e2e_steps + 1)
+        line["gpu_launches"] += 5 * n_batches * (e2e_steps + 1)
         sched.close()
 
     # -- the oracle on this box's host cores (rank 0, N=1 only): a baseline, not the target --

@@ -322,9 +322,12 @@ __device__ __forceinline__ void pool_free(Control& ctl, uint32_t first, uint32_t
 
 // Leader: take the next event and a pool block for it. ts.defer != 0 means "nothing to do here".
 __device__ void leader_fetch(const KernelArgs& a, Control& ctl, TeamShared& ts) {
-  const uint32_t e = atomicAdd(&a.ws.counters[kCtrTicket], 1u);
-  ts.event = e; ts.units = 0; ts.defer = 1; ts.n = 0;
-  if (e >= a.n_events) return;
+  const uint32_t k = atomicAdd(&a.ws.counters[kCtrTicket], 1u);
+  ts.event = k; ts.units = 0; ts.defer = 1; ts.n = 0;
+  if (k >= a.n_events) return;
+  // tickets walk the size-sorted list from both ends in turn: largest, smallest, second largest, ...
+  const uint32_t e = a.ws.order[(k & 1u) ? (k >> 1) : a.n_events - 1u - (k >> 1)];
+  ts.event = e;
   const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
   if (o1 < o0 || o1 - o0 > VELO_MAX_EVENT_HITS) {
     set_status(a.ws.counters, VELO_ERR_INPUT); a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); return;

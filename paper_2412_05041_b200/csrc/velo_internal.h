@@ -57,6 +57,7 @@ struct Workspace {
   uint4* ev_rec;          // n_events: {temp track base, temp hit base, n_tracks, n_track_hits}
   uint32_t* ev_hit_base;  // n_events+1: exclusive scan of n_track_hits over events
   uint32_t* large_list;   // n_events: events deferred to the slab path
+  uint32_t* order;        // n_events: event ids by ascending size class (velo_order_kernel)
   uint32_t* tmp_loff;     // cap_tracks: hit offset of a track inside its event's hit block
   uint32_t* tmp_hits;     // cap_track_hits
   float* tmp_states;      // VELO_N_STATE * cap_tracks

@@ -346,6 +346,45 @@ __global__ void __launch_bounds__(kThreads) velo_event_slab_kernel(const KernelA
   }
 }
 
+// ---- processing order for the team kernel: event ids by ascending size class --------------------
+// Events of a batch differ in size by more than 10x. The team kernel hands out the sorted list
+// from both ends in turn (largest, smallest, second largest, ...), so the handful of events that
+// share an SM's shared memory at any time add up to about the same bytes and the pool neither
+// overflows (teams waiting for memory) nor sits half empty. Counting sort by n_hits / 32, one CTA.
+// The order only schedules: results and their placement do not depend on it.
+constexpr uint32_t kSizeClasses = 512;
+__global__ void __launch_bounds__(1024) velo_order_kernel(const KernelArgs a) {
+  __shared__ uint32_t hist[kSizeClasses];
+  __shared__ uint32_t wsum[32];
+  const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;
+  for (uint32_t c = tid; c < kSizeClasses; c += nthr) hist[c] = 0;
+  __syncthreads();
+  auto size_class = [&](uint32_t e) {
+    const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
+    const uint32_t n = o1 >= o0 ? o1 - o0 : 0u;
+    return min(n >> 5, kSizeClasses - 1u);
+  };
+  for (uint32_t e = tid; e < ne; e += nthr) atomicAdd(&hist[size_class(e)], 1u);
+  __syncthreads();
+  // exclusive scan of the 512 counts by the first 512 threads
+  uint32_t v = tid < kSizeClasses ? hist[tid] : 0u, inc = v;
+  const uint32_t lane = tid & 31u, wid = tid >> 5;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= (uint32_t)d) inc += o; }
+  if (lane == 31) wsum[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t w = wsum[lane], wi = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= (uint32_t)d) wi += o; }
+    wsum[lane] = wi - w;
+  }
+  __syncthreads();
+  if (tid < kSizeClasses) hist[tid] = wsum[wid] + inc - v;
+  __syncthreads();
+  for (uint32_t e = tid; e < ne; e += nthr) a.ws.order[atomicAdd(&hist[size_class(e)], 1u)] = e;
+}
+
 // ---- S7 part 2: exclusive scans of the per-event counts (one CTA) ------------------------------
 __global__ void __launch_bounds__(1024) velo_offsets_kernel(const KernelArgs a) {
   __shared__ unsigned long long warp_sums[33];
@@ -429,6 +468,7 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, ui
   w.ev_rec = (uint4*)take(sizeof(uint4) * ((size_t)n_events + 1));
   w.ev_hit_base = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.large_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
+  w.order = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.tmp_loff = (uint32_t*)take(4 * ((size_t)cap_tracks + 1));
   w.tmp_hits = (uint32_t*)take(4 * ((size_t)cap_track_hits + 1));
   w.tmp_states = (float*)take(4 * (size_t)VELO_N_STATE * ((size_t)cap_tracks + 1));
@@ -449,6 +489,7 @@ int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_
     if (path == kPathSlabOnly) {
       velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a, 0);
     } else {
+      velo_order_kernel<<<1, 1024, 0, stream>>>(a);
       const int rc = launch_event_smem(a, stream, teams);
       if (rc != 0) return rc;
       velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a, 1);   // the deferred events, usually none
