@@ -110,6 +110,42 @@ def test_hits_off_their_module_plane_are_deferred_to_the_general_kernel(velo):
     check(got, cpu(d3))
 
 
+def test_events_the_team_kernel_gives_up_on_midway(velo):
+    """Deferral after work has started: (a) more candidates than the team path's table (n/8 + 32)
+    - an event made of short tracks only; (b) more than 2047 hits in one phi bucket; (c) a module
+    holding every hit. All three continue in the general kernel and must still equal the oracle."""
+    import oracle
+    rng = np.random.default_rng(11)
+    # (a) 120 three-hit tracks on modules 10, 11, 12, spread in phi: 360 hits, 120 candidates > 77
+    xs, ys, zs, ms = [], [], [], []
+    for k in range(120):
+        phi = 2 * np.pi * (k + 0.37) / 120
+        tx, ty = 0.08 * np.cos(phi), 0.08 * np.sin(phi)
+        for m in (10, 11, 12):
+            z = float(T.MODULE_Z[m])
+            xs.append(tx * z); ys.append(ty * z); zs.append(z); ms.append(m)
+    short = (np.array(xs, np.float32), np.array(ys, np.float32), np.array(zs, np.float32), np.array(ms, np.uint8))
+    # (b) 2500 hits of module 7 inside one phi bucket (plus a track elsewhere)
+    r = rng.uniform(6.0, 40.0, 2500); ph = rng.uniform(0.50, 0.52, 2500)
+    line = T.line_event([10, 11, 12, 13], tx=-0.1, ty=0.02)
+    dense = (np.concatenate([(r * np.cos(ph)).astype(np.float32), line[0]]),
+             np.concatenate([(r * np.sin(ph)).astype(np.float32), line[1]]),
+             np.concatenate([np.full(2500, T.MODULE_Z[7], np.float32), line[2]]),
+             np.concatenate([np.full(2500, 7, np.uint8), line[3]]))
+    # (c) 700 hits, all on module 3, all over phi
+    r = rng.uniform(6.0, 40.0, 700); ph = rng.uniform(-np.pi, np.pi, 700)
+    flat = ((r * np.cos(ph)).astype(np.float32), (r * np.sin(ph)).astype(np.float32),
+            np.full(700, T.MODULE_Z[3], np.float32), np.full(700, 3, np.uint8))
+    normal = T.line_event([10, 11, 12, 13, 14])
+    x, y, z, m, off = T.batch_of([normal, short, normal, dense, flat, normal])
+    got = velo.reconstruct(x, y, z, m, off, datagen.MODULE_Z)
+    want = oracle.reconstruct(x, y, z, m, off, M)
+    check(got, want)
+    assert got["n_deferred"] >= 2 and want["n_tracks"] >= 120 + 3 + 1
+    slab = velo.reconstruct(x, y, z, m, off, datagen.MODULE_Z, opts=velo.LaunchOptions(path=velo.VELO_PATH_SLAB_ONLY))
+    check(slab, want)
+
+
 @pytest.mark.parametrize("n_modules", [3, 4, 17, 32])
 def test_other_module_counts(velo, n_modules):
     import oracle
