@@ -29,7 +29,9 @@ if ROOT not in sys.path:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one event-kernel launch, from the ncu --set full
 # capture summarised in profiles/r01c_team_kernel_25k.md; key = (config, path, events per step)
-NCU_DRAM_BYTES_PER_LAUNCH = {(2, 0, 100_000): 674_186_240 + 504_429_312}
+NCU_DRAM_BYTES_PER_LAUNCH = {(2, 0, 100_000): 675_263_488 + 496_218_112}
+# smsp__inst_executed.sum of the same capture / its 25 000 events: what bounds the path in practice
+NCU_WARP_INST_PER_EVENT = {(2, 0): 95_249.0}
 
 METRIC = "velo_tracking_events_per_s"
 UNIT = "events/s"
@@ -113,6 +115,20 @@ class ClockSampler:
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
                 "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def issue_block(args, events_per_s: float, clocks: dict):
+    """The practical limiter beside the HBM roofline: warp instructions issued per second against
+    the issue peak of the chip (148 SMs x 4 schedulers x 1 warp instruction per clock at the SM
+    clock seen during the run). Instructions per event come from the ncu capture in profiles/."""
+    per_event = NCU_WARP_INST_PER_EVENT.get((args.config, args.path))
+    mhz = clocks.get("sm_mhz") or 1965.0
+    if per_event is None:
+        return None
+    peak = 148 * 4 * mhz * 1e6
+    return {"bound": "alu", "achieved": events_per_s * per_event / 1e9, "peak": peak / 1e9, "unit": "G warp instr/s",
+            "frac": events_per_s * per_event / peak, "warp_instructions_per_event": per_event,
+            "source": "profiles/r01c_team_kernel_25k.md"}
 
 
 def measured_peak_gbs() -> tuple[float, str]:
@@ -295,8 +311,9 @@ def run_velo(args):
                      "kernel_share_of_step": avg_kern_ms * n_batches / ms_step,
                      "step_achieved": step_gbs, "step_frac": step_gbs / peak,
                      "frac_of_nominal_8TBs": step_gbs / 8000.0,
-                     "limiter": "instruction issue and latency, not HBM (ncu: issue slots 48.5 % busy, DRAM 3 % busy, "
-                                "92.6 k warp instructions per event; see profiles/)"},
+                     "limiter": "instruction issue and latency, not HBM (ncu: issue slots 51.5 % busy, DRAM 3 % busy, "
+                                "95.2 k warp instructions per event; see profiles/ and DESIGN.md 5.1)"},
+        "issue": issue_block(args, world * n_events / (ms_step * 1e-3), clocks),
         "clocks": clocks,
         "gpu_launches": launches_per_batch * n_batches * (args.steps + args.warmup),
     }

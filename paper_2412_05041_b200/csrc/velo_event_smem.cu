@@ -37,9 +37,9 @@ namespace {
 #endif
 constexpr int kTeamThreads = VELO_TEAM_THREADS;   // tuning builds may try 64 or 256
 constexpr int kTeamWarps = kTeamThreads / 32;
-constexpr uint32_t kUnitBytes = 4096;       // pool allocation unit
-constexpr uint32_t kPoolUnits = 54;         // 216 KB of pool + 8 KB of control = 224 KB per CTA
-constexpr uint32_t kCtlBytes = 2 * kUnitBytes;
+constexpr uint32_t kUnitBytes = 3456;       // pool allocation unit: 64 of them (one bitmap word) make
+constexpr uint32_t kPoolUnits = 64;         //   216 KB of pool; + 8 KB of control = 224 KB per CTA
+constexpr uint32_t kCtlBytes = 8192;
 constexpr uint32_t kClChunk = 256;          // centre hits per seeding chunk (2 per thread)
 constexpr uint32_t kMaxTeams = kTeamsPerCtaMax;
 constexpr uint32_t kMaxTeamHits = kTeamMaxHits;   // <= 32767: the local original index is stored in 15 bits
@@ -295,7 +295,7 @@ __device__ __forceinline__ uint32_t pool_alloc(Control& ctl, uint32_t units) {
   volatile uint32_t* serving = &ctl.alloc_serving;
   while (*serving != my) __nanosleep(1500);
   volatile unsigned long long* bm = &ctl.bitmap;
-  const unsigned long long all = (1ull << kPoolUnits) - 1ull;
+  const unsigned long long all = kPoolUnits >= 64u ? ~0ull : (1ull << (kPoolUnits & 63u)) - 1ull;
   uint32_t first;
   unsigned long long seen = ~0ull;
   for (;;) {
