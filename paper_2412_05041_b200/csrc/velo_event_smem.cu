@@ -140,7 +140,7 @@ struct Layout {
   uint32_t bytes;
 };
 __device__ __forceinline__ uint32_t align16(uint32_t v) { return (v + 15u) & ~15u; }
-constexpr uint32_t kTrackBytes = 22;   // shared-memory bytes per candidate slot (see Ev)
+constexpr uint32_t kTrackBytes = 21;   // shared-memory bytes per candidate slot (see Ev)
 __device__ __forceinline__ Layout event_layout(uint32_t n, uint32_t M) {
   Layout L;
   uint32_t o = 0;
@@ -170,7 +170,7 @@ struct Ev {
   uint16_t* tcentre;     // sorted index of the seed's centre hit
   uint16_t* th0;         // the seed's first hit (row[0]); with tl it flags a track that reaches 4 hits
   uint16_t* act;         // two lists of tcap active-track ids; after the loop: order[] (creation order)
-  uint8_t *tn, *tmiss;   // hits on the track; consecutive misses; after the loop: pass state
+  uint8_t* tmiss;        // consecutive misses; after the loop: pass state (hits on a track = popc(tmask))
   uint32_t tcap;
   // per-team scratch in global memory (L2-resident)
   uint16_t* rows;        // rows[t * 32 + k] = k-th hit (sorted index) of candidate t
@@ -369,7 +369,6 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     ev.tcentre = (uint16_t*)q; q += 2u * T;
     ev.th0 = (uint16_t*)q; q += 2u * T;
     ev.act = (uint16_t*)q; q += 4u * T;
-    ev.tn = q; q += T;
     ev.tmiss = q;
   }
   ev.rows = (uint16_t*)scratch;
@@ -503,7 +502,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
           const uint32_t mask = ev.tmask[t];
           const uint32_t mb = __ffs(mask) - 1u, ma = __ffs(mask & (mask - 1u)) - 1u;
           const float2 p1 = ev.xy[hb], p0 = ev.xy[ha];
-          const uint32_t c = ev.w[hb] >> 16;
+          const uint32_t whb = ev.w[hb], c = whb >> 16;
           const float z1 = mz[mb], z0 = mz[ma];
           VELO_SUB(24);   // list entry, track words, hit words
           const float tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0));
@@ -512,27 +511,28 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
           const Window q = make_window(bo_u, c, P.phi_window_fwd);
           VELO_SUB(25);   // prediction, window
           // branch-free visits (the loops are latency-bound: a taken branch costs more than the math)
-          bool found = false; uint32_t best = 0; float best_sc = 0.0f;
+          bool found = false; uint32_t best = 0, best_w = 0; float best_sc = 0.0f;
           auto visit = [&](uint32_t j, uint32_t wj, float2 p2, bool valid) {
             const float ex = __fsub_rn(px, p2.x), ey = __fsub_rn(py, p2.y);
             const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
             const bool better = valid & in_window(q, wj) & (sc <= max_fwd) & (!found | (sc < best_sc));
-            found |= better; best = better ? j : best; best_sc = better ? sc : best_sc;
+            found |= better; best = better ? j : best; best_w = better ? wj : best_w; best_sc = better ? sc : best_sc;
           };
           scan4(ev, q.b0, q.e0, visit);
           scan4(ev, q.b1, q.e1, visit);   // second run: only for a window across +-pi
           VELO_SUB(26);   // visits
           VELO_COUNT(16, 1); VELO_COUNT(17, (q.e0 - q.b0) + (q.e1 - q.b1));
           if (found) {
-            const uint32_t nh = ev.tn[t];
+            const uint32_t nh = (uint32_t)__popc(mask);   // one hit per module: the mask counts them
             ev.rows[t * 32u + nh] = (uint16_t)best;
-            ev.tn[t] = (uint8_t)(nh + 1);
             ev.tmiss[t] = 0;
             ev.tl[t] = (hb << 16) | best;
             ev.tmask[t] = mask | (1u << u);
             // (B): forwarding never reads flags, so they can be set right away
-            if (nh + 1 == 4) { ev.w[ev.th0[t]] |= kFlagBit; ev.w[ha] |= kFlagBit; ev.w[hb] |= kFlagBit; }
-            if (nh + 1 >= 4) ev.w[best] |= kFlagBit;
+            // (the words of hb and best are in registers: the other bits of a hit word never change
+            // during the loop, so a plain store of word | flag is as good as a read-modify-write)
+            if (nh + 1 == 4) { ev.w[ev.th0[t]] |= kFlagBit; ev.w[ha] |= kFlagBit; ev.w[hb] = whb | kFlagBit; }
+            if (nh + 1 >= 4) ev.w[best] = best_w | kFlagBit;
             alive = true;
           } else {
             const uint32_t miss = (uint32_t)ev.tmiss[t] + 1u;
@@ -628,7 +628,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
             if (slot < T) {
               *reinterpret_cast<uint2*>(ev.rows + slot * 32u) = make_uint2(b0 | (h1 << 16), b2);
               ev.th0[slot] = (uint16_t)b0;
-              ev.tn[slot] = 3; ev.tmiss[slot] = 0;
+              ev.tmiss[slot] = 0;
               ev.tl[slot] = (h1 << 16) | b2;
               ev.tmask[slot] = 7u << u;
               ev.tseed[slot] = best_sc; ev.tcentre[slot] = (uint16_t)h1;
@@ -667,7 +667,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   // ---- O-10 ghost filter part 1 (reads the final flags); tmiss[t] becomes the pass state ---------
   for (uint32_t t = tid; t < nt; t += kTeamThreads) {
     bool pass = true;
-    if (ev.tn[t] == 3) {
+    if (__popc(ev.tmask[t]) == 3) {
       const uint32_t l = ev.tl[t];   // never extended: still (centre, third hit)
       const uint32_t f = ev.w[ev.th0[t]] | ev.w[l >> 16] | ev.w[l & 0xffffu];
       if ((f & kFlagBit) || !(ev.tseed[t] <= P.max_scatter_weak)) pass = false;
@@ -681,7 +681,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   const float inv_s2 = __fdiv_rn(1.0f, sig2);
   for (uint32_t t = tid; t < nt; t += kTeamThreads) {
     if (!ev.tmiss[t]) continue;
-    const uint32_t nh = ev.tn[t];
+    const uint32_t nh = (uint32_t)__popc(ev.tmask[t]);
     const uint32_t centre = ev.tcentre[t];
     float s9[9];
     fit_track(ev, mz, t, nh, ev.tmask[t], sig2, inv_s2, s9);
@@ -703,13 +703,13 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     uint16_t* own = reinterpret_cast<uint16_t*>(ev.w);   // own[2h + 1] = upper half of w[h]
     for (uint32_t t = tid; t < nt; t += kTeamThreads) {
       if (!ev.tmiss[t]) continue;
-      for_hits(ev, t, ev.tn[t], [&](uint32_t, uint32_t h) { own[2u * h + 1u] = (uint16_t)t; });
+      for_hits(ev, t, (uint32_t)__popc(ev.tmask[t]), [&](uint32_t, uint32_t h) { own[2u * h + 1u] = (uint16_t)t; });
     }
     team_sync(team);
     for (uint32_t t = tid; t < nt; t += kTeamThreads) {
       if (!ev.tmiss[t]) continue;
       const unsigned long long key = tkey[t];
-      for_hits(ev, t, ev.tn[t], [&](uint32_t, uint32_t h) {
+      for_hits(ev, t, (uint32_t)__popc(ev.tmask[t]), [&](uint32_t, uint32_t h) {
         uint32_t* wp = &ev.w[h];
         uint32_t old = *(volatile uint32_t*)wp;
         while ((old >> 16) != t && key < tkey[old >> 16]) {
@@ -731,7 +731,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
     const uint32_t t = k < nt ? order[k] : 0u;   // the k-th candidate in creation order
     uint32_t nh = 0, surv = 0;
     if (k < nt && ev.tmiss[t]) {
-      nh = ev.tn[t];
+      nh = (uint32_t)__popc(ev.tmask[t]);
       uint32_t lost = 0;
       for_hits(ev, t, nh, [&](uint32_t, uint32_t h) { lost += ((ev.w[h] >> 16) != t) ? 1u : 0u; });
       surv = !((unsigned long long)lost * P.clone_den > (unsigned long long)nh * P.clone_num) ? 1u : 0u;
@@ -760,7 +760,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   const bool staged = ev_nh <= 2u * n;
   for (uint32_t t = tid; t < nt; t += kTeamThreads) {
     if (ev.tmiss[t] != 2) continue;
-    const uint32_t nh = ev.tn[t], lt = pl[t], lh = ph[t];
+    const uint32_t nh = (uint32_t)__popc(ev.tmask[t]), lt = pl[t], lh = ph[t];
     float s9[9];
 #pragma unroll
     for (uint32_t k = 0; k < 9; ++k) s9[k] = ev.st[k * kTeamMaxTracks + t];
