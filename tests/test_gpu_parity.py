@@ -303,3 +303,65 @@ def test_full_size_sampled_events(velo, config):
     mod = d["module"][th].astype(np.int64)
     same_track = np.ones(th.shape[0] - 1, bool); same_track[tho[1:-1] - 1] = False
     assert (np.diff(mod)[same_track] < 0).all()                              # decreasing module order
+
+
+# ---- the end-to-end call over host buffers: velo_scheduler_run_host (S8) --------------------------
+def _run_scheduler(velo, d, cuts, n_streams, pinned=True):
+    import torch
+    g = velo.velo_geometry_load(datagen.MODULE_Z)
+    P = velo.velo_params_default(g)
+    off = d["event_offsets"]
+    sizes = [(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]])) for b in range(len(cuts) - 1)]
+    sched = velo.Scheduler(g, n_streams, max(1, max(s[0] for s in sizes)), max(s[1] for s in sizes))
+    outs = [velo.HostTracks(ne, nh, pinned=pinned) for ne, nh in sizes]
+    sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off, cuts, outs)
+    torch.cuda.synchronize()
+    res = velo.stitch([o.result() for o in outs])
+    sched.close()
+    return res
+
+
+def test_scheduler_host_buffers_equal_oracle(velo):
+    d = datagen.generate_config(1, n_events=611)
+    want = cpu(d)
+    # ragged batches, more batches than streams (every lane is reused), one empty batch
+    cuts = [0, 100, 100, 333, 334, 500, 611]
+    for n_streams, pinned in ((2, True), (4, False), (1, True)):
+        got = _run_scheduler(velo, d, cuts, n_streams, pinned)
+        info = check(got, want)
+        assert info["bit_identical_states"]
+        np.testing.assert_array_equal(got["track_hits"], want["track_hits"])
+
+
+def test_scheduler_reports_an_oversized_batch(velo):
+    import torch
+    d = datagen.generate_config(0, n_events=20)
+    g = velo.velo_geometry_load(datagen.MODULE_Z)
+    P = velo.velo_params_default(g)
+    off = d["event_offsets"]
+    sched = velo.Scheduler(g, 2, 10, int(off[10]))          # sized for the first ten events only
+    outs = [velo.HostTracks(10, int(off[10])), velo.HostTracks(10, int(off[20]) - int(off[10]))]
+    sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off, [0, 10, 20], outs)
+    torch.cuda.synchronize()
+    first = outs[0].result()
+    assert first["n_tracks"] > 0
+    if int(off[20]) - int(off[10]) > int(off[10]):          # the second batch has more hits than the lanes hold
+        with pytest.raises(velo.VeloError) as e:
+            outs[1].result()
+        assert e.value.code == velo.VELO_ERR_CAPACITY
+    sched.close()
+
+
+def test_config4_full_size_sampled_events(velo):
+    """BASELINE.json:configs[4] at full size (2 000 ion-like events, one call): sampled events
+    against the oracle, among them the largest (general kernel) and mid-sized ones (team kernel)."""
+    d = datagen.generate_config(4)
+    got = gpu(velo, d)
+    nh = np.diff(d["event_offsets"].astype(np.int64))
+    rng = np.random.default_rng(5)
+    order = np.argsort(nh)
+    ids = np.unique(np.concatenate([rng.integers(0, d["n_events"], 40), order[-3:], order[:3],
+                                    order[np.searchsorted(nh[order], [9000, 12000, 13000, 14000])]]))
+    sub = T.gather_events(d, ids)
+    check(T.select_events(got, d, ids), cpu(sub))
+    assert 0 < got["n_deferred"] < d["n_events"]
