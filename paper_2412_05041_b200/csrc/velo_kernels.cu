@@ -14,7 +14,9 @@ namespace velo {
 
 namespace {
 
-constexpr int kThreads = 256;            // CTA size of the event kernel
+constexpr int kThreads = 256;            // CTA size of the slab kernel when it takes every event of a batch
+constexpr int kThreadsLarge = 1024;      // ... and when it takes the events the team kernel deferred: those are
+                                         // the large ones, and a batch waits for the latency of its largest event
 constexpr unsigned kInactive = 255u;     // tmiss value of a track that stopped forwarding
 
 // Per-event arrays (sorted-hit order) and the candidate-track table. The pointers address either
@@ -322,7 +324,8 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
 
 // ---- event kernel, slab variant: persistent CTAs pull events from a ticket counter -------------
 // from_list = 0: every event of the batch; 1: the events the shared-memory kernel deferred (ws.large_list).
-__global__ void __launch_bounds__(kThreads) velo_event_slab_kernel(const KernelArgs a, const int from_list) {
+template <int kCta>
+__global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs a, const int from_list) {
   __shared__ Shared sh;
   const SlabLayout L = slab_layout();
   unsigned char* slab = a.ws.slabs + (size_t)blockIdx.x * L.bytes;
@@ -499,12 +502,12 @@ int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_
   if (a.n_events > 0) {
     const uint32_t grid = a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events;
     if (path == kPathSlabOnly) {
-      velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a, 0);
+      velo_event_slab_kernel<kThreads><<<grid, kThreads, 0, stream>>>(a, 0);
     } else {
       velo_order_kernel<<<1, 1024, 0, stream>>>(a);
       const int rc = launch_event_smem(a, stream, teams);
       if (rc != 0) return rc;
-      velo_event_slab_kernel<<<grid, kThreads, 0, stream>>>(a, 1);   // the deferred events, usually none
+      velo_event_slab_kernel<kThreadsLarge><<<grid, kThreadsLarge, 0, stream>>>(a, 1);   // the deferred events, usually none
     }
   }
   if (ev_stop) cudaEventRecord(ev_stop, stream);
