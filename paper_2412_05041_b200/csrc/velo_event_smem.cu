@@ -782,8 +782,13 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
 }
 
 // ---- the kernel: one CTA per SM, kTeams teams, events by ticket ---------------------------------
+// The launch bound is one team more than the CTA has: it caps the registers (80 for 5 teams) so
+// that about 14 k registers per SM stay free and the small kernels around the event kernel (order,
+// deferred-event list, offsets, compaction) of the neighbouring batches run beside it instead of
+// waiting for a whole SM.
 template <int kTeams>
-__global__ void __launch_bounds__(kTeams* kTeamThreads, 1) velo_event_team_kernel(const KernelArgs a) {
+__global__ void __launch_bounds__((kTeams + 1) * kTeamThreads > 1024 ? 1024 : (kTeams + 1) * kTeamThreads, 1)
+    velo_event_team_kernel(const KernelArgs a) {
   extern __shared__ __align__(16) unsigned char smem[];
   Control& ctl = *reinterpret_cast<Control*>(smem);
   unsigned char* pool = smem + kCtlBytes;

@@ -22,6 +22,7 @@ constexpr uint32_t kSlabHits = 65536;  // >= VELO_MAX_EVENT_HITS, and a multiple
 struct SlabLayout {                    // byte offsets inside a slab
   size_t sx, sy, sz, phi, perm, flag, owner, stash, tmp;            // per sorted hit
   size_t th, tn, tmiss, tcentre, tseed, tkey, tpass;                // per candidate track
+  size_t bins;                                                      // phi-bucket table (when not in shared memory)
   size_t bytes;
 };
 __host__ __device__ inline SlabLayout slab_layout() {
@@ -33,6 +34,7 @@ __host__ __device__ inline SlabLayout slab_layout() {
   L.owner = take(8); L.stash = take(4); L.tmp = take(4);
   L.th = take(2 * VELO_MAX_MODULES); L.tn = take(1); L.tmiss = take(1); L.tcentre = take(2);
   L.tseed = take(4); L.tkey = take(8); L.tpass = take(1);
+  L.bins = o; o += ((sizeof(uint32_t) * (kMaxBins + 1) + 255) / 256) * 256;
   L.bytes = o;
   return L;
 }

@@ -38,7 +38,6 @@ struct Ev {
 };
 
 struct Shared {
-  uint32_t binoff[kMaxBins + 1];      // histogram, then exclusive offsets of the phi buckets
   unsigned long long warp_sums[33];
   uint32_t mod_off[VELO_MAX_MODULES + 1];
   uint32_t ticket, bad, ntracks, tbase, hbase;
@@ -118,7 +117,9 @@ __device__ __forceinline__ void set_status(uint32_t* counters, int code) {
 }
 
 // Reconstructs event e with the CTA's arrays `ev`. Called by all threads of the CTA.
-__device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uint32_t e) {
+// binoff: histogram, then exclusive offsets of the phi buckets (kMaxBins + 1 words, in shared memory
+// or in the CTA's slab).
+__device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uint32_t* binoff, uint32_t e) {
   const uint32_t tid = threadIdx.x, nthr = blockDim.x;
   const uint32_t M = a.n_modules;
   const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
@@ -135,14 +136,14 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
   const uint8_t* gm = a.module + o0;
 
   // ---- S0 decode: phi16 and bucket histogram (O-1) ---------------------------------------------
-  for (uint32_t b = tid; b <= nbins; b += nthr) sh.binoff[b] = 0;
+  for (uint32_t b = tid; b <= nbins; b += nthr) binoff[b] = 0;
   if (tid == 0) { sh.bad = 0; sh.ntracks = 0; }
   __syncthreads();
   for (uint32_t i = tid; i < n; i += nthr) {
     const uint32_t m = gm[i];
     if (m >= M) { sh.bad = 1; continue; }
     const uint32_t pu = (uint32_t)(phi16(gx[i], gy[i]) + 32768);
-    const uint32_t slot = atomicAdd(&sh.binoff[m * kBinsPerModule + (pu >> kBinShift)], 1u);
+    const uint32_t slot = atomicAdd(&binoff[m * kBinsPerModule + (pu >> kBinShift)], 1u);
     ev.stash[i] = (pu << 16) | slot;
   }
   __syncthreads();
@@ -156,27 +157,27 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
     const uint32_t per = (nbins + nthr - 1) / nthr;
     const uint32_t b0 = tid * per, b1 = min(b0 + per, nbins);
     uint32_t s = 0;
-    for (uint32_t b = b0; b < b1; ++b) s += sh.binoff[b];
+    for (uint32_t b = b0; b < b1; ++b) s += binoff[b];
     unsigned long long tot;
     uint32_t run = (uint32_t)block_scan_excl(s, sh.warp_sums, &tot);
-    for (uint32_t b = b0; b < b1; ++b) { const uint32_t c = sh.binoff[b]; sh.binoff[b] = run; run += c; }
-    if (tid == 0) sh.binoff[nbins] = n;
+    for (uint32_t b = b0; b < b1; ++b) { const uint32_t c = binoff[b]; binoff[b] = run; run += c; }
+    if (tid == 0) binoff[nbins] = n;
   }
   __syncthreads();
-  for (uint32_t m = tid; m <= M; m += nthr) sh.mod_off[m] = sh.binoff[m * kBinsPerModule];
+  for (uint32_t m = tid; m <= M; m += nthr) sh.mod_off[m] = binoff[m * kBinsPerModule];
 
   // ---- S1 phi sort (O-2): group by bucket, then rank inside the bucket by (phi16, index) -------
   for (uint32_t i = tid; i < n; i += nthr) {
     const uint32_t st = ev.stash[i], pu = st >> 16;
     const uint32_t bin = (uint32_t)gm[i] * kBinsPerModule + (pu >> kBinShift);
-    ev.tmp[sh.binoff[bin] + (st & 0xffffu)] = (pu << 16) | i;
+    ev.tmp[binoff[bin] + (st & 0xffffu)] = (pu << 16) | i;
   }
   __syncthreads();
   for (uint32_t i = tid; i < n; i += nthr) {
     const uint32_t pu = ev.stash[i] >> 16;
     const uint32_t bin = (uint32_t)gm[i] * kBinsPerModule + (pu >> kBinShift);
     const uint32_t item = (pu << 16) | i;
-    const uint32_t lo = sh.binoff[bin], hi = sh.binoff[bin + 1];
+    const uint32_t lo = binoff[bin], hi = binoff[bin + 1];
     uint32_t r = lo;
     for (uint32_t j = lo; j < hi; ++j) r += (ev.tmp[j] < item) ? 1u : 0u;
     ev.sx[r] = gx[i]; ev.sy[r] = gy[i]; ev.sz[r] = gz[i];
@@ -200,7 +201,7 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
       const float x1 = ev.sx[hb], y1 = ev.sy[hb], z1 = ev.sz[hb];
       const float dx = __fsub_rn(x1, ev.sx[ha]), dy = __fsub_rn(y1, ev.sy[ha]), dz = __fsub_rn(z1, ev.sz[ha]);
       bool found = false; uint32_t best = 0; float best_sc = 0.0f;
-      for_window(ev, sh.binoff, (int)u, (int)ev.phi[hb], P.phi_window_fwd, [&](uint32_t c) {
+      for_window(ev, binoff, (int)u, (int)ev.phi[hb], P.phi_window_fwd, [&](uint32_t c) {
         const float sc = scatter(dx, dy, dz, x1, y1, z1, ev.sx[c], ev.sy[c], ev.sz[c]);
         if (sc <= P.max_scatter_fwd && (!found || sc < best_sc)) { found = true; best = c; best_sc = sc; }
       });
@@ -223,10 +224,10 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
       if (h1 < c_end && !ev.flag[h1]) {
         const float x1 = ev.sx[h1], y1 = ev.sy[h1], z1 = ev.sz[h1];
         const int c = (int)ev.phi[h1];
-        for_window(ev, sh.binoff, (int)s + 1, c, P.phi_window_seed, [&](uint32_t h0) {
+        for_window(ev, binoff, (int)s + 1, c, P.phi_window_seed, [&](uint32_t h0) {
           if (ev.flag[h0]) return;
           const float dx = __fsub_rn(x1, ev.sx[h0]), dy = __fsub_rn(y1, ev.sy[h0]), dz = __fsub_rn(z1, ev.sz[h0]);
-          for_window(ev, sh.binoff, (int)s - 1, c, P.phi_window_seed, [&](uint32_t h2) {
+          for_window(ev, binoff, (int)s - 1, c, P.phi_window_seed, [&](uint32_t h2) {
             if (ev.flag[h2]) return;
             const float sc = scatter(dx, dy, dz, x1, y1, z1, ev.sx[h2], ev.sy[h2], ev.sz[h2]);
             if (sc <= P.max_scatter_seed && (!found || sc < best_sc)) { found = true; b0 = h0; b2 = h2; best_sc = sc; }
@@ -324,9 +325,12 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
 
 // ---- event kernel, slab variant: persistent CTAs pull events from a ticket counter -------------
 // from_list = 0: every event of the batch; 1: the events the shared-memory kernel deferred (ws.large_list).
-template <int kCta>
+// kBinsInSlab: the bucket table lives in the slab too, so that the CTA needs almost no shared memory
+// and fits beside the team kernel of the next batch (the usual case: nothing was deferred).
+template <int kCta, bool kBinsInSlab>
 __global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs a, const int from_list) {
   __shared__ Shared sh;
+  __shared__ uint32_t bins_smem[kBinsInSlab ? 1 : kMaxBins + 1];
   const SlabLayout L = slab_layout();
   unsigned char* slab = a.ws.slabs + (size_t)blockIdx.x * L.bytes;
   Ev ev;
@@ -345,7 +349,7 @@ __global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs 
     const uint32_t k = sh.ticket;
     __syncthreads();
     if (k >= limit) break;
-    process_event(a, ev, sh, from_list ? a.ws.large_list[k] : k);
+    process_event(a, ev, sh, kBinsInSlab ? (uint32_t*)(slab + L.bins) : bins_smem, from_list ? a.ws.large_list[k] : k);
   }
 }
 
@@ -353,19 +357,20 @@ __global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs 
 // Events of a batch differ in size by more than 10x. The team kernel hands out the sorted list
 // from both ends in turn (largest, smallest, second largest, ...), so the handful of events that
 // share an SM's shared memory at any time add up to about the same bytes and the pool neither
-// overflows (teams waiting for memory) nor sits half empty. Counting sort by n_hits / 32, one CTA.
+// overflows (teams waiting for memory) nor sits half empty. Counting sort by n_hits / 64, one CTA.
 // The order only schedules: results and their placement do not depend on it.
-constexpr uint32_t kSizeClasses = 512;
-__global__ void __launch_bounds__(1024) velo_order_kernel(const KernelArgs a) {
+constexpr uint32_t kSizeClasses = 256;   // with the scan scratch: 1.2 KB of shared memory, it fits beside the team kernel
+__global__ void __launch_bounds__(512) velo_order_kernel(const KernelArgs a) {
   __shared__ uint32_t hist[kSizeClasses];
   __shared__ uint32_t wsum[32];
   const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;
   for (uint32_t c = tid; c < kSizeClasses; c += nthr) hist[c] = 0;
+  if (tid < 32) wsum[tid] = 0;
   __syncthreads();
   auto size_class = [&](uint32_t e) {
     const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
     const uint32_t n = o1 >= o0 ? o1 - o0 : 0u;
-    return min(n >> 5, kSizeClasses - 1u);
+    return min(n >> 6, kSizeClasses - 1u);
   };
   for (uint32_t e = tid; e < ne; e += nthr) atomicAdd(&hist[size_class(e)], 1u);
   __syncthreads();
@@ -389,16 +394,19 @@ __global__ void __launch_bounds__(1024) velo_order_kernel(const KernelArgs a) {
 }
 
 // ---- S7 part 2: exclusive scans of the per-event counts (one CTA) ------------------------------
-__global__ void __launch_bounds__(1024) velo_offsets_kernel(const KernelArgs a) {
+// 256 threads and few registers: it fits beside the team kernel of the next batch.
+__global__ void __launch_bounds__(256) velo_offsets_kernel(const KernelArgs a) {
   __shared__ unsigned long long warp_sums[33];
   const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;
   const uint32_t per = (ne + nthr - 1) / nthr;
   const uint32_t e0 = min(tid * per, ne), e1 = min(e0 + per, ne);
   unsigned long long s = 0;
+#pragma unroll 8
   for (uint32_t e = e0; e < e1; ++e) { const uint4 r = a.ws.ev_rec[e]; s += ((unsigned long long)r.w << 32) | r.z; }
   unsigned long long tot;
   unsigned long long run = block_scan_excl(s, warp_sums, &tot);
   const uint32_t n_tracks = (uint32_t)(tot & 0xffffffffu), n_hits = (uint32_t)(tot >> 32);
+#pragma unroll 8
   for (uint32_t e = e0; e < e1; ++e) {
     const uint4 r = a.ws.ev_rec[e];
     a.event_track_offsets[e] = (uint32_t)(run & 0xffffffffu);
@@ -502,16 +510,19 @@ int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_
   if (a.n_events > 0) {
     const uint32_t grid = a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events;
     if (path == kPathSlabOnly) {
-      velo_event_slab_kernel<kThreads><<<grid, kThreads, 0, stream>>>(a, 0);
+      velo_event_slab_kernel<kThreads, false><<<grid, kThreads, 0, stream>>>(a, 0);
     } else {
-      velo_order_kernel<<<1, 1024, 0, stream>>>(a);
+      velo_order_kernel<<<1, 512, 0, stream>>>(a);
       const int rc = launch_event_smem(a, stream, teams);
       if (rc != 0) return rc;
-      velo_event_slab_kernel<kThreadsLarge><<<grid, kThreadsLarge, 0, stream>>>(a, 1);   // the deferred events, usually none
+      // the deferred events: usually none (then the small CTAs come and go beside the next batch's
+      // team kernel); for batches of large events, large CTAs: such a batch waits for its largest event
+      if (a.n_hits / a.n_events >= 4096u) velo_event_slab_kernel<kThreadsLarge, false><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
+      else velo_event_slab_kernel<kThreads, true><<<grid, kThreads, 0, stream>>>(a, 1);
     }
   }
   if (ev_stop) cudaEventRecord(ev_stop, stream);
-  velo_offsets_kernel<<<1, 1024, 0, stream>>>(a);
+  velo_offsets_kernel<<<1, 256, 0, stream>>>(a);
   if (a.n_events > 0) {
     const uint32_t warps_per_cta = 128 / 32;
     uint32_t grid = (a.n_events + warps_per_cta - 1) / warps_per_cta;
