@@ -141,7 +141,8 @@ int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const ve
  * path: VELO_PATH_DEFAULT = the shared-memory team kernel, with the general slab kernel for the
  * events it defers (hits off their module plane, events too large for one SM's shared memory);
  * VELO_PATH_SLAB_ONLY = the general slab kernel for every event. Both give identical results.
- * teams_per_cta: teams of 128 threads per persistent CTA of the team kernel (4 ... 8), 0 = default.
+ * teams_per_cta: teams of 128 threads per persistent CTA of the team kernel (1 ... 8), 0 = default
+ * (as many as mean-sized events of the batch fit one SM's shared memory: 5 at mu = 5).
  * ctas_per_sm: persistent CTAs per SM of the slab kernel, 0 = library default; the workspace must
  * have been sized for the default or for velo_workspace_bytes_opts with the same value. */
 enum { VELO_PATH_DEFAULT = 0, VELO_PATH_SLAB_ONLY = 1 };

@@ -10,7 +10,7 @@
 // in flight per SM and hide each other's shared-memory and barrier latency.
 //
 // Shared memory holds what the module loop touches at random: 12 bytes per hit (x, y, one packed
-// word), the phi-bucket table and 22 bytes per candidate track. The candidates' hit lists (written
+// word), the phi-bucket table and 21 bytes per candidate track. The candidates' hit lists (written
 // once per appended hit, read back only after the loop) and fitted states live in a per-team
 // scratch in global memory that stays L2-resident. Smaller blocks = more events in flight per SM,
 // and events in flight are what hides the latency of the 24 dependent, barrier-separated steps.
