@@ -478,7 +478,7 @@ uint32_t num_sms() {
   return n;
 }
 
-uint32_t default_n_slabs() { return num_sms() * 4u; }
+uint32_t default_n_slabs() { return num_sms() * 2u; }   // two 1024-thread CTAs of the general kernel fit an SM
 
 Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, uint32_t cap_track_hits,
                           uint32_t n_slabs) {
