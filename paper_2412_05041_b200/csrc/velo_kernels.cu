@@ -44,18 +44,18 @@ struct Shared {
 };
 
 // Visits, in ascending sorted index, every hit j of module m with |int16(phi[j] - c)| <= W (O-3).
-template <class F>
+template <int kShift, class F>
 __device__ __forceinline__ void for_window(const Ev& ev, const uint32_t* binoff, int m, int c, int W, F&& f) {
   if (W < 0) return;
-  const uint32_t* bo = binoff + m * kBinsPerModule;
+  const uint32_t* bo = binoff + m * (65536 >> kShift);
   if (2 * (long long)W + 1 >= 65536) {
-    for (uint32_t j = bo[0]; j < bo[kBinsPerModule]; ++j) f(j);
+    for (uint32_t j = bo[0]; j < bo[(65536 >> kShift)]; ++j) f(j);
     return;
   }
   const int lo = c + 32768 - W, hi = c + 32768 + W;  // unsigned-phi interval, may leave [0, 65535]
   auto seg = [&](int a, int b) {
-    const uint32_t j1 = bo[(b >> kBinShift) + 1];
-    for (uint32_t j = bo[a >> kBinShift]; j < j1; ++j) {
+    const uint32_t j1 = bo[(b >> kShift) + 1];
+    for (uint32_t j = bo[a >> kShift]; j < j1; ++j) {
       const int pu = (int)ev.phi[j] + 32768;
       if (pu >= a && pu <= b) f(j);
     }
@@ -119,11 +119,15 @@ __device__ __forceinline__ void set_status(uint32_t* counters, int code) {
 // Reconstructs event e with the CTA's arrays `ev`. Called by all threads of the CTA.
 // binoff: histogram, then exclusive offsets of the phi buckets (kMaxBins + 1 words, in shared memory
 // or in the CTA's slab).
+// kShift: phi units per bucket = 1 << kShift (1024 for ordinary events; 256 for batches of large
+// events, whose buckets would otherwise hold ~50 hits each and every window scan ~100).
+template <int kShift>
 __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uint32_t* binoff, uint32_t e) {
+  constexpr uint32_t kBins = 65536u >> kShift;   // buckets per module
   const uint32_t tid = threadIdx.x, nthr = blockDim.x;
   const uint32_t M = a.n_modules;
   const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
-  const uint32_t nbins = M * kBinsPerModule;
+  const uint32_t nbins = M * kBins;
   const velo_params_t& P = a.P;
 
   // ---- input checks (VELO_ERR_INPUT): the event then contributes zero tracks -------------------
@@ -143,7 +147,7 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
     const uint32_t m = gm[i];
     if (m >= M) { sh.bad = 1; continue; }
     const uint32_t pu = (uint32_t)(phi16(gx[i], gy[i]) + 32768);
-    const uint32_t slot = atomicAdd(&binoff[m * kBinsPerModule + (pu >> kBinShift)], 1u);
+    const uint32_t slot = atomicAdd(&binoff[m * kBins + (pu >> kShift)], 1u);
     ev.stash[i] = (pu << 16) | slot;
   }
   __syncthreads();
@@ -164,18 +168,18 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
     if (tid == 0) binoff[nbins] = n;
   }
   __syncthreads();
-  for (uint32_t m = tid; m <= M; m += nthr) sh.mod_off[m] = binoff[m * kBinsPerModule];
+  for (uint32_t m = tid; m <= M; m += nthr) sh.mod_off[m] = binoff[m * kBins];
 
   // ---- S1 phi sort (O-2): group by bucket, then rank inside the bucket by (phi16, index) -------
   for (uint32_t i = tid; i < n; i += nthr) {
     const uint32_t st = ev.stash[i], pu = st >> 16;
-    const uint32_t bin = (uint32_t)gm[i] * kBinsPerModule + (pu >> kBinShift);
+    const uint32_t bin = (uint32_t)gm[i] * kBins + (pu >> kShift);
     ev.tmp[binoff[bin] + (st & 0xffffu)] = (pu << 16) | i;
   }
   __syncthreads();
   for (uint32_t i = tid; i < n; i += nthr) {
     const uint32_t pu = ev.stash[i] >> 16;
-    const uint32_t bin = (uint32_t)gm[i] * kBinsPerModule + (pu >> kBinShift);
+    const uint32_t bin = (uint32_t)gm[i] * kBins + (pu >> kShift);
     const uint32_t item = (pu << 16) | i;
     const uint32_t lo = binoff[bin], hi = binoff[bin + 1];
     uint32_t r = lo;
@@ -201,7 +205,7 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
       const float x1 = ev.sx[hb], y1 = ev.sy[hb], z1 = ev.sz[hb];
       const float dx = __fsub_rn(x1, ev.sx[ha]), dy = __fsub_rn(y1, ev.sy[ha]), dz = __fsub_rn(z1, ev.sz[ha]);
       bool found = false; uint32_t best = 0; float best_sc = 0.0f;
-      for_window(ev, binoff, (int)u, (int)ev.phi[hb], P.phi_window_fwd, [&](uint32_t c) {
+      for_window<kShift>(ev, binoff, (int)u, (int)ev.phi[hb], P.phi_window_fwd, [&](uint32_t c) {
         const float sc = scatter(dx, dy, dz, x1, y1, z1, ev.sx[c], ev.sy[c], ev.sz[c]);
         if (sc <= P.max_scatter_fwd && (!found || sc < best_sc)) { found = true; best = c; best_sc = sc; }
       });
@@ -224,10 +228,10 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
       if (h1 < c_end && !ev.flag[h1]) {
         const float x1 = ev.sx[h1], y1 = ev.sy[h1], z1 = ev.sz[h1];
         const int c = (int)ev.phi[h1];
-        for_window(ev, binoff, (int)s + 1, c, P.phi_window_seed, [&](uint32_t h0) {
+        for_window<kShift>(ev, binoff, (int)s + 1, c, P.phi_window_seed, [&](uint32_t h0) {
           if (ev.flag[h0]) return;
           const float dx = __fsub_rn(x1, ev.sx[h0]), dy = __fsub_rn(y1, ev.sy[h0]), dz = __fsub_rn(z1, ev.sz[h0]);
-          for_window(ev, binoff, (int)s - 1, c, P.phi_window_seed, [&](uint32_t h2) {
+          for_window<kShift>(ev, binoff, (int)s - 1, c, P.phi_window_seed, [&](uint32_t h2) {
             if (ev.flag[h2]) return;
             const float sc = scatter(dx, dy, dz, x1, y1, z1, ev.sx[h2], ev.sy[h2], ev.sz[h2]);
             if (sc <= P.max_scatter_seed && (!found || sc < best_sc)) { found = true; b0 = h0; b2 = h2; best_sc = sc; }
@@ -327,10 +331,11 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
 // from_list = 0: every event of the batch; 1: the events the shared-memory kernel deferred (ws.large_list).
 // kBinsInSlab: the bucket table lives in the slab too, so that the CTA needs almost no shared memory
 // and fits beside the team kernel of the next batch (the usual case: nothing was deferred).
-template <int kCta, bool kBinsInSlab>
+template <int kCta, bool kBinsInSlab, int kShift>
 __global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs a, const int from_list) {
+  static_assert(!kBinsInSlab || kShift == kBinShift, "the slab's bucket table is sized for the default buckets");
   __shared__ Shared sh;
-  __shared__ uint32_t bins_smem[kBinsInSlab ? 1 : kMaxBins + 1];
+  __shared__ uint32_t bins_smem[kBinsInSlab ? 1 : VELO_MAX_MODULES * (65536 >> kShift) + 1];
   const SlabLayout L = slab_layout();
   unsigned char* slab = a.ws.slabs + (size_t)blockIdx.x * L.bytes;
   Ev ev;
@@ -349,7 +354,7 @@ __global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs 
     const uint32_t k = sh.ticket;
     __syncthreads();
     if (k >= limit) break;
-    process_event(a, ev, sh, kBinsInSlab ? (uint32_t*)(slab + L.bins) : bins_smem, from_list ? a.ws.large_list[k] : k);
+    process_event<kShift>(a, ev, sh, kBinsInSlab ? (uint32_t*)(slab + L.bins) : bins_smem, from_list ? a.ws.large_list[k] : k);
   }
 }
 
@@ -510,15 +515,15 @@ int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_
   if (a.n_events > 0) {
     const uint32_t grid = a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events;
     if (path == kPathSlabOnly) {
-      velo_event_slab_kernel<kThreads, false><<<grid, kThreads, 0, stream>>>(a, 0);
+      velo_event_slab_kernel<kThreads, false, kBinShift><<<grid, kThreads, 0, stream>>>(a, 0);
     } else {
       velo_order_kernel<<<1, 512, 0, stream>>>(a);
       const int rc = launch_event_smem(a, stream, teams);
       if (rc != 0) return rc;
       // the deferred events: usually none (then the small CTAs come and go beside the next batch's
       // team kernel); for batches of large events, large CTAs: such a batch waits for its largest event
-      if (a.n_hits / a.n_events >= 4096u) velo_event_slab_kernel<kThreadsLarge, false><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
-      else velo_event_slab_kernel<kThreads, true><<<grid, kThreads, 0, stream>>>(a, 1);
+      if (a.n_hits / a.n_events >= 4096u) velo_event_slab_kernel<kThreadsLarge, false, 8><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
+      else velo_event_slab_kernel<kThreads, true, kBinShift><<<grid, kThreads, 0, stream>>>(a, 1);
     }
   }
   if (ev_stop) cudaEventRecord(ev_stop, stream);
