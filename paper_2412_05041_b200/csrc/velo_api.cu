@@ -83,6 +83,9 @@ int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, con
   a.x = hits->x; a.y = hits->y; a.z = hits->z; a.module = hits->module;
   a.event_offsets = hits->event_offsets;
   a.n_events = hits->n_events; a.n_modules = g->n_modules; a.n_hits = hits->n_hits;
+  // In a batch of large events (ion-like, mean >= 4096 hits) an event of more than ~6 k hits is
+  // better off in the general kernel with its 1024-thread CTAs than alone on an SM of the team kernel.
+  a.team_max_hits = (hits->n_events && hits->n_hits / hits->n_events >= 4096u) ? 6144u : velo::kTeamMaxHits;
   for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
   a.P = *params;
   if (a.P.max_skipped > 200u) a.P.max_skipped = 200u;  // more misses than modules is all the same

@@ -334,7 +334,7 @@ __device__ void leader_fetch(const KernelArgs& a, Control& ctl, TeamShared& ts) 
   }
   const uint32_t n = o1 - o0;
   if (n == 0) { a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); return; }
-  if (n > kMaxTeamHits) { defer_to_slab(a, e); return; }
+  if (n > a.team_max_hits) { defer_to_slab(a, e); return; }
   const Layout L = event_layout(n, a.n_modules);
   const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;
   if (units > kPoolUnits) { defer_to_slab(a, e); return; }

@@ -80,6 +80,7 @@ struct KernelArgs {
   const uint32_t* event_offsets;
   uint32_t n_events, n_modules;
   uint32_t n_hits;                   // host knowledge of the batch size: only steers launch heuristics
+  uint32_t team_max_hits;            // events with more hits go to the general kernel
   float module_z[VELO_MAX_MODULES];  // geometry: the shared-memory path requires z[i] == module_z[module[i]]
   velo_params_t P;
   // output
