@@ -43,6 +43,10 @@ constexpr uint32_t kCtlBytes = 8192;
 constexpr uint32_t kClChunk = 256;          // centre hits per seeding chunk (2 per thread)
 constexpr uint32_t kMaxTeams = kTeamsPerCtaMax;
 constexpr uint32_t kMaxTeamHits = kTeamMaxHits;   // <= 32767: the local original index is stored in 15 bits
+#ifndef VELO_SEED_LANES
+#define VELO_SEED_LANES 4
+#endif
+constexpr uint32_t kSeedLanes = VELO_SEED_LANES;   // lanes that share the search of one seed centre
 constexpr uint32_t kMaxBinSlot = 2047;      // slot inside a phi bucket is stashed in 11 bits
 constexpr uint32_t kFlagBit = 0x8000u;      // O-5 flag[h] inside the packed hit word
 
@@ -585,8 +589,8 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
         cpar ^= 1u;
         // (C2) four lanes per unflagged centre hit: lane `sub` takes every 4th h0 of the window; the
         // quad's best (h0, h2) under (scatter, h0, h2) is reduced with shuffles
-        for (uint32_t k0 = 0; k0 < ncl; k0 += kTeamThreads / 4) {
-          const uint32_t k = k0 + (tid >> 2), sub = tid & 3u;
+        for (uint32_t k0 = 0; k0 < ncl; k0 += kTeamThreads / kSeedLanes) {
+          const uint32_t k = k0 + tid / kSeedLanes, sub = tid % kSeedLanes;
           bool found = false; uint32_t b0 = 0, b2 = 0, h1 = 0; float best_sc = 0.0f;
           if (k < ncl) {
             h1 = ts.cl[k];
@@ -596,7 +600,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
             const Window q2 = make_window(bo_2, w1 >> 16, P.phi_window_seed);
             const uint32_t end0 = q0.e0 + (q0.e1 - q0.b1);
             VELO_COUNT(18, 1); VELO_COUNT(19, end0 - q0.b0);
-            for (uint32_t jo = q0.b0 + sub; jo < end0; jo += 4) {
+            for (uint32_t jo = q0.b0 + sub; jo < end0; jo += kSeedLanes) {
               const uint32_t h0 = jo < q0.e0 ? jo : jo - q0.e0 + q0.b1;
               const uint32_t w0 = ev.w[h0];
               if ((w0 & kFlagBit) || !in_window(q0, w0)) continue;
@@ -616,7 +620,7 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
             }
           }
 #pragma unroll
-          for (uint32_t d = 1; d <= 2; d <<= 1) {   // minimum over the quad, ties: lowest h0, then lowest h2
+          for (uint32_t d = 1; d < kSeedLanes; d <<= 1) {   // minimum over the group, ties: lowest h0, then lowest h2
             const bool of = __shfl_xor_sync(0xffffffffu, (int)found, d) != 0;
             const float osc = __shfl_xor_sync(0xffffffffu, best_sc, d);
             const uint32_t ob0 = __shfl_xor_sync(0xffffffffu, b0, d), ob2 = __shfl_xor_sync(0xffffffffu, b2, d);
