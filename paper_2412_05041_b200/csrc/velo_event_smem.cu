@@ -487,6 +487,12 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   team_sync(team);
   for (uint32_t s = M - 2; s >= 1; --s) {
     const uint32_t u = s - 1, nxt = cur ^ 1u;
+    // No hit in modules 0 .. u: forwarding can only miss and seeding finds no third hit, in this step
+    // and in all that follow, and what a miss changes (the miss counter) is not read after the loop.
+    if (ev.bo[(u + 1) * kBinsPerModule] == 0) {
+      for (uint32_t r = tid + 1u; r <= s; r += kTeamThreads) ts.sstart[r] = ts.nt;   // nothing is created any more
+      break;
+    }
     VELO_SUB_START();
     // (A) O-7 forwarding into module u of every track active at the start of the step
     {
