@@ -29,9 +29,9 @@ if ROOT not in sys.path:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one event-kernel launch, from the ncu --set full
 # capture summarised in profiles/r01c_team_kernel_25k.md; key = (config, path, events per step)
-NCU_DRAM_BYTES_PER_LAUNCH = {(2, 0, 100_000): 674_300_672 + 494_879_488}
+NCU_DRAM_BYTES_PER_LAUNCH = {(2, 0, 100_000): 676_917_248 + 496_348_160}
 # smsp__inst_executed.sum of the same capture / its 25 000 events: what bounds the path in practice
-NCU_WARP_INST_PER_EVENT = {(2, 0): 97_007.0}
+NCU_WARP_INST_PER_EVENT = {(2, 0): 94_811.0}
 
 METRIC = "velo_tracking_events_per_s"
 UNIT = "events/s"
@@ -311,8 +311,8 @@ def run_velo(args):
                      "kernel_share_of_step": avg_kern_ms * n_batches / ms_step,
                      "step_achieved": step_gbs, "step_frac": step_gbs / peak,
                      "frac_of_nominal_8TBs": step_gbs / 8000.0,
-                     "limiter": "instruction issue and latency, not HBM (ncu: issue slots 52.1 % busy, DRAM 3 % busy, "
-                                "97.0 k warp instructions per event; see profiles/ and DESIGN.md 5.1)"},
+                     "limiter": "instruction issue and latency, not HBM (ncu: issue slots 52.0 % busy, DRAM 3 % busy, "
+                                "94.8 k warp instructions per event; see profiles/ and DESIGN.md 5.1)"},
         "issue": issue_block(args, world * n_events / (ms_step * 1e-3), clocks),
         "clocks": clocks,
         "gpu_launches": launches_per_batch * n_batches * (args.steps + args.warmup),
