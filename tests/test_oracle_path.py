@@ -224,22 +224,7 @@ def test_filters_bruteforce_on_generated_events(cfg0):
     assert tot_killed > 0
 
 
-def test_clone_pair_differing_in_one_hit():
-    # two 4-hit candidates sharing three hits: the better chi2 survives, the other is killed
-    # (it loses 3 of 4 hits; 3*3 > 4*1). Built from one clean line + a displaced duplicate on
-    # the first module so that two seeds forward onto the same three hits.
-    ev = line_event([13, 12, 11, 10], extra=[(0.1 * 126 + 0.11, 0.0, 13)])
-    c = oracle.event_candidates(*ev, 26)
-    four = [t for t in range(c["n_cand"]) if c["n"][t] == 4]
-    if len(four) == 2:
-        a, b = four
-        shared = set(c["hits"][a, :4]) & set(c["hits"][b, :4])
-        assert len(shared) == 3
-        worse = a if c["states"][a, 11] > c["states"][b, 11] else b
-        assert not c["survive"][worse] and c["survive"][a + b - worse]
-    r = run(ev)
-    assert track_modules(r, ev[3]) == [(13, 12, 11, 10)]
-    assert split_tracks(r, 0)[0][0] == (0, 1, 2, 3)
+# (the clone rule on real candidate pairs with stated outcomes: tests/test_oracle_hand_events.py)
 
 
 # ---------------------------------------------------------------- (vi), (vii), edge cases

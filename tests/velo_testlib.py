@@ -172,3 +172,119 @@ def _oracle_range(job):
                            (off[e0:e1 + 1].astype(np.int64) - h0).astype(np.uint32), n_modules, params)
     r["track_hits"] = r["track_hits"] + np.uint32(h0)
     return r
+
+
+# ---- hand-made events with STATED outcomes (round 2 pins of O-7, O-8, O-6(B), O-12, A11) ----------
+# Each builder returns (event, expected): event = (x, y, z, module) arrays, expected = the list of
+# output tracks as tuples of ORIGINAL hit indices in discovery order, in canonical order (O-16).
+# The expectations are worked out by hand from SURVEY.md §8(c); nothing here was produced by the
+# oracle or by the CUDA path. Modules 5 ... 18 are 25 mm apart (A1), so mirrored displacements
+# about a middle module are exactly collinear.
+def _hits(rows):
+    x = np.array([r[0] for r in rows], np.float32); y = np.array([r[1] for r in rows], np.float32)
+    m = np.array([r[2] for r in rows], np.uint8)
+    return x, y, MODULE_Z[m.astype(np.int64)].astype(np.float32), m
+
+
+def _line_a(first_module, n):
+    """x = 10 + 0.1 z, y = 0 on n consecutive modules downwards from first_module (phi16 = 0)."""
+    return [(10.0 + 0.1 * float(MODULE_Z[m]), 0.0, m) for m in range(first_module, first_module - n, -1)]
+
+
+def pin_forward_tie(top=13):
+    """O-7 tie -> LOWEST sorted index: the forwarding target module holds the same hit twice
+    (A14). Sorted index ties resolve by original index (O-2), so the track ends on hit 3, not 4."""
+    rows = _line_a(top, 4)
+    rows.append(rows[3])                       # duplicate of the hit on the target module
+    return _hits(rows), [(0, 1, 2, 3)]
+
+
+def pin_forward_window_centre():
+    """O-7 window is centred on hb (the LATEST hit), not on ha. The line x = 10, y = 0.0077 z is
+    straight (scatter 0) but turns by ~201 phi16 units per module: the module-10 hit lies 201
+    units from hb (inside W = 300) and 402 units from ha (outside)."""
+    rows = [(10.0, 0.0077 * float(MODULE_Z[m]), m) for m in (13, 12, 11, 10)]
+    return _hits(rows), [(0, 1, 2, 3)]
+
+
+def pin_forward_miss_reset():
+    """O-7: n_missed returns to 0 after a found hit. Hits on modules 16, 15, 14, 12, 11, 9, 8: each
+    gap is ONE missed module, max_skipped = 1 bridges both -> one 7-hit track."""
+    rows = [(10.0 + 0.1 * float(MODULE_Z[m]), 0.0, m) for m in (16, 15, 14, 12, 11, 9, 8)]
+    return _hits(rows), [(0, 1, 2, 3, 4, 5, 6)]
+
+
+def pin_seed_flagged_centre(top=13):
+    """O-8: a flagged hit is not a seed centre, and O-6(B): the flags of step s are visible to the
+    seeding of the SAME step. Line A on modules top ... top-5 reaches 4 hits in (A) of step top-2,
+    which flags its hit on module top-2 (hit 2). Strays U(top-1), U(top-3) mirror each other about
+    that hit (exactly collinear through it) and U(top-4) continues their line: if hit 2 seeded at
+    step top-2 it would give the 4-hit track (U, 2, U, U). It must not: the strays stay unused."""
+    rows = _line_a(top, 6)
+    xa = lambda m: 10.0 + 0.1 * float(MODULE_Z[m])
+    rows += [(xa(top - 1), 0.2, top - 1), (xa(top - 3), -0.2, top - 3), (xa(top - 4), -0.4, top - 4)]
+    return _hits(rows), [(0, 1, 2, 3, 4, 5)]
+
+
+def pin_seed_flagged_h0(top=13):
+    """O-8: a flagged hit is not used as h0. Strays C(top-3), C(top-4), C(top-5) are exactly
+    collinear with line A's hit on module top-2 (hit 2, flagged at step top-2). At step top-3 the
+    centre C(top-3) has only that flagged hit in its module-(top-2) window -> no seed; at step
+    top-4 the three strays seed on their own and survive as a weak 3-hit track (scatter 0)."""
+    rows = _line_a(top, 6)
+    xa = lambda m: 10.0 + 0.1 * float(MODULE_Z[m])
+    rows += [(xa(top - 3), 0.15, top - 3), (xa(top - 4), 0.30, top - 4), (xa(top - 5), 0.45, top - 5)]
+    return _hits(rows), [(0, 1, 2, 3, 4, 5), (6, 7, 8)]
+
+
+def pin_seed_flagged_h2(top=13):
+    """O-8: a flagged hit is not used as h2, including one flagged in (A)/(B) of the same step.
+    Strays V(top-2) = A + 2d, V(top-3) = A + d are exactly collinear with line A's hit on module
+    top-4 (hit 4, picked up and flagged at step top-3), and V(top-5) = A - d continues that line.
+    At step top-3 the centre V(top-3) finds only the flagged hit 4 in its module-(top-4) window ->
+    no seed; used as h2 it would give the 4-hit track (V, V, 4, V)."""
+    rows = _line_a(top, 6)
+    xa = lambda m: 10.0 + 0.1 * float(MODULE_Z[m])
+    rows += [(xa(top - 2), 0.30, top - 2), (xa(top - 3), 0.15, top - 3), (xa(top - 5), -0.15, top - 5)]
+    return _hits(rows), [(0, 1, 2, 3, 4, 5)]
+
+
+def pin_chi2_track(n):
+    """O-12: a track with a known chi2. n hits on modules 12 ... 12-n+1 at y = 0, x = 10 except one
+    hit displaced by e = 0.03 mm (n = 3: the middle one; n = 5: the middle one). Unweighted LSQ
+    leaves residuals (-e/3, 2e/3, -e/3) resp. (-e/5, -e/5, 4e/5, -e/5, -e/5): sum of squares
+    2e^2/3 resp. 4e^2/5; chi2 = that / sigma^2 with sigma^2 = 0.055^2/12; ndof = 2n - 4.
+    Returns (event, expected track, chi2 in float64)."""
+    e = 0.03
+    mods = list(range(12, 12 - n, -1))
+    rows = [(10.0 + (e if i == n // 2 else 0.0), 0.0, m) for i, m in enumerate(mods)]
+    ss = 2 * e * e / 3 if n == 3 else 4 * e * e / 5
+    x = np.array([r[0] for r in rows], np.float32).astype(np.float64)
+    ss32 = float(((x - x.mean()) ** 2).sum())          # the same sum on the fp32-rounded inputs
+    assert abs(ss32 - ss) < 1e-3 * ss
+    return _hits(rows), [tuple(range(n))], ss32 / (0.055 ** 2 / 12.0)
+
+
+def pin_clone_pair():
+    """O-13 on a real pair: two centre hits 0.1 mm apart on module 12 both seed with the same h0
+    and h2 (seed scatter 0 and 0.04) and both forward onto the same module-10 hit, giving two
+    4-hit candidates that share three hits. The straight one has the lower chi2 and owns the
+    shared hits; the other loses 3 of 4 (3*3 > 4*1) and is killed."""
+    rows = _line_a(13, 4)
+    rows.append((rows[1][0], 0.1, 12))
+    return _hits(rows), [(0, 1, 2, 3)]
+
+
+def pin_clone_tie():
+    """O-13 tie: two centre hits mirrored about the line (y = +0.1 and -0.1) give candidates with
+    bit-identical chi2; the key falls back to the centre's sorted index, and y < 0 sorts first."""
+    a = _line_a(13, 4)
+    rows = [a[0], (a[1][0], 0.1, 12), (a[1][0], -0.1, 12), a[2], a[3]]
+    return _hits(rows), [(0, 2, 3, 4)]
+
+
+PIN_EVENTS = [pin_forward_tie, lambda: pin_forward_tie(14), pin_forward_window_centre, pin_forward_miss_reset,
+              pin_seed_flagged_centre, lambda: pin_seed_flagged_centre(14), pin_seed_flagged_h0,
+              lambda: pin_seed_flagged_h0(14), pin_seed_flagged_h2, lambda: pin_seed_flagged_h2(14),
+              lambda: pin_chi2_track(3)[:2], lambda: pin_chi2_track(5)[:2],
+              pin_clone_pair, pin_clone_tie]
