@@ -49,6 +49,13 @@ def parse_args():
     ap.add_argument("--ctas-per-sm", type=int, default=0, help="slab-kernel launch option (0 = library default)")
     ap.add_argument("--teams", type=int, default=0, help="teams per CTA of the team kernel (0 = library default)")
     ap.add_argument("--path", type=int, default=0, help="0 = team kernel + slab for deferred events, 1 = slab only")
+    ap.add_argument("--track-group", type=int, default=0, help="threads per event of the module-loop kernel (0 = default)")
+    ap.add_argument("--track-teams", type=int, default=0)
+    ap.add_argument("--fit-teams", type=int, default=0)
+    ap.add_argument("--sort-teams", type=int, default=0)
+    ap.add_argument("--pool-units", type=int, default=0)
+    ap.add_argument("--timeline", action="store_true",
+                    help="instrumented build: print when each pipeline stage of each batch ran, then exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -224,9 +231,13 @@ def run_velo(args):
     g = velo.velo_geometry_load(datagen.MODULE_Z, half_shift_x=cfg.half_shift_x)
     P = velo.velo_params_default(g)
     dh = velo.DeviceHits(d["x"], d["y"], d["z"], d["module"], off)
-    opts0 = velo.LaunchOptions(ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams)
+    tune = dict(track_group=args.track_group, track_teams=args.track_teams, fit_teams=args.fit_teams,
+                sort_teams=args.sort_teams, pool_units=args.pool_units)
+    opts0 = velo.LaunchOptions(ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams, **tune)
     launches_per_batch = 3 if args.path == 1 else 5   # [order, team kernel,] slab kernel, offsets, compaction
     streams = [torch.cuda.Stream() for _ in range(n_batches)]
+    if os.environ.get('VELO_BENCH_SERIAL'):
+        streams = [streams[0]] * n_batches
     main = torch.cuda.current_stream()
     outs, hstructs = [], []
     for b in range(n_batches):
@@ -247,7 +258,7 @@ def run_velo(args):
             ks, ke = kev[i][b]
             ks.record(streams[b]); ke.record(streams[b])
             o = velo.LaunchOptions(event_kernel_start=ks.cuda_event, event_kernel_stop=ke.cuda_event,
-                                   ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams)
+                                   ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams, **tune)
             velo.velo_reconstruct(g, hstructs[b], P, outs[b], streams[b], o)
             joins[b].record(streams[b])
             main.wait_event(joins[b])
@@ -260,6 +271,18 @@ def run_velo(args):
     for i in range(args.warmup):
         step(i)
     barrier()
+    if args.timeline:
+        # windows of the sort / track / fit kernels of the last warm-up step's batches (GPU global timer)
+        rows = []
+        for b, o in enumerate(outs):
+            skip = o.workspace_ptr - o.workspace.data_ptr() + 256
+            clk = o.workspace[skip:skip + 48].cpu().numpy().view(np.uint64)
+            rows.append([(int(~clk[2 * k]), int(clk[2 * k + 1])) for k in range(3)])
+        t0 = min(r[0][0] for r in rows)
+        for b, r in enumerate(rows):
+            print("batch %d: " % b + "  ".join("%s %8.3f .. %8.3f ms" % (nm, (s - t0) / 1e6, (e - t0) / 1e6)
+                                                 for nm, (s, e) in zip(("sort", "track", "fit"), r)), flush=True)
+        return
     sampler = ClockSampler(local); sampler.start()
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0.record(main)
@@ -366,6 +389,9 @@ def run_velo(args):
 
 def main():
     args = parse_args()
+    if args.timeline:
+        os.environ["VELO_TIMELINE_BUILD"] = "1"
+
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -145,14 +145,18 @@ int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const ve
  * (as many as mean-sized events of the batch fit one SM's shared memory: 5 at mu = 5).
  * ctas_per_sm: persistent CTAs per SM of the slab kernel, 0 = library default; the workspace must
  * have been sized for the default or for velo_workspace_bytes_opts with the same value. */
-enum { VELO_PATH_DEFAULT = 0, VELO_PATH_SLAB_ONLY = 1 };
+enum { VELO_PATH_DEFAULT = 0, VELO_PATH_SLAB_ONLY = 1, VELO_PATH_TEAM_LEGACY = 2 };
 typedef struct {
   void* event_kernel_start;
   void* event_kernel_stop;
   uint32_t ctas_per_sm;
   uint32_t path;
   uint32_t teams_per_cta;
-  uint32_t reserved;
+  uint32_t track_group;   /* threads per event in the module-loop kernel: 32, 64 or 128; 0 = default  */
+  uint32_t track_teams;   /* events in flight per persistent CTA of the module-loop kernel; 0 = default */
+  uint32_t fit_teams;     /* ... of the fit/output kernel; 0 = default                                  */
+  uint32_t sort_teams;    /* ... of the sort kernel; 0 = default                                        */
+  uint32_t pool_units;    /* shared-memory pool per CTA in units of 3456 bytes, 1..64; 0 = 64           */
 } velo_launch_options_t;
 size_t velo_workspace_bytes_opts(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks,
                                  uint32_t cap_track_hits, const velo_launch_options_t* opts);
@@ -173,7 +177,7 @@ void velo_scheduler_free(velo_scheduler_t* s);
  * (event indices, batch_begin[0] = 0, batch_begin[n_batches] = hits->n_events); batch b runs on
  * stream b % n_streams: host->device copy of its slice, velo_reconstruct, device->host copy of
  * exactly the produced tracks into out[b] (HOST pointers, capacities per batch; summary is a
- * HOST u32[4]). Offsets in out[b] are batch-local; track_hits are absolute hit indices.
+ * HOST u32[VELO_N_SUMMARY]). Offsets in out[b] are batch-local; track_hits are absolute hit indices.
  * Returns after every copy has completed. A batch larger than the scheduler's limits or an
  * output capacity below cap_tracks = n_hits/4 + n_events, cap_track_hits = 2*n_hits of the
  * device buffers is reported per batch through out[b].summary[2]. */

@@ -12,8 +12,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libvelo.so")
-SOURCES = ["velo_api.cu", "velo_kernels.cu", "velo_event_smem.cu", "velo_scheduler.cu"]
-HEADERS = ["velo_device.cuh", "velo_internal.h"]
+SOURCES = ["velo_api.cu", "velo_kernels.cu", "velo_sort.cu", "velo_track.cu", "velo_fit.cu", "velo_event_smem.cu",
+           "velo_scheduler.cu"]
+HEADERS = ["velo_device.cuh", "velo_internal.h", "velo_pool.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-shared"]
 
@@ -31,6 +32,18 @@ def _stale() -> bool:
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(INCLUDE, "velo.h")]
     return any(os.path.getmtime(d) > t for d in deps)
+
+
+LIB_TIMELINE = os.path.join(_HERE, "libvelo_timeline.so")
+
+
+def build_timeline() -> str:
+    """The same library with -DVELO_TIMELINE: every pipeline kernel records the window in which its
+    CTAs ran (GPU global timer), for `bench.py --timeline`. Never used by the product path."""
+    cmd = [_nvcc(), *NVCC_FLAGS, "-DVELO_TIMELINE", "-I", INCLUDE, "-o", LIB_TIMELINE] + \
+          [os.path.join(CSRC, f) for f in SOURCES]
+    subprocess.run(cmd, check=True)
+    return LIB_TIMELINE
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

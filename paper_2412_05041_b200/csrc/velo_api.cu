@@ -9,12 +9,6 @@
 
 #include "velo_internal.h"
 
-struct velo_geometry {
-  uint32_t n_modules;
-  float module_z[VELO_MAX_MODULES];
-  float r_in, r_out, pitch, half_shift_x;
-};
-
 extern "C" {
 
 const char* velo_version(void) { return "velo-b200 0.1 (sm_100a)"; }
@@ -58,17 +52,20 @@ static uint32_t n_slabs_for(const velo_launch_options_t* opts) {
 
 size_t velo_workspace_bytes_opts(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits,
                                  const velo_launch_options_t* opts) {
-  (void)n_hits;
-  return velo::carve_workspace(nullptr, n_events, cap_tracks, cap_track_hits, n_slabs_for(opts)).bytes;
+  return velo::carve_workspace(nullptr, n_events, n_hits, cap_tracks, cap_track_hits, n_slabs_for(opts)).bytes;
 }
 
 size_t velo_workspace_bytes(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits) {
   return velo_workspace_bytes_opts(n_events, n_hits, cap_tracks, cap_track_hits, nullptr);
 }
 
-int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
-                          velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
-                          const velo_launch_options_t* opts) {
+}  // extern "C"
+
+namespace velo {
+
+int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
+                     const velo_launch_options_t* opts, uint32_t hit_base) {
   if (!g || !hits || !params || !out || !workspace) return VELO_ERR_ARG;
   if (!hits->event_offsets || !out->event_track_offsets || !out->track_hit_offsets || !out->summary)
     return VELO_ERR_ARG;
@@ -79,24 +76,47 @@ int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, con
   const size_t need = velo_workspace_bytes_opts(hits->n_events, hits->n_hits, out->cap_tracks, out->cap_track_hits, opts);
   if (workspace_bytes < need) return VELO_ERR_WORKSPACE;
 
-  velo::KernelArgs a{};
+  KernelArgs a{};
   a.x = hits->x; a.y = hits->y; a.z = hits->z; a.module = hits->module;
   a.event_offsets = hits->event_offsets;
   a.n_events = hits->n_events; a.n_modules = g->n_modules; a.n_hits = hits->n_hits;
-  // In a batch of large events (ion-like, mean >= 4096 hits) an event of more than ~6 k hits is
-  // better off in the general kernel with its 1024-thread CTAs than alone on an SM of the team kernel.
-  a.team_max_hits = (hits->n_events && hits->n_hits / hits->n_events >= 4096u) ? 6144u : velo::kTeamMaxHits;
+  a.hit_base = hit_base;
+  const uint32_t path = opts ? opts->path : 0u;
+  if (path == kPathTeamLegacy) {
+    // In a batch of large events (ion-like, mean >= 4096 hits) an event of more than ~6 k hits is
+    // better off in the general kernel with its 1024-thread CTAs than alone on an SM of the team kernel.
+    a.team_max_hits = (hits->n_events && hits->n_hits / hits->n_events >= 4096u) ? 6144u : kTeamMaxHits;
+  } else {
+    a.team_max_hits = kPipeMaxHits;
+  }
   for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
   a.P = *params;
   if (a.P.max_skipped > 200u) a.P.max_skipped = 200u;  // more misses than modules is all the same
+  // A negative window holds no hit (O-3). The kernels take windows >= 0; the same result follows
+  // from a scatter cut that nothing passes (scatter is a sum of squares, never below zero).
+  if (a.P.phi_window_seed < 0) { a.P.phi_window_seed = 0; a.P.max_scatter_seed = -1.0f; }
+  if (a.P.phi_window_fwd < 0) { a.P.phi_window_fwd = 0; a.P.max_scatter_fwd = -1.0f; }
   a.event_track_offsets = out->event_track_offsets; a.track_hit_offsets = out->track_hit_offsets;
   a.track_hits = out->track_hits; a.states = out->states;
   a.cap_tracks = out->cap_tracks; a.cap_track_hits = out->cap_track_hits; a.summary = out->summary;
-  a.ws = velo::carve_workspace(workspace, hits->n_events, out->cap_tracks, out->cap_track_hits, n_slabs_for(opts));
-  const int err = velo::launch_reconstruct(a, (cudaStream_t)stream, opts ? (cudaEvent_t)opts->event_kernel_start : nullptr,
-                                           opts ? (cudaEvent_t)opts->event_kernel_stop : nullptr,
-                                           opts ? opts->path : 0u, opts ? opts->teams_per_cta : 0u);
+  a.ws = carve_workspace(workspace, hits->n_events, hits->n_hits, out->cap_tracks, out->cap_track_hits, n_slabs_for(opts));
+  PipeOpts po{};
+  if (opts) { po.track_group = opts->track_group; po.track_teams = opts->track_teams; po.fit_teams = opts->fit_teams;
+              po.sort_teams = opts->sort_teams; po.pool_units = opts->pool_units; }
+  const int err = launch_reconstruct(a, (cudaStream_t)stream, opts ? (cudaEvent_t)opts->event_kernel_start : nullptr,
+                                     opts ? (cudaEvent_t)opts->event_kernel_stop : nullptr, path,
+                                     opts ? opts->teams_per_cta : 0u, po);
   return err == 0 ? VELO_OK : VELO_ERR_CUDA;
+}
+
+}  // namespace velo
+
+extern "C" {
+
+int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                          velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
+                          const velo_launch_options_t* opts) {
+  return velo::reconstruct_impl(g, hits, params, out, workspace, workspace_bytes, stream, opts, 0u);
 }
 
 int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,

@@ -378,8 +378,9 @@ __device__ void team_event(const KernelArgs& a, Control& ctl, TeamShared& ts, un
   ev.rows = (uint16_t*)scratch;
   ev.st = (float*)(scratch + (size_t)kTeamMaxTracks * 64u);
   unsigned long long* tkey = (unsigned long long*)ev.tl;   // 8 bytes per track over (tl, tseed), used after O-10
-  const float* gx = a.x + o0; const float* gy = a.y + o0; const float* gz = a.z + o0;
-  const uint8_t* gm = a.module + o0;
+  const size_t g0 = (size_t)(o0 - a.hit_base);
+  const float* gx = a.x + g0; const float* gy = a.y + g0; const float* gz = a.z + g0;
+  const uint8_t* gm = a.module + g0;
 
   // ---- S0 decode: phi16, bucket histogram (O-1); the plane check of the team path ---------------
   const uint32_t nwords = nbins / 2u;
@@ -830,12 +831,8 @@ int launch_teams(const KernelArgs& a, cudaStream_t stream) {
     return launch_teams<1024 / kTeamThreads>(a, stream);
   } else {
   const uint32_t smem = kCtlBytes + kPoolUnits * kUnitBytes;
-  static bool configured = false;   // per process; the attribute is sticky per function and device
-  if (!configured) {
-    cudaError_t err = cudaFuncSetAttribute(velo_event_team_kernel<kTeams>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return (int)err;
-    configured = true;
-  }
+  cudaError_t err = cudaFuncSetAttribute(velo_event_team_kernel<kTeams>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (err != cudaSuccess) return (int)err;   // per device and cheap: set on every launch
   const uint32_t sms = num_sms();
   const uint32_t want = (a.n_events + kTeams - 1) / kTeams;
   const uint32_t grid = want < sms ? (want ? want : 1u) : sms;

@@ -1,0 +1,383 @@
+// velo_fit.cu — stage 3 of the pipeline: O-10 weak-track filter, O-11 straight-line fit, O-12 chi2
+// cut, O-13 clone filter (hit ownership by 64-bit key), then S7 output as count -> scan -> write,
+// every final array written once (sm_100a).
+//
+// velo_fit_kernel: teams of G threads in persistent CTAs take the events largest-first. An event's
+// sorted (x, y) arrive in shared memory by a 1-D TMA bulk copy; its candidates (rows of sorted hit
+// indices, module masks, seed scatters) and final flag bits come from stage 2's global scratch. One
+// thread per candidate fits and filters. What leaves: per candidate its fate and nine state words
+// (coalesced planes in global scratch), per event the number of surviving tracks and track hits.
+// velo_offsets_kernel (velo_kernels.cu) scans those counts into event_track_offsets. Then
+// velo_write_kernel, a streaming kernel with one warp per event and no shared memory, places every
+// surviving track: state planes, track_hit_offsets, and track_hits as original hit indices. Events
+// that the pipeline deferred to the general slab kernel (whose tracks sit in temp blocks) are
+// copied into place by the same kernel.
+//
+// Step semantics: SURVEY.md §8(c) O-10 ... O-14; every float operation is a round-to-nearest
+// intrinsic in the oracle's order (no FMA contraction), so states are bit-identical to the oracle's.
+#include "velo_device.cuh"
+#include "velo_internal.h"
+#include "velo_pool.cuh"
+
+namespace velo {
+
+namespace {
+
+
+template <int G>
+struct FitTeam {
+  unsigned long long mbar;
+  uint32_t wsum[4 * (G / 32)];
+  uint32_t event, skip, n, sb, o0;
+  uint32_t units, first_unit, pool_off;
+  uint32_t cbase, ncand;
+};
+
+template <int G, int kTeams>
+struct FitCtl {
+  PoolCtl pool;
+  float module_z[VELO_MAX_MODULES];
+  FitTeam<G> team[kTeams];
+};
+
+__device__ __forceinline__ uint32_t a16(uint32_t v) { return (v + 15u) & ~15u; }
+
+struct FitLayout { uint32_t xy, own, fbits, key, mask, state, bytes; };
+__device__ __forceinline__ FitLayout fit_layout(uint32_t n, uint32_t nt) {
+  FitLayout L;
+  uint32_t o = 0;
+  L.xy = o; o += a16(8u * n);            // sorted (x, y)
+  L.own = o; o += a16(4u * n);           // O-13 owner (candidate id) per hit
+  L.fbits = o; o += a16(4u * ((n + 31u) >> 5));
+  L.key = o; o += a16(8u * nt);
+  L.mask = o; o += a16(4u * nt);
+  L.state = o; o += a16(nt);
+  L.bytes = o;
+  return L;
+}
+
+// Calls f(i, h) for the hits h (sorted indices) of candidate row `row` in discovery order.
+template <class F>
+__device__ __forceinline__ void for_hits(const uint16_t* row, uint32_t n, F&& f) {
+  const uint4* r4 = reinterpret_cast<const uint4*>(row);
+  for (uint32_t g = 0; g * 8u < n; ++g) {
+    const uint4 v = r4[g];
+    const uint32_t q[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (uint32_t j = 0; j < 8; ++j) {
+      if (g * 8u + j < n) f(g * 8u + j, (q[j >> 1] >> ((j & 1u) * 16u)) & 0xffffu);
+    }
+  }
+}
+
+// ---- O-11 straight-line fit with z taken from the module planes ---------------------------------
+// s9 = x, y, tx, ty, z, cxx, cxtx, vt, chi2 (the 13 state words repeat cxx, cxtx, vt for y and add n).
+// Hits are visited in discovery order = decreasing module = the set bits of `mask` from the top.
+__device__ __forceinline__ void fit_track(const float2* xy, const float* mz, const uint16_t* row, uint32_t n, uint32_t mask,
+                                          float sig2, float inv_s2, float* s9) {
+  float sz = 0.0f, sx = 0.0f, sy = 0.0f;
+  uint32_t mk = mask;
+  for_hits(row, n, [&](uint32_t, uint32_t h) {
+    const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
+    const float2 p = xy[h];
+    sz = __fadd_rn(sz, mz[m]); sx = __fadd_rn(sx, p.x); sy = __fadd_rn(sy, p.y);
+  });
+  const float nf = (float)n;
+  const float zb = __fdiv_rn(sz, nf), xb = __fdiv_rn(sx, nf), yb = __fdiv_rn(sy, nf);
+  float sdd = 0.0f, sdx = 0.0f, sdy = 0.0f;
+  mk = mask;
+  for_hits(row, n, [&](uint32_t, uint32_t h) {
+    const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
+    const float2 p = xy[h];
+    const float d = __fsub_rn(mz[m], zb);
+    sdd = __fadd_rn(sdd, __fmul_rn(d, d));
+    sdx = __fadd_rn(sdx, __fmul_rn(d, __fsub_rn(p.x, xb)));
+    sdy = __fadd_rn(sdy, __fmul_rn(d, __fsub_rn(p.y, yb)));
+  });
+  const float tx = __fdiv_rn(sdx, sdd), ty = __fdiv_rn(sdy, sdd);
+  float c = 0.0f;
+  mk = mask;
+  for_hits(row, n, [&](uint32_t, uint32_t h) {
+    const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
+    const float2 p = xy[h];
+    const float d = __fsub_rn(mz[m], zb);
+    const float rx = __fsub_rn(__fsub_rn(p.x, xb), __fmul_rn(tx, d));
+    const float ry = __fsub_rn(__fsub_rn(p.y, yb), __fmul_rn(ty, d));
+    c = __fadd_rn(c, __fmul_rn(rx, rx));
+    c = __fadd_rn(c, __fmul_rn(ry, ry));
+  });
+  const float s2 = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
+  float dzb;
+  if (s2 < 1e-12f) dzb = 0.0f;
+  else dzb = -__fdiv_rn(__fadd_rn(__fmul_rn(xb, tx), __fmul_rn(yb, ty)), s2);
+  const float vt = __fdiv_rn(sig2, sdd);
+  s9[0] = __fadd_rn(xb, __fmul_rn(tx, dzb));
+  s9[1] = __fadd_rn(yb, __fmul_rn(ty, dzb));
+  s9[2] = tx; s9[3] = ty;
+  s9[4] = __fadd_rn(zb, dzb);
+  s9[5] = __fadd_rn(__fdiv_rn(sig2, nf), __fmul_rn(__fmul_rn(dzb, dzb), vt));
+  s9[6] = __fmul_rn(dzb, vt);
+  s9[7] = vt;
+  s9[8] = __fmul_rn(c, inv_s2);
+}
+
+template <int G>
+__device__ void fit_fetch(const KernelArgs& a, PoolCtl& pool, FitTeam<G>& ts) {
+  const uint32_t k = atomicAdd(&a.ws.counters[kCtrFitTicket], 1u);
+  ts.event = k; ts.units = 0; ts.skip = 1;
+  if (k >= a.n_events) return;
+  // largest first, then smallest, second largest, ... (velo_order_kernel): the order only schedules
+  const uint32_t e = a.ws.order[(k & 1u) ? (k >> 1) : a.n_events - 1u - (k >> 1)];
+  ts.event = e;
+  const EvInfo info = a.ws.ev_info[e];
+  if (info.state == kEvDeferred) return;           // the slab kernel has written this event's counts
+  if (info.state != kEvReady || info.ncand == 0) { a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); return; }
+  const FitLayout L = fit_layout(info.n, info.ncand);
+  const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;   // fits the pool: stage 1 checked fit_smem_bound
+  const uint32_t first = pool_alloc(pool, units);
+  ts.n = info.n; ts.cbase = info.cbase; ts.ncand = info.ncand;
+  ts.o0 = a.event_offsets[e];
+  ts.sb = sorted_base(ts.o0 - a.event_offsets[0], e);
+  ts.units = units; ts.first_unit = first; ts.pool_off = first * kUnitBytes; ts.skip = 0;
+}
+
+// ---- one pipeline event, by one team ------------------------------------------------------------
+template <int G>
+__device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, unsigned char* blk, uint32_t team,
+                          uint32_t tid, uint32_t& parity, uint32_t& phase) {
+  const velo_params_t& P = a.P;
+  const uint32_t e = ts.event, n = ts.n, nt = ts.ncand, o0 = ts.o0;
+  const FitLayout L = fit_layout(n, nt);
+  float2* xy = (float2*)(blk + L.xy);
+  uint32_t* own = (uint32_t*)(blk + L.own);
+  uint32_t* fbits = (uint32_t*)(blk + L.fbits);
+  unsigned long long* tkey = (unsigned long long*)(blk + L.key);
+  uint32_t* tmask = (uint32_t*)(blk + L.mask);
+  uint8_t* tstate = blk + L.state;       // 0 dropped by O-10/O-12, 1 passed, 2 survives O-13
+  const uint16_t* rows = a.ws.rows + (size_t)ts.cbase * 32u;
+  const uint2* cmeta = a.ws.cmeta + ts.cbase;
+  float* cfit = a.ws.cfit + ts.cbase;    // plane k of candidate t: cfit[k * cand_total + t]
+  const size_t cs = a.ws.cand_total;
+
+  // sorted coordinates: one bulk copy (size rounded up to 16 bytes: the scratch slots are spaced for it)
+  if (tid == 0) {
+    const uint32_t bxy = a16(8u * n);
+    mbar_arrive_expect_tx(&ts.mbar, bxy);
+    tma_load_1d(xy, a.ws.sxy + ts.sb, bxy, &ts.mbar);
+  }
+  {
+    const uint32_t* fb = a.ws.flag_bits + ((o0 - a.event_offsets[0]) >> 5) + e;
+    for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) fbits[i] = fb[i];
+  }
+  team_sync<G>(team);
+  // ---- O-10 ghost filter part 1 (reads the final flags) -------------------------------------------
+  for (uint32_t t = tid; t < nt; t += G) {
+    const uint2 cm = cmeta[t];
+    tmask[t] = cm.x;
+    bool pass = true;
+    if (__popc(cm.x) == 3) {
+      const uint2 r = *reinterpret_cast<const uint2*>(rows + t * 32u);
+      const uint32_t h0 = r.x & 0xffffu, h1 = r.x >> 16, h2 = r.y & 0xffffu;
+      const uint32_t f = ((fbits[h0 >> 5] >> (h0 & 31u)) | (fbits[h1 >> 5] >> (h1 & 31u)) | (fbits[h2 >> 5] >> (h2 & 31u))) & 1u;
+      if (f || !(__uint_as_float(cm.y) <= P.max_scatter_weak)) pass = false;
+    }
+    tstate[t] = pass ? 1 : 0;
+  }
+  mbar_wait(&ts.mbar, phase & 1u); phase ^= 1u;
+  // ---- O-11 fit, O-12 chi2 cut, O-13 key -----------------------------------------------------------
+  const float sig2 = __fmul_rn(P.sigma_hit, P.sigma_hit);
+  const float inv_s2 = __fdiv_rn(1.0f, sig2);
+  for (uint32_t t = tid; t < nt; t += G) {
+    if (!tstate[t]) continue;
+    const uint32_t mask = tmask[t], nh = (uint32_t)__popc(mask);
+    float s9[9];
+    fit_track(xy, mz, rows + t * 32u, nh, mask, sig2, inv_s2, s9);
+    const float lim = __fmul_rn(P.max_chi2_ndof, (float)(2 * (int)nh - 4));
+    if (s9[8] > lim) { tstate[t] = 0; continue; }
+    const uint32_t centre = rows[t * 32u + 1u];
+    tkey[t] = ((unsigned long long)(255u - nh) << 56) | ((unsigned long long)__float_as_uint(s9[8]) << 24) |
+              (unsigned long long)centre;
+#pragma unroll
+    for (uint32_t k = 0; k < 9; ++k) cfit[k * cs + t] = s9[k];
+  }
+  team_sync<G>(team);
+  // ---- O-13 owners: owner[h] = the candidate with the smallest key among those that contain h ----
+  // Step 1: every passing candidate writes its id on its hits (plain stores: where several share a
+  // hit, any one of them lands). Step 2: a candidate that finds another id on one of its hits
+  // settles it with a compare-and-swap on the 64-bit keys. Hits are shared rarely, so the common
+  // path has no atomics.
+  for (uint32_t t = tid; t < nt; t += G) {
+    if (!tstate[t]) continue;
+    for_hits(rows + t * 32u, (uint32_t)__popc(tmask[t]), [&](uint32_t, uint32_t h) { own[h] = t; });
+  }
+  team_sync<G>(team);
+  for (uint32_t t = tid; t < nt; t += G) {
+    if (!tstate[t]) continue;
+    const unsigned long long key = tkey[t];
+    for_hits(rows + t * 32u, (uint32_t)__popc(tmask[t]), [&](uint32_t, uint32_t h) {
+      uint32_t old = *(volatile uint32_t*)&own[h];
+      while (old != t && key < tkey[old]) {
+        const uint32_t seen = atomicCAS(&own[h], old, t);
+        if (seen == old) break;
+        old = seen;
+      }
+    });
+  }
+  team_sync<G>(team);
+  // ---- O-13 clone filter; the event's counts --------------------------------------------------------
+  uint32_t run_t = 0, run_h = 0;
+  uint8_t* cstate = a.ws.cstate + ts.cbase;
+  for (uint32_t t0 = 0; t0 < nt; t0 += G) {
+    const uint32_t t = t0 + tid;
+    uint32_t nh = 0, surv = 0;
+    if (t < nt && tstate[t]) {
+      nh = (uint32_t)__popc(tmask[t]);
+      uint32_t lost = 0;
+      for_hits(rows + t * 32u, nh, [&](uint32_t, uint32_t h) { lost += (own[h] != t) ? 1u : 0u; });
+      surv = !((unsigned long long)lost * P.clone_den > (unsigned long long)nh * P.clone_num) ? 1u : 0u;
+      if (!surv) nh = 0;
+    }
+    if (t < nt) cstate[t] = (uint8_t)surv;
+    uint32_t tot_h, pre_t, tot_t;
+    team_scan2<G>(nh, surv, ts.wsum, team, parity, &tot_h, &pre_t, &tot_t);
+    run_t += tot_t; run_h += tot_h;
+  }
+  if (tid == 0) a.ws.ev_rec[e] = make_uint4(0, 0, run_t, run_h);
+}
+
+// ---- the fit kernel: one CTA per SM, kTeams teams of G threads ------------------------------------
+template <int G, int kTeams>
+__global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArgs a, const uint32_t pool_units) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  using Ctl = FitCtl<G, kTeams>;
+  constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
+  Ctl& ctl = *reinterpret_cast<Ctl*>(smem);
+  unsigned char* pool = smem + kCtl;
+  const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
+  if (threadIdx.x == 0) { ctl.pool.bitmap = 0ull; ctl.pool.alloc_next = 0; ctl.pool.alloc_serving = 0; ctl.pool.units = pool_units; }
+  if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
+  FitTeam<G>& ts = ctl.team[team];
+  if (tid == 0) { mbar_init(&ts.mbar, 1u); mbar_fence_init(); }
+  __syncthreads();
+  VELO_STAGE_BEGIN(a.ws.phase_clk, 2);
+  uint32_t parity = 0, phase = 0;
+  for (;;) {
+    if (tid == 0) fit_fetch<G>(a, ctl.pool, ts);
+    team_sync<G>(team);
+    if (ts.event >= a.n_events) break;
+    if (!ts.skip) fit_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity, phase);
+    team_sync<G>(team);
+    if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
+  }
+  VELO_STAGE_END(a.ws.phase_clk, 2);
+}
+
+// ---- S7 write: one warp per event places its surviving tracks in the final arrays ----------------
+// Offsets come from velo_offsets_kernel (event_track_offsets, ws.ev_hit_base). Candidates are in
+// creation order, so a running count over them is the track's place inside the event.
+__global__ void __launch_bounds__(128, 8) velo_write_kernel(const KernelArgs a) {
+  const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t tot_t = a.event_track_offsets[a.n_events], tot_h = a.ws.ev_hit_base[a.n_events];
+  if (tot_t > a.cap_tracks || tot_h > a.cap_track_hits) return;  // VELO_ERR_CAPACITY: nothing valid
+  const size_t cs = a.cap_tracks, cc = a.ws.cand_total;
+  const uint32_t obase = a.event_offsets[0];
+  for (uint32_t e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; e < a.n_events; e += warps) {
+    const uint4 r = a.ws.ev_rec[e];
+    if (r.z == 0) continue;
+    const uint32_t dst_t = a.event_track_offsets[e], dst_h = a.ws.ev_hit_base[e];
+    EvInfo info{0u, kEvDeferred, 0u, 0u};
+    if (!a.all_deferred) info = a.ws.ev_info[e];
+    if (info.state == kEvDeferred) {
+      // tracks of the general kernel: temp block -> place (four independent loads per lane and trip)
+      const uint32_t* src = a.ws.tmp_hits + r.y;
+      uint32_t* dst = a.track_hits + dst_h;
+      for (uint32_t k = lane; k < r.w; k += 128u) {
+        uint32_t v[4];
+#pragma unroll
+        for (uint32_t q = 0; q < 4; ++q) v[q] = (k + 32u * q < r.w) ? src[k + 32u * q] : 0u;
+#pragma unroll
+        for (uint32_t q = 0; q < 4; ++q) if (k + 32u * q < r.w) dst[k + 32u * q] = v[q];
+      }
+      for (uint32_t k = lane; k < r.z; k += 32u) {
+        float v[VELO_N_STATE];
+        const uint32_t lo = a.ws.tmp_loff[r.x + k];
+#pragma unroll
+        for (int p = 0; p < VELO_N_STATE; ++p) v[p] = a.ws.tmp_states[(size_t)p * cs + r.x + k];
+        a.track_hit_offsets[dst_t + k] = dst_h + lo;
+#pragma unroll
+        for (int p = 0; p < VELO_N_STATE; ++p) a.states[(size_t)p * cs + dst_t + k] = v[p];
+      }
+      continue;
+    }
+    const uint32_t o0 = a.event_offsets[e];
+    const uint16_t* orig = a.ws.sorig + sorted_base(o0 - obase, e);
+    const uint16_t* rows = a.ws.rows + (size_t)info.cbase * 32u;
+    const uint2* cmeta = a.ws.cmeta + info.cbase;
+    const uint8_t* cstate = a.ws.cstate + info.cbase;
+    const float* cfit = a.ws.cfit + info.cbase;
+    uint32_t run_t = 0, run_h = 0;
+    for (uint32_t t0 = 0; t0 < info.ncand; t0 += 32u) {
+      const uint32_t t = t0 + lane;
+      const bool surv = t < info.ncand && cstate[t] != 0;
+      const uint32_t nh = surv ? (uint32_t)__popc(cmeta[t].x) : 0u;
+      const uint32_t b = __ballot_sync(0xffffffffu, surv);
+      uint32_t inc = nh;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= (uint32_t)d) inc += o; }
+      const uint32_t lt = run_t + (uint32_t)__popc(b & ((1u << lane) - 1u)), lh = run_h + inc - nh;
+      run_t += (uint32_t)__popc(b); run_h += __shfl_sync(0xffffffffu, inc, 31);
+      if (!surv) continue;
+      float s9[9];
+#pragma unroll
+      for (uint32_t k = 0; k < 9; ++k) s9[k] = cfit[k * cc + t];
+      float* dst_s = a.states + dst_t + lt;
+      dst_s[0] = s9[0]; dst_s[cs] = s9[1]; dst_s[2 * cs] = s9[2]; dst_s[3 * cs] = s9[3]; dst_s[4 * cs] = s9[4];
+      dst_s[5 * cs] = s9[5]; dst_s[6 * cs] = s9[6]; dst_s[7 * cs] = s9[7];
+      dst_s[8 * cs] = s9[5]; dst_s[9 * cs] = s9[6]; dst_s[10 * cs] = s9[7];
+      dst_s[11 * cs] = s9[8]; dst_s[12 * cs] = __uint_as_float(nh);
+      a.track_hit_offsets[dst_t + lt] = dst_h + lh;
+      uint32_t* dst = a.track_hits + dst_h + lh;
+      for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) { dst[i] = o0 + orig[h]; });
+    }
+  }
+}
+
+template <int G, int kTeams>
+int launch_fit_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
+  static_assert(G == 32 || kTeams <= 15, "named barriers 1..15");
+  using Ctl = FitCtl<G, kTeams>;
+  constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
+  const uint32_t smem = kCtl + pool_units * kUnitBytes;
+  cudaError_t err = cudaFuncSetAttribute(velo_fit_kernel<G, kTeams>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (err != cudaSuccess) return (int)err;
+  const uint32_t sms = num_sms();
+  const uint32_t want = (a.n_events + kTeams - 1) / kTeams;
+  const uint32_t grid = want < sms ? (want ? want : 1u) : sms;
+  velo_fit_kernel<G, kTeams><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
+  return (int)cudaGetLastError();
+}
+
+}  // namespace
+
+int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
+  if (a.n_events == 0) return 0;
+  const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
+  switch (o.fit_teams) {
+    case 4: return launch_fit_t<128, 4>(a, stream, pu);
+    case 6: return launch_fit_t<128, 6>(a, stream, pu);
+    case 12: return launch_fit_t<64, 12>(a, stream, pu);
+    case 15: return launch_fit_t<64, 15>(a, stream, pu);
+    default: return launch_fit_t<128, 8>(a, stream, pu);
+  }
+}
+
+int launch_write(const KernelArgs& a, cudaStream_t stream) {
+  if (a.n_events == 0) return 0;
+  uint32_t grid = (a.n_events + 3u) / 4u;
+  if (grid > num_sms() * 16u) grid = num_sms() * 16u;
+  velo_write_kernel<<<grid, 128, 0, stream>>>(a);
+  return (int)cudaGetLastError();
+}
+
+}  // namespace velo

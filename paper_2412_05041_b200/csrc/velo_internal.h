@@ -51,10 +51,47 @@ constexpr uint32_t kTeamsPerCtaMax = 8;
 // counters: u32[16]: 0 tracks allocated, 1 track-hits allocated, 2 status, 3 candidates,
 //           4 event ticket, 5 large-event list length, 6 large-event ticket
 enum { kCtrTracks = 0, kCtrHits = 1, kCtrStatus = 2, kCtrCand = 3, kCtrTicket = 4, kCtrLargeN = 5,
-       kCtrLargeTicket = 6, kNumCounters = 16, kNumPhaseClocks = 32 };
+       kCtrLargeTicket = 6, kCtrSortTicket = 7, kCtrTrackTicket = 8, kCtrFitTicket = 9, kCtrCandAlloc = 10,
+       kNumCounters = 16, kNumPhaseClocks = 32 };
+
+// ---- the three-stage pipeline (velo_sort.cu -> velo_track.cu -> velo_fit.cu) ---------------------
+// Stage 1 writes every event's phi-sorted hits to global scratch; stage 2 streams them module by
+// module into shared memory (TMA) and writes candidate tracks; stage 3 fits, filters and writes the
+// final arrays. Scratch index of sorted hit h of event e: sorted_base(e) + h, with sorted_base(e) =
+// align8(event_offsets[e] - event_offsets[0]) + 16 e: disjoint slots whose 2-, 8- and 16-byte
+// element arrays all start 16-byte aligned and leave room to round a bulk copy up to 16 bytes.
+__host__ __device__ inline uint32_t sorted_base(uint32_t o0_local, uint32_t e) { return ((o0_local + 7u) & ~7u) + 16u * e; }
+__host__ __device__ inline size_t sorted_capacity(uint32_t n_events, uint32_t n_hits) { return (size_t)n_hits + 16ull * n_events + 32ull; }
+// Flag bits of event e start at word (o0_local >> 5) + e (disjoint for consecutive events).
+__host__ __device__ inline size_t flag_words(uint32_t n_events, uint32_t n_hits) { return (size_t)(n_hits >> 5) + n_events + 2ull; }
+// Candidate-table capacity of an event of n hits in the pipeline path (candidates ~0.107/hit at
+// mu = 5, 0.19/hit for the open VELO; an event that needs more is deferred to the general kernel).
+__host__ __device__ inline uint32_t cand_capacity(uint32_t n) { return ((n >> 3) + (n >> 4) + 32u + 15u) & ~15u; }
+// Active-track list capacity (tracks alive at the same time: 0.07/hit on average, 0.104/hit at most
+// in 600 events of configs[1]; small events of the open VELO reach 0.14/hit, which the + 32 covers).
+__host__ __device__ inline uint32_t active_capacity(uint32_t n) { return (((n * 13u) >> 7) + 32u + 7u) & ~7u; }
+constexpr uint32_t kModOffStride = 40;   // u16 per event: mod_off[0 .. M] (M <= 32), [39] = largest module
+constexpr uint32_t kPipeMaxHits = 12000; // largest event the pipeline path takes (stage 1: 17 B/hit, stage 3: ~18 B/hit of shared memory)
+// Upper bound of stage 3's shared-memory block for an event of n hits (velo_fit.cu: fit_layout with
+// every candidate slot used): stage 1 defers an event to the general kernel if this does not fit.
+__host__ __device__ inline uint32_t fit_smem_bound(uint32_t n) { return 14u * n + (n >> 3) + 21u * cand_capacity(n) + 256u; }
+// per-event state written by stage 1, updated by stage 2
+enum { kEvEmpty = 0, kEvReady = 1, kEvDeferred = 2, kEvBad = 3 };
+struct EvInfo { uint32_t n, state, cbase, ncand; };   // cbase: first candidate slot; ncand: candidates created
 
 struct Workspace {
   uint32_t* counters;     // kNumCounters
+  EvInfo* ev_info;        // n_events
+  uint4* rec16;           // sorted_capacity: {x, y, phi16u << 16 | start(m+1), start(m-1) << 16 | start(m-2)}
+  float2* sxy;            // sorted_capacity: sorted (x, y) for stage 3
+  uint16_t* sorig;        // sorted_capacity: sorted position -> original event-local index
+  uint16_t* mod_off;      // n_events * kModOffStride
+  uint32_t* flag_bits;    // flag_words: final O-5 flags, one bit per sorted hit
+  uint16_t* rows;         // cand_total * 32: hit lists (sorted indices) of the candidates
+  uint2* cmeta;           // cand_total: {module mask of the hits, seed scatter bits}
+  size_t cand_total;      // capacity of rows / cmeta in candidates
+  float* cfit;            // 9 planes of cand_total: fitted state words of the candidates (stage 3)
+  uint8_t* cstate;        // cand_total: 1 = the candidate survives every filter
   unsigned long long* phase_clk;  // kNumPhaseClocks SM-clock accumulators (written only by -DVELO_PHASE_CLOCKS builds)
   uint4* ev_rec;          // n_events: {temp track base, temp hit base, n_tracks, n_track_hits}
   uint32_t* ev_hit_base;  // n_events+1: exclusive scan of n_track_hits over events
@@ -68,7 +105,7 @@ struct Workspace {
   uint32_t n_slabs;
   size_t bytes;
 };
-Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, uint32_t cap_track_hits,
+Workspace carve_workspace(void* base, uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits,
                           uint32_t n_slabs);
 uint32_t default_n_slabs();
 uint32_t num_sms();  // SM count of the current device (148 on B200); 148 if no device is present
@@ -79,8 +116,10 @@ struct KernelArgs {
   const uint8_t* module;
   const uint32_t* event_offsets;
   uint32_t n_events, n_modules;
-  uint32_t n_hits;                   // host knowledge of the batch size: only steers launch heuristics
+  uint32_t n_hits;                   // host knowledge of the batch size: sizes the scratch, steers launch heuristics
+  uint32_t hit_base;                 // x, y, z, module point at absolute hit index hit_base (0 for velo_reconstruct)
   uint32_t team_max_hits;            // events with more hits go to the general kernel
+  uint32_t all_deferred;             // slab-only path: every event was reconstructed by the general kernel
   float module_z[VELO_MAX_MODULES];  // geometry: the shared-memory path requires z[i] == module_z[module[i]]
   velo_params_t P;
   // output
@@ -94,12 +133,34 @@ struct KernelArgs {
 };
 
 // Which event kernel(s) a batch runs through (velo_launch_options_t.path).
-enum { kPathDefault = 0,   // shared-memory team kernel, slab kernel for the events it defers
-       kPathSlabOnly = 1 };  // slab kernel for every event (the general path on its own)
+enum { kPathDefault = 0,     // three-stage pipeline, slab kernel for the events it defers
+       kPathSlabOnly = 1,    // slab kernel for every event (the general path on its own)
+       kPathTeamLegacy = 2 };  // round-1 shared-memory team kernel (kept for comparison)
+
+// Launch geometry of the pipeline kernels (0 = default), from velo_launch_options_t.
+struct PipeOpts { uint32_t track_group, track_teams, fit_teams, sort_teams, pool_units; };
+int launch_sort(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o);
+int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o);
+int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o);
+int launch_write(const KernelArgs& a, cudaStream_t stream);
 
 // Enqueues the whole path for one batch on `stream`. Returns a cudaError_t as int.
 int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop,
-                       uint32_t path, uint32_t teams);
+                       uint32_t path, uint32_t teams, const PipeOpts& po);
+
+}  // namespace velo
+struct velo_geometry {
+  uint32_t n_modules;
+  float module_z[VELO_MAX_MODULES];
+  float r_in, r_out, pitch, half_shift_x;
+};
+namespace velo {
+
+// velo_reconstruct with the hit planes pointing at absolute hit index `hit_base` instead of 0 (the
+// scheduler's device buffers hold one batch's slice; emitted track_hits stay absolute indices).
+int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
+                     const velo_launch_options_t* opts, uint32_t hit_base);
 
 // velo_event_smem.cu: the shared-memory event kernel (persistent, one CTA per SM, `teams` teams of
 // 128 threads). Events it cannot hold are appended to ws.large_list. Returns a cudaError_t as int.

@@ -131,13 +131,15 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
   const velo_params_t& P = a.P;
 
   // ---- input checks (VELO_ERR_INPUT): the event then contributes zero tracks -------------------
-  if (o1 < o0 || o1 - o0 > VELO_MAX_EVENT_HITS) {
+  const uint32_t obase = a.event_offsets[0];
+  if (o1 < o0 || o0 < obase || o1 - obase > a.n_hits || o1 - o0 > VELO_MAX_EVENT_HITS) {   // stays inside the batch
     if (tid == 0) { set_status(a.ws.counters, VELO_ERR_INPUT); a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); }
     return;
   }
   const uint32_t n = o1 - o0;
-  const float* gx = a.x + o0; const float* gy = a.y + o0; const float* gz = a.z + o0;
-  const uint8_t* gm = a.module + o0;
+  const size_t g0 = (size_t)(o0 - a.hit_base);
+  const float* gx = a.x + g0; const float* gy = a.y + g0; const float* gz = a.z + g0;
+  const uint8_t* gm = a.module + g0;
 
   // ---- S0 decode: phi16 and bucket histogram (O-1) ---------------------------------------------
   for (uint32_t b = tid; b <= nbins; b += nthr) binoff[b] = 0;
@@ -471,21 +473,18 @@ __global__ void __launch_bounds__(128, 8) velo_compact_kernel(const KernelArgs a
 
 // ---- host side -----------------------------------------------------------------------------------
 uint32_t num_sms() {
-  static const uint32_t n = [] {
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
-      cudaGetLastError();
-      return 148u;
-    }
-    return (uint32_t)sms;
-  }();
-  return n;
+  int dev = 0, sms = 0;   // per current device (a process may use several GPUs); the query is cheap
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+    cudaGetLastError();
+    return 148u;
+  }
+  return (uint32_t)sms;
 }
 
 uint32_t default_n_slabs() { return num_sms() * 2u; }   // two 1024-thread CTAs of the general kernel fit an SM
 
-Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, uint32_t cap_track_hits,
+Workspace carve_workspace(void* base, uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks, uint32_t cap_track_hits,
                           uint32_t n_slabs) {
   Workspace w{};
   size_t o = 0;
@@ -493,10 +492,22 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, ui
   auto take = [&](size_t bytes) { size_t r = o; o += ((bytes + 255) / 256) * 256; return b + r; };
   w.counters = (uint32_t*)take(sizeof(uint32_t) * kNumCounters);                 // offset 0
   w.phase_clk = (unsigned long long*)take(sizeof(unsigned long long) * kNumPhaseClocks);   // offset 256
+  w.ev_info = (EvInfo*)take(sizeof(EvInfo) * ((size_t)n_events + 1));
   w.ev_rec = (uint4*)take(sizeof(uint4) * ((size_t)n_events + 1));
   w.ev_hit_base = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.large_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.order = (uint32_t*)take(4 * ((size_t)n_events + 1));
+  const size_t sc = sorted_capacity(n_events, n_hits);
+  w.rec16 = (uint4*)take(16 * sc);
+  w.sxy = (float2*)take(8 * sc);
+  w.sorig = (uint16_t*)take(2 * sc);
+  w.mod_off = (uint16_t*)take(2 * (size_t)kModOffStride * ((size_t)n_events + 1));
+  w.flag_bits = (uint32_t*)take(4 * flag_words(n_events, n_hits));
+  w.cand_total = (size_t)(n_hits >> 3) + (n_hits >> 4) + 48ull * n_events + 64ull;   // >= sum of cand_capacity(n_e)
+  w.rows = (uint16_t*)take(64 * w.cand_total);
+  w.cmeta = (uint2*)take(8 * w.cand_total);
+  w.cfit = (float*)take(4 * 9 * w.cand_total);
+  w.cstate = (uint8_t*)take(w.cand_total);
   w.tmp_loff = (uint32_t*)take(4 * ((size_t)cap_tracks + 1));
   w.tmp_hits = (uint32_t*)take(4 * ((size_t)cap_track_hits + 1));
   w.tmp_states = (float*)take(4 * (size_t)VELO_N_STATE * ((size_t)cap_tracks + 1));
@@ -507,34 +518,59 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t cap_tracks, ui
   return w;
 }
 
-int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop,
-                       uint32_t path, uint32_t teams) {
+int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop,
+                       uint32_t path, uint32_t teams, const PipeOpts& po) {
+  KernelArgs a = a_in;
+  a.all_deferred = path == kPathSlabOnly ? 1u : 0u;
   cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);   // phase_clk accumulates
   if (err != cudaSuccess) return (int)err;
+#ifdef VELO_TIMELINE
+  cudaMemsetAsync(a.ws.phase_clk, 0, sizeof(unsigned long long) * kNumPhaseClocks, stream);
+#endif
   if (ev_start) cudaEventRecord(ev_start, stream);
-  if (a.n_events > 0) {
-    const uint32_t grid = a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events;
-    if (path == kPathSlabOnly) {
-      velo_event_slab_kernel<kThreads, false, kBinShift><<<grid, kThreads, 0, stream>>>(a, 0);
-    } else {
+  const uint32_t grid = a.n_events ? (a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events) : 0u;
+  const bool large_events = a.n_events && a.n_hits / a.n_events >= 4096u;
+  if (path == kPathTeamLegacy) {
+    if (a.n_events > 0) {
       velo_order_kernel<<<1, 512, 0, stream>>>(a);
       const int rc = launch_event_smem(a, stream, teams);
       if (rc != 0) return rc;
-      // the deferred events: usually none (then the small CTAs come and go beside the next batch's
-      // team kernel); for batches of large events, large CTAs: such a batch waits for its largest event
-      if (a.n_hits / a.n_events >= 4096u) velo_event_slab_kernel<kThreadsLarge, false, 8><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
+      if (large_events) velo_event_slab_kernel<kThreadsLarge, false, 8><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
+      else velo_event_slab_kernel<kThreads, true, kBinShift><<<grid, kThreads, 0, stream>>>(a, 1);
+    }
+    if (ev_stop) cudaEventRecord(ev_stop, stream);
+    velo_offsets_kernel<<<1, 256, 0, stream>>>(a);
+    if (a.n_events > 0) {
+      const uint32_t warps_per_cta = 128 / 32;
+      uint32_t cgrid = (a.n_events + warps_per_cta - 1) / warps_per_cta;
+      if (cgrid > num_sms() * 16u) cgrid = num_sms() * 16u;
+      velo_compact_kernel<<<cgrid, 128, 0, stream>>>(a);
+    }
+    return (int)cudaGetLastError();
+  }
+  if (a.n_events > 0) {
+    if (path == kPathSlabOnly) {
+      velo_event_slab_kernel<kThreads, false, kBinShift><<<grid, kThreads, 0, stream>>>(a, 0);
+    } else {
+      // stage 1: sort; stage 2: module loop (events by size, largest first); then the general kernel
+      // for whatever the pipeline deferred (usually nothing: its CTAs come and go); stage 3 below
+      int rc = launch_sort(a, stream, po);
+      if (rc != 0) return rc;
+      velo_order_kernel<<<1, 512, 0, stream>>>(a);
+      rc = launch_track(a, stream, po);
+      if (rc != 0) return rc;
+      if (large_events) velo_event_slab_kernel<kThreadsLarge, false, 8><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
       else velo_event_slab_kernel<kThreads, true, kBinShift><<<grid, kThreads, 0, stream>>>(a, 1);
     }
   }
-  if (ev_stop) cudaEventRecord(ev_stop, stream);
-  velo_offsets_kernel<<<1, 256, 0, stream>>>(a);
-  if (a.n_events > 0) {
-    const uint32_t warps_per_cta = 128 / 32;
-    uint32_t grid = (a.n_events + warps_per_cta - 1) / warps_per_cta;
-    if (grid > num_sms() * 16u) grid = num_sms() * 16u;
-    velo_compact_kernel<<<grid, 128, 0, stream>>>(a);
+  if (path != kPathSlabOnly) {
+    const int rc = launch_fit(a, stream, po);   // fit and filters: per-candidate results, per-event counts
+    if (rc != 0) return rc;
   }
-  return (int)cudaGetLastError();
+  velo_offsets_kernel<<<1, 256, 0, stream>>>(a);   // counts -> event_track_offsets, summary
+  const int rc = launch_write(a, stream);          // every final array, once
+  if (ev_stop) cudaEventRecord(ev_stop, stream);
+  return rc != 0 ? rc : (int)cudaGetLastError();
 }
 
 }  // namespace velo

@@ -148,12 +148,12 @@ int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, co
     good &= ok(cudaMemcpyAsync(l.offsets, hits->event_offsets + e0, 4 * ((size_t)ne + 1), cudaMemcpyHostToDevice,
                                l.stream));
     if (!good) { rc = VELO_ERR_CUDA; break; }
-    // the device copy holds hits [h0, h1) at index 0: shift the pointers so that the batch's
-    // absolute offsets address it, and the emitted track_hits stay absolute hit indices
+    // the device copy holds hits [h0, h1) at index 0; the batch keeps its absolute offsets, so the
+    // emitted track_hits stay absolute hit indices
     velo_hits_t dh{};
-    dh.x = l.x - h0; dh.y = l.y - h0; dh.z = l.z - h0; dh.module = l.module - h0;
+    dh.x = l.x; dh.y = l.y; dh.z = l.z; dh.module = l.module;
     dh.event_offsets = l.offsets; dh.n_events = ne; dh.n_hits = nh;
-    rc = velo_reconstruct(s->g, &dh, params, &l.out, l.workspace, l.workspace_bytes, (void*)l.stream);
+    rc = velo::reconstruct_impl(s->g, &dh, params, &l.out, l.workspace, l.workspace_bytes, (void*)l.stream, nullptr, h0);
     if (rc != VELO_OK) break;
     good &= ok(cudaMemcpyAsync(l.summary_host, l.out.summary, 4 * VELO_N_SUMMARY, cudaMemcpyDeviceToHost, l.stream));
     good &= ok(cudaMemcpyAsync(o.event_track_offsets, l.out.event_track_offsets, 4 * ((size_t)ne + 1),

@@ -1,0 +1,299 @@
+// velo_sort.cu — stage 1 of the pipeline: S0 decode + S1 per-module phi sort (sm_100a).
+//
+// A streaming kernel: every event is read once from the caller's SoA planes (128-bit loads on the
+// aligned interior), gets its phi16 (O-1) and its (module, phi16, original index) order (O-2) in
+// shared memory, and leaves as one contiguous, 16-byte aligned block of sorted 16-byte hit records
+// in global scratch, which stage 2 pulls into shared memory module by module with 1-D TMA copies:
+//
+//   rec16[h] = { x, y, (phi16 + 32768) << 16 | start(m+1), start(m-1) << 16 | start(m-2) }
+//
+// start(m') = position inside module m' of its first hit with phi >= phi(h) - W (W = the wider of
+// the two O-3 windows), i.e. where a window scan of module m' around h begins: stage 2 then never
+// searches, it scans from `start` until the window test fails (a window across +-pi has a second
+// run that starts at position 0). Also written: sorted (x, y) and original indices for stage 3,
+// the module offsets, and the event's state (ready / deferred to the general kernel / bad input).
+//
+// Shared memory is held only for the sort (17 bytes per hit + the bucket table). Step semantics:
+// SURVEY.md §8(c) O-1, O-2, O-3.
+#include "velo_device.cuh"
+#include "velo_internal.h"
+#include "velo_pool.cuh"
+
+namespace velo {
+
+namespace {
+
+constexpr uint32_t kMaxBinSlot = 2047;      // slot inside a phi bucket is stashed in 11 bits
+
+template <int G>
+struct SortTeam {
+  uint32_t wsum[4 * (G / 32)];
+  uint32_t event, n, o0, ol;         // event index, hits, first hit (absolute), first hit relative to the batch
+  uint32_t units, first_unit, pool_off;
+  uint32_t skip;                     // nothing to sort (empty / bad / deferred before the sort)
+  uint32_t trouble;                  // bit 0: defer to the general kernel, bit 31: bad input
+};
+
+template <int G, int kTeams>
+struct SortCtl {
+  PoolCtl pool;
+  float module_z[VELO_MAX_MODULES];
+  SortTeam<G> team[kTeams];
+};
+
+__device__ __forceinline__ uint32_t align16u(uint32_t v) { return (v + 15u) & ~15u; }
+
+struct SortLayout { uint32_t xy, w, bins, stash, mod8, bytes; };
+__device__ __forceinline__ SortLayout sort_layout(uint32_t n, uint32_t M) {
+  SortLayout L;
+  uint32_t o = 0;
+  L.xy = o; o += align16u(8u * n);
+  L.w = o; o += align16u(4u * n);
+  L.bins = o; o += align16u(2u * (M * kBinsPerModule + 2u));
+  L.stash = o; o += align16u(4u * n);
+  L.mod8 = o; o += align16u(n);
+  L.bytes = o;
+  return L;
+}
+
+__device__ __forceinline__ void set_status(uint32_t* counters, int code) {
+  atomicCAS(&counters[kCtrStatus], 0u, (uint32_t)code);   // first error wins
+}
+
+template <int G>
+__device__ void sort_fetch(const KernelArgs& a, PoolCtl& pool, SortTeam<G>& ts) {
+  const uint32_t e = atomicAdd(&a.ws.counters[kCtrSortTicket], 1u);
+  ts.event = e; ts.units = 0; ts.skip = 1; ts.n = 0; ts.trouble = 0;
+  if (e >= a.n_events) return;
+  const uint32_t base = a.event_offsets[0];
+  const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
+  EvInfo info{0u, kEvEmpty, 0u, 0u};
+  // every event must stay inside the batch, [base, base + n_hits]: nothing is read out of bounds
+  if (o1 < o0 || o0 < base || o1 - base > a.n_hits || o1 - o0 > VELO_MAX_EVENT_HITS) {
+    set_status(a.ws.counters, VELO_ERR_INPUT);
+    info.state = kEvBad; a.ws.ev_info[e] = info;
+    return;
+  }
+  const uint32_t n = o1 - o0;
+  info.n = n;
+  if (n == 0) { a.ws.ev_info[e] = info; return; }
+  const SortLayout L = sort_layout(n, a.n_modules);
+  const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;
+  if (n > a.team_max_hits || units > pool.units || fit_smem_bound(n) > pool.units * kUnitBytes) {
+    info.state = kEvDeferred; a.ws.ev_info[e] = info;
+    a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+    return;
+  }
+  const uint32_t first = pool_alloc(pool, units);
+  ts.n = n; ts.o0 = o0; ts.ol = o0 - base; ts.units = units; ts.first_unit = first; ts.pool_off = first * kUnitBytes;
+  ts.skip = 0;
+}
+
+template <int G>
+__device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts, unsigned char* blk, uint32_t team,
+                           uint32_t tid, uint32_t& parity) {
+  const uint32_t M = a.n_modules, nbins = M * kBinsPerModule;
+  const uint32_t e = ts.event, n = ts.n;
+  const SortLayout L = sort_layout(n, M);
+  float2* xyo = (float2*)(blk + L.xy);          // (x, y) by ORIGINAL index
+  uint32_t* w = (uint32_t*)(blk + L.w);
+  uint32_t* binsw = (uint32_t*)(blk + L.bins);
+  uint16_t* bo = (uint16_t*)binsw;
+  uint32_t* stash = (uint32_t*)(blk + L.stash);
+  uint8_t* mod8 = blk + L.mod8;                 // module by SORTED position
+  const size_t g0 = (size_t)(ts.o0 - a.hit_base);
+  const float* gx = a.x + g0; const float* gy = a.y + g0; const float* gz = a.z + g0;
+  const uint8_t* gm = a.module + g0;
+
+  // ---- S0 decode: phi16 (O-1), bucket histogram; the plane check of the pipeline path -------------
+  const uint32_t nwords = nbins / 2u;
+  for (uint32_t b = tid; b <= nwords; b += G) binsw[b] = 0;
+  team_sync<G>(team);
+  {
+    uint32_t trouble = 0;
+    auto decode = [&](uint32_t i, float x, float y, float z, uint32_t m) {
+      if (m >= M) { trouble |= 0x80000000u; return; }
+      if (__float_as_uint(z) != __float_as_uint(mz[m])) trouble |= 1u;
+      const uint32_t pu = (uint32_t)(phi16(x, y) + 32768);
+      const uint32_t bin = m * kBinsPerModule + (pu >> kBinShift);
+      const uint32_t sh = (bin & 1u) * 16u;
+      const uint32_t slot = (atomicAdd(&binsw[bin >> 1], 1u << sh) >> sh) & 0xffffu;
+      if (slot > kMaxBinSlot) trouble |= 1u;
+      stash[i] = (m << 27) | (pu << 11) | (slot & kMaxBinSlot);
+      xyo[i] = make_float2(x, y);
+    };
+    // 128-bit loads where the planes allow them. The three float planes and the byte plane are
+    // indexed by the same hit index, so with the usual allocations they reach 16-byte (4-byte for
+    // the modules) alignment after the same number of leading hits; otherwise everything is scalar.
+    const uint32_t px = (uint32_t)(((uintptr_t)gx >> 2) & 3u), py = (uint32_t)(((uintptr_t)gy >> 2) & 3u),
+                   pz = (uint32_t)(((uintptr_t)gz >> 2) & 3u), pm = (uint32_t)((uintptr_t)gm & 3u);
+    const bool vec = (((uintptr_t)gx | (uintptr_t)gy | (uintptr_t)gz) & 3u) == 0 && px == py && px == pz &&
+                     (((4u - px) & 3u) == ((4u - pm) & 3u));
+    uint32_t head = vec ? ((4u - px) & 3u) : n;
+    if (head > n) head = n;
+    const uint32_t nq = (n - head) / 4u;
+    for (uint32_t i = tid; i < head; i += G) decode(i, gx[i], gy[i], gz[i], gm[i]);
+    {
+      const float4* vx = (const float4*)(gx + head); const float4* vy = (const float4*)(gy + head);
+      const float4* vz = (const float4*)(gz + head); const uint32_t* vm = (const uint32_t*)(gm + head);
+      for (uint32_t q = tid; q < nq; q += G) {
+        const float4 X = vx[q], Y = vy[q], Z = vz[q]; const uint32_t Mq = vm[q];
+        const uint32_t i = head + 4u * q;
+        decode(i, X.x, Y.x, Z.x, Mq & 0xffu);
+        decode(i + 1, X.y, Y.y, Z.y, (Mq >> 8) & 0xffu);
+        decode(i + 2, X.z, Y.z, Z.z, (Mq >> 16) & 0xffu);
+        decode(i + 3, X.w, Y.w, Z.w, Mq >> 24);
+      }
+    }
+    for (uint32_t i = head + 4u * nq + tid; i < n; i += G) decode(i, gx[i], gy[i], gz[i], gm[i]);
+    if (trouble) atomicOr(&ts.trouble, trouble);
+  }
+  team_sync<G>(team);
+  if (ts.trouble) {
+    if (tid == 0) {
+      EvInfo info{n, kEvDeferred, 0u, 0u};
+      if (ts.trouble & 0x80000000u) { set_status(a.ws.counters, VELO_ERR_INPUT); info.state = kEvBad; }
+      else a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+      a.ws.ev_info[e] = info;
+    }
+    return;
+  }
+  // exclusive scan of the packed histogram -> bucket offsets; bo[nbins] = n
+  {
+    const uint32_t per = (nwords + G - 1) / G;
+    const uint32_t w0 = min(tid * per, nwords), w1 = min(w0 + per, nwords);
+    uint32_t s = 0;
+    for (uint32_t k = w0; k < w1; ++k) { const uint32_t v = binsw[k]; s += (v & 0xffffu) + (v >> 16); }
+    uint32_t tot, p2, t2;
+    uint32_t run = team_scan2<G>(s, 0u, ts.wsum, team, parity, &tot, &p2, &t2);
+    for (uint32_t k = w0; k < w1; ++k) {
+      const uint32_t v = binsw[k], c0 = v & 0xffffu, c1 = v >> 16;
+      binsw[k] = run | ((run + c0) << 16);
+      run += c0 + c1;
+    }
+    if (tid == 0) bo[nbins] = (uint16_t)n;
+  }
+  team_sync<G>(team);
+  // ---- S1 phi sort (O-2): group by bucket in w[], rank inside the bucket by (phi16, index), place --
+  for (uint32_t i = tid; i < n; i += G) {
+    const uint32_t st = stash[i], pu = (st >> 11) & 0xffffu;
+    const uint32_t bin = (st >> 27) * kBinsPerModule + (pu >> kBinShift);
+    w[(uint32_t)bo[bin] + (st & kMaxBinSlot)] = (pu << 16) | i;
+  }
+  team_sync<G>(team);
+  for (uint32_t i = tid; i < n; i += G) {
+    const uint32_t st = stash[i], pu = (st >> 11) & 0xffffu;
+    const uint32_t bin = (st >> 27) * kBinsPerModule + (pu >> kBinShift);
+    const uint32_t item = (pu << 16) | i;
+    const uint32_t lo = bo[bin], hi = bo[bin + 1];
+    uint32_t r = 0;                      // rank inside the bucket: at most kMaxBinSlot
+    for (uint32_t j = lo; j < hi; ++j) r += (w[j] < item) ? 1u : 0u;
+    stash[i] = (st & ~kMaxBinSlot) | r;
+  }
+  team_sync<G>(team);                    // every rank is known: w[] can take its final content
+  for (uint32_t i = tid; i < n; i += G) {
+    const uint32_t st = stash[i], pu = (st >> 11) & 0xffffu, m = st >> 27;
+    const uint32_t r = (uint32_t)bo[m * kBinsPerModule + (pu >> kBinShift)] + (st & kMaxBinSlot);
+    w[r] = (pu << 16) | i;
+    mod8[r] = (uint8_t)m;
+  }
+  team_sync<G>(team);
+  // ---- window starts and the event's sorted block -------------------------------------------------
+  const int Wseed = a.P.phi_window_seed, Wfwd = a.P.phi_window_fwd;
+  const int W = Wseed > Wfwd ? Wseed : Wfwd;                 // >= 0 (the host clamps negative windows)
+  const bool whole = 2 * (long long)W + 1 >= 65536;
+  // position inside module mm of its first hit with unsigned phi >= lo
+  auto start_in = [&](uint32_t mm, uint32_t lo) -> uint32_t {
+    const uint16_t* bm = bo + mm * kBinsPerModule;
+    uint32_t j0 = bm[lo >> kBinShift], j1 = bm[(lo >> kBinShift) + 1];
+    while (j0 < j1) {                                        // binary search inside one phi bucket
+      const uint32_t mid = (j0 + j1) >> 1;
+      if ((w[mid] >> 16) < lo) j0 = mid + 1u; else j1 = mid;
+    }
+    return j0 - (uint32_t)bm[0];
+  };
+  const uint32_t sb = sorted_base(ts.ol, e);
+  uint4* rec = a.ws.rec16 + sb;
+  float2* sxy = a.ws.sxy + sb;
+  uint16_t* sorig = a.ws.sorig + sb;
+  for (uint32_t h = tid; h < n; h += G) {
+    const uint32_t item = w[h], pu = item >> 16, i = item & 0xffffu, m = mod8[h];
+    const float2 p = xyo[i];
+    uint32_t sp1 = 0, sm1 = 0, sm2 = 0;
+    if (!whole) {
+      const uint32_t lo = (pu - (uint32_t)W) & 0xffffu;
+      if (m + 1u < M) sp1 = start_in(m + 1u, lo);
+      if (m >= 1u) sm1 = start_in(m - 1u, lo);
+      if (m >= 2u) sm2 = start_in(m - 2u, lo);
+    }
+    rec[h] = make_uint4(__float_as_uint(p.x), __float_as_uint(p.y), (pu << 16) | sp1, (sm1 << 16) | sm2);
+    sxy[h] = p;
+    sorig[h] = (uint16_t)i;
+  }
+  // module offsets and the largest module
+  uint16_t* mo = a.ws.mod_off + (size_t)e * kModOffStride;
+  if (tid < 32) {
+    const uint32_t lo = tid <= M ? (uint32_t)bo[tid * kBinsPerModule] : n;
+    const uint32_t hi = tid < M ? (uint32_t)bo[(tid + 1u) * kBinsPerModule] : lo;
+    uint32_t sz = hi - lo;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sz = max(sz, __shfl_xor_sync(0xffffffffu, sz, o));
+    mo[tid] = (uint16_t)lo;
+    if (tid == 0) { mo[32] = (uint16_t)n; mo[kModOffStride - 1] = (uint16_t)sz; }
+  }
+  if (tid == 0) a.ws.ev_info[e] = EvInfo{n, kEvReady, 0u, 0u};
+}
+
+// ---- the kernel: one CTA per SM, kTeams teams of G threads, events by ticket in event order -----
+template <int G, int kTeams>
+__global__ void __launch_bounds__(G * kTeams, 1) velo_sort_kernel(const KernelArgs a, const uint32_t pool_units) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  using Ctl = SortCtl<G, kTeams>;
+  constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
+  Ctl& ctl = *reinterpret_cast<Ctl*>(smem);
+  unsigned char* pool = smem + kCtl;
+  const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
+  if (threadIdx.x == 0) { ctl.pool.bitmap = 0ull; ctl.pool.alloc_next = 0; ctl.pool.alloc_serving = 0; ctl.pool.units = pool_units; }
+  if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
+  __syncthreads();
+  VELO_STAGE_BEGIN(a.ws.phase_clk, 0);
+  SortTeam<G>& ts = ctl.team[team];
+  uint32_t parity = 0;
+  for (;;) {
+    if (tid == 0) sort_fetch<G>(a, ctl.pool, ts);
+    team_sync<G>(team);
+    if (ts.event >= a.n_events) break;
+    if (!ts.skip) sort_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity);
+    team_sync<G>(team);
+    if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
+  }
+  VELO_STAGE_END(a.ws.phase_clk, 0);
+}
+
+template <int G, int kTeams>
+int launch_sort_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
+  using Ctl = SortCtl<G, kTeams>;
+  constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
+  const uint32_t smem = kCtl + pool_units * kUnitBytes;
+  cudaError_t err = cudaFuncSetAttribute(velo_sort_kernel<G, kTeams>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (err != cudaSuccess) return (int)err;
+  const uint32_t sms = num_sms();
+  const uint32_t want = (a.n_events + kTeams - 1) / kTeams;
+  const uint32_t grid = want < sms ? (want ? want : 1u) : sms;
+  velo_sort_kernel<G, kTeams><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
+  return (int)cudaGetLastError();
+}
+
+}  // namespace
+
+int launch_sort(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
+  const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
+  switch (o.sort_teams) {
+    case 4: return launch_sort_t<128, 4>(a, stream, pu);
+    case 6: return launch_sort_t<128, 6>(a, stream, pu);
+    case 8: return launch_sort_t<128, 8>(a, stream, pu);
+    default: return launch_sort_t<128, 7>(a, stream, pu);
+  }
+}
+
+}  // namespace velo

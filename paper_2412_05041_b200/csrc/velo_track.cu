@@ -1,0 +1,423 @@
+// velo_track.cu — stage 2 of the pipeline: the O-6 module loop (S3 forwarding, S2 search-by-triplet
+// seeding, hit flags) over the phi-sorted blocks that stage 1 left in global scratch (sm_100a).
+//
+// One persistent CTA per SM owns the SM's shared memory as a pool; a team of G threads (a warp by
+// default: every phase boundary of the loop is then a __syncwarp, not a barrier) takes an event and
+// holds, instead of the whole event, only what a step touches at random:
+//   * a ring of four module slots fed by 1-D TMA bulk copies (cp.async.bulk + mbarrier): step s
+//     reads modules s+1, s, s-1 while module s-2 is in flight, a full step ahead of its use;
+//   * the list of ACTIVE tracks as self-contained 32-byte records (last two hits' coordinates,
+//     phi and window starts of the latest hit, hit indices, module mask, candidate id), compacted
+//     in place every step, so the lanes of the forwarding pass are always dense;
+//   * one flag byte per hit, the first hit of every candidate, the list of unflagged centre hits.
+// About 19 KB for a mu = 5 event of 1.9 k hits instead of the 34 KB of the whole sorted event, and
+// only for the duration of the loop: the sort (stage 1) and the fit/filters/output (stage 3) run
+// in their own kernels. Candidates leave as 64-byte rows of sorted hit indices plus {module mask,
+// seed scatter}; the final flags leave as one bit per hit.
+//
+// Window scans never search: stage 1 stored with every hit where its window starts in the three
+// modules a scan can target (records' words 2 and 3); a scan runs from there, four hits per trip
+// with the loads issued first, until the window test fails. A window across +-pi first visits its
+// low-phi run from position 0, so hits are always met in ascending sorted index and ties resolve
+// to the lowest index by strict comparison (O-7, O-8). Step semantics: SURVEY.md §8(c) O-3 ... O-9;
+// every float operation is a round-to-nearest intrinsic in the oracle's order (no FMA contraction).
+#include "velo_device.cuh"
+#include "velo_internal.h"
+#include "velo_pool.cuh"
+
+namespace velo {
+
+namespace {
+
+template <int G>
+struct TrackTeam {
+  unsigned long long mbar[4];        // one mbarrier per ring slot
+  uint32_t wsum[2 * (G / 32)];
+  uint32_t event, n, sb;             // event index, hits, first record in the sorted scratch
+  uint32_t units, first_unit, pool_off, skip;
+  uint32_t maxmod, cbase, tcap, acap;
+  uint32_t defer;                    // set by any thread: the event continues in the general kernel
+  uint16_t mod_off[kModOffStride];
+};
+
+template <int G, int kTeams>
+struct TrackCtl {
+  PoolCtl pool;
+  float module_z[VELO_MAX_MODULES];
+  TrackTeam<G> team[kTeams];
+};
+
+__device__ __forceinline__ uint32_t al16(uint32_t v) { return (v + 15u) & ~15u; }
+
+struct TrackLayout { uint32_t ring, act, flags, th0, cl, bytes; };
+__device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod, uint32_t tcap, uint32_t acap) {
+  TrackLayout L;
+  uint32_t o = 0;
+  L.ring = o; o += 4u * 16u * maxmod;
+  L.act = o; o += 32u * acap;
+  L.flags = o; o += al16(n);
+  L.th0 = o; o += al16(2u * tcap);
+  L.cl = o; o += al16(2u * maxmod);
+  L.bytes = o;
+  return L;
+}
+
+template <int G>
+__device__ void track_fetch(const KernelArgs& a, PoolCtl& pool, TrackTeam<G>& ts) {
+  const uint32_t k = atomicAdd(&a.ws.counters[kCtrTrackTicket], 1u);
+  ts.event = k; ts.units = 0; ts.skip = 1; ts.defer = 0;
+  if (k >= a.n_events) return;
+  // tickets walk the size-sorted list from both ends in turn: largest, smallest, second largest, ...
+  const uint32_t e = a.ws.order[(k & 1u) ? (k >> 1) : a.n_events - 1u - (k >> 1)];
+  ts.event = e;
+  const EvInfo info = a.ws.ev_info[e];
+  if (info.state != kEvReady) return;
+  const uint32_t n = info.n;
+  const uint32_t maxmod = a.ws.mod_off[(size_t)e * kModOffStride + kModOffStride - 1];
+  const uint32_t tcap = cand_capacity(n), acap = active_capacity(n);
+  const TrackLayout L = track_layout(n, maxmod, tcap, acap);
+  const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;
+  if (units > pool.units) {
+    a.ws.ev_info[e].state = kEvDeferred;
+    a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+    return;
+  }
+  ts.cbase = atomicAdd(&a.ws.counters[kCtrCandAlloc], tcap);
+  const uint32_t first = pool_alloc(pool, units);
+  ts.n = n; ts.sb = sorted_base(a.event_offsets[e] - a.event_offsets[0], e);
+  ts.maxmod = maxmod; ts.tcap = tcap; ts.acap = acap;
+  ts.units = units; ts.first_unit = first; ts.pool_off = first * kUnitBytes; ts.skip = 0;
+}
+
+// Visits positions j0, j0 + 1, ... of a module slot (nm hits) while they lie inside the wide window
+// (lo16w, limw), four per trip: the four 16-byte loads of a trip are issued before its arithmetic.
+// f(jj, rec, in) must be branch-free; for padding lanes `in` is false and jj repeats nm - 1.
+template <class F>
+__device__ __forceinline__ void scan_run(const uint4* slot, uint32_t j0, uint32_t nm, uint32_t lo16w, uint32_t limw, F&& f) {
+  for (uint32_t j = j0; j < nm; j += 4u) {
+    uint4 r[4]; uint32_t jj[4];
+#pragma unroll
+    for (uint32_t k = 0; k < 4; ++k) { jj[k] = min(j + k, nm - 1u); r[k] = slot[jj[k]]; }
+    bool in = false;
+#pragma unroll
+    for (uint32_t k = 0; k < 4; ++k) { in = (j + k < nm) & (r[k].z - lo16w <= limw); f(jj[k], r[k], in); }
+    if (!in) break;     // the last of the four is outside (or past the module): so is everything after it
+  }
+}
+
+// O-3 window about unsigned phi c with half-width W, as a test on the phi field of a record word.
+struct Win { uint32_t lo16, lim; bool wrapped; };
+__device__ __forceinline__ Win make_win(uint32_t c, int W) {
+  Win q;
+  if (2 * (long long)W + 1 >= 65536) { q.lo16 = 0; q.lim = 0xffffffffu; q.wrapped = false; return q; }
+  const uint32_t lo = (c - (uint32_t)W) & 0xffffu, hi = (c + (uint32_t)W) & 0xffffu;
+  q.lo16 = lo << 16; q.lim = ((2u * (uint32_t)W) << 16) | 0xffffu; q.wrapped = lo > hi;
+  return q;
+}
+
+// ---- one event, by one team ---------------------------------------------------------------------
+template <int G, bool kSameW>
+__device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& ts, unsigned char* blk, uint32_t team,
+                            uint32_t tid, uint32_t& parity, uint32_t& phases) {
+  const uint32_t M = a.n_modules, n = ts.n, e = ts.event;
+  const velo_params_t& P = a.P;
+  const uint32_t slotcap = ts.maxmod, tcap = ts.tcap, acap = ts.acap;
+  const TrackLayout L = track_layout(n, slotcap, tcap, acap);
+  uint4* ring = (uint4*)(blk + L.ring);
+  uint4* act = (uint4*)(blk + L.act);
+  uint8_t* flags = blk + L.flags;
+  uint16_t* th0 = (uint16_t*)(blk + L.th0);
+  uint16_t* cl = (uint16_t*)(blk + L.cl);
+  const uint16_t* mo = ts.mod_off;
+  const uint4* grec = a.ws.rec16 + ts.sb;
+  uint16_t* rows = a.ws.rows + (size_t)ts.cbase * 32u;
+  uint2* cmeta = a.ws.cmeta + ts.cbase;
+  const int Wseed = P.phi_window_seed, Wfwd = P.phi_window_fwd;
+  const int Wwide = Wseed > Wfwd ? Wseed : Wfwd;
+
+  for (uint32_t i = tid; i < kModOffStride; i += G) ts.mod_off[i] = a.ws.mod_off[(size_t)e * kModOffStride + i];
+  for (uint32_t i = tid; i < al16(n) / 4u; i += G) ((uint32_t*)flags)[i] = 0;
+  team_sync<G>(team);
+
+  // ring: module m lives in slot m & 3; loads are issued and waited for in descending module order
+  auto issue = [&](uint32_t m) {
+    if (tid == 0) {
+      const uint32_t bytes = 16u * ((uint32_t)mo[m + 1] - (uint32_t)mo[m]);
+      mbar_arrive_expect_tx(&ts.mbar[m & 3u], bytes);
+      if (bytes) tma_load_1d(ring + (m & 3u) * slotcap, grec + mo[m], bytes, &ts.mbar[m & 3u]);
+    }
+  };
+  auto wait = [&](uint32_t m) {
+    mbar_wait(&ts.mbar[m & 3u], (phases >> (m & 3u)) & 1u);
+    phases ^= 1u << (m & 3u);
+  };
+  uint32_t issued = M, waited = M;       // lowest module issued / waited for so far
+  for (uint32_t k = 0; k < 4 && issued > 0; ++k) issue(--issued);
+  wait(--waited); wait(--waited);        // modules M-1 and M-2
+
+  uint32_t nact = 0, ncand = 0;
+  const float max_fwd = P.max_scatter_fwd, max_seed = P.max_scatter_seed;
+  for (uint32_t s = M - 2; s >= 1; --s) {
+    const uint32_t u = s - 1;
+    // No hit in modules 0 .. u: forwarding can only miss and seeding finds no third hit, in this step
+    // and in all that follow, and what a miss changes (the miss count) is not read after the loop.
+    if (mo[u + 1] == 0) break;
+    wait(--waited);                      // module u has landed
+    const uint32_t off_u = mo[u], nu = (uint32_t)mo[u + 1] - off_u;
+    const uint32_t off_s = mo[s], ns = (uint32_t)mo[s + 1] - off_s;
+    const uint32_t off_p = mo[s + 1], np = (uint32_t)mo[s + 2] - off_p;
+    const uint4* ring_u = ring + (u & 3u) * slotcap;
+    const uint4* ring_s = ring + (s & 3u) * slotcap;
+    const uint4* ring_p = ring + ((s + 1u) & 3u) * slotcap;
+    const float z2 = mz[u];
+
+    // ---- (A) O-7 forwarding into module u of every track active at the start of the step ----------
+    uint32_t wbase = 0;
+    for (uint32_t p0 = 0; p0 < nact; p0 += G) {
+      const uint32_t k = p0 + tid;
+      bool alive = false;
+      uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0;
+      if (k < nact) {
+        q0 = act[2u * k]; q1 = act[2u * k + 1u];
+        const float x0 = __uint_as_float(q0.x), y0 = __uint_as_float(q0.y);
+        const float x1 = __uint_as_float(q0.z), y1 = __uint_as_float(q0.w);
+        const uint32_t c = q1.x >> 16, id = q1.x & 0xffffu, w3 = q1.y, hab = q1.z, mask = q1.w;
+        const uint32_t mb = __ffs(mask) - 1u, ma = __ffs(mask & (mask - 1u)) - 1u;
+        const float z1 = mz[mb], z0 = mz[ma];
+        const float tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0));
+        const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, x0), tz));
+        const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, y0), tz));
+        const Win wx = make_win(c, Wfwd);
+        bool found = false; uint32_t best = 0; float best_sc = 0.0f;
+        auto visit = [&](uint32_t jj, const uint4& r, bool in) {
+          const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+          const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+          bool ok = in & (sc <= max_fwd) & (!found | (sc < best_sc));
+          if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
+          found |= ok; best = ok ? jj : best; best_sc = ok ? sc : best_sc;
+        };
+        const uint32_t pend = mb - s;      // modules already missed since the latest hit
+        if (pend <= 1u) {
+          const Win ww = kSameW ? wx : make_win(c, Wwide);
+          if (ww.wrapped) scan_run(ring_u, 0u, nu, ww.lo16, ww.lim, visit);          // low-phi run of a window across +-pi
+          scan_run(ring_u, pend ? (w3 & 0xffffu) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
+        } else {
+          // no stored start for a target this far from the latest hit (max_skipped >= 2): whole module
+          for (uint32_t j = 0; j < nu; ++j) {
+            const uint4 r = ring_u[j];
+            const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+            const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+            const bool ok = (r.z - wx.lo16 <= wx.lim) & (sc <= max_fwd) & (!found | (sc < best_sc));
+            found |= ok; best = ok ? j : best; best_sc = ok ? sc : best_sc;
+          }
+        }
+        if (found) {
+          const uint4 r2 = ring_u[best];
+          const uint32_t h2 = off_u + best, nh = (uint32_t)__popc(mask);
+          rows[id * 32u + nh] = (uint16_t)h2;
+          // (B): forwarding never reads flags, so they can be set right away
+          if (nh + 1u == 4u) { flags[th0[id]] = 1; flags[hab >> 16] = 1; flags[hab & 0xffffu] = 1; }
+          if (nh + 1u >= 4u) flags[h2] = 1;
+          q0 = make_uint4(q0.z, q0.w, r2.x, r2.y);
+          q1 = make_uint4((r2.z & 0xffff0000u) | id, r2.w, (hab << 16) | h2, mask | (1u << u));
+          alive = true;
+        } else {
+          alive = (mb - u) <= P.max_skipped;       // consecutive misses so far, this one included
+          if (!alive && __popc(mask) > 3) cmeta[id].x = mask;
+        }
+      }
+      uint32_t total;
+      const uint32_t pos = team_scan_pred<G>(alive, ts.wsum, team, parity, &total);   // (also: every read of this pass is done)
+      if (alive) { act[2u * (wbase + pos)] = q0; act[2u * (wbase + pos) + 1u] = q1; }
+      wbase += total;
+    }
+    nact = wbase;
+    team_sync<G>(team);                  // flags and the compacted list are visible
+
+    // ---- (C) O-8 seeding with centre module s -----------------------------------------------------
+    // (C1) the unflagged centre hits, in ascending order (flags are final for this step)
+    uint32_t ncl = 0;
+    for (uint32_t c0 = 0; c0 < ns; c0 += G) {
+      const uint32_t j = c0 + tid;
+      const bool open = j < ns && !flags[off_s + j];
+      uint32_t total;
+      const uint32_t pos = team_scan_pred<G>(open, ts.wsum, team, parity, &total);
+      if (open) cl[ncl + pos] = (uint16_t)j;
+      ncl += total;
+    }
+    team_sync<G>(team);
+    // (C2) one lane per unflagged centre hit: best (h0, h2) under (scatter, h0, h2)
+    if (ncl) {
+      const float zc0 = mz[s + 1], zc1 = mz[s];
+      const float tz = __fdiv_rn(__fsub_rn(z2, zc1), __fsub_rn(zc1, zc0));
+      for (uint32_t k0 = 0; k0 < ncl; k0 += G) {
+        const uint32_t k = k0 + tid;
+        bool found = false; uint32_t b0 = 0, b2 = 0, j1 = 0; float best_sc = 0.0f;
+        uint4 r1 = make_uint4(0, 0, 0, 0);
+        if (k < ncl) {
+          j1 = cl[k];
+          r1 = ring_s[j1];
+          const float x1 = __uint_as_float(r1.x), y1 = __uint_as_float(r1.y);
+          const uint32_t c = r1.z >> 16;
+          const Win wx = make_win(c, Wseed);
+          const Win ww = kSameW ? wx : make_win(c, Wwide);
+          for (uint32_t run0 = ww.wrapped ? 0u : 1u; run0 < 2u; ++run0) {
+            for (uint32_t j0 = run0 ? (r1.z & 0xffffu) : 0u; j0 < np; ++j0) {
+              const uint4 r0 = ring_p[j0];
+              if (!(r0.z - ww.lo16 <= ww.lim)) break;
+              if (!kSameW && !(r0.z - wx.lo16 <= wx.lim)) continue;
+              if (flags[off_p + j0]) continue;
+              const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tz));
+              const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tz));
+              // h0 and h2 ascending: strict < keeps the lexicographic minimum; branch-free body
+              auto visit2 = [&](uint32_t jj, const uint4& r, bool in) {
+                const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+                const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+                bool ok = in & !flags[off_u + jj] & (sc <= max_seed) & (!found | (sc < best_sc));
+                if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
+                found |= ok; b0 = ok ? j0 : b0; b2 = ok ? jj : b2; best_sc = ok ? sc : best_sc;
+              };
+              if (ww.wrapped) scan_run(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
+              scan_run(ring_u, r1.w >> 16, nu, ww.lo16, ww.lim, visit2);
+            }
+          }
+        }
+        uint32_t total;
+        const uint32_t pos = team_scan_pred<G>(found, ts.wsum, team, parity, &total);
+        if (found && ncand + pos < tcap && nact + pos < acap) {
+          const uint32_t id = ncand + pos;
+          const uint32_t h0 = off_p + b0, h1 = off_s + j1, h2 = off_u + b2;
+          const uint4 r2 = ring_u[b2];
+          *reinterpret_cast<uint2*>(rows + id * 32u) = make_uint2(h0 | (h1 << 16), h2);
+          cmeta[id] = make_uint2(7u << u, __float_as_uint(best_sc));
+          th0[id] = (uint16_t)h0;
+          act[2u * (nact + pos)] = make_uint4(r1.x, r1.y, r2.x, r2.y);
+          act[2u * (nact + pos) + 1u] = make_uint4((r2.z & 0xffff0000u) | id, r2.w, (h1 << 16) | h2, 7u << u);
+        }
+        ncand += total; nact += total;
+      }
+    }
+    if (ncand > tcap || nact > acap) { if (tid == 0) ts.defer = 1; }
+    team_sync<G>(team);                  // the new tracks are visible; module s+1 has been read for the last time
+    if (ts.defer) break;
+    if (issued > 0) issue(--issued);     // module s-3 into the slot of module s+1
+  }
+  // every load that was issued must land before the block can be freed
+  while (waited > issued) wait(--waited);
+  if (ts.defer) {
+    if (tid == 0) {
+      a.ws.ev_info[e].state = kEvDeferred;
+      a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+    }
+    return;
+  }
+  // tracks still active take their final module mask; the final flags leave as bits
+  for (uint32_t k = tid; k < nact; k += G) {
+    const uint4 q1 = act[2u * k + 1u];
+    if (__popc(q1.w) > 3) cmeta[q1.x & 0xffffu].x = q1.w;
+  }
+  {
+    uint32_t* fb = a.ws.flag_bits + ((a.event_offsets[e] - a.event_offsets[0]) >> 5) + e;
+    for (uint32_t j0 = 0; j0 < n; j0 += G) {
+      const uint32_t j = j0 + tid;
+      const uint32_t b = __ballot_sync(0xffffffffu, j < n && flags[j]);
+      if ((tid & 31u) == 0 && j < n) fb[j >> 5] = b;
+    }
+  }
+  if (tid == 0) {
+    a.ws.ev_info[e] = EvInfo{n, kEvReady, ts.cbase, ncand};
+    atomicAdd(&a.ws.counters[kCtrCand], ncand);
+  }
+}
+
+// ---- the kernel: one CTA per SM, kTeams teams of G threads ---------------------------------------
+template <int G, int kTeams, bool kSameW>
+__global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelArgs a, const uint32_t pool_units) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  using Ctl = TrackCtl<G, kTeams>;
+  constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
+  Ctl& ctl = *reinterpret_cast<Ctl*>(smem);
+  unsigned char* pool = smem + kCtl;
+  const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
+  if (threadIdx.x == 0) { ctl.pool.bitmap = 0ull; ctl.pool.alloc_next = 0; ctl.pool.alloc_serving = 0; ctl.pool.units = pool_units; }
+  if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
+  TrackTeam<G>& ts = ctl.team[team];
+  if (tid == 0) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) mbar_init(&ts.mbar[k], 1u);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  VELO_STAGE_BEGIN(a.ws.phase_clk, 1);
+  uint32_t parity = 0, phases = 0;
+  for (;;) {
+    if (tid == 0) track_fetch<G>(a, ctl.pool, ts);
+    team_sync<G>(team);
+    if (ts.event >= a.n_events) break;
+    if (!ts.skip) track_event<G, kSameW>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity, phases);
+    team_sync<G>(team);   // every thread is done with the block and with ts before the leader reuses them
+    if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
+  }
+  VELO_STAGE_END(a.ws.phase_clk, 1);
+}
+
+template <int G, int kTeams>
+int launch_track_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
+  static_assert(G == 32 || kTeams <= 15, "named barriers 1..15");
+  using Ctl = TrackCtl<G, kTeams>;
+  constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
+  const uint32_t smem = kCtl + pool_units * kUnitBytes;
+  const bool same = a.P.phi_window_seed == a.P.phi_window_fwd;
+  const uint32_t sms = num_sms();
+  const uint32_t want = (a.n_events + kTeams - 1) / kTeams;
+  const uint32_t grid = want < sms ? (want ? want : 1u) : sms;
+  cudaError_t err;
+  if (same) {
+    err = cudaFuncSetAttribute(velo_track_kernel<G, kTeams, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return (int)err;
+    velo_track_kernel<G, kTeams, true><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
+  } else {
+    err = cudaFuncSetAttribute(velo_track_kernel<G, kTeams, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return (int)err;
+    velo_track_kernel<G, kTeams, false><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
+  }
+  return (int)cudaGetLastError();
+}
+
+}  // namespace
+
+int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
+  const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
+  uint32_t g = o.track_group, t = o.track_teams;
+  if (g == 0) {
+    // a warp per event for mu = 5 sized events; more threads per event when the events are large
+    const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
+    g = mean >= 6144u ? 128u : 32u;
+  }
+  if (g == 128) {
+    if (t == 0) t = 6;
+    switch (t) {
+      case 4: return launch_track_t<128, 4>(a, stream, pu);
+      case 8: return launch_track_t<128, 8>(a, stream, pu);
+      default: return launch_track_t<128, 6>(a, stream, pu);
+    }
+  }
+  if (g == 64) {
+    if (t == 0) t = 12;
+    switch (t) {
+      case 8: return launch_track_t<64, 8>(a, stream, pu);
+      case 15: return launch_track_t<64, 15>(a, stream, pu);
+      default: return launch_track_t<64, 12>(a, stream, pu);
+    }
+  }
+  if (t == 0) t = 16;
+  switch (t) {
+    case 8: return launch_track_t<32, 8>(a, stream, pu);
+    case 12: return launch_track_t<32, 12>(a, stream, pu);
+    case 20: return launch_track_t<32, 20>(a, stream, pu);
+    case 24: return launch_track_t<32, 24>(a, stream, pu);
+    default: return launch_track_t<32, 16>(a, stream, pu);
+  }
+}
+
+}  // namespace velo

@@ -17,7 +17,7 @@ from . import build as _build
 VELO_OK, VELO_ERR_ARG, VELO_ERR_GEOMETRY, VELO_ERR_WORKSPACE = 0, -1, -2, -3
 VELO_ERR_CUDA, VELO_ERR_CAPACITY, VELO_ERR_INPUT = -4, -5, -6
 VELO_MAX_MODULES, VELO_MAX_EVENT_HITS, VELO_N_STATE = 32, 65535, 13
-VELO_PATH_DEFAULT, VELO_PATH_SLAB_ONLY = 0, 1
+VELO_PATH_DEFAULT, VELO_PATH_SLAB_ONLY, VELO_PATH_TEAM_LEGACY = 0, 1, 2
 VELO_N_SUMMARY = 8
 STATE_NAMES = ("x", "y", "tx", "ty", "z", "cxx", "cxtx", "ctxtx", "cyy", "cyty", "ctyty", "chi2", "n_hits")
 ERROR_NAMES = {0: "VELO_OK", -1: "VELO_ERR_ARG", -2: "VELO_ERR_GEOMETRY", -3: "VELO_ERR_WORKSPACE",
@@ -61,7 +61,9 @@ class Tracks(ctypes.Structure):
 
 class LaunchOptions(ctypes.Structure):
     _fields_ = [("event_kernel_start", c_void_p), ("event_kernel_stop", c_void_p), ("ctas_per_sm", c_uint32),
-                ("path", c_uint32), ("teams_per_cta", c_uint32), ("reserved", c_uint32)]
+                ("path", c_uint32), ("teams_per_cta", c_uint32), ("track_group", c_uint32),
+                ("track_teams", c_uint32), ("fit_teams", c_uint32), ("sort_teams", c_uint32),
+                ("pool_units", c_uint32)]
 
 
 _lib = None
@@ -72,6 +74,8 @@ def lib():
     global _lib
     if _lib is None:
         path = _build.LIB
+        if os.environ.get("VELO_TIMELINE_BUILD"):          # bench.py --timeline: the instrumented build
+            path = _build.build_timeline()
         if not os.path.exists(path):
             raise RuntimeError(f"{path} is missing: run `python -m paper_2412_05041_b200.build` "
                                "(there is no fallback path)")
@@ -255,14 +259,12 @@ def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None 
     off = np.ascontiguousarray(event_offsets, dtype=np.uint32).astype(np.int64)
     cuts = [dh.n_events * b // n_batches for b in range(n_batches + 1)]
     streams = [torch.cuda.Stream() for _ in range(n_batches)]
-    outs = []
+    sizes = [(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]] - off[cuts[b]])) for b in range(n_batches)]
+    # every buffer exists (and its zero-fill on the current stream is done) before the side streams start
+    outs = [DeviceTracks(ne, nh, cap_tracks, cap_track_hits, opts=opts) for ne, nh in sizes]
     torch.cuda.synchronize()
     for b in range(n_batches):
-        e0, e1 = cuts[b], cuts[b + 1]
-        nh = int(off[e1] - off[e0])
-        o = DeviceTracks(e1 - e0, nh, cap_tracks, cap_track_hits, opts=opts)
-        velo_reconstruct(g, dh.slice_struct(e0, e1, nh), P, o, streams[b], opts)
-        outs.append(o)
+        velo_reconstruct(g, dh.slice_struct(cuts[b], cuts[b + 1], sizes[b][1]), P, outs[b], streams[b], opts)
     torch.cuda.synchronize()
     return stitch([o.to_host() for o in outs])
 

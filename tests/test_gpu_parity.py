@@ -45,7 +45,7 @@ def test_config0_full(velo):
     info = check(got, want)
     assert info["bit_identical_states"]
     assert got["n_candidates"] == want["n_candidates"]
-    assert got["n_deferred"] == 0            # every event ran in the shared-memory team kernel
+    assert got["n_deferred"] == 0            # every event ran in the pipeline kernels
     assert want["n_tracks"] > 15000          # 100 events x ~190 tracks: the comparison is not vacuous
 
 
@@ -77,16 +77,48 @@ def test_run_to_run_determinism(velo):
         np.testing.assert_array_equal(ref["states"].view(np.uint32), r["states"].view(np.uint32))
 
 
-# ---- the two event kernels: shared-memory teams (default) and the general slab kernel -----------
-def test_team_and_slab_paths_agree(velo):
+# ---- the event kernels: the three-stage pipeline (default) in several launch geometries, the general
+# slab kernel on its own, and the round-1 team kernel --------------------------------------------------
+@pytest.mark.parametrize("kw", [
+    {"path": 1}, {"path": 2},                                     # general slab kernel only; round-1 team kernel
+    {"track_group": 32, "track_teams": 8}, {"track_group": 32, "track_teams": 24},
+    {"track_group": 64}, {"track_group": 64, "track_teams": 15}, {"track_group": 128},
+    {"fit_teams": 4}, {"fit_teams": 12}, {"sort_teams": 4}, {"sort_teams": 8},
+    {"pool_units": 24}, {"pool_units": 12, "track_group": 64}], ids=str)
+def test_pipeline_geometries_and_other_paths_agree(velo, kw):
     d = datagen.generate_config(0)
     want = cpu(d)
-    for kw in ({"path": velo.VELO_PATH_SLAB_ONLY}, {"teams_per_cta": 4}, {"teams_per_cta": 5}, {"teams_per_cta": 7},
-               {"teams_per_cta": 8}):
-        got = gpu(velo, d, opts=velo.LaunchOptions(**kw))
-        info = check(got, want)
-        assert info["bit_identical_states"], kw
-        np.testing.assert_array_equal(got["track_hits"], want["track_hits"])    # emitted in the oracle's order
+    got = gpu(velo, d, opts=velo.LaunchOptions(**kw))
+    info = check(got, want)
+    assert info["bit_identical_states"], kw
+    np.testing.assert_array_equal(got["track_hits"], want["track_hits"])    # emitted in the oracle's order
+    if kw.get("path", 0) == 0 and "pool_units" not in kw:
+        assert got["n_deferred"] == 0, kw
+
+
+def test_hand_made_pin_events(velo):
+    """The events of tests/test_oracle_hand_events.py (stated outcomes: forwarding tie, window centre,
+    miss reset, flagged hits in seeding, same-step flags, chi2 cut, clone pairs) through the CUDA path."""
+    import oracle
+    built = [f() for f in T.PIN_EVENTS]
+    events = [b[0] for b in built]
+    x, y, z, m, off = T.batch_of(events)
+    for kw in ({}, {"track_group": 64}, {"path": velo.VELO_PATH_SLAB_ONLY}):
+        got = velo.reconstruct(x, y, z, m, off, datagen.MODULE_Z, opts=velo.LaunchOptions(**kw))
+        for e, b in enumerate(built):
+            o0 = int(off[e])
+            assert sorted(tuple(h - o0 for h in hits) for hits, _ in T.split_tracks(got, e)) == b[1], (e, kw)
+        check(got, oracle.reconstruct(x, y, z, m, off, M))
+    # the chi2 cut on both sides of the threshold (O-12)
+    g = velo.velo_geometry_load(datagen.MODULE_Z)
+    for n in (3, 5):
+        ev, want, chi2 = T.pin_chi2_track(n)
+        xe, ye, ze, me, offe = T.batch_of([ev])
+        for factor, expect in ((1.04, want), (0.96, [])):
+            p = velo.velo_params_default(g)
+            p.max_chi2_ndof = float(np.float32(chi2 / (2 * n - 4) * factor))
+            got = velo.reconstruct(xe, ye, ze, me, offe, datagen.MODULE_Z, params=p)
+            assert sorted(hits for hits, _ in T.split_tracks(got, 0)) == expect
 
 
 def test_hits_off_their_module_plane_are_deferred_to_the_general_kernel(velo):
@@ -281,17 +313,24 @@ def test_status_codes(velo):
     assert e.value.code == velo.VELO_ERR_INPUT
 
 
-# ---- full size, in the launch configuration bench.py times: sampled events -----------------------
+# ---- full size, in the launch configuration bench.py times: EVERY event against the oracle ----------
+def _compare_in_chunks(got, d, chunk):
+    """All events, a chunk of events at a time (bounds the host memory of the comparison)."""
+    identical = True
+    for e0 in range(0, d["n_events"], chunk):
+        ids = np.arange(e0, min(e0 + chunk, d["n_events"]))
+        sub = T.gather_events(d, ids)
+        info = check(T.select_events(got, d, ids), cpu(sub))
+        identical &= info["bit_identical_states"]
+    return identical
+
+
 @pytest.mark.parametrize("config", [2, 3])
-def test_full_size_sampled_events(velo, config):
+def test_full_size_every_event(velo, config):
     d = datagen.generate_config(config)
     got = gpu(velo, d, n_batches=4)
-    rng = np.random.default_rng(7)
-    nh = np.diff(d["event_offsets"].astype(np.int64))
-    ids = np.unique(np.concatenate([rng.integers(0, d["n_events"], 400), np.argsort(nh)[-8:], np.argsort(nh)[:8],
-                                    [0, 24999, 25000, 49999, 50000, 99999]]))
-    sub = T.gather_events(d, ids)
-    check(T.select_events(got, d, ids), cpu(sub))
+    assert got["n_deferred"] == 0
+    assert _compare_in_chunks(got, d, 25000)
     # properties that hold at any size
     eto = got["event_track_offsets"].astype(np.int64); tho = got["track_hit_offsets"].astype(np.int64)
     assert (np.diff(eto) >= 0).all() and (np.diff(tho) >= 3).all() and tho[-1] == got["n_track_hits"]
@@ -352,16 +391,29 @@ def test_scheduler_reports_an_oversized_batch(velo):
     sched.close()
 
 
-def test_config4_full_size_sampled_events(velo):
-    """BASELINE.json:configs[4] at full size (2 000 ion-like events, one call): sampled events
-    against the oracle, among them the largest (general kernel) and mid-sized ones (team kernel)."""
+def test_config4_full_size_every_event(velo):
+    """BASELINE.json:configs[4] at full size (2 000 ion-like events, one call): every event against the
+    oracle; the largest run in the general kernel, the others in the pipeline."""
     d = datagen.generate_config(4)
     got = gpu(velo, d)
-    nh = np.diff(d["event_offsets"].astype(np.int64))
-    rng = np.random.default_rng(5)
-    order = np.argsort(nh)
-    ids = np.unique(np.concatenate([rng.integers(0, d["n_events"], 40), order[-3:], order[:3],
-                                    order[np.searchsorted(nh[order], [9000, 12000, 13000, 14000])]]))
-    sub = T.gather_events(d, ids)
-    check(T.select_events(got, d, ids), cpu(sub))
     assert 0 < got["n_deferred"] < d["n_events"]
+    assert _compare_in_chunks(got, d, 500)
+
+
+def test_scheduler_summary_is_eight_words(velo):
+    """include/velo.h: out[b].summary is a HOST u32[VELO_N_SUMMARY]; nothing is written past it."""
+    import ctypes
+    import torch
+    d = datagen.generate_config(0, n_events=16)
+    g = velo.velo_geometry_load(datagen.MODULE_Z)
+    P = velo.velo_params_default(g)
+    off = d["event_offsets"]
+    sched = velo.Scheduler(g, 2, 16, int(off[16]))
+    out = velo.HostTracks(16, int(off[16]))
+    guard = torch.full((velo.VELO_N_SUMMARY + 8,), 0x5A5A5A5A, dtype=torch.int32)
+    out.summary = guard[:velo.VELO_N_SUMMARY]
+    sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off, [0, 16], [out])
+    torch.cuda.synchronize()
+    assert (guard[velo.VELO_N_SUMMARY:] == 0x5A5A5A5A).all()
+    assert out.result()["n_tracks"] > 0
+    sched.close()
