@@ -156,7 +156,7 @@ typedef struct {
   uint32_t track_teams;   /* events in flight per persistent CTA of the module-loop kernel; 0 = default */
   uint32_t fit_teams;     /* ... of the fit/output kernel; 0 = default                                  */
   uint32_t sort_teams;    /* ... of the sort kernel; 0 = default                                        */
-  uint32_t pool_units;    /* shared-memory pool per CTA in units of 3456 bytes, 1..64; 0 = 64           */
+  uint32_t pool_units;    /* shared-memory pool per CTA in units of 1728 bytes, 1..128; 0 = 128         */
 } velo_launch_options_t;
 size_t velo_workspace_bytes_opts(uint32_t n_events, uint32_t n_hits, uint32_t cap_tracks,
                                  uint32_t cap_track_hits, const velo_launch_options_t* opts);

@@ -16,7 +16,8 @@ SOURCES = ["velo_api.cu", "velo_kernels.cu", "velo_sort.cu", "velo_track.cu", "v
            "velo_scheduler.cu"]
 HEADERS = ["velo_device.cuh", "velo_internal.h", "velo_pool.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-shared"]
+              "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC"]
+OBJ_DIR = os.path.join(_HERE, "build")
 
 
 def _nvcc() -> str:
@@ -37,23 +38,35 @@ def _stale() -> bool:
 LIB_TIMELINE = os.path.join(_HERE, "libvelo_timeline.so")
 
 
+def _compile(lib: str, extra: list[str], tag: str, verbose: bool = False) -> str:
+    """nvcc -c every source (in parallel: they are independent translation units), then link."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    objs = [os.path.join(OBJ_DIR, f"{tag}_{f[:-3]}.o") for f in SOURCES]
+
+    def one(src, obj):
+        cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-I", INCLUDE, "-c", "-o", obj, os.path.join(CSRC, src)]
+        if verbose:
+            cmd[1:1] = ["-Xptxas", "-v"]
+        subprocess.run(cmd, check=True)
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as ex:
+        list(ex.map(one, SOURCES, objs))
+    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", lib, *objs], check=True)
+    return lib
+
+
 def build_timeline() -> str:
     """The same library with -DVELO_TIMELINE: every pipeline kernel records the window in which its
     CTAs ran (GPU global timer), for `bench.py --timeline`. Never used by the product path."""
-    cmd = [_nvcc(), *NVCC_FLAGS, "-DVELO_TIMELINE", "-I", INCLUDE, "-o", LIB_TIMELINE] + \
-          [os.path.join(CSRC, f) for f in SOURCES]
-    subprocess.run(cmd, check=True)
-    return LIB_TIMELINE
+    return _compile(LIB_TIMELINE, ["-DVELO_TIMELINE"], "tl")
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile libvelo.so if missing or older than its sources. Returns its path."""
     if force or _stale():
-        cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
-        if verbose:
-            cmd.insert(1, "-Xptxas")
-            cmd.insert(2, "-v")
-        subprocess.run(cmd, check=True)
+        _compile(LIB, [], "velo", verbose)
     return LIB
 
 

@@ -3,9 +3,10 @@
 // every final array written once (sm_100a).
 //
 // velo_fit_kernel: teams of G threads in persistent CTAs take the events largest-first. An event's
-// sorted (x, y) arrive in shared memory by a 1-D TMA bulk copy; its candidates (rows of sorted hit
-// indices, module masks, seed scatters) and final flag bits come from stage 2's global scratch. One
-// thread per candidate fits and filters. What leaves: per candidate its fate and nine state words
+// candidates (rows of sorted hit indices and of hit coordinates in discovery order, module masks,
+// seed scatters) and final flag bits come from stage 2's global scratch: a thread fits its candidate
+// straight from its coordinate row, no gather. Shared memory holds only what threads share: the
+// O-13 owner per hit and the candidates' keys. One thread per candidate fits and filters. What leaves: per candidate its fate and nine state words
 // (coalesced planes in global scratch), per event the number of surviving tracks and track hits.
 // velo_offsets_kernel (velo_kernels.cu) scans those counts into event_track_offsets. Then
 // velo_write_kernel, a streaming kernel with one warp per event and no shared memory, places every
@@ -26,7 +27,6 @@ namespace {
 
 template <int G>
 struct FitTeam {
-  unsigned long long mbar;
   uint32_t wsum[4 * (G / 32)];
   uint32_t event, skip, n, sb, o0;
   uint32_t units, first_unit, pool_off;
@@ -42,11 +42,10 @@ struct FitCtl {
 
 __device__ __forceinline__ uint32_t a16(uint32_t v) { return (v + 15u) & ~15u; }
 
-struct FitLayout { uint32_t xy, own, fbits, key, mask, state, bytes; };
+struct FitLayout { uint32_t own, fbits, key, mask, state, bytes; };
 __device__ __forceinline__ FitLayout fit_layout(uint32_t n, uint32_t nt) {
   FitLayout L;
   uint32_t o = 0;
-  L.xy = o; o += a16(8u * n);            // sorted (x, y)
   L.own = o; o += a16(4u * n);           // O-13 owner (candidate id) per hit
   L.fbits = o; o += a16(4u * ((n + 31u) >> 5));
   L.key = o; o += a16(8u * nt);
@@ -73,22 +72,49 @@ __device__ __forceinline__ void for_hits(const uint16_t* row, uint32_t n, F&& f)
 // ---- O-11 straight-line fit with z taken from the module planes ---------------------------------
 // s9 = x, y, tx, ty, z, cxx, cxtx, vt, chi2 (the 13 state words repeat cxx, cxtx, vt for y and add n).
 // Hits are visited in discovery order = decreasing module = the set bits of `mask` from the top.
-__device__ __forceinline__ void fit_track(const float2* xy, const float* mz, const uint16_t* row, uint32_t n, uint32_t mask,
+// The (x, y) of a candidate's hits in discovery order: the first 16 hits are loaded into registers
+// up front (eight independent 16-byte loads in flight per thread), the rare rest comes on demand.
+struct XyRow {
+  float4 v[8];
+  const float4* r4;
+  __device__ __forceinline__ void load(const float2* rxy, uint32_t n) {
+    r4 = reinterpret_cast<const float4*>(rxy);
+#pragma unroll
+    for (uint32_t g = 0; g < 8; ++g) v[g] = 2u * g < n ? __ldcs(r4 + g) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+};
+// Calls f(p) for the hits in discovery order.
+template <class F>
+__device__ __forceinline__ void for_xy(const XyRow& r, uint32_t n, F&& f) {
+#pragma unroll
+  for (uint32_t g = 0; g < 8; ++g) {
+    if (2u * g >= n) break;
+    f(make_float2(r.v[g].x, r.v[g].y));
+    if (2u * g + 1u < n) f(make_float2(r.v[g].z, r.v[g].w));
+  }
+  for (uint32_t g = 8; 2u * g < n; ++g) {
+    const float4 v = r.r4[g];
+    f(make_float2(v.x, v.y));
+    if (2u * g + 1u < n) f(make_float2(v.z, v.w));
+  }
+}
+
+__device__ __forceinline__ void fit_track(const float2* rxy_g, const float* mz, uint32_t n, uint32_t mask,
                                           float sig2, float inv_s2, float* s9) {
+  XyRow rxy;
+  rxy.load(rxy_g, n);
   float sz = 0.0f, sx = 0.0f, sy = 0.0f;
   uint32_t mk = mask;
-  for_hits(row, n, [&](uint32_t, uint32_t h) {
+  for_xy(rxy, n, [&](const float2 p) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float2 p = xy[h];
     sz = __fadd_rn(sz, mz[m]); sx = __fadd_rn(sx, p.x); sy = __fadd_rn(sy, p.y);
   });
   const float nf = (float)n;
   const float zb = __fdiv_rn(sz, nf), xb = __fdiv_rn(sx, nf), yb = __fdiv_rn(sy, nf);
   float sdd = 0.0f, sdx = 0.0f, sdy = 0.0f;
   mk = mask;
-  for_hits(row, n, [&](uint32_t, uint32_t h) {
+  for_xy(rxy, n, [&](const float2 p) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float2 p = xy[h];
     const float d = __fsub_rn(mz[m], zb);
     sdd = __fadd_rn(sdd, __fmul_rn(d, d));
     sdx = __fadd_rn(sdx, __fmul_rn(d, __fsub_rn(p.x, xb)));
@@ -97,9 +123,8 @@ __device__ __forceinline__ void fit_track(const float2* xy, const float* mz, con
   const float tx = __fdiv_rn(sdx, sdd), ty = __fdiv_rn(sdy, sdd);
   float c = 0.0f;
   mk = mask;
-  for_hits(row, n, [&](uint32_t, uint32_t h) {
+  for_xy(rxy, n, [&](const float2 p) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float2 p = xy[h];
     const float d = __fsub_rn(mz[m], zb);
     const float rx = __fsub_rn(__fsub_rn(p.x, xb), __fmul_rn(tx, d));
     const float ry = __fsub_rn(__fsub_rn(p.y, yb), __fmul_rn(ty, d));
@@ -144,11 +169,10 @@ __device__ void fit_fetch(const KernelArgs& a, PoolCtl& pool, FitTeam<G>& ts) {
 // ---- one pipeline event, by one team ------------------------------------------------------------
 template <int G>
 __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, unsigned char* blk, uint32_t team,
-                          uint32_t tid, uint32_t& parity, uint32_t& phase) {
+                          uint32_t tid, uint32_t& parity) {
   const velo_params_t& P = a.P;
   const uint32_t e = ts.event, n = ts.n, nt = ts.ncand, o0 = ts.o0;
   const FitLayout L = fit_layout(n, nt);
-  float2* xy = (float2*)(blk + L.xy);
   uint32_t* own = (uint32_t*)(blk + L.own);
   uint32_t* fbits = (uint32_t*)(blk + L.fbits);
   unsigned long long* tkey = (unsigned long long*)(blk + L.key);
@@ -156,15 +180,10 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
   uint8_t* tstate = blk + L.state;       // 0 dropped by O-10/O-12, 1 passed, 2 survives O-13
   const uint16_t* rows = a.ws.rows + (size_t)ts.cbase * 32u;
   const uint2* cmeta = a.ws.cmeta + ts.cbase;
+  const float2* rows_xy = a.ws.rows_xy + (size_t)ts.cbase * kXyStride;
   float* cfit = a.ws.cfit + ts.cbase;    // plane k of candidate t: cfit[k * cand_total + t]
   const size_t cs = a.ws.cand_total;
 
-  // sorted coordinates: one bulk copy (size rounded up to 16 bytes: the scratch slots are spaced for it)
-  if (tid == 0) {
-    const uint32_t bxy = a16(8u * n);
-    mbar_arrive_expect_tx(&ts.mbar, bxy);
-    tma_load_1d(xy, a.ws.sxy + ts.sb, bxy, &ts.mbar);
-  }
   {
     const uint32_t* fb = a.ws.flag_bits + ((o0 - a.event_offsets[0]) >> 5) + e;
     for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) fbits[i] = fb[i];
@@ -183,7 +202,6 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
     }
     tstate[t] = pass ? 1 : 0;
   }
-  mbar_wait(&ts.mbar, phase & 1u); phase ^= 1u;
   // ---- O-11 fit, O-12 chi2 cut, O-13 key -----------------------------------------------------------
   const float sig2 = __fmul_rn(P.sigma_hit, P.sigma_hit);
   const float inv_s2 = __fdiv_rn(1.0f, sig2);
@@ -191,7 +209,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
     if (!tstate[t]) continue;
     const uint32_t mask = tmask[t], nh = (uint32_t)__popc(mask);
     float s9[9];
-    fit_track(xy, mz, rows + t * 32u, nh, mask, sig2, inv_s2, s9);
+    fit_track(rows_xy + t * kXyStride, mz, nh, mask, sig2, inv_s2, s9);
     const float lim = __fmul_rn(P.max_chi2_ndof, (float)(2 * (int)nh - 4));
     if (s9[8] > lim) { tstate[t] = 0; continue; }
     const uint32_t centre = rows[t * 32u + 1u];
@@ -254,18 +272,17 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArg
   Ctl& ctl = *reinterpret_cast<Ctl*>(smem);
   unsigned char* pool = smem + kCtl;
   const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
-  if (threadIdx.x == 0) { ctl.pool.bitmap = 0ull; ctl.pool.alloc_next = 0; ctl.pool.alloc_serving = 0; ctl.pool.units = pool_units; }
+  if (threadIdx.x == 0) pool_init(ctl.pool, pool_units);
   if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
   FitTeam<G>& ts = ctl.team[team];
-  if (tid == 0) { mbar_init(&ts.mbar, 1u); mbar_fence_init(); }
   __syncthreads();
   VELO_STAGE_BEGIN(a.ws.phase_clk, 2);
-  uint32_t parity = 0, phase = 0;
+  uint32_t parity = 0;
   for (;;) {
     if (tid == 0) fit_fetch<G>(a, ctl.pool, ts);
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
-    if (!ts.skip) fit_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity, phase);
+    if (!ts.skip) fit_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity);
     team_sync<G>(team);
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
   }
@@ -275,7 +292,8 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArg
 // ---- S7 write: one warp per event places its surviving tracks in the final arrays ----------------
 // Offsets come from velo_offsets_kernel (event_track_offsets, ws.ev_hit_base). Candidates are in
 // creation order, so a running count over them is the track's place inside the event.
-__global__ void __launch_bounds__(128, 8) velo_write_kernel(const KernelArgs a) {
+template <int kMinBlocks>
+__global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const KernelArgs a) {
   const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t tot_t = a.event_track_offsets[a.n_events], tot_h = a.ws.ev_hit_base[a.n_events];
@@ -368,15 +386,15 @@ int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
     case 6: return launch_fit_t<128, 6>(a, stream, pu);
     case 12: return launch_fit_t<64, 12>(a, stream, pu);
     case 15: return launch_fit_t<64, 15>(a, stream, pu);
+    case 254: return launch_fit_t<256, 4>(a, stream, pu);
     default: return launch_fit_t<128, 8>(a, stream, pu);
   }
 }
 
 int launch_write(const KernelArgs& a, cudaStream_t stream) {
   if (a.n_events == 0) return 0;
-  uint32_t grid = (a.n_events + 3u) / 4u;
-  if (grid > num_sms() * 16u) grid = num_sms() * 16u;
-  velo_write_kernel<<<grid, 128, 0, stream>>>(a);
+  const uint32_t grid = (a.n_events + 3u) / 4u;     // a warp per event
+  velo_write_kernel<8><<<grid, 128, 0, stream>>>(a);
   return (int)cudaGetLastError();
 }
 

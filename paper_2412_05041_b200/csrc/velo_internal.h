@@ -67,14 +67,18 @@ __host__ __device__ inline size_t flag_words(uint32_t n_events, uint32_t n_hits)
 // Candidate-table capacity of an event of n hits in the pipeline path (candidates ~0.107/hit at
 // mu = 5, 0.19/hit for the open VELO; an event that needs more is deferred to the general kernel).
 __host__ __device__ inline uint32_t cand_capacity(uint32_t n) { return ((n >> 3) + (n >> 4) + 32u + 15u) & ~15u; }
-// Active-track list capacity (tracks alive at the same time: 0.07/hit on average, 0.104/hit at most
-// in 600 events of configs[1]; small events of the open VELO reach 0.14/hit, which the + 32 covers).
-__host__ __device__ inline uint32_t active_capacity(uint32_t n) { return (((n * 13u) >> 7) + 32u + 7u) & ~7u; }
+// Shared-memory part of the active-track list (tracks alive at the same time: 0.07/hit at the peak
+// of a mean mu = 5 event, 0.104/hit at most in 600 events of configs[1]): what does not fit spills
+// to global scratch (velo_track.cu), so this capacity trades shared memory against rare L2 trips.
+__host__ __device__ inline uint32_t active_capacity(uint32_t n) { return (((n * 7u) >> 7) + 24u + 7u) & ~7u; }
 constexpr uint32_t kModOffStride = 40;   // u16 per event: mod_off[0 .. M] (M <= 32), [39] = largest module
 constexpr uint32_t kPipeMaxHits = 12000; // largest event the pipeline path takes (stage 1: 17 B/hit, stage 3: ~18 B/hit of shared memory)
 // Upper bound of stage 3's shared-memory block for an event of n hits (velo_fit.cu: fit_layout with
 // every candidate slot used): stage 1 defers an event to the general kernel if this does not fit.
-__host__ __device__ inline uint32_t fit_smem_bound(uint32_t n) { return 14u * n + (n >> 3) + 21u * cand_capacity(n) + 256u; }
+__host__ __device__ inline uint32_t fit_smem_bound(uint32_t n) { return 4u * n + (n >> 3) + 13u * cand_capacity(n) + 256u; }
+// (x, y) of a candidate's hits in discovery order, written by stage 2 as it appends them: stage 3
+// fits from these rows and needs no gather. kXyStride float2 per candidate (16-byte aligned rows).
+constexpr uint32_t kXyStride = VELO_MAX_MODULES;
 // per-event state written by stage 1, updated by stage 2
 enum { kEvEmpty = 0, kEvReady = 1, kEvDeferred = 2, kEvBad = 3 };
 struct EvInfo { uint32_t n, state, cbase, ncand; };   // cbase: first candidate slot; ncand: candidates created
@@ -83,7 +87,7 @@ struct Workspace {
   uint32_t* counters;     // kNumCounters
   EvInfo* ev_info;        // n_events
   uint4* rec16;           // sorted_capacity: {x, y, phi16u << 16 | start(m+1), start(m-1) << 16 | start(m-2)}
-  float2* sxy;            // sorted_capacity: sorted (x, y) for stage 3
+  float2* rows_xy;        // cand_total * kXyStride: (x, y) of the candidates' hits, discovery order
   uint16_t* sorig;        // sorted_capacity: sorted position -> original event-local index
   uint16_t* mod_off;      // n_events * kModOffStride
   uint32_t* flag_bits;    // flag_words: final O-5 flags, one bit per sorted hit

@@ -499,12 +499,12 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t n_hits, uint32
   w.order = (uint32_t*)take(4 * ((size_t)n_events + 1));
   const size_t sc = sorted_capacity(n_events, n_hits);
   w.rec16 = (uint4*)take(16 * sc);
-  w.sxy = (float2*)take(8 * sc);
   w.sorig = (uint16_t*)take(2 * sc);
   w.mod_off = (uint16_t*)take(2 * (size_t)kModOffStride * ((size_t)n_events + 1));
   w.flag_bits = (uint32_t*)take(4 * flag_words(n_events, n_hits));
   w.cand_total = (size_t)(n_hits >> 3) + (n_hits >> 4) + 48ull * n_events + 64ull;   // >= sum of cand_capacity(n_e)
   w.rows = (uint16_t*)take(64 * w.cand_total);
+  w.rows_xy = (float2*)take(sizeof(float2) * kXyStride * w.cand_total);
   w.cmeta = (uint2*)take(8 * w.cand_total);
   w.cfit = (float*)take(4 * 9 * w.cand_total);
   w.cstate = (uint8_t*)take(w.cand_total);

@@ -1,7 +1,7 @@
 // velo_pool.cuh — persistent-CTA infrastructure shared by the three pipeline kernels of libvelo
 // (velo_sort.cu, velo_track.cu, velo_fit.cu; sm_100a).
 //
-// One persistent CTA per SM owns the SM's shared memory as a pool of 64 units. The CTA is cut into
+// One persistent CTA per SM owns the SM's shared memory as a pool of 128 units. The CTA is cut into
 // teams of G threads (a warp, or a few warps behind a named barrier); a team's leader takes the
 // next event from a global ticket and allocates from the pool exactly what that event needs in
 // this stage (events span 0 ... ~6 k hits at mu = 5: a fixed slot per event would waste more than
@@ -14,15 +14,18 @@
 
 namespace velo {
 
-constexpr uint32_t kUnitBytes = 3456;   // pool allocation unit: at most 64 of them (one bitmap word)
-constexpr uint32_t kPoolUnitsMax = 64;  //   = 216 KB of pool; + the control block <= 227 KB per CTA
+constexpr uint32_t kUnitBytes = 1728;    // pool allocation unit: at most 128 of them (two bitmap words)
+constexpr uint32_t kPoolUnitsMax = 128;  //   = 216 KB of pool; + the control block <= 227 KB per CTA
 
 struct PoolCtl {
-  unsigned long long bitmap;            // 1 = unit in use
+  unsigned long long bitmap[2];         // 1 = unit in use; unit u is bit u & 63 of word u >> 6
   uint32_t alloc_next, alloc_serving;   // FIFO ticket lock around the allocator: no starvation
   uint32_t units;                       // units in this CTA's pool (set at kernel start)
   uint32_t pad;
 };
+__device__ __forceinline__ void pool_init(PoolCtl& ctl, uint32_t units) {
+  ctl.bitmap[0] = 0ull; ctl.bitmap[1] = 0ull; ctl.alloc_next = 0; ctl.alloc_serving = 0; ctl.units = units;
+}
 
 // ---- stage windows for `bench.py --timeline` (a -DVELO_TIMELINE build only) -----------------------
 // phase_clk[2k] = ~(earliest start) and phase_clk[2k + 1] = latest end of stage k's CTAs, in ns of
@@ -108,35 +111,63 @@ __device__ __forceinline__ uint32_t team_scan2(uint32_t v, uint32_t v2, uint32_t
 }
 
 // ---- pool allocator (called by a team's leader thread only) ------------------------------------
+// First fit over a 128-bit occupancy map. Allocations are serialised by the FIFO ticket, so only
+// the ticket holder ever sets bits; frees (any leader, any time) only clear bits. The holder may
+// therefore read a stale map, which errs on the safe side, and no compare-and-swap is needed.
+struct Bits128 { unsigned long long lo, hi; };
+__device__ __forceinline__ Bits128 shr128(Bits128 v, uint32_t s) {     // 0 < s < 128
+  Bits128 r;
+  if (s >= 64u) { r.lo = v.hi >> (s - 64u); r.hi = 0ull; }
+  else { r.lo = (v.lo >> s) | (v.hi << (64u - s)); r.hi = v.hi >> s; }
+  return r;
+}
+__device__ __forceinline__ Bits128 ones128(uint32_t first, uint32_t count) {   // bits first .. first+count-1, count >= 1
+  const uint32_t end = first + count;                                          // <= 128
+  Bits128 r;
+  const unsigned long long below_end_lo = end >= 64u ? ~0ull : ((1ull << end) - 1ull);
+  const unsigned long long below_first_lo = first >= 64u ? ~0ull : ((1ull << first) - 1ull);
+  r.lo = below_end_lo & ~below_first_lo;
+  const unsigned long long below_end_hi = end >= 128u ? ~0ull : (end > 64u ? ((1ull << (end - 64u)) - 1ull) : 0ull);
+  const unsigned long long below_first_hi = first > 64u ? ((1ull << (first - 64u)) - 1ull) : 0ull;
+  r.hi = below_end_hi & ~below_first_hi;
+  return r;
+}
 __device__ __forceinline__ uint32_t pool_alloc(PoolCtl& ctl, uint32_t units) {
   const uint32_t my = atomicAdd(&ctl.alloc_next, 1u);
   volatile uint32_t* serving = &ctl.alloc_serving;
-  while (*serving != my) __nanosleep(400);
-  volatile unsigned long long* bm = &ctl.bitmap;
-  const uint32_t pu = ctl.units;
-  const unsigned long long all = pu >= 64u ? ~0ull : (1ull << pu) - 1ull;
+  while (*serving != my) __nanosleep(1000);
+  volatile unsigned long long* bm = ctl.bitmap;
+  const Bits128 all = ones128(0u, ctl.units);
   uint32_t first;
-  unsigned long long seen = ~0ull;
+  Bits128 seen{~0ull, ~0ull};
   for (;;) {
-    const unsigned long long used = *bm;
-    if (used == seen) { __nanosleep(400); continue; }   // nothing was freed since the last failed try
-    unsigned long long r = ~used & all;          // bit p: unit p free
-    for (uint32_t i = 1; i < units && r; ++i) r &= (r >> 1);   // bit p: units p .. p+i free
-    if (r) {
-      first = (uint32_t)__ffsll((long long)r) - 1u;
-      const unsigned long long claim = ((units >= 64u ? ~0ull : ((1ull << units) - 1ull)) << first);
-      if (atomicCAS(&ctl.bitmap, used, used | claim) == used) break;
-    } else {
-      seen = used;
+    const Bits128 used{bm[0], bm[1]};
+    if (used.lo == seen.lo && used.hi == seen.hi) { __nanosleep(500); continue; }   // nothing was freed since the last failed try
+    Bits128 r{~used.lo & all.lo, ~used.hi & all.hi};   // bit p: unit p free
+    // after the loop, bit p: units p .. p+units-1 free (run length doubles per trip)
+    for (uint32_t len = 1; len < units && (r.lo | r.hi); ) {
+      const uint32_t sh = min(len, units - len);
+      const Bits128 t = shr128(r, sh);
+      r.lo &= t.lo; r.hi &= t.hi;
+      len += sh;
     }
+    if (r.lo | r.hi) {
+      first = r.lo ? (uint32_t)__ffsll((long long)r.lo) - 1u : 63u + (uint32_t)__ffsll((long long)r.hi);
+      const Bits128 claim = ones128(first, units);
+      if (claim.lo) atomicOr(&ctl.bitmap[0], claim.lo);
+      if (claim.hi) atomicOr(&ctl.bitmap[1], claim.hi);
+      break;
+    }
+    seen = used;
   }
   __threadfence_block();
   *serving = my + 1u;
   return first;
 }
 __device__ __forceinline__ void pool_free(PoolCtl& ctl, uint32_t first, uint32_t units) {
-  const unsigned long long claim = ((units >= 64u ? ~0ull : ((1ull << units) - 1ull)) << first);
-  atomicAnd(&ctl.bitmap, ~claim);
+  const Bits128 claim = ones128(first, units);
+  if (claim.lo) atomicAnd(&ctl.bitmap[0], ~claim.lo);
+  if (claim.hi) atomicAnd(&ctl.bitmap[1], ~claim.hi);
 }
 
 // ---- mbarrier + 1-D TMA bulk copy (global -> shared::cta), PTX ISA 8.x --------------------------

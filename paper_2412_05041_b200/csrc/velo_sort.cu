@@ -214,7 +214,6 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
   };
   const uint32_t sb = sorted_base(ts.ol, e);
   uint4* rec = a.ws.rec16 + sb;
-  float2* sxy = a.ws.sxy + sb;
   uint16_t* sorig = a.ws.sorig + sb;
   for (uint32_t h = tid; h < n; h += G) {
     const uint32_t item = w[h], pu = item >> 16, i = item & 0xffffu, m = mod8[h];
@@ -227,7 +226,6 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
       if (m >= 2u) sm2 = start_in(m - 2u, lo);
     }
     rec[h] = make_uint4(__float_as_uint(p.x), __float_as_uint(p.y), (pu << 16) | sp1, (sm1 << 16) | sm2);
-    sxy[h] = p;
     sorig[h] = (uint16_t)i;
   }
   // module offsets and the largest module
@@ -253,7 +251,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_sort_kernel(const KernelAr
   Ctl& ctl = *reinterpret_cast<Ctl*>(smem);
   unsigned char* pool = smem + kCtl;
   const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
-  if (threadIdx.x == 0) { ctl.pool.bitmap = 0ull; ctl.pool.alloc_next = 0; ctl.pool.alloc_serving = 0; ctl.pool.units = pool_units; }
+  if (threadIdx.x == 0) pool_init(ctl.pool, pool_units);
   if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
   __syncthreads();
   VELO_STAGE_BEGIN(a.ws.phase_clk, 0);
@@ -291,8 +289,11 @@ int launch_sort(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   switch (o.sort_teams) {
     case 4: return launch_sort_t<128, 4>(a, stream, pu);
     case 6: return launch_sort_t<128, 6>(a, stream, pu);
+    case 7: return launch_sort_t<128, 7>(a, stream, pu);
     case 8: return launch_sort_t<128, 8>(a, stream, pu);
-    default: return launch_sort_t<128, 7>(a, stream, pu);
+    case 253: return launch_sort_t<256, 3>(a, stream, pu);
+    case 252: return launch_sort_t<512, 2>(a, stream, pu);
+    default: return launch_sort_t<256, 4>(a, stream, pu);   // 22 us per event with 256 threads, 43 us with 128
   }
 }
 

@@ -55,7 +55,7 @@ __device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod,
   uint32_t o = 0;
   L.ring = o; o += 4u * 16u * maxmod;
   L.act = o; o += 32u * acap;
-  L.flags = o; o += al16(n);
+  L.flags = o; o += al16(4u * ((n + 31u) >> 5));
   L.th0 = o; o += al16(2u * tcap);
   L.cl = o; o += al16(2u * maxmod);
   L.bytes = o;
@@ -125,18 +125,33 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
   const TrackLayout L = track_layout(n, slotcap, tcap, acap);
   uint4* ring = (uint4*)(blk + L.ring);
   uint4* act = (uint4*)(blk + L.act);
-  uint8_t* flags = blk + L.flags;
+  uint32_t* flags = (uint32_t*)(blk + L.flags);   // one bit per sorted hit
+  auto flagged = [&](uint32_t h) -> bool { return (flags[h >> 5] >> (h & 31u)) & 1u; };
+  auto set_flag = [&](uint32_t h) { atomicOr(&flags[h >> 5], 1u << (h & 31u)); };
+  // Active tracks beyond the shared-memory list (rare: it holds 0.055 per hit + 24, the mean peak is
+  // 0.07 per hit at mu = 5 but lasts a step or two) live in global scratch: stage 3's state planes,
+  // which nothing reads before stage 3 writes them.
+  uint4* act_ovf = reinterpret_cast<uint4*>(a.ws.cfit) + 2u * (size_t)ts.cbase;
+  auto act_load = [&](uint32_t k, uint4& q0, uint4& q1) {
+    if (k < acap) { q0 = act[2u * k]; q1 = act[2u * k + 1u]; }
+    else { q0 = __ldcg(act_ovf + 2u * (k - acap)); q1 = __ldcg(act_ovf + 2u * (k - acap) + 1u); }
+  };
+  auto act_store = [&](uint32_t k, const uint4& q0, const uint4& q1) {
+    if (k < acap) { act[2u * k] = q0; act[2u * k + 1u] = q1; }
+    else { act_ovf[2u * (k - acap)] = q0; act_ovf[2u * (k - acap) + 1u] = q1; }
+  };
   uint16_t* th0 = (uint16_t*)(blk + L.th0);
   uint16_t* cl = (uint16_t*)(blk + L.cl);
   const uint16_t* mo = ts.mod_off;
   const uint4* grec = a.ws.rec16 + ts.sb;
   uint16_t* rows = a.ws.rows + (size_t)ts.cbase * 32u;
   uint2* cmeta = a.ws.cmeta + ts.cbase;
+  float2* rows_xy = a.ws.rows_xy + (size_t)ts.cbase * kXyStride;
   const int Wseed = P.phi_window_seed, Wfwd = P.phi_window_fwd;
   const int Wwide = Wseed > Wfwd ? Wseed : Wfwd;
 
   for (uint32_t i = tid; i < kModOffStride; i += G) ts.mod_off[i] = a.ws.mod_off[(size_t)e * kModOffStride + i];
-  for (uint32_t i = tid; i < al16(n) / 4u; i += G) ((uint32_t*)flags)[i] = 0;
+  for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) flags[i] = 0;
   team_sync<G>(team);
 
   // ring: module m lives in slot m & 3; loads are issued and waited for in descending module order
@@ -178,7 +193,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
       bool alive = false;
       uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0;
       if (k < nact) {
-        q0 = act[2u * k]; q1 = act[2u * k + 1u];
+        act_load(k, q0, q1);
         const float x0 = __uint_as_float(q0.x), y0 = __uint_as_float(q0.y);
         const float x1 = __uint_as_float(q0.z), y1 = __uint_as_float(q0.w);
         const uint32_t c = q1.x >> 16, id = q1.x & 0xffffu, w3 = q1.y, hab = q1.z, mask = q1.w;
@@ -215,9 +230,10 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
           const uint4 r2 = ring_u[best];
           const uint32_t h2 = off_u + best, nh = (uint32_t)__popc(mask);
           rows[id * 32u + nh] = (uint16_t)h2;
+          rows_xy[id * kXyStride + nh] = make_float2(__uint_as_float(r2.x), __uint_as_float(r2.y));
           // (B): forwarding never reads flags, so they can be set right away
-          if (nh + 1u == 4u) { flags[th0[id]] = 1; flags[hab >> 16] = 1; flags[hab & 0xffffu] = 1; }
-          if (nh + 1u >= 4u) flags[h2] = 1;
+          if (nh + 1u == 4u) { set_flag(th0[id]); set_flag(hab >> 16); set_flag(hab & 0xffffu); }
+          if (nh + 1u >= 4u) set_flag(h2);
           q0 = make_uint4(q0.z, q0.w, r2.x, r2.y);
           q1 = make_uint4((r2.z & 0xffff0000u) | id, r2.w, (hab << 16) | h2, mask | (1u << u));
           alive = true;
@@ -228,7 +244,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
       }
       uint32_t total;
       const uint32_t pos = team_scan_pred<G>(alive, ts.wsum, team, parity, &total);   // (also: every read of this pass is done)
-      if (alive) { act[2u * (wbase + pos)] = q0; act[2u * (wbase + pos) + 1u] = q1; }
+      if (alive) act_store(wbase + pos, q0, q1);
       wbase += total;
     }
     nact = wbase;
@@ -239,7 +255,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     uint32_t ncl = 0;
     for (uint32_t c0 = 0; c0 < ns; c0 += G) {
       const uint32_t j = c0 + tid;
-      const bool open = j < ns && !flags[off_s + j];
+      const bool open = j < ns && !flagged(off_s + j);
       uint32_t total;
       const uint32_t pos = team_scan_pred<G>(open, ts.wsum, team, parity, &total);
       if (open) cl[ncl + pos] = (uint16_t)j;
@@ -266,14 +282,14 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
               const uint4 r0 = ring_p[j0];
               if (!(r0.z - ww.lo16 <= ww.lim)) break;
               if (!kSameW && !(r0.z - wx.lo16 <= wx.lim)) continue;
-              if (flags[off_p + j0]) continue;
+              if (flagged(off_p + j0)) continue;
               const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tz));
               const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tz));
               // h0 and h2 ascending: strict < keeps the lexicographic minimum; branch-free body
               auto visit2 = [&](uint32_t jj, const uint4& r, bool in) {
                 const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
                 const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-                bool ok = in & !flags[off_u + jj] & (sc <= max_seed) & (!found | (sc < best_sc));
+                bool ok = in & !flagged(off_u + jj) & (sc <= max_seed) & (!found | (sc < best_sc));
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
                 found |= ok; b0 = ok ? j0 : b0; b2 = ok ? jj : b2; best_sc = ok ? sc : best_sc;
               };
@@ -284,20 +300,24 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
         }
         uint32_t total;
         const uint32_t pos = team_scan_pred<G>(found, ts.wsum, team, parity, &total);
-        if (found && ncand + pos < tcap && nact + pos < acap) {
+        if (found && ncand + pos < tcap) {
           const uint32_t id = ncand + pos;
           const uint32_t h0 = off_p + b0, h1 = off_s + j1, h2 = off_u + b2;
           const uint4 r2 = ring_u[b2];
           *reinterpret_cast<uint2*>(rows + id * 32u) = make_uint2(h0 | (h1 << 16), h2);
+          const uint4 r0 = ring_p[b0];
+          float4* rxy = reinterpret_cast<float4*>(rows_xy + id * kXyStride);
+          rxy[0] = make_float4(__uint_as_float(r0.x), __uint_as_float(r0.y), __uint_as_float(r1.x), __uint_as_float(r1.y));
+          rows_xy[id * kXyStride + 2u] = make_float2(__uint_as_float(r2.x), __uint_as_float(r2.y));
           cmeta[id] = make_uint2(7u << u, __float_as_uint(best_sc));
           th0[id] = (uint16_t)h0;
-          act[2u * (nact + pos)] = make_uint4(r1.x, r1.y, r2.x, r2.y);
-          act[2u * (nact + pos) + 1u] = make_uint4((r2.z & 0xffff0000u) | id, r2.w, (h1 << 16) | h2, 7u << u);
+          act_store(nact + pos, make_uint4(r1.x, r1.y, r2.x, r2.y),
+                    make_uint4((r2.z & 0xffff0000u) | id, r2.w, (h1 << 16) | h2, 7u << u));
         }
         ncand += total; nact += total;
       }
     }
-    if (ncand > tcap || nact > acap) { if (tid == 0) ts.defer = 1; }
+    if (ncand > tcap) { if (tid == 0) ts.defer = 1; }
     team_sync<G>(team);                  // the new tracks are visible; module s+1 has been read for the last time
     if (ts.defer) break;
     if (issued > 0) issue(--issued);     // module s-3 into the slot of module s+1
@@ -313,16 +333,13 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
   }
   // tracks still active take their final module mask; the final flags leave as bits
   for (uint32_t k = tid; k < nact; k += G) {
-    const uint4 q1 = act[2u * k + 1u];
+    uint4 q0, q1;
+    act_load(k, q0, q1);
     if (__popc(q1.w) > 3) cmeta[q1.x & 0xffffu].x = q1.w;
   }
   {
     uint32_t* fb = a.ws.flag_bits + ((a.event_offsets[e] - a.event_offsets[0]) >> 5) + e;
-    for (uint32_t j0 = 0; j0 < n; j0 += G) {
-      const uint32_t j = j0 + tid;
-      const uint32_t b = __ballot_sync(0xffffffffu, j < n && flags[j]);
-      if ((tid & 31u) == 0 && j < n) fb[j >> 5] = b;
-    }
+    for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) fb[i] = flags[i];
   }
   if (tid == 0) {
     a.ws.ev_info[e] = EvInfo{n, kEvReady, ts.cbase, ncand};
@@ -339,7 +356,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
   Ctl& ctl = *reinterpret_cast<Ctl*>(smem);
   unsigned char* pool = smem + kCtl;
   const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
-  if (threadIdx.x == 0) { ctl.pool.bitmap = 0ull; ctl.pool.alloc_next = 0; ctl.pool.alloc_serving = 0; ctl.pool.units = pool_units; }
+  if (threadIdx.x == 0) pool_init(ctl.pool, pool_units);
   if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
   TrackTeam<G>& ts = ctl.team[team];
   if (tid == 0) {
@@ -390,9 +407,9 @@ int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
   uint32_t g = o.track_group, t = o.track_teams;
   if (g == 0) {
-    // a warp per event for mu = 5 sized events; more threads per event when the events are large
+    // two warps per event for mu = 5 sized events; more threads per event when the events are large
     const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
-    g = mean >= 6144u ? 128u : 32u;
+    g = mean >= 6144u ? 128u : 64u;
   }
   if (g == 128) {
     if (t == 0) t = 6;

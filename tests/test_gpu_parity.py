@@ -83,8 +83,8 @@ def test_run_to_run_determinism(velo):
     {"path": 1}, {"path": 2},                                     # general slab kernel only; round-1 team kernel
     {"track_group": 32, "track_teams": 8}, {"track_group": 32, "track_teams": 24},
     {"track_group": 64}, {"track_group": 64, "track_teams": 15}, {"track_group": 128},
-    {"fit_teams": 4}, {"fit_teams": 12}, {"sort_teams": 4}, {"sort_teams": 8},
-    {"pool_units": 24}, {"pool_units": 12, "track_group": 64}], ids=str)
+    {"fit_teams": 4}, {"fit_teams": 12}, {"fit_teams": 254}, {"sort_teams": 4}, {"sort_teams": 7}, {"sort_teams": 252},
+    {"pool_units": 48}, {"pool_units": 24, "track_group": 64}], ids=str)
 def test_pipeline_geometries_and_other_paths_agree(velo, kw):
     d = datagen.generate_config(0)
     want = cpu(d)
