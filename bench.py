@@ -273,15 +273,25 @@ def run_velo(args):
     barrier()
     if args.timeline:
         # windows of the sort / track / fit kernels of the last warm-up step's batches (GPU global timer)
-        rows = []
+        rows, phases = [], []
         for b, o in enumerate(outs):
             skip = o.workspace_ptr - o.workspace.data_ptr() + 256
-            clk = o.workspace[skip:skip + 48].cpu().numpy().view(np.uint64)
+            clk = o.workspace[skip:skip + 512].cpu().numpy().view(np.uint64)
             rows.append([(int(~clk[2 * k]), int(clk[2 * k + 1])) for k in range(3)])
+            phases.append(clk.copy())
         t0 = min(r[0][0] for r in rows)
         for b, r in enumerate(rows):
             print("batch %d: " % b + "  ".join("%s %8.3f .. %8.3f ms" % (nm, (s - t0) / 1e6, (e - t0) / 1e6)
                                                  for nm, (s, e) in zip(("sort", "track", "fit"), r)), flush=True)
+        # SM clocks per event and phase, summed over the team leaders (batch 0)
+        names = {"sort": (8, ["fetch", "decode", "scan", "scatter+rank", "place", "starts+write", "free"]),
+                 "track": (16, ["fetch", "setup", "wait module", "forwarding", "centre list", "seeding", "tail"]),
+                 "fit": (32, ["fetch", "weak filter", "fit", "owners 1", "owners 2", "clone+counts"])}
+        clk = phases[0]
+        for nm, (base, labels) in names.items():
+            nev = max(int(clk[base]), 1)
+            print("%s: %d events; SM clocks per event: " % (nm, nev) +
+                  ", ".join("%s %.0f" % (l, clk[base + 1 + i] / nev) for i, l in enumerate(labels)), flush=True)
         return
     sampler = ClockSampler(local); sampler.start()
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -31,6 +31,7 @@ struct FitTeam {
   uint32_t event, skip, n, sb, o0;
   uint32_t units, first_unit, pool_off;
   uint32_t cbase, ncand;
+  unsigned long long ph_last;        // phase clocks (-DVELO_TIMELINE builds)
 };
 
 template <int G, int kTeams>
@@ -202,6 +203,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
     }
     tstate[t] = pass ? 1 : 0;
   }
+  VELO_PH(a.ws.phase_clk, ts, 34);
   // ---- O-11 fit, O-12 chi2 cut, O-13 key -----------------------------------------------------------
   const float sig2 = __fmul_rn(P.sigma_hit, P.sigma_hit);
   const float inv_s2 = __fdiv_rn(1.0f, sig2);
@@ -219,6 +221,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
     for (uint32_t k = 0; k < 9; ++k) cfit[k * cs + t] = s9[k];
   }
   team_sync<G>(team);
+  VELO_PH(a.ws.phase_clk, ts, 35);
   // ---- O-13 owners: owner[h] = the candidate with the smallest key among those that contain h ----
   // Step 1: every passing candidate writes its id on its hits (plain stores: where several share a
   // hit, any one of them lands). Step 2: a candidate that finds another id on one of its hits
@@ -229,6 +232,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
     for_hits(rows + t * 32u, (uint32_t)__popc(tmask[t]), [&](uint32_t, uint32_t h) { own[h] = t; });
   }
   team_sync<G>(team);
+  VELO_PH(a.ws.phase_clk, ts, 36);
   for (uint32_t t = tid; t < nt; t += G) {
     if (!tstate[t]) continue;
     const unsigned long long key = tkey[t];
@@ -242,6 +246,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
     });
   }
   team_sync<G>(team);
+  VELO_PH(a.ws.phase_clk, ts, 37);
   // ---- O-13 clone filter; the event's counts --------------------------------------------------------
   uint32_t run_t = 0, run_h = 0;
   uint8_t* cstate = a.ws.cstate + ts.cbase;
@@ -278,13 +283,17 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArg
   __syncthreads();
   VELO_STAGE_BEGIN(a.ws.phase_clk, 2);
   uint32_t parity = 0;
+  VELO_PH_START(ts);
   for (;;) {
     if (tid == 0) fit_fetch<G>(a, ctl.pool, ts);
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
+    VELO_PH(a.ws.phase_clk, ts, 33);     // ticket, descriptors, pool
     if (!ts.skip) fit_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity);
     team_sync<G>(team);
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
+    VELO_PH(a.ws.phase_clk, ts, 38);     // clone filter, counts
+    VELO_PH_COUNT(a.ws.phase_clk, 32, 1);
   }
   VELO_STAGE_END(a.ws.phase_clk, 2);
 }

@@ -52,7 +52,7 @@ constexpr uint32_t kTeamsPerCtaMax = 8;
 //           4 event ticket, 5 large-event list length, 6 large-event ticket
 enum { kCtrTracks = 0, kCtrHits = 1, kCtrStatus = 2, kCtrCand = 3, kCtrTicket = 4, kCtrLargeN = 5,
        kCtrLargeTicket = 6, kCtrSortTicket = 7, kCtrTrackTicket = 8, kCtrFitTicket = 9, kCtrCandAlloc = 10,
-       kNumCounters = 16, kNumPhaseClocks = 32 };
+       kNumCounters = 16, kNumPhaseClocks = 64 };
 
 // ---- the three-stage pipeline (velo_sort.cu -> velo_track.cu -> velo_fit.cu) ---------------------
 // Stage 1 writes every event's phi-sorted hits to global scratch; stage 2 streams them module by

@@ -38,7 +38,15 @@ __device__ __forceinline__ unsigned long long velo_globaltimer() {
 }
 #define VELO_STAGE_BEGIN(clk, k) do { if (threadIdx.x == 0) atomicMax(&(clk)[2 * (k)], ~velo_globaltimer()); } while (0)
 #define VELO_STAGE_END(clk, k) do { __syncthreads(); if (threadIdx.x == 0) atomicMax(&(clk)[2 * (k) + 1], velo_globaltimer()); } while (0)
+// Phase clocks: the team leader adds the SM clocks since its previous mark to phase_clk[i] (sort 8..15,
+// track 16..27, fit 32..43; slot i + 0 of each range counts events).
+#define VELO_PH_START(ts) do { if (tid == 0) (ts).ph_last = clock64(); } while (0)
+#define VELO_PH(clk, ts, i) do { if (tid == 0) { const unsigned long long now_ = clock64(); atomicAdd(&(clk)[i], now_ - (ts).ph_last); (ts).ph_last = now_; } } while (0)
+#define VELO_PH_COUNT(clk, i, v) do { if (tid == 0) atomicAdd(&(clk)[i], (unsigned long long)(v)); } while (0)
 #else
+#define VELO_PH_START(ts) do { } while (0)
+#define VELO_PH(clk, ts, i) do { } while (0)
+#define VELO_PH_COUNT(clk, i, v) do { } while (0)
 #define VELO_STAGE_BEGIN(clk, k) do { } while (0)
 #define VELO_STAGE_END(clk, k) do { } while (0)
 #endif

@@ -32,6 +32,7 @@ struct SortTeam {
   uint32_t units, first_unit, pool_off;
   uint32_t skip;                     // nothing to sort (empty / bad / deferred before the sort)
   uint32_t trouble;                  // bit 0: defer to the general kernel, bit 31: bad input
+  unsigned long long ph_last;        // phase clocks (-DVELO_TIMELINE builds)
 };
 
 template <int G, int kTeams>
@@ -149,6 +150,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
     if (trouble) atomicOr(&ts.trouble, trouble);
   }
   team_sync<G>(team);
+  VELO_PH(a.ws.phase_clk, ts, 10);
   if (ts.trouble) {
     if (tid == 0) {
       EvInfo info{n, kEvDeferred, 0u, 0u};
@@ -174,6 +176,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
     if (tid == 0) bo[nbins] = (uint16_t)n;
   }
   team_sync<G>(team);
+  VELO_PH(a.ws.phase_clk, ts, 11);
   // ---- S1 phi sort (O-2): group by bucket in w[], rank inside the bucket by (phi16, index), place --
   for (uint32_t i = tid; i < n; i += G) {
     const uint32_t st = stash[i], pu = (st >> 11) & 0xffffu;
@@ -191,6 +194,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
     stash[i] = (st & ~kMaxBinSlot) | r;
   }
   team_sync<G>(team);                    // every rank is known: w[] can take its final content
+  VELO_PH(a.ws.phase_clk, ts, 12);
   for (uint32_t i = tid; i < n; i += G) {
     const uint32_t st = stash[i], pu = (st >> 11) & 0xffffu, m = st >> 27;
     const uint32_t r = (uint32_t)bo[m * kBinsPerModule + (pu >> kBinShift)] + (st & kMaxBinSlot);
@@ -198,6 +202,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
     mod8[r] = (uint8_t)m;
   }
   team_sync<G>(team);
+  VELO_PH(a.ws.phase_clk, ts, 13);
   // ---- window starts and the event's sorted block -------------------------------------------------
   const int Wseed = a.P.phi_window_seed, Wfwd = a.P.phi_window_fwd;
   const int W = Wseed > Wfwd ? Wseed : Wfwd;                 // >= 0 (the host clamps negative windows)
@@ -240,6 +245,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
     if (tid == 0) { mo[32] = (uint16_t)n; mo[kModOffStride - 1] = (uint16_t)sz; }
   }
   if (tid == 0) a.ws.ev_info[e] = EvInfo{n, kEvReady, 0u, 0u};
+  VELO_PH(a.ws.phase_clk, ts, 14);
 }
 
 // ---- the kernel: one CTA per SM, kTeams teams of G threads, events by ticket in event order -----
@@ -257,13 +263,17 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_sort_kernel(const KernelAr
   VELO_STAGE_BEGIN(a.ws.phase_clk, 0);
   SortTeam<G>& ts = ctl.team[team];
   uint32_t parity = 0;
+  VELO_PH_START(ts);
   for (;;) {
     if (tid == 0) sort_fetch<G>(a, ctl.pool, ts);
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
+    VELO_PH(a.ws.phase_clk, ts, 9);      // ticket, offsets, pool
     if (!ts.skip) sort_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity);
     team_sync<G>(team);
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
+    VELO_PH(a.ws.phase_clk, ts, 15);
+    VELO_PH_COUNT(a.ws.phase_clk, 8, 1);
   }
   VELO_STAGE_END(a.ws.phase_clk, 0);
 }

@@ -37,6 +37,7 @@ struct TrackTeam {
   uint32_t units, first_unit, pool_off, skip;
   uint32_t maxmod, cbase, tcap, acap;
   uint32_t defer;                    // set by any thread: the event continues in the general kernel
+  unsigned long long ph_last;        // phase clocks (-DVELO_TIMELINE builds)
   uint16_t mod_off[kModOffStride];
 };
 
@@ -169,6 +170,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
   uint32_t issued = M, waited = M;       // lowest module issued / waited for so far
   for (uint32_t k = 0; k < 4 && issued > 0; ++k) issue(--issued);
   wait(--waited); wait(--waited);        // modules M-1 and M-2
+  VELO_PH(a.ws.phase_clk, ts, 18);       // descriptors, flags, first loads
 
   uint32_t nact = 0, ncand = 0;
   const float max_fwd = P.max_scatter_fwd, max_seed = P.max_scatter_seed;
@@ -178,6 +180,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     // and in all that follow, and what a miss changes (the miss count) is not read after the loop.
     if (mo[u + 1] == 0) break;
     wait(--waited);                      // module u has landed
+    VELO_PH(a.ws.phase_clk, ts, 19);
     const uint32_t off_u = mo[u], nu = (uint32_t)mo[u + 1] - off_u;
     const uint32_t off_s = mo[s], ns = (uint32_t)mo[s + 1] - off_s;
     const uint32_t off_p = mo[s + 1], np = (uint32_t)mo[s + 2] - off_p;
@@ -249,6 +252,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     }
     nact = wbase;
     team_sync<G>(team);                  // flags and the compacted list are visible
+    VELO_PH(a.ws.phase_clk, ts, 20);
 
     // ---- (C) O-8 seeding with centre module s -----------------------------------------------------
     // (C1) the unflagged centre hits, in ascending order (flags are final for this step)
@@ -262,6 +266,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
       ncl += total;
     }
     team_sync<G>(team);
+    VELO_PH(a.ws.phase_clk, ts, 21);
     // (C2) one lane per unflagged centre hit: best (h0, h2) under (scatter, h0, h2)
     if (ncl) {
       const float zc0 = mz[s + 1], zc1 = mz[s];
@@ -319,6 +324,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     }
     if (ncand > tcap) { if (tid == 0) ts.defer = 1; }
     team_sync<G>(team);                  // the new tracks are visible; module s+1 has been read for the last time
+    VELO_PH(a.ws.phase_clk, ts, 22);
     if (ts.defer) break;
     if (issued > 0) issue(--issued);     // module s-3 into the slot of module s+1
   }
@@ -367,13 +373,17 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
   __syncthreads();
   VELO_STAGE_BEGIN(a.ws.phase_clk, 1);
   uint32_t parity = 0, phases = 0;
+  VELO_PH_START(ts);
   for (;;) {
     if (tid == 0) track_fetch<G>(a, ctl.pool, ts);
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
+    VELO_PH(a.ws.phase_clk, ts, 17);     // ticket, descriptors, pool
     if (!ts.skip) track_event<G, kSameW>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity, phases);
     team_sync<G>(team);   // every thread is done with the block and with ts before the leader reuses them
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
+    VELO_PH(a.ws.phase_clk, ts, 23);     // tail: remaining loads, masks, flag bits
+    VELO_PH_COUNT(a.ws.phase_clk, 16, 1);
   }
   VELO_STAGE_END(a.ws.phase_clk, 1);
 }
