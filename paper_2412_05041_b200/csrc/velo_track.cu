@@ -267,12 +267,16 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     }
     team_sync<G>(team);
     VELO_PH(a.ws.phase_clk, ts, 21);
-    // (C2) one lane per unflagged centre hit: best (h0, h2) under (scatter, h0, h2)
+    // (C2) L = 1, 2 or 4 adjacent lanes per unflagged centre hit (as many as the team can seat at once),
+    // lane q taking every L-th h0 of the window: best (h0, h2) under (scatter, h0, h2), reduced over
+    // the L lanes with shuffles under the same lexicographic order
     if (ncl) {
       const float zc0 = mz[s + 1], zc1 = mz[s];
       const float tz = __fdiv_rn(__fsub_rn(z2, zc1), __fsub_rn(zc1, zc0));
-      for (uint32_t k0 = 0; k0 < ncl; k0 += G) {
-        const uint32_t k = k0 + tid;
+      const uint32_t lsh = (4u * ncl <= (uint32_t)G) ? 2u : (2u * ncl <= (uint32_t)G) ? 1u : 0u;
+      const uint32_t L = 1u << lsh;
+      for (uint32_t k0 = 0; k0 < ncl; k0 += (uint32_t)G >> lsh) {
+        const uint32_t k = k0 + (tid >> lsh), q = tid & (L - 1u);
         bool found = false; uint32_t b0 = 0, b2 = 0, j1 = 0; float best_sc = 0.0f;
         uint4 r1 = make_uint4(0, 0, 0, 0);
         if (k < ncl) {
@@ -283,7 +287,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
           const Win wx = make_win(c, Wseed);
           const Win ww = kSameW ? wx : make_win(c, Wwide);
           for (uint32_t run0 = ww.wrapped ? 0u : 1u; run0 < 2u; ++run0) {
-            for (uint32_t j0 = run0 ? (r1.z & 0xffffu) : 0u; j0 < np; ++j0) {
+            for (uint32_t j0 = (run0 ? (r1.z & 0xffffu) : 0u) + q; j0 < np; j0 += L) {
               const uint4 r0 = ring_p[j0];
               if (!(r0.z - ww.lo16 <= ww.lim)) break;
               if (!kSameW && !(r0.z - wx.lo16 <= wx.lim)) continue;
@@ -303,6 +307,15 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
             }
           }
         }
+        for (uint32_t d = 1; d < L; d <<= 1) {
+          const bool o_found = __shfl_xor_sync(0xffffffffu, (int)found, d) != 0;
+          const float o_sc = __shfl_xor_sync(0xffffffffu, best_sc, d);
+          const uint32_t o_b0 = __shfl_xor_sync(0xffffffffu, b0, d), o_b2 = __shfl_xor_sync(0xffffffffu, b2, d);
+          const bool better = o_found & (!found | (o_sc < best_sc) |
+                                         ((o_sc == best_sc) & ((o_b0 < b0) | ((o_b0 == b0) & (o_b2 < b2)))));
+          found |= o_found; b0 = better ? o_b0 : b0; b2 = better ? o_b2 : b2; best_sc = better ? o_sc : best_sc;
+        }
+        found &= (q == 0u);                // one lane speaks for the centre
         uint32_t total;
         const uint32_t pos = team_scan_pred<G>(found, ts.wsum, team, parity, &total);
         if (found && ncand + pos < tcap) {
