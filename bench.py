@@ -27,11 +27,16 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one event-kernel launch, from the ncu --set full
-# capture summarised in profiles/r01c_team_kernel_25k.md; key = (config, path, events per step)
-NCU_DRAM_BYTES_PER_LAUNCH = {(2, 0, 100_000): 676_917_248 + 496_348_160}
-# smsp__inst_executed.sum of the same capture / its 25 000 events: what bounds the path in practice
-NCU_WARP_INST_PER_EVENT = {(2, 0): 94_811.0}
+# ncu --set full counters of one 25 000-event launch of every kernel of the path (configs[2] batch size),
+# written from the capture summarised in profiles/r02e_pipeline.md; read by name, never pasted here
+STAGE_COUNTERS_CSV = os.path.join(ROOT, "profiles", "r02e_stage_counters.csv")
+STAGE_COUNTERS_EVENTS = 25_000
+# stage k runs between stage events k and k+1 of velo_launch_options_t (include/velo.h)
+STAGES = [("sort", ["velo_sort_kernel", "velo_order_kernel"]),
+          ("track", ["velo_track_kernel", "velo_event_slab_kernel"]),
+          ("fit", ["velo_fit_kernel"]),
+          ("offsets", ["velo_offsets_kernel"]),
+          ("write", ["velo_write_kernel"])]
 
 METRIC = "velo_tracking_events_per_s"
 UNIT = "events/s"
@@ -47,8 +52,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json:configs index (default 2)")
     ap.add_argument("--events", type=int, default=None, help="override the number of events (debugging)")
     ap.add_argument("--ctas-per-sm", type=int, default=0, help="slab-kernel launch option (0 = library default)")
-    ap.add_argument("--teams", type=int, default=0, help="teams per CTA of the team kernel (0 = library default)")
-    ap.add_argument("--path", type=int, default=0, help="0 = team kernel + slab for deferred events, 1 = slab only")
+    ap.add_argument("--path", type=int, default=0, help="0 = three-stage pipeline + slab kernel for deferred events, 1 = slab only")
+    ap.add_argument("--no-other-workloads", action="store_true", help="skip the short configs[3] and configs[4] legs")
     ap.add_argument("--track-group", type=int, default=0, help="threads per event of the module-loop kernel (0 = default)")
     ap.add_argument("--track-teams", type=int, default=0)
     ap.add_argument("--fit-teams", type=int, default=0)
@@ -124,18 +129,14 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def issue_block(args, events_per_s: float, clocks: dict):
-    """The practical limiter beside the HBM roofline: warp instructions issued per second against
-    the issue peak of the chip (148 SMs x 4 schedulers x 1 warp instruction per clock at the SM
-    clock seen during the run). Instructions per event come from the ncu capture in profiles/."""
-    per_event = NCU_WARP_INST_PER_EVENT.get((args.config, args.path))
-    mhz = clocks.get("sm_mhz") or 1965.0
-    if per_event is None:
-        return None
-    peak = 148 * 4 * mhz * 1e6
-    return {"bound": "alu", "achieved": events_per_s * per_event / 1e9, "peak": peak / 1e9, "unit": "G warp instr/s",
-            "frac": events_per_s * per_event / peak, "warp_instructions_per_event": per_event,
-            "source": "profiles/r01c_team_kernel_25k.md"}
+def stage_counters() -> dict:
+    """kernel name -> counters of one 25 000-event launch (profiles/r02e_stage_counters.csv); {} if absent."""
+    import csv
+    try:
+        with open(STAGE_COUNTERS_CSV) as f:
+            return {r["kernel"]: r for r in csv.DictReader(f)}
+    except OSError:
+        return {}
 
 
 def measured_peak_gbs() -> tuple[float, str]:
@@ -193,6 +194,119 @@ def run_reference(args):
 
 
 # ---- the CUDA arm ----------------------------------------------------------------------------------
+class Workload:
+    """One BASELINE.json config resident in HBM: pinned host arrays, device hits, per-batch outputs."""
+
+    def __init__(self, velo, datagen, sharding, torch, cfg_index, n_events_override, rank, opts_kw):
+        self.torch, self.velo = torch, velo
+        self.cfg_index = cfg_index
+        cfg, n_events, n_batches = datagen.CONFIGS[cfg_index]
+        if n_events_override:
+            n_events = n_events_override
+        self.n_events, self.n_batches = n_events, n_batches
+        self.keep = []
+
+        def pinned(shape, dtype):
+            t = torch.empty(int(np.prod(shape)) if not np.isscalar(shape) else int(shape),
+                            dtype={np.float32: torch.float32, np.uint8: torch.uint8}[np.dtype(dtype).type],
+                            pin_memory=True)
+            self.keep.append(t)
+            return t.numpy()
+
+        e0, _ = sharding.weak_event_range(rank, n_events)   # every rank its own events: weak scaling
+        self.d = d = datagen.generate(cfg, e0, n_events, alloc=pinned)
+        self.off = off = d["event_offsets"]
+        self.n_hits = d["n_hits"]
+        self.cuts = cuts = [n_events * b // n_batches for b in range(n_batches + 1)]
+        self.g = velo.velo_geometry_load(datagen.MODULE_Z, half_shift_x=cfg.half_shift_x)
+        self.P = velo.velo_params_default(self.g)
+        self.dh = velo.DeviceHits(d["x"], d["y"], d["z"], d["module"], off)
+        self.opts_kw = opts_kw
+        opts0 = velo.LaunchOptions(**opts_kw)
+        self.outs, self.hstructs = [], []
+        for b in range(n_batches):
+            nh = int(off[cuts[b + 1]]) - int(off[cuts[b]])
+            self.outs.append(velo.DeviceTracks(cuts[b + 1] - cuts[b], nh, opts=opts0))
+            self.hstructs.append(self.dh.slice_struct(cuts[b], cuts[b + 1], nh))
+        self.streams = [torch.cuda.Stream() for _ in range(n_batches)]
+        self.main = torch.cuda.current_stream()
+        self.fork = torch.cuda.Event()
+        self.joins = [torch.cuda.Event() for _ in range(n_batches)]
+
+    def step(self):
+        """One pass of the whole hot path over the workload: every batch on its own stream."""
+        velo = self.velo
+        self.fork.record(self.main)
+        o = velo.LaunchOptions(**self.opts_kw)
+        for b in range(self.n_batches):
+            self.streams[b].wait_event(self.fork)
+            velo.velo_reconstruct(self.g, self.hstructs[b], self.P, self.outs[b], self.streams[b], o)
+            self.joins[b].record(self.streams[b])
+            self.main.wait_event(self.joins[b])
+
+    def stage_pass(self, reps):
+        """The same batches one after the other on ONE stream with an event at every stage boundary
+        (velo_launch_options_t.stage_events): the duration of every kernel of the path, measured
+        with CUDA events on the stream it is launched on. Returns {stage: mean ms per launch}."""
+        torch, velo = self.torch, self.velo
+        st = self.streams[0]
+        ev = [[[torch.cuda.Event(enable_timing=True) for _ in range(velo.VELO_N_STAGE_EVENTS)]
+               for _ in range(self.n_batches)] for _ in range(reps)]
+        torch.cuda.synchronize()
+        for r in range(reps):
+            for b in range(self.n_batches):
+                o = velo.LaunchOptions(**self.opts_kw)
+                for k in range(velo.VELO_N_STAGE_EVENTS):
+                    ev[r][b][k].record(st)      # a torch event is created lazily by its first record()
+                    o.stage_events[k] = ev[r][b][k].cuda_event
+                velo.velo_reconstruct(self.g, self.hstructs[b], self.P, self.outs[b], st, o)
+        torch.cuda.synchronize()
+        out = {}
+        for k, (name, _) in enumerate(STAGES):
+            out[name] = float(np.mean([ev[r][b][k].elapsed_time(ev[r][b][k + 1])
+                                       for r in range(reps) for b in range(self.n_batches)]))
+        return out
+
+    def results(self):
+        return [o.to_host() for o in self.outs]          # raises on any device-side status
+
+    def alg_bytes(self, res):
+        off, cuts = self.off, self.cuts
+        return [algorithmic_bytes(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]]),
+                                  res[b]["n_tracks"], res[b]["n_track_hits"]) for b in range(self.n_batches)]
+
+    def free(self):
+        self.outs = self.hstructs = self.dh = self.d = self.keep = None
+        self.torch.cuda.empty_cache()
+
+
+def timed_steps(torch, dist, world, wl, warmup, steps, sampler=None):
+    """W untimed steps, then exactly K timed steps between barrier + synchronize; device time with CUDA
+    events on the launching stream, max over ranks. Returns (total ms, [ms of every step])."""
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        wl.step()
+    barrier()
+    if sampler:
+        sampler.start()
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    marks[0].record(wl.main)
+    for i in range(steps):
+        wl.step()
+        marks[i + 1].record(wl.main)
+    barrier()
+    total = marks[0].elapsed_time(marks[steps])
+    per_step = [marks[i].elapsed_time(marks[i + 1]) for i in range(steps)]
+    if world > 1:
+        t = torch.tensor([total] + per_step, device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total, per_step = float(t[0].item()), [float(v) for v in t[1:].tolist()]
+    return total, per_step
+
+
 def run_velo(args):
     import torch
     import torch.distributed as dist
@@ -210,71 +324,21 @@ def run_velo(args):
     vbuild.build()
     velo.lib()
 
-    # -- synthetic workload: this rank's own events (weak scaling) --
-    cfg, n_events, n_batches = datagen.CONFIGS[args.config]
-    if args.events:
-        n_events = args.events
-    keep = []  # pinned host tensors behind the numpy views
+    opts_kw = dict(ctas_per_sm=args.ctas_per_sm, path=args.path, track_group=args.track_group,
+                   track_teams=args.track_teams, fit_teams=args.fit_teams, sort_teams=args.sort_teams,
+                   pool_units=args.pool_units)
+    kernels_per_batch = 3 if args.path == 1 else 7   # sort, order, track, slab, fit, offsets, write
+    wl = Workload(velo, datagen, sharding, torch, args.config, args.events, rank, opts_kw)
+    n_events, n_batches, n_hits, off, cuts = wl.n_events, wl.n_batches, wl.n_hits, wl.off, wl.cuts
+    launches = 0
 
-    def pinned(shape, dtype):
-        t = torch.empty(int(np.prod(shape)) if not np.isscalar(shape) else int(shape),
-                        dtype={np.float32: torch.float32, np.uint8: torch.uint8}[np.dtype(dtype).type],
-                        pin_memory=True)
-        keep.append(t)
-        return t.numpy()
-
-    e0, _ = sharding.weak_event_range(rank, n_events)   # every rank its own events: weak scaling
-    d = datagen.generate(cfg, e0, n_events, alloc=pinned)
-    off = d["event_offsets"]
-    n_hits = d["n_hits"]
-    cuts = [n_events * b // n_batches for b in range(n_batches + 1)]
-    g = velo.velo_geometry_load(datagen.MODULE_Z, half_shift_x=cfg.half_shift_x)
-    P = velo.velo_params_default(g)
-    dh = velo.DeviceHits(d["x"], d["y"], d["z"], d["module"], off)
-    tune = dict(track_group=args.track_group, track_teams=args.track_teams, fit_teams=args.fit_teams,
-                sort_teams=args.sort_teams, pool_units=args.pool_units)
-    opts0 = velo.LaunchOptions(ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams, **tune)
-    launches_per_batch = 3 if args.path == 1 else 5   # [order, team kernel,] slab kernel, offsets, compaction
-    streams = [torch.cuda.Stream() for _ in range(n_batches)]
-    if os.environ.get('VELO_BENCH_SERIAL'):
-        streams = [streams[0]] * n_batches
-    main = torch.cuda.current_stream()
-    outs, hstructs = [], []
-    for b in range(n_batches):
-        e0, e1 = cuts[b], cuts[b + 1]
-        nh = int(off[e1]) - int(off[e0])
-        outs.append(velo.DeviceTracks(e1 - e0, nh, opts=opts0))
-        hstructs.append(dh.slice_struct(e0, e1, nh))
-    n_steps_total = args.warmup + args.steps
-    kev = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_batches)]
-           for _ in range(n_steps_total)]
-    fork = torch.cuda.Event(); joins = [torch.cuda.Event() for _ in range(n_batches)]
-
-    def step(i):
-        fork.record(main)
-        for b in range(n_batches):
-            streams[b].wait_event(fork)
-            # raw cudaEvent_t handles: a torch event is created lazily by its first record()
-            ks, ke = kev[i][b]
-            ks.record(streams[b]); ke.record(streams[b])
-            o = velo.LaunchOptions(event_kernel_start=ks.cuda_event, event_kernel_stop=ke.cuda_event,
-                                   ctas_per_sm=args.ctas_per_sm, path=args.path, teams_per_cta=args.teams, **tune)
-            velo.velo_reconstruct(g, hstructs[b], P, outs[b], streams[b], o)
-            joins[b].record(streams[b])
-            main.wait_event(joins[b])
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for i in range(args.warmup):
-        step(i)
-    barrier()
     if args.timeline:
+        for _ in range(args.warmup):
+            wl.step()
+        torch.cuda.synchronize()
         # windows of the sort / track / fit kernels of the last warm-up step's batches (GPU global timer)
         rows, phases = [], []
-        for b, o in enumerate(outs):
+        for b, o in enumerate(wl.outs):
             skip = o.workspace_ptr - o.workspace.data_ptr() + 256
             clk = o.workspace[skip:skip + 512].cpu().numpy().view(np.uint64)
             rows.append([(int(~clk[2 * k]), int(clk[2 * k + 1])) for k in range(3)])
@@ -293,70 +357,91 @@ def run_velo(args):
             print("%s: %d events; SM clocks per event: " % (nm, nev) +
                   ", ".join("%s %.0f" % (l, clk[base + 1 + i] / nev) for i, l in enumerate(labels)), flush=True)
         return
-    sampler = ClockSampler(local); sampler.start()
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t0.record(main)
-    for i in range(args.warmup, n_steps_total):
-        step(i)
-    t1.record(main)
-    barrier()
+
+    sampler = ClockSampler(local)
+    ms_total, per_step = timed_steps(torch, dist, world, wl, args.warmup, args.steps, sampler)
     clocks = sampler.stop()
-    ms_total = t0.elapsed_time(t1)
-    if world > 1:
-        t = torch.tensor([ms_total], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms_total = float(t.item())
-    ms_step = ms_total / args.steps
+    launches += kernels_per_batch * n_batches * (args.steps + args.warmup)
+    ms_step = float(np.median(per_step))
 
     # -- results of the last step: sizes for the byte counts, status for validity --
-    res = [o.to_host() for o in outs]          # raises on any device-side status
+    res = wl.results()
     n_tracks = sum(r["n_tracks"] for r in res); n_thits = sum(r["n_track_hits"] for r in res)
     n_deferred = sum(r["n_deferred"] for r in res)
-    alg_batch = [algorithmic_bytes(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]]),
-                                   res[b]["n_tracks"], res[b]["n_track_hits"]) for b in range(n_batches)]
-    # The event kernels of a step's batches each fill the GPU (one persistent CTA per SM), so they run
-    # back to back even though they are launched on different streams. Their average duration is the
-    # span from the first start mark to the last stop mark of the step, divided by the launches.
-    span_ms = []
-    for i in range(args.warmup, n_steps_total):
-        first = min(range(n_batches), key=lambda b: kev[i][0][0].elapsed_time(kev[i][b][0]))
-        span_ms.append(max(kev[i][first][0].elapsed_time(kev[i][b][1]) for b in range(n_batches)))
-    avg_kern_ms = float(np.mean(span_ms)) / n_batches
-    peak, peak_src = measured_peak_gbs()
-    achieved = float(np.mean(alg_batch)) / (avg_kern_ms * 1e-3) / 1e9
-    step_gbs = float(sum(alg_batch)) / (ms_step * 1e-3) / 1e9
+    alg_batch = wl.alg_bytes(res)
+    alg_launch = float(np.mean(alg_batch))
 
-    value = world * n_events / (ms_step * 1e-3)
+    # -- every kernel of the path timed on its own stream (one stream, stage events) --
+    stage_reps = max(1, min(args.steps, 5))
+    stage_ms = wl.stage_pass(stage_reps)
+    launches += kernels_per_batch * n_batches * stage_reps
+    stage_sum = sum(stage_ms.values())
+    peak, peak_src = measured_peak_gbs()
+    counters = stage_counters() if (args.config == 2 and args.path == 0 and n_events // n_batches == STAGE_COUNTERS_EVENTS) else {}
+
+    def traffic_of(kernels):
+        if not counters or any(k not in counters for k in kernels):
+            return None
+        return sum(int(counters[k]["dram_bytes_read"]) + int(counters[k]["dram_bytes_write"]) for k in kernels)
+
+    stages = []
+    for name, kernels in STAGES:
+        ms = stage_ms[name]
+        stages.append({"stage": name, "kernels": kernels, "ms_per_launch": ms, "share_of_path": ms / stage_sum,
+                       "achieved": alg_launch / (ms * 1e-3) / 1e9 if ms > 0 else None, "traffic": traffic_of(kernels)})
+    dom = max(stages, key=lambda s_: s_["ms_per_launch"])
+    step_gbs = float(sum(alg_batch)) / (ms_step * 1e-3) / 1e9
+    all_kernels = [k for _, ks in STAGES for k in ks]
+    step_traffic = traffic_of(all_kernels)
+    warp_inst = sum(int(counters[k]["warp_instructions"]) for k in all_kernels) / STAGE_COUNTERS_EVENTS if counters else None
+    mhz = clocks.get("sm_mhz") or 1965.0
+    issue_peak = 148 * 4 * mhz * 1e6
+    events_per_s = world * n_events / (ms_step * 1e-3)
+
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic",
+        "metric": METRIC, "value": events_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "ms_per_step_mean": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "hits_per_s": world * n_hits / (ms_step * 1e-3),
         "config": {"workload": workload_name(args.config, n_events, n_batches), "events_per_gpu": n_events,
                    "hits_per_gpu": n_hits, "tracks": n_tracks, "track_hits": n_thits, "streams": n_batches,
                    "events_deferred_to_slab_kernel": n_deferred,
-                   "event_kernels": "slab only" if args.path == 1 else "shared-memory teams + slab for deferred events",
+                   "event_kernels": "slab only" if args.path == 1 else
+                                    "three-stage pipeline (sort, module loop, fit) + slab kernel for deferred events",
                    "cache": "inputs larger than L2 (%.2f GB per step)" % (13 * n_hits / 1e9),
+                   "timing": "median of the steps (device time, CUDA events, max over ranks)",
                    "parallelism": f"events sharded over {world} GPU(s), no collective"},
-        "roofline": {"bound": "hbm", "kernel": "velo_event_slab_kernel" if args.path == 1 else "velo_event_team_kernel (+ slab kernel for deferred events)", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, args.path, n_events)),
-                     "traffic_source": "profiles/r01c_team_kernel_25k.md (ncu --set full, one 25 000-event launch)",
-                     "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": float(np.mean(alg_batch)), "kernel_ms_per_launch": avg_kern_ms,
-                     "kernel_share_of_step": avg_kern_ms * n_batches / ms_step,
-                     "step_achieved": step_gbs, "step_frac": step_gbs / peak,
-                     "frac_of_nominal_8TBs": step_gbs / 8000.0,
-                     "limiter": "instruction issue and latency, not HBM (ncu: issue slots 52.0 % busy, DRAM 3 % busy, "
-                                "94.8 k warp instructions per event; see profiles/ and DESIGN.md 5.1)"},
-        "issue": issue_block(args, world * n_events / (ms_step * 1e-3), clocks),
+        "roofline": {"bound": "hbm", "kernel": " + ".join(dom["kernels"][:1]), "stage": dom["stage"],
+                     "achieved": dom["achieved"], "peak": peak, "unit": "GB/s", "frac": dom["achieved"] / peak,
+                     "traffic": dom["traffic"],
+                     "traffic_source": "profiles/r02e_stage_counters.csv (ncu --set full, one 25 000-event launch of every kernel)"
+                                       if counters else None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_launch,
+                     "kernel_ms_per_launch": dom["ms_per_launch"], "kernel_share_of_step": dom["share_of_path"],
+                     "how": "algorithmic bytes of one batch / duration of that batch's launch of the stage, CUDA events "
+                            "at the stage boundaries on the launching stream, batches one after the other on one stream, "
+                            "%d passes after the timed region" % stage_reps,
+                     "stages": stages, "path_ms_per_launch": stage_sum,
+                     "step_achieved": step_gbs, "step_frac": step_gbs / peak, "step_traffic": step_traffic,
+                     "step_traffic_over_algorithmic": step_traffic * n_batches / float(sum(alg_batch)) if step_traffic else None,
+                     "frac_of_nominal_8TBs": step_gbs / 8000.0, "target_frac": 0.40, "target_met": step_gbs / peak >= 0.40,
+                     "limiter": "instruction issue and event latency, not HBM: every stage holds an event's shared memory "
+                                "for the length of its dependent instruction chains (profiles/r02e_pipeline.md)"},
+        "issue": ({"bound": "alu", "achieved": events_per_s / world * warp_inst / 1e9, "peak": issue_peak / 1e9,
+                   "unit": "G warp instr/s", "frac": events_per_s / world * warp_inst / issue_peak,
+                   "warp_instructions_per_event": warp_inst, "source": "profiles/r02e_stage_counters.csv"}
+                  if warp_inst else None),
         "clocks": clocks,
-        "gpu_launches": launches_per_batch * n_batches * (args.steps + args.warmup),
     }
 
     # -- end to end through the host-buffer C-ABI call (velo_scheduler_run_host): pinned host
     #    inputs -> H2D -> kernels -> D2H of the produced tracks, all inside the timed region --
+    d = wl.d
     if not args.no_e2e:
         max_ev = max(cuts[b + 1] - cuts[b] for b in range(n_batches))
         max_h = max(int(off[cuts[b + 1]]) - int(off[cuts[b]]) for b in range(n_batches))
-        del outs, dh
+        g, P = wl.g, wl.P
+        wl.outs = wl.hstructs = wl.dh = None
         torch.cuda.empty_cache()
         sched = velo.Scheduler(g, n_batches, max_ev, max_h)
         houts = [velo.HostTracks(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]])) for b in range(n_batches)]
@@ -365,36 +450,76 @@ def run_velo(args):
         run = lambda: sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off_pinned.numpy().view(np.uint32),
                                      cuts, houts)
         run()  # warm-up
-        barrier()
-        w0 = time.perf_counter()
-        for _ in range(e2e_steps):
-            run()
+        if world > 1:
+            dist.barrier()
         torch.cuda.synchronize()
-        e2e_s = (time.perf_counter() - w0) / e2e_steps
+        times = []
+        for _ in range(e2e_steps):
+            w0 = time.perf_counter()
+            run()                      # returns after every copy has completed
+            times.append(time.perf_counter() - w0)
+        e2e_s = float(np.median(times))
         if world > 1:
             t = torch.tensor([e2e_s], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
         hres = [h.result() for h in houts]
         assert sum(r["n_tracks"] for r in hres) == n_tracks and sum(r["n_track_hits"] for r in hres) == n_thits
         h2d = 13 * n_hits + sum(4 * (cuts[b + 1] - cuts[b] + 1) for b in range(n_batches))
-        d2h = sum(16 + 4 * (cuts[b + 1] - cuts[b] + 1) + 4 * (r["n_tracks"] + 1) + 52 * r["n_tracks"] + 4 * r["n_track_hits"]
+        d2h = sum(4 * velo.VELO_N_SUMMARY + 4 * (cuts[b + 1] - cuts[b] + 1) + 4 * (r["n_tracks"] + 1) + 52 * r["n_tracks"] + 4 * r["n_track_hits"]
                   for b, r in enumerate(hres))
         line["e2e"] = {"value": world * n_events / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s, "steps": e2e_steps,
+                       "pcie_gbs": (h2d + d2h) / e2e_s / 1e9,
                        "api": "velo_scheduler_run_host (pinned host buffers, %d streams)" % n_batches}
-        line["gpu_launches"] += 5 * n_batches * (e2e_steps + 1)
+        launches += kernels_per_batch * n_batches * (e2e_steps + 1)
         sched.close()
 
     # -- the oracle on this box's host cores (rank 0, N=1 only): a baseline, not the target --
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         sample = min(n_events, 4000 if args.config != 4 else 60)
-        dt, nh = time_oracle(d, sample)
+        runs = [time_oracle(d, sample) for _ in range(3)]
+        dt = float(np.median([r[0] for r in runs])); nh = runs[0][1]
         line["cpu_baseline"] = {"value": sample / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "hits_per_s": nh / dt, "host_cores_available": os.cpu_count(),
-                                "sample": f"first {sample} events of the workload, one pass, {dt:.1f} s"}
+                                "sample": f"first {sample} events of the workload, median of 3 passes, {dt:.1f} s each"}
+
+    # -- the small- and large-event regimes: short legs on configs[3] and configs[4] (device-resident) --
+    if args.config == 2 and not args.events and not args.no_other_workloads and world == 1:
+        wl.free()
+        others = []
+        for ci in (3, 4):
+            w2 = Workload(velo, datagen, sharding, torch, ci, None, rank, opts_kw)
+            k2 = max(3, min(args.steps, 5))
+            _, ps = timed_steps(torch, dist, world, w2, 3, k2)
+            r2 = w2.results()
+            ms2 = float(np.median(ps))
+            gbs2 = float(sum(w2.alg_bytes(r2))) / (ms2 * 1e-3) / 1e9
+            st2 = w2.stage_pass(2)
+            launches += kernels_per_batch * w2.n_batches * (3 + k2 + 2)
+            others.append({"workload": workload_name(ci, w2.n_events, w2.n_batches), "value": w2.n_events / (ms2 * 1e-3),
+                           "unit": UNIT, "hits_per_s": w2.n_hits / (ms2 * 1e-3), "ms_per_step": ms2, "steps": k2,
+                           "hits": w2.n_hits, "tracks": sum(r["n_tracks"] for r in r2),
+                           "events_deferred_to_slab_kernel": sum(r["n_deferred"] for r in r2),
+                           "roofline": {"bound": "hbm", "step_achieved": gbs2, "peak": peak, "unit": "GB/s", "step_frac": gbs2 / peak,
+                                        "stage_ms_per_launch": st2}})
+            w2.free()
+        line["other_workloads"] = others
+    line["gpu_launches"] = launches
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start N ranks of this script
+    under torch.distributed.run on this node (one process per GPU) and pass their output through."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -404,6 +529,8 @@ def main():
 
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(respawn_under_torchrun(args))
     else:
         run_velo(args)
 

@@ -135,23 +135,22 @@ int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const ve
                      velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream);
 
 /* Same call with launch options, for measurement and tuning. opts may be NULL (= velo_reconstruct).
- * event_kernel_start/stop: cudaEvent_t handles (or NULL) recorded on `stream` immediately before
- * and after the event kernels (the kernels that carry S0 ... S6), so that a benchmark can time the
- * dominant part of a batch on the stream it runs on.
- * path: VELO_PATH_DEFAULT = the shared-memory team kernel, with the general slab kernel for the
- * events it defers (hits off their module plane, events too large for one SM's shared memory);
+ * stage_events: cudaEvent_t handles (or NULL) recorded on `stream` at the stage boundaries of the
+ * batch, so that a benchmark can time every stage on the stream it runs on: [0] before stage 1,
+ * [1] after stage 1 (sort: S0, S1), [2] after stage 2 (module loop: S2, S3, and the general kernel
+ * for deferred events), [3] after stage 3 (fit and filters: S4, S5, S6), [4] after the offsets scan,
+ * [5] after the write kernel (S7).
+ * path: VELO_PATH_DEFAULT = the three-stage pipeline, with the general slab kernel for the events it
+ * defers (hits off their module plane, events too large for one SM's shared memory);
  * VELO_PATH_SLAB_ONLY = the general slab kernel for every event. Both give identical results.
- * teams_per_cta: teams of 128 threads per persistent CTA of the team kernel (1 ... 8), 0 = default
- * (as many as mean-sized events of the batch fit one SM's shared memory: 5 at mu = 5).
  * ctas_per_sm: persistent CTAs per SM of the slab kernel, 0 = library default; the workspace must
  * have been sized for the default or for velo_workspace_bytes_opts with the same value. */
-enum { VELO_PATH_DEFAULT = 0, VELO_PATH_SLAB_ONLY = 1, VELO_PATH_TEAM_LEGACY = 2 };
+enum { VELO_PATH_DEFAULT = 0, VELO_PATH_SLAB_ONLY = 1 };
+#define VELO_N_STAGE_EVENTS 6
 typedef struct {
-  void* event_kernel_start;
-  void* event_kernel_stop;
+  void* stage_events[VELO_N_STAGE_EVENTS];
   uint32_t ctas_per_sm;
   uint32_t path;
-  uint32_t teams_per_cta;
   uint32_t track_group;   /* threads per event in the module-loop kernel: 32, 64 or 128; 0 = default  */
   uint32_t track_teams;   /* events in flight per persistent CTA of the module-loop kernel; 0 = default */
   uint32_t fit_teams;     /* ... of the fit/output kernel; 0 = default                                  */

@@ -82,13 +82,7 @@ int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const ve
   a.n_events = hits->n_events; a.n_modules = g->n_modules; a.n_hits = hits->n_hits;
   a.hit_base = hit_base;
   const uint32_t path = opts ? opts->path : 0u;
-  if (path == kPathTeamLegacy) {
-    // In a batch of large events (ion-like, mean >= 4096 hits) an event of more than ~6 k hits is
-    // better off in the general kernel with its 1024-thread CTAs than alone on an SM of the team kernel.
-    a.team_max_hits = (hits->n_events && hits->n_hits / hits->n_events >= 4096u) ? 6144u : kTeamMaxHits;
-  } else {
-    a.team_max_hits = kPipeMaxHits;
-  }
+  a.team_max_hits = kPipeMaxHits;
   for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
   a.P = *params;
   if (a.P.max_skipped > 200u) a.P.max_skipped = 200u;  // more misses than modules is all the same
@@ -103,9 +97,7 @@ int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const ve
   PipeOpts po{};
   if (opts) { po.track_group = opts->track_group; po.track_teams = opts->track_teams; po.fit_teams = opts->fit_teams;
               po.sort_teams = opts->sort_teams; po.pool_units = opts->pool_units; }
-  const int err = launch_reconstruct(a, (cudaStream_t)stream, opts ? (cudaEvent_t)opts->event_kernel_start : nullptr,
-                                     opts ? (cudaEvent_t)opts->event_kernel_stop : nullptr, path,
-                                     opts ? opts->teams_per_cta : 0u, po);
+  const int err = launch_reconstruct(a, (cudaStream_t)stream, opts ? opts->stage_events : nullptr, path, po);
   return err == 0 ? VELO_OK : VELO_ERR_CUDA;
 }
 

@@ -39,14 +39,6 @@ __host__ __device__ inline SlabLayout slab_layout() {
   return L;
 }
 
-// ---- per-team scratch of the shared-memory team kernel (velo_event_smem.cu) --------------------
-// The candidates' hit lists (32 x u16 per candidate) and fitted states (9 x f32) of the event a
-// team is working on. Rewritten for every event, so it stays L2-resident.
-constexpr uint32_t kTeamMaxHits = 13312;                       // largest event the team path takes
-constexpr uint32_t kTeamMaxTracks = kTeamMaxHits / 8 + 64;     // >= its candidate-table capacity
-constexpr uint32_t kTeamScratchBytes = kTeamMaxTracks * (64 + 36);
-constexpr uint32_t kTeamsPerCtaMax = 8;
-
 // ---- workspace layout (device) ---------------------------------------------------------------
 // counters: u32[16]: 0 tracks allocated, 1 track-hits allocated, 2 status, 3 candidates,
 //           4 event ticket, 5 large-event list length, 6 large-event ticket
@@ -104,7 +96,6 @@ struct Workspace {
   uint32_t* tmp_loff;     // cap_tracks: hit offset of a track inside its event's hit block
   uint32_t* tmp_hits;     // cap_track_hits
   float* tmp_states;      // VELO_N_STATE * cap_tracks
-  unsigned char* team_scratch;  // num_sms * kTeamsPerCtaMax * kTeamScratchBytes
   unsigned char* slabs;   // n_slabs * slab bytes
   uint32_t n_slabs;
   size_t bytes;
@@ -138,8 +129,7 @@ struct KernelArgs {
 
 // Which event kernel(s) a batch runs through (velo_launch_options_t.path).
 enum { kPathDefault = 0,     // three-stage pipeline, slab kernel for the events it defers
-       kPathSlabOnly = 1,    // slab kernel for every event (the general path on its own)
-       kPathTeamLegacy = 2 };  // round-1 shared-memory team kernel (kept for comparison)
+       kPathSlabOnly = 1 };  // slab kernel for every event (the general path on its own)
 
 // Launch geometry of the pipeline kernels (0 = default), from velo_launch_options_t.
 struct PipeOpts { uint32_t track_group, track_teams, fit_teams, sort_teams, pool_units; };
@@ -149,8 +139,8 @@ int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o);
 int launch_write(const KernelArgs& a, cudaStream_t stream);
 
 // Enqueues the whole path for one batch on `stream`. Returns a cudaError_t as int.
-int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop,
-                       uint32_t path, uint32_t teams, const PipeOpts& po);
+int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, void* const* stage_events, uint32_t path,
+                       const PipeOpts& po);
 
 }  // namespace velo
 struct velo_geometry {
@@ -165,9 +155,5 @@ namespace velo {
 int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
                      velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
                      const velo_launch_options_t* opts, uint32_t hit_base);
-
-// velo_event_smem.cu: the shared-memory event kernel (persistent, one CTA per SM, `teams` teams of
-// 128 threads). Events it cannot hold are appended to ws.large_list. Returns a cudaError_t as int.
-int launch_event_smem(const KernelArgs& a, cudaStream_t stream, uint32_t teams);
 
 }  // namespace velo

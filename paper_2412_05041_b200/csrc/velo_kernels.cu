@@ -434,41 +434,6 @@ __global__ void __launch_bounds__(256) velo_offsets_kernel(const KernelArgs a) {
   }
 }
 
-// ---- S7 part 3: move every event's temp block to its place in event order ----------------------
-// One warp per event keeps the copies coalesced (tracks of an event are contiguous on both sides).
-// Every lane has 4 (hit lists) or 14 (state planes, offsets) independent loads in flight per trip:
-// with one load per trip the copy ran at 1.8 TB/s, like this at 3.8 TB/s.
-__global__ void __launch_bounds__(128, 8) velo_compact_kernel(const KernelArgs a) {
-  const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
-  const uint32_t lane = threadIdx.x & 31u;
-  const uint32_t tot_t = a.event_track_offsets[a.n_events], tot_h = a.ws.ev_hit_base[a.n_events];
-  if (tot_t > a.cap_tracks || tot_h > a.cap_track_hits) return;  // VELO_ERR_CAPACITY: nothing valid
-  const size_t cs = a.cap_tracks;
-  for (uint32_t e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; e < a.n_events; e += warps) {
-    const uint4 r = a.ws.ev_rec[e];
-    const uint32_t dst_t = a.event_track_offsets[e], dst_h = a.ws.ev_hit_base[e];
-    // hit lists: four independent loads per lane and trip (the copy is latency-bound otherwise)
-    const uint32_t* src = a.ws.tmp_hits + r.y;
-    uint32_t* dst = a.track_hits + dst_h;
-    for (uint32_t k = lane; k < r.w; k += 128u) {
-      uint32_t v[4];
-#pragma unroll
-      for (uint32_t q = 0; q < 4; ++q) v[q] = (k + 32u * q < r.w) ? src[k + 32u * q] : 0u;
-#pragma unroll
-      for (uint32_t q = 0; q < 4; ++q) if (k + 32u * q < r.w) dst[k + 32u * q] = v[q];
-    }
-    for (uint32_t k = lane; k < r.z; k += 32u) {
-      float v[VELO_N_STATE];
-      const uint32_t lo = a.ws.tmp_loff[r.x + k];
-#pragma unroll
-      for (int p = 0; p < VELO_N_STATE; ++p) v[p] = a.ws.tmp_states[(size_t)p * cs + r.x + k];
-      a.track_hit_offsets[dst_t + k] = dst_h + lo;
-#pragma unroll
-      for (int p = 0; p < VELO_N_STATE; ++p) a.states[(size_t)p * cs + dst_t + k] = v[p];
-    }
-  }
-}
-
 }  // namespace
 
 // ---- host side -----------------------------------------------------------------------------------
@@ -511,45 +476,28 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t n_hits, uint32
   w.tmp_loff = (uint32_t*)take(4 * ((size_t)cap_tracks + 1));
   w.tmp_hits = (uint32_t*)take(4 * ((size_t)cap_track_hits + 1));
   w.tmp_states = (float*)take(4 * (size_t)VELO_N_STATE * ((size_t)cap_tracks + 1));
-  w.team_scratch = take((size_t)num_sms() * kTeamsPerCtaMax * kTeamScratchBytes);
   w.n_slabs = n_slabs;
   w.slabs = take((size_t)n_slabs * slab_layout().bytes);
   w.bytes = o;
   return w;
 }
 
-int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, cudaEvent_t ev_start, cudaEvent_t ev_stop,
-                       uint32_t path, uint32_t teams, const PipeOpts& po) {
+int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const* stage_events, uint32_t path,
+                       const PipeOpts& po) {
   KernelArgs a = a_in;
   a.all_deferred = path == kPathSlabOnly ? 1u : 0u;
-  cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);   // phase_clk accumulates
+  auto mark = [&](int k) { if (stage_events && stage_events[k]) cudaEventRecord((cudaEvent_t)stage_events[k], stream); };
+  cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);
   if (err != cudaSuccess) return (int)err;
 #ifdef VELO_TIMELINE
   cudaMemsetAsync(a.ws.phase_clk, 0, sizeof(unsigned long long) * kNumPhaseClocks, stream);
 #endif
-  if (ev_start) cudaEventRecord(ev_start, stream);
+  mark(0);
   const uint32_t grid = a.n_events ? (a.ws.n_slabs < a.n_events ? a.ws.n_slabs : a.n_events) : 0u;
   const bool large_events = a.n_events && a.n_hits / a.n_events >= 4096u;
-  if (path == kPathTeamLegacy) {
-    if (a.n_events > 0) {
-      velo_order_kernel<<<1, 512, 0, stream>>>(a);
-      const int rc = launch_event_smem(a, stream, teams);
-      if (rc != 0) return rc;
-      if (large_events) velo_event_slab_kernel<kThreadsLarge, false, 8><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
-      else velo_event_slab_kernel<kThreads, true, kBinShift><<<grid, kThreads, 0, stream>>>(a, 1);
-    }
-    if (ev_stop) cudaEventRecord(ev_stop, stream);
-    velo_offsets_kernel<<<1, 256, 0, stream>>>(a);
-    if (a.n_events > 0) {
-      const uint32_t warps_per_cta = 128 / 32;
-      uint32_t cgrid = (a.n_events + warps_per_cta - 1) / warps_per_cta;
-      if (cgrid > num_sms() * 16u) cgrid = num_sms() * 16u;
-      velo_compact_kernel<<<cgrid, 128, 0, stream>>>(a);
-    }
-    return (int)cudaGetLastError();
-  }
   if (a.n_events > 0) {
     if (path == kPathSlabOnly) {
+      mark(1);
       velo_event_slab_kernel<kThreads, false, kBinShift><<<grid, kThreads, 0, stream>>>(a, 0);
     } else {
       // stage 1: sort; stage 2: module loop (events by size, largest first); then the general kernel
@@ -557,19 +505,25 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, cudaEvent_t 
       int rc = launch_sort(a, stream, po);
       if (rc != 0) return rc;
       velo_order_kernel<<<1, 512, 0, stream>>>(a);
+      mark(1);
       rc = launch_track(a, stream, po);
       if (rc != 0) return rc;
       if (large_events) velo_event_slab_kernel<kThreadsLarge, false, 8><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
       else velo_event_slab_kernel<kThreads, true, kBinShift><<<grid, kThreads, 0, stream>>>(a, 1);
     }
+  } else {
+    mark(1);
   }
+  mark(2);
   if (path != kPathSlabOnly) {
     const int rc = launch_fit(a, stream, po);   // fit and filters: per-candidate results, per-event counts
     if (rc != 0) return rc;
   }
+  mark(3);
   velo_offsets_kernel<<<1, 256, 0, stream>>>(a);   // counts -> event_track_offsets, summary
+  mark(4);
   const int rc = launch_write(a, stream);          // every final array, once
-  if (ev_stop) cudaEventRecord(ev_stop, stream);
+  mark(5);
   return rc != 0 ? rc : (int)cudaGetLastError();
 }
 

@@ -17,7 +17,8 @@ from . import build as _build
 VELO_OK, VELO_ERR_ARG, VELO_ERR_GEOMETRY, VELO_ERR_WORKSPACE = 0, -1, -2, -3
 VELO_ERR_CUDA, VELO_ERR_CAPACITY, VELO_ERR_INPUT = -4, -5, -6
 VELO_MAX_MODULES, VELO_MAX_EVENT_HITS, VELO_N_STATE = 32, 65535, 13
-VELO_PATH_DEFAULT, VELO_PATH_SLAB_ONLY, VELO_PATH_TEAM_LEGACY = 0, 1, 2
+VELO_PATH_DEFAULT, VELO_PATH_SLAB_ONLY = 0, 1
+VELO_N_STAGE_EVENTS = 6
 VELO_N_SUMMARY = 8
 STATE_NAMES = ("x", "y", "tx", "ty", "z", "cxx", "cxtx", "ctxtx", "cyy", "cyty", "ctyty", "chi2", "n_hits")
 ERROR_NAMES = {0: "VELO_OK", -1: "VELO_ERR_ARG", -2: "VELO_ERR_GEOMETRY", -3: "VELO_ERR_WORKSPACE",
@@ -60,8 +61,8 @@ class Tracks(ctypes.Structure):
 
 
 class LaunchOptions(ctypes.Structure):
-    _fields_ = [("event_kernel_start", c_void_p), ("event_kernel_stop", c_void_p), ("ctas_per_sm", c_uint32),
-                ("path", c_uint32), ("teams_per_cta", c_uint32), ("track_group", c_uint32),
+    _fields_ = [("stage_events", c_void_p * VELO_N_STAGE_EVENTS), ("ctas_per_sm", c_uint32),
+                ("path", c_uint32), ("track_group", c_uint32),
                 ("track_teams", c_uint32), ("fit_teams", c_uint32), ("sort_teams", c_uint32),
                 ("pool_units", c_uint32)]
 

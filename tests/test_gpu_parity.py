@@ -80,7 +80,7 @@ def test_run_to_run_determinism(velo):
 # ---- the event kernels: the three-stage pipeline (default) in several launch geometries, the general
 # slab kernel on its own, and the round-1 team kernel --------------------------------------------------
 @pytest.mark.parametrize("kw", [
-    {"path": 1}, {"path": 2},                                     # general slab kernel only; round-1 team kernel
+    {"path": 1},                                                  # general slab kernel only
     {"track_group": 32, "track_teams": 8}, {"track_group": 32, "track_teams": 24},
     {"track_group": 64}, {"track_group": 64, "track_teams": 15}, {"track_group": 128},
     {"fit_teams": 4}, {"fit_teams": 12}, {"fit_teams": 254}, {"sort_teams": 4}, {"sort_teams": 7}, {"sort_teams": 252},
