@@ -166,3 +166,108 @@ def event_candidates(x, y, z, module, n_modules: int, params: Params | None = No
             "pass": meta[:nc, 2].astype(bool), "survive": meta[:nc, 3].astype(bool), "lost": meta[:nc, 4],
             "key": key, "seed_scatter": meta[:nc, 7].copy().view(np.float32), "states": states[:nc],
             "perm": perm[:n], "phi": phi[:n], "mod_off": mod_off, "flags": flags[:n].astype(bool)}
+
+
+# ---- the steps after the hot path: oracle/velo_next_oracle.c ------------------
+_SRC_NEXT = os.path.join(_HERE, "velo_next_oracle.c")
+_LIB_NEXT = os.path.join(_HERE, "libvelo_next_oracle.so")
+MS_THETA2_DEFAULT = float(np.float32(9.0e-8))      # K-1: (0.3 mrad)^2
+
+
+class PvParams(ctypes.Structure):
+    """DESIGN.md §2 readings P-1 ... P-6 (paper silent)."""
+    _fields_ = [("z_min", ctypes.c_float), ("bin_width", ctypes.c_float), ("n_bins", ctypes.c_uint32),
+                ("seed_min_sum", ctypes.c_uint32), ("seed_half_window", ctypes.c_uint32),
+                ("chi2_max", ctypes.c_float), ("n_iterations", ctypes.c_uint32), ("min_tracks", ctypes.c_uint32),
+                ("max_pv_per_event", ctypes.c_uint32)]
+
+
+def default_pv_params() -> PvParams:
+    return PvParams(z_min=-300.0, bin_width=0.25, n_bins=2400, seed_min_sum=5, seed_half_window=6,
+                    chi2_max=16.0, n_iterations=4, min_tracks=4, max_pv_per_event=32)
+
+
+def build_next(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB_NEXT) or os.path.getmtime(_LIB_NEXT) < os.path.getmtime(_SRC_NEXT):
+        subprocess.run(["gcc", *CFLAGS, "-o", _LIB_NEXT, _SRC_NEXT, "-lm"], check=True)
+    return _LIB_NEXT
+
+
+_lib_next = None
+
+
+def lib_next():
+    global _lib_next
+    if _lib_next is None:
+        L = ctypes.CDLL(build_next())
+        vp = ctypes.c_void_p
+        L.vn_kalman.argtypes = [ctypes.c_uint32, vp, vp, vp, ctypes.c_float, ctypes.c_float, vp]
+        L.vn_kalman.restype = None
+        L.vn_kalman_tracks.argtypes = [ctypes.c_uint32, vp, vp, vp, vp, vp, ctypes.c_float, ctypes.c_float, vp]
+        L.vn_kalman_tracks.restype = None
+        L.vn_pv_bin.argtypes = [ctypes.c_float, ctypes.c_float, ctypes.c_float, ctypes.c_uint32]
+        L.vn_pv_bin.restype = ctypes.c_int32
+        L.vn_pv_seeds.argtypes = [vp, ctypes.c_uint32, ctypes.POINTER(PvParams), vp]
+        L.vn_pv_seeds.restype = ctypes.c_uint32
+        L.vn_pv_event.argtypes = [vp, ctypes.c_size_t, ctypes.c_uint32, ctypes.c_uint32, ctypes.POINTER(PvParams), vp]
+        L.vn_pv_event.restype = ctypes.c_uint32
+        L.vn_pv_find.argtypes = [ctypes.c_uint32, vp, vp, ctypes.c_size_t, ctypes.POINTER(PvParams), vp, vp,
+                                 ctypes.c_uint32]
+        L.vn_pv_find.restype = ctypes.c_uint32
+        _lib_next = L
+    return _lib_next
+
+
+def kalman(hx, hy, hz, sigma_hit, ms_theta2=MS_THETA2_DEFAULT) -> np.ndarray:
+    """K-1 ... K-5 on one track's hits (discovery order). 13 state words (O-11 layout)."""
+    hx = _f32(hx); hy = _f32(hy); hz = _f32(hz)
+    out = np.zeros(13, np.float32)
+    lib_next().vn_kalman(hx.shape[0], _p(hx), _p(hy), _p(hz), float(np.float32(sigma_hit)),
+                         float(np.float32(ms_theta2)), _p(out))
+    return out
+
+
+def kalman_tracks(res: dict, x, y, z, sigma_hit, ms_theta2=MS_THETA2_DEFAULT) -> np.ndarray:
+    """The filter on every track of a reconstruct() result. Returns 13 x n_tracks f32."""
+    x = _f32(x); y = _f32(y); z = _f32(z)
+    nt = int(res["n_tracks"])
+    tho = np.ascontiguousarray(res["track_hit_offsets"], dtype=np.uint32)
+    th = np.ascontiguousarray(res["track_hits"], dtype=np.uint32)
+    if th.shape[0] == 0:
+        th = np.zeros(1, np.uint32)
+    out = np.zeros((13, max(nt, 1)), np.float32)
+    if nt:
+        lib_next().vn_kalman_tracks(nt, _p(tho), _p(th), _p(x), _p(y), _p(z), float(np.float32(sigma_hit)),
+                                    float(np.float32(ms_theta2)), _p(out))
+    return out[:, :nt]
+
+
+def pv_bin(z, params: PvParams | None = None) -> int:
+    P = params if params is not None else default_pv_params()
+    inv_w = float(np.float32(1.0) / np.float32(P.bin_width))
+    return int(lib_next().vn_pv_bin(float(np.float32(z)), P.z_min, inv_w, P.n_bins))
+
+
+def pv_seeds(hist, params: PvParams | None = None) -> np.ndarray:
+    P = params if params is not None else default_pv_params()
+    h = np.ascontiguousarray(hist, dtype=np.uint32)
+    out = np.zeros(32, np.uint32)
+    n = lib_next().vn_pv_seeds(_p(h), h.shape[0], ctypes.byref(P), _p(out))
+    return out[:n].copy()
+
+
+def pv_find(event_track_offsets, states, params: PvParams | None = None) -> dict:
+    """P-1 ... P-6 on a batch of reconstructed tracks (states: 13 x n_tracks). Returns
+    event_pv_offsets (u32[n_events+1]), pvs (5 x n_pvs f32: x, y, z, sum of weights, n_tracks bits)."""
+    P = params if params is not None else default_pv_params()
+    eto = np.ascontiguousarray(event_track_offsets, dtype=np.uint32)
+    st = np.ascontiguousarray(states, dtype=np.float32)
+    ne = eto.shape[0] - 1
+    cap = max(32 * ne, 1)
+    epo = np.zeros(ne + 1, np.uint32)
+    pvs = np.zeros((5, cap), np.float32)
+    stride = st.shape[1] if st.ndim == 2 and st.shape[1] > 0 else 1
+    if st.size == 0:
+        st = np.zeros((13, 1), np.float32)
+    n = lib_next().vn_pv_find(ne, _p(eto), _p(st), stride, ctypes.byref(P), _p(epo), _p(pvs), cap)
+    return {"event_pv_offsets": epo, "pvs": pvs[:, :n].copy(), "n_pvs": int(n)}
