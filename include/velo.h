@@ -183,6 +183,58 @@ void velo_scheduler_free(velo_scheduler_t* s);
 int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, const velo_hits_t* hits,
                             const uint32_t* batch_begin, uint32_t n_batches, velo_tracks_t* out);
 
+/* ---- after the hot path: SURVEY.md §8(f) f2 and f3 ------------------------------------------- */
+/* f2. Parameterised Kalman filter on the VELO segment of every track (§5: "the Kalman
+ * filtering process on track uses a parameterised approach ... only the segment of a track inside
+ * the VELO is considered for the filtering process"; the paper gives no formula: readings K-1 ... K-5
+ * of DESIGN.md §2). x(z) and y(z) are independent lines; every hit measures both with variance
+ * sigma_hit^2; at every measured plane the slopes pick up noise ms_theta2 * (1 + tx^2 + ty^2); the
+ * filter starts from the exact two-point state of the two most downstream hits, runs towards the
+ * beamline and reports the state at closest approach to the z axis in the 13-word layout of
+ * velo_tracks_t.states (chi2 = sum of squared innovations over their variances, ndof = 2 n - 4).
+ * hits: the DEVICE planes velo_reconstruct was given (absolute hit index 0 at x[0]); tracks: its
+ * DEVICE outputs (track_hit_offsets, track_hits, summary, cap_tracks are read); kalman_states: DEVICE,
+ * 13 planes of tracks->cap_tracks words, written for the tracks the batch produced (none if the
+ * batch reported an error). Asynchronous on `stream`; returns VELO_ERR_ARG / VELO_ERR_CUDA. */
+int velo_kalman_fit(const velo_hits_t* hits, const velo_tracks_t* tracks, float sigma_hit, float ms_theta2,
+                    float* kalman_states, void* stream);
+
+/* f3. Primary vertices from the beamline states (§5: VELO tracks are straight
+ * lines; displaced-vertex lines need primary vertices; the paper gives no algorithm: readings
+ * P-1 ... P-6 of DESIGN.md §2). Per event: histogram of the tracks' z at the beamline; seeds = local
+ * maxima of the (1, 2, 1)-smoothed counts; every track goes to the seed nearest in z; each seed is
+ * fitted as the weighted least-squares point of its tracks' lines, weights 1/cxx times a Tukey
+ * factor (1 - chi2/chi2_max)^2, n_iterations times from (0, 0, z_seed); kept with >= min_tracks
+ * tracks of non-zero weight. Sums over tracks run as 32 partial sums by track index mod 32,
+ * combined by a butterfly (the order is part of the definition: the oracle does the same). */
+#define VELO_PV_MAX_PER_EVENT 32u
+#define VELO_PV_MAX_BINS 4096u
+#define VELO_N_PV_WORDS 5          /* planes of velo_pvs_t.pvs: x, y, z, sum of weights, n_tracks (u32 bits) */
+typedef struct {
+  float z_min, bin_width;          /* -300 mm, 0.25 mm */
+  uint32_t n_bins;                 /* 2400; at most VELO_PV_MAX_BINS */
+  uint32_t seed_min_sum;           /* 5 */
+  uint32_t seed_half_window;       /* 6 bins */
+  float chi2_max;                  /* 16 */
+  uint32_t n_iterations;           /* 4 */
+  uint32_t min_tracks;             /* 4 */
+  uint32_t max_pv_per_event;       /* 32 = VELO_PV_MAX_PER_EVENT (larger values are clamped); lowest z first */
+} velo_pv_params_t;
+void velo_pv_params_default(velo_pv_params_t* p);
+typedef struct {                   /* caller-allocated DEVICE buffers */
+  uint32_t* event_pv_offsets;      /* n_events+1: vertices of event e are [off[e], off[e+1]), ascending seed z */
+  float* pvs;                      /* VELO_N_PV_WORDS planes x cap_pvs */
+  uint32_t cap_pvs;                /* 32 * n_events can never overflow */
+  uint32_t* summary;               /* u32[4]: n_pvs (or the required capacity), status, 0, 0 */
+} velo_pvs_t;
+size_t velo_pv_workspace_bytes(uint32_t n_events, uint32_t cap_tracks);
+/* tracks: DEVICE outputs of velo_reconstruct (event_track_offsets, states, summary, cap_tracks are
+ * read); workspace: DEVICE, 256-byte aligned, velo_pv_workspace_bytes(n_events, tracks->cap_tracks).
+ * Asynchronous on `stream`. More vertices than cap_pvs -> out->summary[1] = VELO_ERR_CAPACITY and
+ * summary[0] = the required capacity; a failed velo_reconstruct status is passed on. */
+int velo_pv_find(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_params_t* params, velo_pvs_t* out,
+                 void* workspace, size_t workspace_bytes, void* stream);
+
 /* Library version string, e.g. "velo-b200 0.1 (sm_100a)". */
 const char* velo_version(void);
 

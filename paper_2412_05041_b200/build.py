@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libvelo.so")
-SOURCES = ["velo_api.cu", "velo_kernels.cu", "velo_sort.cu", "velo_track.cu", "velo_fit.cu",
+SOURCES = ["velo_api.cu", "velo_kernels.cu", "velo_sort.cu", "velo_track.cu", "velo_fit.cu", "velo_next.cu",
            "velo_scheduler.cu"]
 HEADERS = ["velo_device.cuh", "velo_internal.h", "velo_pool.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

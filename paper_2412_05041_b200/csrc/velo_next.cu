@@ -1,0 +1,318 @@
+// velo_next.cu — the two steps that follow the VELO hot path (sm_100a):
+//   velo_kalman_fit: a parameterised Kalman filter on the VELO segment of every track (§5,
+//     "the Kalman filtering process on track uses a parameterised approach ... only the segment of a
+//     track inside the VELO is considered"), readings K-1 ... K-5 of DESIGN.md §2;
+//   velo_pv_find: primary vertices from the beamline states (§5: VELO tracks are
+//     straight lines; displaced-vertex lines need primary vertices), readings P-1 ... P-6.
+// Both consume the device outputs of velo_reconstruct. Every float operation is a round-to-nearest
+// intrinsic in the order DESIGN.md §2 fixes (no FMA contraction): the filter's chi2 and the fitted
+// vertex decide integers (track weights > 0, vertices kept), so the order is part of the method.
+#include "velo_device.cuh"
+#include "velo_internal.h"
+
+namespace velo {
+
+namespace {
+
+// ---- f2: one thread per track -----------------------------------------------------------------------
+// The hits of a track are gathered through track_hits (absolute hit indices, discovery order =
+// decreasing z). The next hit's index and coordinates are loaded while the current one is filtered.
+__global__ void __launch_bounds__(256) velo_kalman_kernel(const float* __restrict__ hx, const float* __restrict__ hy,
+                                                          const float* __restrict__ hz, const uint32_t* __restrict__ tho,
+                                                          const uint32_t* __restrict__ th, const uint32_t* __restrict__ summary,
+                                                          float sigma_hit, float ms_theta2, float* __restrict__ out,
+                                                          uint32_t cap_tracks) {
+  const uint32_t n_tracks = summary[2] == 0u ? summary[0] : 0u;     // a failed batch has no tracks to fit
+  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_tracks || t >= cap_tracks) return;
+  const uint32_t a = tho[t], n = tho[t + 1] - a;
+  const float s2 = __fmul_rn(sigma_hit, sigma_hit);
+  uint32_t i0 = th[a], i1 = th[a + 1];
+  const float x0 = hx[i0], y0 = hy[i0], z0 = hz[i0];
+  float zp = hz[i1];
+  float x = hx[i1], y = hy[i1];
+  float dz = __fsub_rn(zp, z0);
+  float tx = __fdiv_rn(__fsub_rn(x, x0), dz), ty = __fdiv_rn(__fsub_rn(y, y0), dz);
+  float cxx = s2, cxtx = __fdiv_rn(s2, dz), ctxtx = __fdiv_rn(__fadd_rn(s2, s2), __fmul_rn(dz, dz));
+  float chi2 = 0.0f;
+  // software pipeline: hit i+1 is in flight while hit i is processed
+  float nx = 0.0f, ny = 0.0f, nz = 0.0f;
+  if (n > 2) { const uint32_t j = th[a + 2]; nx = hx[j]; ny = hy[j]; nz = hz[j]; }
+  for (uint32_t i = 2; i < n; ++i) {
+    const float mx = nx, my = ny, mzz = nz;
+    if (i + 1 < n) { const uint32_t j = th[a + i + 1]; nx = hx[j]; ny = hy[j]; nz = hz[j]; }
+    const float sl = __fadd_rn(1.0f, __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty)));
+    ctxtx = __fadd_rn(ctxtx, __fmul_rn(ms_theta2, sl));
+    dz = __fsub_rn(mzz, zp);
+    const float xp = __fadd_rn(x, __fmul_rn(tx, dz)), yp = __fadd_rn(y, __fmul_rn(ty, dz));
+    const float cxtx_p = __fadd_rn(cxtx, __fmul_rn(dz, ctxtx));
+    const float cxx_p = __fadd_rn(__fadd_rn(cxx, __fmul_rn(dz, cxtx)), __fmul_rn(dz, cxtx_p));
+    const float S = __fadd_rn(cxx_p, s2);
+    const float k0 = __fdiv_rn(cxx_p, S), k1 = __fdiv_rn(cxtx_p, S);
+    const float rx = __fsub_rn(mx, xp), ry = __fsub_rn(my, yp);
+    x = __fadd_rn(xp, __fmul_rn(k0, rx)); y = __fadd_rn(yp, __fmul_rn(k0, ry));
+    tx = __fadd_rn(tx, __fmul_rn(k1, rx)); ty = __fadd_rn(ty, __fmul_rn(k1, ry));
+    cxx = __fmul_rn(__fsub_rn(1.0f, k0), cxx_p);
+    cxtx = __fmul_rn(__fsub_rn(1.0f, k0), cxtx_p);
+    ctxtx = __fsub_rn(ctxtx, __fmul_rn(k1, cxtx_p));
+    const float r2 = __fadd_rn(__fmul_rn(rx, rx), __fmul_rn(ry, ry));
+    chi2 = __fadd_rn(chi2, __fdiv_rn(r2, S));
+    zp = mzz;
+  }
+  const float ss = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
+  ctxtx = __fadd_rn(ctxtx, __fmul_rn(ms_theta2, __fadd_rn(1.0f, ss)));
+  float dzb;
+  if (ss < 1e-12f) dzb = 0.0f;
+  else dzb = -__fdiv_rn(__fadd_rn(__fmul_rn(x, tx), __fmul_rn(y, ty)), ss);
+  const float cxtx_b = __fadd_rn(cxtx, __fmul_rn(dzb, ctxtx));
+  const float cxx_b = __fadd_rn(__fadd_rn(cxx, __fmul_rn(dzb, cxtx)), __fmul_rn(dzb, cxtx_b));
+  const size_t cs = cap_tracks;
+  float* o = out + t;
+  o[0] = __fadd_rn(x, __fmul_rn(tx, dzb)); o[cs] = __fadd_rn(y, __fmul_rn(ty, dzb));
+  o[2 * cs] = tx; o[3 * cs] = ty; o[4 * cs] = __fadd_rn(zp, dzb);
+  o[5 * cs] = cxx_b; o[6 * cs] = cxtx_b; o[7 * cs] = ctxtx;
+  o[8 * cs] = cxx_b; o[9 * cs] = cxtx_b; o[10 * cs] = ctxtx;
+  o[11 * cs] = chi2; o[12 * cs] = __uint_as_float(n);
+}
+
+// ---- f3: one warp per event ---------------------------------------------------------------------------
+constexpr uint32_t kPvMax = VELO_PV_MAX_PER_EVENT;   // 32: a seed per lane
+constexpr uint32_t kPvWarps = 4;                      // events per CTA
+
+struct PvArgs {
+  const uint32_t* eto;        // event_track_offsets[n_events + 1]
+  const float* states;        // 13 planes of `stride` words
+  const uint32_t* summary;    // velo_reconstruct's summary (status)
+  size_t stride;
+  uint32_t n_events;
+  velo_pv_params_t P;
+  float inv_w;                // 1.0f / bin_width, computed once on the host in fp32
+  float* tmp_pv;              // n_events * kPvMax * 5
+  uint32_t* tmp_cnt;          // n_events
+  uint8_t* asg;               // one byte per track (global track index)
+};
+
+__device__ __forceinline__ float warp_butterfly(float v) {
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) v = __fadd_rn(v, __shfl_xor_sync(0xffffffffu, v, d));
+  return v;
+}
+
+__global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const uint32_t wid = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+  const uint32_t nb = a.P.n_bins, nbw = (nb + 1u) >> 1;          // bins; packed-u16 words
+  const uint32_t per_warp = 4u * nbw + 4u * nb + 4u * kPvMax;
+  uint32_t* hw = reinterpret_cast<uint32_t*>(smem + (size_t)wid * per_warp);   // P-1 histogram, two u16 counts per word
+  uint32_t* s = hw + nbw;                                                       // P-2 smoothed counts
+  float* zs = reinterpret_cast<float*>(s + nb);                                 // seed z
+  const bool failed = a.summary[2] != 0u;
+  const float* X = a.states; const float* Y = X + a.stride; const float* TX = Y + a.stride; const float* TY = TX + a.stride;
+  const float* Z = TY + a.stride; const float* CXX = Z + a.stride;
+  auto hist = [&](uint32_t b) -> uint32_t { return (hw[b >> 1] >> ((b & 1u) * 16u)) & 0xffffu; };
+  for (uint32_t e = blockIdx.x * kPvWarps + wid; e < a.n_events; e += gridDim.x * kPvWarps) {
+    const uint32_t t0 = failed ? 0u : a.eto[e], nt = failed ? 0u : a.eto[e + 1] - t0;
+    // P-1
+    for (uint32_t k = lane; k < nbw; k += 32u) hw[k] = 0u;
+    __syncwarp();
+    for (uint32_t i = lane; i < nt; i += 32u) {
+      const float t = __fmul_rn(__fsub_rn(Z[t0 + i], a.P.z_min), a.inv_w);
+      if (t >= 0.0f && t < (float)nb) { const uint32_t b = (uint32_t)(int)t; atomicAdd(&hw[b >> 1], 1u << ((b & 1u) * 16u)); }
+    }
+    __syncwarp();
+    // P-2 smoothed counts, then seeds in ascending bin order (ballot keeps the order)
+    for (uint32_t b = lane; b < nb; b += 32u) {
+      uint32_t v = 2u * hist(b);
+      if (b > 0u) v += hist(b - 1u);
+      if (b + 1u < nb) v += hist(b + 1u);
+      s[b] = v;
+    }
+    __syncwarp();
+    uint32_t ns = 0;
+    const uint32_t cap = a.P.max_pv_per_event < kPvMax ? a.P.max_pv_per_event : kPvMax;
+    for (uint32_t b0 = 0; b0 < nb && ns < cap; b0 += 32u) {
+      const uint32_t b = b0 + lane;
+      bool ok = false;
+      if (b < nb) {
+        const uint32_t c = s[b];
+        ok = c >= a.P.seed_min_sum && c > 0u;
+        for (uint32_t j = 1; j <= a.P.seed_half_window && ok; ++j) {
+          const uint32_t left = b >= j ? s[b - j] : 0u, right = b + j < nb ? s[b + j] : 0u;
+          ok = (c > left) && (c >= right);
+        }
+      }
+      const uint32_t m = __ballot_sync(0xffffffffu, ok);
+      const uint32_t pos = ns + (uint32_t)__popc(m & ((1u << lane) - 1u));
+      if (ok && pos < cap) zs[pos] = __fadd_rn(a.P.z_min, __fmul_rn(__fadd_rn((float)b, 0.5f), a.P.bin_width));
+      ns = min(ns + (uint32_t)__popc(m), cap);
+    }
+    __syncwarp();
+    uint32_t nout = 0;
+    if (ns > 0) {
+      // P-3 every track to its nearest seed (ties to the lower seed)
+      for (uint32_t i = lane; i < nt; i += 32u) {
+        const float z = Z[t0 + i];
+        uint32_t best = 0; float bd = fabsf(__fsub_rn(z, zs[0]));
+        for (uint32_t v = 1; v < ns; ++v) { const float dd = fabsf(__fsub_rn(z, zs[v])); if (dd < bd) { bd = dd; best = v; } }
+        a.asg[t0 + i] = (uint8_t)best;
+      }
+      __syncwarp();
+      // P-4, P-5, P-6: lane l sums the tracks with i mod 32 == l in increasing i, butterfly combine
+      for (uint32_t v = 0; v < ns; ++v) {
+        float xv = 0.0f, yv = 0.0f, zv = zs[v], S0 = 0.0f;
+        uint32_t ntrk = 0; bool alive = true;
+        for (uint32_t it = 0; it < a.P.n_iterations && alive; ++it) {
+          float l0 = 0.0f, lx = 0.0f, ly = 0.0f, lxx = 0.0f, la = 0.0f, lb = 0.0f, lc = 0.0f, ln = 0.0f;
+          for (uint32_t i = lane; i < nt; i += 32u) {
+            if (a.asg[t0 + i] != v) continue;
+            const float x = X[t0 + i], y = Y[t0 + i], tx = TX[t0 + i], ty = TY[t0 + i], z = Z[t0 + i];
+            const float dz = __fsub_rn(zv, z);
+            const float rx = __fsub_rn(__fadd_rn(x, __fmul_rn(tx, dz)), xv);
+            const float ry = __fsub_rn(__fadd_rn(y, __fmul_rn(ty, dz)), yv);
+            const float w0 = __fdiv_rn(1.0f, CXX[t0 + i]);
+            const float c = __fmul_rn(w0, __fadd_rn(__fmul_rn(rx, rx), __fmul_rn(ry, ry)));
+            float wt = 0.0f;
+            if (c < a.P.chi2_max) { const float u = __fsub_rn(1.0f, __fdiv_rn(c, a.P.chi2_max)); wt = __fmul_rn(u, u); }
+            const float w = __fmul_rn(w0, wt);
+            const float aa = __fsub_rn(x, __fmul_rn(tx, z)), bb = __fsub_rn(y, __fmul_rn(ty, z));
+            const float t2 = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
+            const float ab = __fadd_rn(__fmul_rn(tx, aa), __fmul_rn(ty, bb));
+            l0 = __fadd_rn(l0, w);
+            lx = __fadd_rn(lx, __fmul_rn(w, tx)); ly = __fadd_rn(ly, __fmul_rn(w, ty));
+            lxx = __fadd_rn(lxx, __fmul_rn(w, t2));
+            la = __fadd_rn(la, __fmul_rn(w, aa)); lb = __fadd_rn(lb, __fmul_rn(w, bb));
+            lc = __fadd_rn(lc, __fmul_rn(w, ab));
+            if (wt > 0.0f) ln = __fadd_rn(ln, 1.0f);
+          }
+          S0 = warp_butterfly(l0);
+          const float Sx = warp_butterfly(lx), Sy = warp_butterfly(ly), Sxx = warp_butterfly(lxx);
+          const float A = warp_butterfly(la), B = warp_butterfly(lb), C = warp_butterfly(lc);
+          ntrk = (uint32_t)warp_butterfly(ln);
+          if (!(S0 > 0.0f)) { alive = false; break; }
+          const float den = __fsub_rn(Sxx, __fdiv_rn(__fadd_rn(__fmul_rn(Sx, Sx), __fmul_rn(Sy, Sy)), S0));
+          if (!(den > 0.0f)) { alive = false; break; }
+          zv = __fdiv_rn(__fsub_rn(__fdiv_rn(__fadd_rn(__fmul_rn(Sx, A), __fmul_rn(Sy, B)), S0), C), den);
+          xv = __fdiv_rn(__fadd_rn(A, __fmul_rn(Sx, zv)), S0);
+          yv = __fdiv_rn(__fadd_rn(B, __fmul_rn(Sy, zv)), S0);
+        }
+        if (alive && ntrk >= a.P.min_tracks) {
+          if (lane == 0) {
+            float* o = a.tmp_pv + ((size_t)e * kPvMax + nout) * 5u;
+            o[0] = xv; o[1] = yv; o[2] = zv; o[3] = S0; o[4] = __uint_as_float(ntrk);
+          }
+          ++nout;
+        }
+      }
+    }
+    if (lane == 0) a.tmp_cnt[e] = nout;
+    __syncwarp();
+  }
+}
+
+// counts -> event_pv_offsets, then every event's vertices to their place (one CTA)
+__global__ void __launch_bounds__(1024) velo_pv_offsets_kernel(const PvArgs a, uint32_t* event_pv_offsets, float* pvs,
+                                                               uint32_t cap_pvs, uint32_t* pv_summary) {
+  __shared__ unsigned long long warp_sums[33];
+  const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;
+  const uint32_t per = (ne + nthr - 1) / nthr;
+  const uint32_t e0 = min(tid * per, ne), e1 = min(e0 + per, ne);
+  unsigned long long sum = 0;
+  for (uint32_t e = e0; e < e1; ++e) sum += a.tmp_cnt[e];
+  unsigned long long tot;
+  unsigned long long run = block_scan_excl(sum, warp_sums, &tot);
+  const bool over = tot > cap_pvs;
+  for (uint32_t e = e0; e < e1; ++e) {
+    const uint32_t n = a.tmp_cnt[e];
+    event_pv_offsets[e] = (uint32_t)run;
+    if (!over) {
+      for (uint32_t k = 0; k < n; ++k) {
+        const float* src = a.tmp_pv + ((size_t)e * kPvMax + k) * 5u;
+#pragma unroll
+        for (uint32_t p = 0; p < 5; ++p) pvs[(size_t)p * cap_pvs + (uint32_t)run + k] = src[p];
+      }
+    }
+    run += n;
+  }
+  if (tid == 0) {
+    event_pv_offsets[ne] = (uint32_t)tot;
+    uint32_t status = a.summary[2];
+    if (status == 0u && over) status = (uint32_t)VELO_ERR_CAPACITY;
+    pv_summary[0] = (uint32_t)tot; pv_summary[1] = status; pv_summary[2] = 0u; pv_summary[3] = 0u;
+  }
+}
+
+struct PvWorkspace { float* tmp_pv; uint32_t* tmp_cnt; uint8_t* asg; size_t bytes; };
+PvWorkspace carve_pv(void* base, uint32_t n_events, uint32_t cap_tracks) {
+  PvWorkspace w{};
+  size_t o = 0;
+  unsigned char* b = (unsigned char*)base;
+  auto take = [&](size_t bytes) { size_t r = o; o += ((bytes + 255) / 256) * 256; return b + r; };
+  w.tmp_pv = (float*)take(sizeof(float) * 5u * kPvMax * ((size_t)n_events + 1));
+  w.tmp_cnt = (uint32_t*)take(4 * ((size_t)n_events + 1));
+  w.asg = (uint8_t*)take((size_t)cap_tracks + 1);
+  w.bytes = o;
+  return w;
+}
+
+}  // namespace
+
+}  // namespace velo
+
+extern "C" {
+
+int velo_kalman_fit(const velo_hits_t* hits, const velo_tracks_t* tracks, float sigma_hit, float ms_theta2,
+                    float* kalman_states, void* stream) {
+  if (!hits || !tracks || !kalman_states) return VELO_ERR_ARG;
+  if (!tracks->track_hit_offsets || !tracks->track_hits || !tracks->summary || tracks->cap_tracks == 0) return VELO_ERR_ARG;
+  if (hits->n_hits && (!hits->x || !hits->y || !hits->z)) return VELO_ERR_ARG;
+  if (!(sigma_hit > 0.0f) || !(ms_theta2 >= 0.0f)) return VELO_ERR_ARG;
+  const uint32_t threads = 256, grid = (tracks->cap_tracks + threads - 1) / threads;
+  velo::velo_kalman_kernel<<<grid, threads, 0, (cudaStream_t)stream>>>(
+      hits->x, hits->y, hits->z, tracks->track_hit_offsets, tracks->track_hits, tracks->summary, sigma_hit, ms_theta2,
+      kalman_states, tracks->cap_tracks);
+  return cudaGetLastError() == cudaSuccess ? VELO_OK : VELO_ERR_CUDA;
+}
+
+void velo_pv_params_default(velo_pv_params_t* p) {
+  if (!p) return;
+  p->z_min = -300.0f; p->bin_width = 0.25f; p->n_bins = 2400;
+  p->seed_min_sum = 5; p->seed_half_window = 6;
+  p->chi2_max = 16.0f; p->n_iterations = 4; p->min_tracks = 4; p->max_pv_per_event = VELO_PV_MAX_PER_EVENT;
+}
+
+size_t velo_pv_workspace_bytes(uint32_t n_events, uint32_t cap_tracks) {
+  return velo::carve_pv(nullptr, n_events, cap_tracks).bytes;
+}
+
+int velo_pv_find(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_params_t* params, velo_pvs_t* out,
+                 void* workspace, size_t workspace_bytes, void* stream) {
+  using namespace velo;
+  if (!tracks || !params || !out || !workspace) return VELO_ERR_ARG;
+  if (!tracks->event_track_offsets || !tracks->states || !tracks->summary || tracks->cap_tracks == 0) return VELO_ERR_ARG;
+  if (!out->event_pv_offsets || !out->pvs || !out->summary || out->cap_pvs == 0) return VELO_ERR_ARG;
+  if (params->n_bins == 0 || params->n_bins > VELO_PV_MAX_BINS || !(params->bin_width > 0.0f) || !(params->chi2_max > 0.0f))
+    return VELO_ERR_ARG;
+  if (((uintptr_t)workspace & 255u) != 0) return VELO_ERR_ARG;
+  const PvWorkspace w = carve_pv(workspace, n_events, tracks->cap_tracks);
+  if (workspace_bytes < w.bytes) return VELO_ERR_WORKSPACE;
+  PvArgs a{};
+  a.eto = tracks->event_track_offsets; a.states = tracks->states; a.summary = tracks->summary;
+  a.stride = tracks->cap_tracks; a.n_events = n_events; a.P = *params;
+  a.inv_w = 1.0f / params->bin_width;
+  a.tmp_pv = w.tmp_pv; a.tmp_cnt = w.tmp_cnt; a.asg = w.asg;
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint32_t nbw = (params->n_bins + 1u) >> 1;
+  const uint32_t smem = kPvWarps * (4u * nbw + 4u * params->n_bins + 4u * kPvMax);
+  cudaError_t err = cudaFuncSetAttribute(velo_pv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (err != cudaSuccess) return VELO_ERR_CUDA;
+  if (n_events > 0) {
+    uint32_t grid = (n_events + kPvWarps - 1) / kPvWarps;
+    const uint32_t most = num_sms() * 8u;
+    if (grid > most) grid = most;
+    velo_pv_kernel<<<grid, 32 * kPvWarps, smem, st>>>(a);
+  }
+  velo_pv_offsets_kernel<<<1, 1024, 0, st>>>(a, out->event_pv_offsets, out->pvs, out->cap_pvs, out->summary);
+  return cudaGetLastError() == cudaSuccess ? VELO_OK : VELO_ERR_CUDA;
+}
+
+}  // extern "C"

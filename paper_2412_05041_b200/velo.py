@@ -28,7 +28,8 @@ ERROR_NAMES = {0: "VELO_OK", -1: "VELO_ERR_ARG", -2: "VELO_ERR_GEOMETRY", -3: "V
 EXPORTS = ("velo_version", "velo_geometry_load", "velo_geometry_free", "velo_geometry_n_modules",
            "velo_params_default", "velo_workspace_bytes", "velo_workspace_bytes_opts", "velo_reconstruct",
            "velo_reconstruct_opts", "velo_scheduler_create",
-           "velo_scheduler_free", "velo_scheduler_run_host")
+           "velo_scheduler_free", "velo_scheduler_run_host",
+           "velo_kalman_fit", "velo_pv_params_default", "velo_pv_workspace_bytes", "velo_pv_find")
 
 
 class VeloError(RuntimeError):
@@ -66,6 +67,19 @@ class LaunchOptions(ctypes.Structure):
                 ("track_teams", c_uint32), ("fit_teams", c_uint32), ("sort_teams", c_uint32),
                 ("pool_units", c_uint32)]
 
+
+class PvParams(ctypes.Structure):
+    _fields_ = [("z_min", c_float), ("bin_width", c_float), ("n_bins", c_uint32), ("seed_min_sum", c_uint32),
+                ("seed_half_window", c_uint32), ("chi2_max", c_float), ("n_iterations", c_uint32),
+                ("min_tracks", c_uint32), ("max_pv_per_event", c_uint32)]
+
+
+class Pvs(ctypes.Structure):
+    _fields_ = [("event_pv_offsets", c_void_p), ("pvs", c_void_p), ("cap_pvs", c_uint32), ("summary", c_void_p)]
+
+
+VELO_N_PV_WORDS = 5
+MS_THETA2_DEFAULT = 9.0e-8      # K-1: (0.3 mrad)^2
 
 _lib = None
 
@@ -107,6 +121,15 @@ def lib():
         L.velo_scheduler_run_host.argtypes = [c_void_p, POINTER(Params), POINTER(Hits), c_void_p, c_uint32,
                                               POINTER(Tracks)]
         L.velo_scheduler_run_host.restype = c_int
+        L.velo_kalman_fit.argtypes = [POINTER(Hits), POINTER(Tracks), c_float, c_float, c_void_p, c_void_p]
+        L.velo_kalman_fit.restype = c_int
+        L.velo_pv_params_default.argtypes = [POINTER(PvParams)]
+        L.velo_pv_params_default.restype = None
+        L.velo_pv_workspace_bytes.argtypes = [c_uint32, c_uint32]
+        L.velo_pv_workspace_bytes.restype = c_size_t
+        L.velo_pv_find.argtypes = [POINTER(Tracks), c_uint32, POINTER(PvParams), POINTER(Pvs), c_void_p, c_size_t,
+                                   c_void_p]
+        L.velo_pv_find.restype = c_int
         _lib = L
     return _lib
 
@@ -246,6 +269,71 @@ def velo_reconstruct(geometry: Geometry, hits: Hits, params: Params, out: Device
 
 
 velo_reconstruct_opts = velo_reconstruct
+
+
+# ---- after the hot path: Kalman filter on the VELO segment, primary vertices ----
+def velo_kalman_fit(hits: Hits, tracks: DeviceTracks, sigma_hit: float, ms_theta2: float = MS_THETA2_DEFAULT,
+                    stream=None):
+    """Enqueues the filter for every track of `tracks` (the outputs of velo_reconstruct for `hits`).
+    Returns a device tensor of 13 planes x cap_tracks."""
+    torch = _torch()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    out = torch.empty((VELO_N_STATE, tracks.cap_tracks), dtype=torch.float32, device=tracks.states.device)
+    tr = tracks.struct()
+    rc = lib().velo_kalman_fit(byref(hits), byref(tr), c_float(sigma_hit), c_float(ms_theta2), c_void_p(out.data_ptr()),
+                               c_void_p(st.cuda_stream))
+    if rc != VELO_OK:
+        raise VeloError(rc, "velo_kalman_fit")
+    return out
+
+
+def velo_pv_params_default() -> PvParams:
+    p = PvParams()
+    lib().velo_pv_params_default(byref(p))
+    return p
+
+
+def velo_pv_workspace_bytes(n_events: int, cap_tracks: int) -> int:
+    return int(lib().velo_pv_workspace_bytes(n_events, cap_tracks))
+
+
+class DevicePvs:
+    """Caller-allocated output buffers of velo_pv_find (velo_pvs_t) plus its workspace."""
+
+    def __init__(self, n_events: int, cap_tracks: int, cap_pvs: int | None = None, device="cuda"):
+        torch = _torch()
+        self.n_events = n_events
+        self.cap_pvs = int(cap_pvs if cap_pvs is not None else 32 * n_events + 1)
+        i32 = dict(dtype=torch.int32, device=device)
+        self.event_pv_offsets = torch.empty(n_events + 1, **i32)
+        self.pvs = torch.empty((VELO_N_PV_WORDS, self.cap_pvs), dtype=torch.float32, device=device)
+        self.summary = torch.zeros(4, **i32)
+        self.workspace_bytes = velo_pv_workspace_bytes(n_events, cap_tracks)
+        self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=device)
+        self.workspace_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+
+    def struct(self) -> Pvs:
+        return Pvs(event_pv_offsets=self.event_pv_offsets.data_ptr(), pvs=self.pvs.data_ptr(), cap_pvs=self.cap_pvs,
+                   summary=self.summary.data_ptr())
+
+    def to_host(self) -> dict:
+        s = self.summary.cpu().numpy().view(np.uint32)
+        n, status = int(s[0]), int(np.int32(s[1]))
+        if status != VELO_OK:
+            raise VeloError(status, f"velo_pv_find (device status; required cap_pvs={n})")
+        return {"event_pv_offsets": self.event_pv_offsets.cpu().numpy().view(np.uint32),
+                "pvs": self.pvs[:, :n].cpu().numpy(), "n_pvs": n}
+
+
+def velo_pv_find(tracks: DeviceTracks, out: DevicePvs, params: PvParams | None = None, stream=None) -> None:
+    torch = _torch()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    P = params if params is not None else velo_pv_params_default()
+    tr = tracks.struct(); pv = out.struct()
+    rc = lib().velo_pv_find(byref(tr), tracks.n_events, byref(P), byref(pv), c_void_p(out.workspace_ptr),
+                            c_size_t(out.workspace_bytes), c_void_p(st.cuda_stream))
+    if rc != VELO_OK:
+        raise VeloError(rc, "velo_pv_find")
 
 
 def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None = None, n_batches: int = 1,
