@@ -267,6 +267,31 @@ class Workload:
                                        for r in range(reps) for b in range(self.n_batches)]))
         return out
 
+    def after_path_pass(self, reps):
+        """The two steps after the hot path on the batches' device outputs:
+        velo_kalman_fit and velo_pv_find, timed with CUDA events on one stream."""
+        torch, velo = self.torch, self.velo
+        st = self.streams[0]
+        pvs = [velo.DevicePvs(o.n_events, o.cap_tracks) for o in self.outs]
+        kal = torch.empty((velo.VELO_N_STATE, max(o.cap_tracks for o in self.outs)), dtype=torch.float32, device="cuda")
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(reps * self.n_batches)]
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            for r in range(reps):
+                for b in range(self.n_batches):
+                    e = ev[r * self.n_batches + b]
+                    e[0].record(st)
+                    velo.velo_kalman_fit(self.hstructs[b], self.outs[b], self.P.sigma_hit, stream=st, out=kal)
+                    e[1].record(st)
+                    velo.velo_pv_find(self.outs[b], pvs[b], stream=st)
+                    e[2].record(st)
+        torch.cuda.synchronize()
+        n_pvs = sum(p.to_host()["n_pvs"] for p in pvs)
+        return {"kalman_ms_per_launch": float(np.mean([e[0].elapsed_time(e[1]) for e in ev])),
+                "pv_ms_per_launch": float(np.mean([e[1].elapsed_time(e[2]) for e in ev])), "n_pvs": n_pvs,
+                "what": "velo_kalman_fit (parameterised Kalman filter on the VELO segment) and velo_pv_find (primary "
+                        "vertices) on each batch's device outputs; not part of `value`"}
+
     def results(self):
         return [o.to_host() for o in self.outs]          # raises on any device-side status
 
@@ -376,6 +401,8 @@ def run_velo(args):
     stage_ms = wl.stage_pass(stage_reps)
     launches += kernels_per_batch * n_batches * stage_reps
     stage_sum = sum(stage_ms.values())
+    after_path = wl.after_path_pass(stage_reps)
+    launches += 3 * n_batches * stage_reps
     peak, peak_src = measured_peak_gbs()
     counters = stage_counters() if (args.config == 2 and args.path == 0 and n_events // n_batches == STAGE_COUNTERS_EVENTS) else {}
 
@@ -431,6 +458,7 @@ def run_velo(args):
                    "unit": "G warp instr/s", "frac": events_per_s / world * warp_inst / issue_peak,
                    "warp_instructions_per_event": warp_inst, "source": "profiles/r02e_stage_counters.csv"}
                   if warp_inst else None),
+        "after_path": after_path,
         "clocks": clocks,
     }
 

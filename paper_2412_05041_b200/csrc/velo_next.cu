@@ -149,14 +149,33 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
     __syncwarp();
     uint32_t nout = 0;
     if (ns > 0) {
+      // Once the seeds are known the histogram is dead: its shared memory takes the event's tracks
+      // (six words and the seed index each), so that the fit iterations touch no global memory. An
+      // event with more tracks than fit there reads them from global memory instead, in the same order.
+      const uint32_t stage_cap = (4u * nbw + 4u * nb) / 25u;
+      const bool resident = nt <= stage_cap;
+      float* sx = reinterpret_cast<float*>(hw);
+      float* sy = sx + stage_cap; float* stx = sy + stage_cap; float* sty = stx + stage_cap;
+      float* sz = sty + stage_cap; float* sw0 = sz + stage_cap;
+      uint8_t* sasg = reinterpret_cast<uint8_t*>(sw0 + stage_cap);
       // P-3 every track to its nearest seed (ties to the lower seed)
       for (uint32_t i = lane; i < nt; i += 32u) {
         const float z = Z[t0 + i];
         uint32_t best = 0; float bd = fabsf(__fsub_rn(z, zs[0]));
         for (uint32_t v = 1; v < ns; ++v) { const float dd = fabsf(__fsub_rn(z, zs[v])); if (dd < bd) { bd = dd; best = v; } }
-        a.asg[t0 + i] = (uint8_t)best;
+        if (resident) {
+          sasg[i] = (uint8_t)best;
+          sx[i] = X[t0 + i]; sy[i] = Y[t0 + i]; stx[i] = TX[t0 + i]; sty[i] = TY[t0 + i]; sz[i] = z;
+          sw0[i] = __fdiv_rn(1.0f, CXX[t0 + i]);
+        } else {
+          a.asg[t0 + i] = (uint8_t)best;
+        }
       }
       __syncwarp();
+      const float* PX = resident ? sx : X + t0; const float* PY = resident ? sy : Y + t0;
+      const float* PTX = resident ? stx : TX + t0; const float* PTY = resident ? sty : TY + t0;
+      const float* PZ = resident ? sz : Z + t0; const float* PW = resident ? sw0 : CXX + t0;
+      const uint8_t* PA = resident ? sasg : a.asg + t0;
       // P-4, P-5, P-6: lane l sums the tracks with i mod 32 == l in increasing i, butterfly combine
       for (uint32_t v = 0; v < ns; ++v) {
         float xv = 0.0f, yv = 0.0f, zv = zs[v], S0 = 0.0f;
@@ -164,12 +183,12 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
         for (uint32_t it = 0; it < a.P.n_iterations && alive; ++it) {
           float l0 = 0.0f, lx = 0.0f, ly = 0.0f, lxx = 0.0f, la = 0.0f, lb = 0.0f, lc = 0.0f, ln = 0.0f;
           for (uint32_t i = lane; i < nt; i += 32u) {
-            if (a.asg[t0 + i] != v) continue;
-            const float x = X[t0 + i], y = Y[t0 + i], tx = TX[t0 + i], ty = TY[t0 + i], z = Z[t0 + i];
+            if (PA[i] != v) continue;
+            const float x = PX[i], y = PY[i], tx = PTX[i], ty = PTY[i], z = PZ[i];
+            const float w0 = resident ? PW[i] : __fdiv_rn(1.0f, PW[i]);
             const float dz = __fsub_rn(zv, z);
             const float rx = __fsub_rn(__fadd_rn(x, __fmul_rn(tx, dz)), xv);
             const float ry = __fsub_rn(__fadd_rn(y, __fmul_rn(ty, dz)), yv);
-            const float w0 = __fdiv_rn(1.0f, CXX[t0 + i]);
             const float c = __fmul_rn(w0, __fadd_rn(__fmul_rn(rx, rx), __fmul_rn(ry, ry)));
             float wt = 0.0f;
             if (c < a.P.chi2_max) { const float u = __fsub_rn(1.0f, __fdiv_rn(c, a.P.chi2_max)); wt = __fmul_rn(u, u); }
@@ -209,36 +228,38 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
   }
 }
 
-// counts -> event_pv_offsets, then every event's vertices to their place (one CTA)
-__global__ void __launch_bounds__(1024) velo_pv_offsets_kernel(const PvArgs a, uint32_t* event_pv_offsets, float* pvs,
-                                                               uint32_t cap_pvs, uint32_t* pv_summary) {
+// counts -> event_pv_offsets (one CTA), then every event's vertices to their place (a thread per slot)
+__global__ void __launch_bounds__(1024) velo_pv_offsets_kernel(const PvArgs a, uint32_t* event_pv_offsets, uint32_t cap_pvs,
+                                                               uint32_t* pv_summary) {
   __shared__ unsigned long long warp_sums[33];
   const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;
   const uint32_t per = (ne + nthr - 1) / nthr;
   const uint32_t e0 = min(tid * per, ne), e1 = min(e0 + per, ne);
   unsigned long long sum = 0;
+#pragma unroll 8
   for (uint32_t e = e0; e < e1; ++e) sum += a.tmp_cnt[e];
   unsigned long long tot;
   unsigned long long run = block_scan_excl(sum, warp_sums, &tot);
-  const bool over = tot > cap_pvs;
-  for (uint32_t e = e0; e < e1; ++e) {
-    const uint32_t n = a.tmp_cnt[e];
-    event_pv_offsets[e] = (uint32_t)run;
-    if (!over) {
-      for (uint32_t k = 0; k < n; ++k) {
-        const float* src = a.tmp_pv + ((size_t)e * kPvMax + k) * 5u;
-#pragma unroll
-        for (uint32_t p = 0; p < 5; ++p) pvs[(size_t)p * cap_pvs + (uint32_t)run + k] = src[p];
-      }
-    }
-    run += n;
-  }
+#pragma unroll 8
+  for (uint32_t e = e0; e < e1; ++e) { event_pv_offsets[e] = (uint32_t)run; run += a.tmp_cnt[e]; }
   if (tid == 0) {
     event_pv_offsets[ne] = (uint32_t)tot;
     uint32_t status = a.summary[2];
-    if (status == 0u && over) status = (uint32_t)VELO_ERR_CAPACITY;
+    if (status == 0u && tot > cap_pvs) status = (uint32_t)VELO_ERR_CAPACITY;
     pv_summary[0] = (uint32_t)tot; pv_summary[1] = status; pv_summary[2] = 0u; pv_summary[3] = 0u;
   }
+}
+
+__global__ void __launch_bounds__(256) velo_pv_place_kernel(const PvArgs a, const uint32_t* event_pv_offsets, float* pvs,
+                                                            uint32_t cap_pvs) {
+  if (event_pv_offsets[a.n_events] > cap_pvs) return;      // VELO_ERR_CAPACITY: nothing valid
+  const size_t slot = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t e = (uint32_t)(slot / kPvMax), k = (uint32_t)(slot % kPvMax);
+  if (e >= a.n_events || k >= a.tmp_cnt[e]) return;
+  const float* src = a.tmp_pv + slot * 5u;
+  const uint32_t dst = event_pv_offsets[e] + k;
+#pragma unroll
+  for (uint32_t p = 0; p < 5; ++p) pvs[(size_t)p * cap_pvs + dst] = src[p];
 }
 
 struct PvWorkspace { float* tmp_pv; uint32_t* tmp_cnt; uint8_t* asg; size_t bytes; };
@@ -311,7 +332,11 @@ int velo_pv_find(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_p
     if (grid > most) grid = most;
     velo_pv_kernel<<<grid, 32 * kPvWarps, smem, st>>>(a);
   }
-  velo_pv_offsets_kernel<<<1, 1024, 0, st>>>(a, out->event_pv_offsets, out->pvs, out->cap_pvs, out->summary);
+  velo_pv_offsets_kernel<<<1, 1024, 0, st>>>(a, out->event_pv_offsets, out->cap_pvs, out->summary);
+  if (n_events > 0) {
+    const size_t slots = (size_t)n_events * kPvMax;
+    velo_pv_place_kernel<<<(uint32_t)((slots + 255) / 256), 256, 0, st>>>(a, out->event_pv_offsets, out->pvs, out->cap_pvs);
+  }
   return cudaGetLastError() == cudaSuccess ? VELO_OK : VELO_ERR_CUDA;
 }
 

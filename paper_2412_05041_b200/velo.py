@@ -273,12 +273,15 @@ velo_reconstruct_opts = velo_reconstruct
 
 # ---- after the hot path: Kalman filter on the VELO segment, primary vertices ----
 def velo_kalman_fit(hits: Hits, tracks: DeviceTracks, sigma_hit: float, ms_theta2: float = MS_THETA2_DEFAULT,
-                    stream=None):
+                    stream=None, out=None):
     """Enqueues the filter for every track of `tracks` (the outputs of velo_reconstruct for `hits`).
-    Returns a device tensor of 13 planes x cap_tracks."""
+    Returns a device tensor whose first 13 x cap_tracks words are the state planes (`out`, if given,
+    must hold at least that many)."""
     torch = _torch()
     st = stream if stream is not None else torch.cuda.current_stream()
-    out = torch.empty((VELO_N_STATE, tracks.cap_tracks), dtype=torch.float32, device=tracks.states.device)
+    if out is None:
+        out = torch.empty((VELO_N_STATE, tracks.cap_tracks), dtype=torch.float32, device=tracks.states.device)
+    assert out.numel() >= VELO_N_STATE * tracks.cap_tracks
     tr = tracks.struct()
     rc = lib().velo_kalman_fit(byref(hits), byref(tr), c_float(sigma_hit), c_float(ms_theta2), c_void_p(out.data_ptr()),
                                c_void_p(st.cuda_stream))
