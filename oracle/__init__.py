@@ -201,6 +201,9 @@ def lib_next():
     if _lib_next is None:
         L = ctypes.CDLL(build_next())
         vp = ctypes.c_void_p
+        L.vn_pixel_decode.argtypes = [ctypes.c_uint32, vp, ctypes.c_double, ctypes.c_double, vp, ctypes.c_uint32,
+                                      vp, vp, vp, vp]
+        L.vn_pixel_decode.restype = ctypes.c_int
         L.vn_kalman.argtypes = [ctypes.c_uint32, vp, vp, vp, ctypes.c_float, ctypes.c_float, vp]
         L.vn_kalman.restype = None
         L.vn_kalman_tracks.argtypes = [ctypes.c_uint32, vp, vp, vp, vp, vp, ctypes.c_float, ctypes.c_float, vp]
@@ -271,3 +274,18 @@ def pv_find(event_track_offsets, states, params: PvParams | None = None) -> dict
         st = np.zeros((13, 1), np.float32)
     n = lib_next().vn_pv_find(ne, _p(eto), _p(st), stride, ctypes.byref(P), _p(epo), _p(pvs), cap)
     return {"event_pv_offsets": epo, "pvs": pvs[:, :n].copy(), "n_pvs": int(n)}
+
+
+def pixel_decode(pixel, module_z, pitch: float = 0.055, half_shift_x: float = 0.0) -> dict:
+    """F-1, F-2: packed pixel addresses -> x, y, z (f32), module (u8)."""
+    px = np.ascontiguousarray(pixel, dtype=np.uint32)
+    mz = _f32(module_z)
+    n = px.shape[0]
+    x = np.zeros(max(n, 1), np.float32); y = np.zeros(max(n, 1), np.float32); z = np.zeros(max(n, 1), np.float32)
+    m = np.zeros(max(n, 1), np.uint8)
+    if n:
+        rc = lib_next().vn_pixel_decode(n, _p(px), float(pitch), float(half_shift_x), _p(mz), mz.shape[0],
+                                        _p(x), _p(y), _p(z), _p(m))
+        if rc != 0:
+            raise ValueError("module id out of range")
+    return {"x": x[:n], "y": y[:n], "z": z[:n], "module": m[:n]}

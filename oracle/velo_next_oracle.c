@@ -1,6 +1,6 @@
-/* velo_next_oracle.c — plain, slow, single-threaded CPU oracle for the two steps that follow the
- * VELO hot path in SURVEY.md §8(f): f2, a parameterised Kalman filter on the VELO segment of every
- * track, and f3, primary-vertex finding from the beamline states.
+/* velo_next_oracle.c — plain, slow, single-threaded CPU oracle for the steps around the VELO hot path
+ * in SURVEY.md §8(f): f1, the decode of packed pixel hits in front of it; f2, a parameterised Kalman
+ * filter on the VELO segment of every track, and f3, primary-vertex finding from the beamline states.
  *
  * TEST INFRASTRUCTURE ONLY: only tests/, __graft_entry__.smoke() and bench.py's CPU legs may build,
  * load or call it. It shares no code, header, table or helper with paper_2412_05041_b200/csrc.
@@ -30,6 +30,30 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+
+/* ================================ f1: packed pixel hits ======================================== */
+/* The paper says only that the VELO is a pixel detector read out as raw data (PAPER.md:24 §2, :42 §3);
+ * the format is this repository's (DESIGN.md §2 F-1, F-2):
+ * F-1 one u32 per hit: bits 0-10 column + 1024, bits 11-21 row + 1024, bit 22 half (1 = the +x half),
+ *     bits 23-27 module; column and row count pixels of `pitch` from the half's local origin.
+ * F-2 decode: x = fl32(((double)column + 0.5) * pitch + h * half_shift_x), y = fl32(((double)row + 0.5) * pitch)
+ *     with h = +1 / -1 for the half bit, in double precision with one final rounding; z = module_z[module].
+ * Returns 0, or -1 if a module id is out of range (nothing else can be wrong in a 28-bit address). */
+int vn_pixel_decode(uint32_t n, const uint32_t* pixel, double pitch, double half_shift_x, const float* module_z,
+                    uint32_t n_modules, float* x, float* y, float* z, uint8_t* module) {
+  for (uint32_t i = 0; i < n; ++i) {
+    const uint32_t w = pixel[i];
+    const int32_t col = (int32_t)(w & 2047u) - 1024, row = (int32_t)((w >> 11) & 2047u) - 1024;
+    const double h = ((w >> 22) & 1u) ? 1.0 : -1.0;
+    const uint32_t m = w >> 23;
+    if (m >= n_modules) return -1;
+    x[i] = (float)(((double)col + 0.5) * pitch + h * half_shift_x);
+    y[i] = (float)(((double)row + 0.5) * pitch);
+    z[i] = module_z[m];
+    module[i] = (uint8_t)m;
+  }
+  return 0;
+}
 
 /* ================================ f2: Kalman filter on the VELO segment ======================= */
 /* K-1 model: x(z) and y(z) are independent straight lines with state (x, tx), (y, ty); z is exact;

@@ -98,6 +98,9 @@ def _load():
         lib.velogen_fill.argtypes = [ctypes.POINTER(_CConfig), ctypes.c_void_p, ctypes.c_uint64,
                                      ctypes.c_uint32] + [ctypes.c_void_p] * 8 + [ctypes.c_int]
         lib.velogen_fill.restype = ctypes.c_int
+        lib.velogen_pixels.argtypes = [ctypes.POINTER(_CConfig), ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32,
+                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
+        lib.velogen_pixels.restype = ctypes.c_int
         del u32p
         _lib = lib
     return _lib
@@ -118,12 +121,13 @@ def _ptr(a):
 
 
 def generate(cfg: GenConfig, e0: int, n_events: int, truth: bool = False, nthreads: int | None = None,
-             alloc=None) -> dict:
+             alloc=None, pixels: bool = False) -> dict:
     """Generate events [e0, e0+n_events). Returns numpy arrays:
     x, y, z (f32[n_hits]), module (u8[n_hits]), event_offsets (u32[n_events+1]); with truth=True
     also hit_track (i32[n_hits], -1 = noise), trk_offsets (u32[n_events+1]), trk_truth
-    (f64[n_trk, 5] = xv, yv, zv, tx, ty). `alloc(shape, dtype)` may supply the hit buffers
-    (e.g. views of pinned host memory)."""
+    (f64[n_trk, 5] = xv, yv, zv, tx, ty); with pixels=True (quantised recipes only) also pixel
+    (u32[n_hits], the packed pixel address of every hit: include/velo.h velo_pixel_hits_t).
+    `alloc(shape, dtype)` may supply the hit buffers (e.g. views of pinned host memory)."""
     lib = _load()
     if nthreads is None:
         nthreads = os.cpu_count() or 1
@@ -157,6 +161,12 @@ def generate(cfg: GenConfig, e0: int, n_events: int, truth: bool = False, nthrea
            "n_hits": tot_h, "module_z": mz.astype(np.float32), "cfg": cfg}
     if truth:
         out.update(hit_track=ht, trk_offsets=toff, trk_truth=tt)
+    if pixels:
+        px = mk(tot_h, np.uint32)
+        rc = lib.velogen_pixels(ctypes.byref(cc), _ptr(mz), e0, n_events, _ptr(hoff), _ptr(px), nthreads)
+        if rc != 0:
+            raise RuntimeError(f"velogen_pixels failed: {rc} (-3: the recipe is not quantised to pixels)")
+        out["pixel"] = px
     return out
 
 

@@ -78,7 +78,7 @@ struct Rng {
   uint32_t below(uint32_t n) { return (uint32_t)(uniform() * (double)n); }  // [0,n)
 };
 
-struct Hit { float x, y, z; uint8_t module; int32_t track; };
+struct Hit { float x, y, z; uint8_t module; int32_t track; uint32_t pixel; };
 struct Trk { double xv, yv, zv, tx, ty; };
 
 struct EventBuf {
@@ -104,6 +104,14 @@ bool record(const velogen_config_t& c, const double* mz, EventBuf& b, uint32_t m
     yo = ((double)iy + 0.5) * c.pitch;
   }
   Hit hit;
+  hit.pixel = 0xffffffffu;
+  if (c.quantise) {
+    // the detector's packed pixel address (include/velo.h, velo_pixel_hits_t): column and row biased
+    // by 1024, half bit, module
+    long ix = (long)std::floor(xl / c.pitch), iy = (long)std::floor(y / c.pitch);
+    if (ix >= -1024 && ix < 1024 && iy >= -1024 && iy < 1024)
+      hit.pixel = (uint32_t)(ix + 1024) | ((uint32_t)(iy + 1024) << 11) | ((uint32_t)(h > 0) << 22) | (m << 23);
+  }
   hit.x = (float)(xo + (double)h * c.half_shift_x);
   hit.y = (float)yo;
   hit.z = (float)mz[m];
@@ -247,6 +255,26 @@ int velogen_fill(const velogen_config_t* cfg, const double* module_z, uint64_t e
     }
   });
   return bad[0] ? -2 : 0;
+}
+
+// The same events as packed pixel addresses (one u32 per hit, same order as velogen_fill's arrays).
+// Needs cfg->quantise; returns -3 if a hit has no pixel address.
+int velogen_pixels(const velogen_config_t* cfg, const double* module_z, uint64_t e0, uint32_t n,
+                   const uint32_t* hit_off, uint32_t* pixel, int nthreads) {
+  if (!cfg || !module_z || cfg->n_modules < 1 || cfg->n_modules > 32) return -1;
+  velogen_config_t c = *cfg;
+  std::vector<int> bad(2, 0);
+  int* badp = bad.data();
+  parallel_events(n, nthreads, [&, c, badp](uint32_t i, EventBuf& b) {
+    gen_event(c, module_z, e0 + i, b);
+    if (b.hits.size() != (size_t)(hit_off[i + 1] - hit_off[i])) { badp[0] = 1; return; }
+    const uint32_t o = hit_off[i];
+    for (size_t k = 0; k < b.hits.size(); ++k) {
+      pixel[o + k] = b.hits[k].pixel;
+      if (b.hits[k].pixel == 0xffffffffu) badp[1] = 1;
+    }
+  });
+  return bad[0] ? -2 : (bad[1] ? -3 : 0);
 }
 
 }  // extern "C"

@@ -273,3 +273,34 @@ def test_pv_efficiency_and_resolution_against_generator_vertices():
     assert found / total >= 0.90, found / total
     assert np.std(res) < 0.2, np.std(res)
     assert 4.0 < pv["n_pvs"] / ne < 7.0                                # mu = 5
+
+
+# ---- f1: packed pixel hits -------------------------------------------------------------------------
+def test_pixel_decode_hand_values():
+    """F-1, F-2 by hand: column 0 of the +x half is centred on pitch/2; column -1 of the -x half on
+    -pitch/2; the open VELO shifts the halves by +-24.5 mm; rows likewise; z is the module's plane."""
+    mz = datagen.MODULE_Z
+    w = lambda col, row, half, m: (col + 1024) | ((row + 1024) << 11) | (half << 22) | (m << 23)
+    px = np.array([w(0, 0, 1, 8), w(-1, -1, 0, 8), w(100, -200, 1, 25), w(-1024, 1023, 0, 0)], np.uint32)
+    d = oracle.pixel_decode(px, mz)
+    np.testing.assert_array_equal(d["x"], np.array([0.0275, -0.0275, 100.5 * 0.055, -1023.5 * 0.055]).astype(np.float32))
+    np.testing.assert_array_equal(d["y"], np.array([0.0275, -0.0275, -199.5 * 0.055, 1023.5 * 0.055]).astype(np.float32))
+    np.testing.assert_array_equal(d["z"], np.array([1, 1, 751, -289], np.float32))
+    np.testing.assert_array_equal(d["module"], [8, 8, 25, 0])
+    d = oracle.pixel_decode(px[:2], mz, half_shift_x=24.5)
+    np.testing.assert_array_equal(d["x"], np.array([24.5275, -24.5275]).astype(np.float32))
+    with pytest.raises(ValueError):
+        oracle.pixel_decode(np.array([w(0, 0, 1, 26)], np.uint32), mz)
+    assert oracle.pixel_decode(np.zeros(0, np.uint32), mz)["x"].shape == (0,)
+
+
+@pytest.mark.parametrize("config", [0, 3, 4])
+def test_pixel_decode_round_trip_with_the_generator(config):
+    """The generator writes the pixel addresses it quantised the hits to; decoding them gives its
+    fp32 x, y, z and module bit for bit (closed and open VELO, ion-like events)."""
+    d = datagen.generate_config(config, n_events=40, pixels=True)
+    got = oracle.pixel_decode(d["pixel"], datagen.MODULE_Z, half_shift_x=d["cfg"].half_shift_x)
+    for k in ("x", "y", "z"):
+        np.testing.assert_array_equal(got[k].view(np.uint32), d[k].view(np.uint32))
+    np.testing.assert_array_equal(got["module"], d["module"])
+    assert len(d["pixel"]) > 1000
