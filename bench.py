@@ -197,24 +197,24 @@ def run_reference(args):
 class Workload:
     """One BASELINE.json config resident in HBM: pinned host arrays, device hits, per-batch outputs."""
 
-    def __init__(self, velo, datagen, sharding, torch, cfg_index, n_events_override, rank, opts_kw):
+    def __init__(self, velo, datagen, sharding, torch, cfg_index, n_events_override, rank, opts_kw, want_pixels=False):
         self.torch, self.velo = torch, velo
         self.cfg_index = cfg_index
         cfg, n_events, n_batches = datagen.CONFIGS[cfg_index]
         if n_events_override:
             n_events = n_events_override
-        self.n_events, self.n_batches = n_events, n_batches
+        self.n_events, self.n_batches, self.cfg = n_events, n_batches, cfg
         self.keep = []
 
         def pinned(shape, dtype):
             t = torch.empty(int(np.prod(shape)) if not np.isscalar(shape) else int(shape),
-                            dtype={np.float32: torch.float32, np.uint8: torch.uint8}[np.dtype(dtype).type],
+                            dtype={np.float32: torch.float32, np.uint8: torch.uint8, np.uint32: torch.int32}[np.dtype(dtype).type],
                             pin_memory=True)
             self.keep.append(t)
-            return t.numpy()
+            return t.numpy().view(np.dtype(dtype))
 
         e0, _ = sharding.weak_event_range(rank, n_events)   # every rank its own events: weak scaling
-        self.d = d = datagen.generate(cfg, e0, n_events, alloc=pinned)
+        self.d = d = datagen.generate(cfg, e0, n_events, alloc=pinned, pixels=want_pixels)
         self.off = off = d["event_offsets"]
         self.n_hits = d["n_hits"]
         self.cuts = cuts = [n_events * b // n_batches for b in range(n_batches + 1)]
@@ -353,7 +353,7 @@ def run_velo(args):
                    track_teams=args.track_teams, fit_teams=args.fit_teams, sort_teams=args.sort_teams,
                    pool_units=args.pool_units)
     kernels_per_batch = 3 if args.path == 1 else 7   # sort, order, track, slab, fit, offsets, write
-    wl = Workload(velo, datagen, sharding, torch, args.config, args.events, rank, opts_kw)
+    wl = Workload(velo, datagen, sharding, torch, args.config, args.events, rank, opts_kw, want_pixels=not args.no_e2e)
     n_events, n_batches, n_hits, off, cuts = wl.n_events, wl.n_batches, wl.n_hits, wl.off, wl.cuts
     launches = 0
 
@@ -475,30 +475,50 @@ def run_velo(args):
         houts = [velo.HostTracks(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]])) for b in range(n_batches)]
         off_pinned = torch.from_numpy(off.view(np.int32).copy()).pin_memory()
         e2e_steps = max(1, min(args.steps, 5))
-        run = lambda: sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off_pinned.numpy().view(np.uint32),
-                                     cuts, houts)
-        run()  # warm-up
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-        times = []
-        for _ in range(e2e_steps):
-            w0 = time.perf_counter()
-            run()                      # returns after every copy has completed
-            times.append(time.perf_counter() - w0)
-        e2e_s = float(np.median(times))
-        if world > 1:
-            t = torch.tensor([e2e_s], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
-        hres = [h.result() for h in houts]
-        assert sum(r["n_tracks"] for r in hres) == n_tracks and sum(r["n_track_hits"] for r in hres) == n_thits
-        h2d = 13 * n_hits + sum(4 * (cuts[b + 1] - cuts[b] + 1) for b in range(n_batches))
+        off_u32 = off_pinned.numpy().view(np.uint32)
+        fmt = velo.PixelFormat(pitch=wl.cfg.pitch, half_shift_x=wl.cfg.half_shift_x)
+        px_pinned = torch.from_numpy(d["pixel"].view(np.int32)) if "pixel" in d else None
+
+        def measure(run):
+            run()  # warm-up
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+            times = []
+            for _ in range(e2e_steps):
+                w0 = time.perf_counter()
+                run()                      # returns after every copy has completed
+                times.append(time.perf_counter() - w0)
+            t_ = float(np.median(times))
+            if world > 1:
+                tt = torch.tensor([t_], device="cuda"); dist.all_reduce(tt, op=dist.ReduceOp.MAX); t_ = float(tt.item())
+            hres = [h.result() for h in houts]
+            assert sum(r["n_tracks"] for r in hres) == n_tracks and sum(r["n_track_hits"] for r in hres) == n_thits
+            return t_, hres
+
+        soa_s, hres = measure(lambda: sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off_u32, cuts, houts))
         d2h = sum(4 * velo.VELO_N_SUMMARY + 4 * (cuts[b + 1] - cuts[b] + 1) + 4 * (r["n_tracks"] + 1) + 52 * r["n_tracks"] + 4 * r["n_track_hits"]
                   for b, r in enumerate(hres))
-        line["e2e"] = {"value": world * n_events / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                       "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s, "steps": e2e_steps,
-                       "pcie_gbs": (h2d + d2h) / e2e_s / 1e9,
-                       "api": "velo_scheduler_run_host (pinned host buffers, %d streams)" % n_batches}
+        off_bytes = sum(4 * (cuts[b + 1] - cuts[b] + 1) for b in range(n_batches))
+        e2e_soa = {"value": world * n_events / soa_s, "unit": UNIT, "h2d_bytes_per_step": 13 * n_hits + off_bytes,
+                   "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * soa_s, "steps": e2e_steps,
+                   "pcie_gbs": (13 * n_hits + off_bytes + d2h) / soa_s / 1e9,
+                   "input": "fp32 SoA hits (x, y, z f32 + module u8: 13 B per hit)",
+                   "api": "velo_scheduler_run_host (pinned host buffers, %d streams)" % n_batches}
         launches += kernels_per_batch * n_batches * (e2e_steps + 1)
+        if px_pinned is not None:
+            px_s, _ = measure(lambda: sched.run_host_pixels(P, px_pinned, off_u32, fmt, cuts, houts))
+            line["e2e"] = {"value": world * n_events / px_s, "unit": UNIT, "h2d_bytes_per_step": 4 * n_hits + off_bytes,
+                           "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * px_s, "steps": e2e_steps,
+                           "pcie_gbs": (4 * n_hits + off_bytes + d2h) / px_s / 1e9,
+                           "input": "packed pixel addresses (4 B per hit; include/velo.h velo_pixel_hits_t), decoded inside "
+                                    "stage 1; identical tracks to the fp32 path (tests/test_gpu_pixels.py)",
+                           "bound": "PCIe: the device->host copy of the produced tracks (%.2f GB per step)" % (d2h / 1e9),
+                           "api": "velo_scheduler_run_host_pixels (pinned host buffers, %d streams)" % n_batches}
+            line["e2e_fp32_soa"] = e2e_soa
+            launches += kernels_per_batch * n_batches * (e2e_steps + 1)
+        else:
+            line["e2e"] = e2e_soa
         sched.close()
 
     # -- the oracle on this box's host cores (rank 0, N=1 only): a baseline, not the target --

@@ -183,6 +183,31 @@ void velo_scheduler_free(velo_scheduler_t* s);
 int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, const velo_hits_t* hits,
                             const uint32_t* batch_begin, uint32_t n_batches, velo_tracks_t* out);
 
+/* ---- in front of the hot path: SURVEY.md §8(f) f1, packed pixel hits decoded inside S0 -------- */
+/* The VELO is a pixel detector read out as raw data (PAPER.md:24 §2, :42 §3); the paper gives no
+ * format, so this one is the repository's (DESIGN.md §2 F-1, F-2). One u32 per hit:
+ *   bits 0-10 column + 1024, bits 11-21 row + 1024, bit 22 half (1 = the +x half), bits 23-27 module;
+ * column and row count pixels of `pitch` from the half's local origin. Decode, in double precision
+ * with one final rounding: x = fl32((column + 0.5) * pitch + h * half_shift_x), h = +1 / -1 for the
+ * half bit; y = fl32((row + 0.5) * pitch); z = module_z[module]. 4 bytes per hit instead of 13. */
+typedef struct {                 /* DEVICE pointers for velo_reconstruct_pixels, HOST for the scheduler call */
+  const uint32_t* pixel;         /* n_hits packed addresses, indexed by absolute hit index */
+  const uint32_t* event_offsets; /* n_events+1, as in velo_hits_t */
+  uint32_t n_events, n_hits;
+} velo_pixel_hits_t;
+typedef struct { double pitch, half_shift_x; } velo_pixel_format_t;   /* 0.055 mm; 0 closed, 24.5 open */
+/* velo_reconstruct with the decode fused into stage 1 (S0): same outputs, same workspace size, same
+ * error behaviour (a module id >= n_modules -> VELO_ERR_INPUT). The fp32 coordinates exist only
+ * inside the kernels; events that the pipeline defers to the general kernel are decoded into the
+ * workspace first. opts may be NULL. */
+int velo_reconstruct_pixels(const velo_geometry_t* g, const velo_pixel_hits_t* hits, const velo_pixel_format_t* fmt,
+                            const velo_params_t* params, velo_tracks_t* out, void* workspace, size_t workspace_bytes,
+                            void* stream, const velo_launch_options_t* opts);
+/* velo_scheduler_run_host over packed HOST input: 4 bytes per hit cross the bus instead of 13. */
+int velo_scheduler_run_host_pixels(velo_scheduler_t* s, const velo_params_t* params, const velo_pixel_hits_t* hits,
+                                   const velo_pixel_format_t* fmt, const uint32_t* batch_begin, uint32_t n_batches,
+                                   velo_tracks_t* out);
+
 /* ---- after the hot path: SURVEY.md §8(f) f2 and f3 ------------------------------------------- */
 /* f2. Parameterised Kalman filter on the VELO segment of every track (§5: "the Kalman
  * filtering process on track uses a parameterised approach ... only the segment of a track inside

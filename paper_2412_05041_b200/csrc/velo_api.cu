@@ -63,24 +63,18 @@ size_t velo_workspace_bytes(uint32_t n_events, uint32_t n_hits, uint32_t cap_tra
 
 namespace velo {
 
-int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
-                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
-                     const velo_launch_options_t* opts, uint32_t hit_base) {
-  if (!g || !hits || !params || !out || !workspace) return VELO_ERR_ARG;
-  if (!hits->event_offsets || !out->event_track_offsets || !out->track_hit_offsets || !out->summary)
-    return VELO_ERR_ARG;
-  if (hits->n_hits && (!hits->x || !hits->y || !hits->z || !hits->module)) return VELO_ERR_ARG;
+namespace {
+
+// Argument checks and kernel arguments shared by the fp32 and the packed-pixel entry points.
+int run_batch(const velo_geometry_t* g, KernelArgs& a, uint32_t n_events, uint32_t n_hits, const velo_params_t* params,
+              velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream, const velo_launch_options_t* opts) {
+  if (!out->event_track_offsets || !out->track_hit_offsets || !out->summary) return VELO_ERR_ARG;
   if (!out->track_hits || !out->states || out->cap_tracks == 0 || out->cap_track_hits == 0) return VELO_ERR_ARG;
   if (((uintptr_t)workspace & 255u) != 0) return VELO_ERR_ARG;
   if (params->clone_den == 0) return VELO_ERR_ARG;
-  const size_t need = velo_workspace_bytes_opts(hits->n_events, hits->n_hits, out->cap_tracks, out->cap_track_hits, opts);
+  const size_t need = velo_workspace_bytes_opts(n_events, n_hits, out->cap_tracks, out->cap_track_hits, opts);
   if (workspace_bytes < need) return VELO_ERR_WORKSPACE;
-
-  KernelArgs a{};
-  a.x = hits->x; a.y = hits->y; a.z = hits->z; a.module = hits->module;
-  a.event_offsets = hits->event_offsets;
-  a.n_events = hits->n_events; a.n_modules = g->n_modules; a.n_hits = hits->n_hits;
-  a.hit_base = hit_base;
+  a.n_events = n_events; a.n_modules = g->n_modules; a.n_hits = n_hits;
   const uint32_t path = opts ? opts->path : 0u;
   a.team_max_hits = kPipeMaxHits;
   for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
@@ -93,12 +87,37 @@ int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const ve
   a.event_track_offsets = out->event_track_offsets; a.track_hit_offsets = out->track_hit_offsets;
   a.track_hits = out->track_hits; a.states = out->states;
   a.cap_tracks = out->cap_tracks; a.cap_track_hits = out->cap_track_hits; a.summary = out->summary;
-  a.ws = carve_workspace(workspace, hits->n_events, hits->n_hits, out->cap_tracks, out->cap_track_hits, n_slabs_for(opts));
+  a.ws = carve_workspace(workspace, n_events, n_hits, out->cap_tracks, out->cap_track_hits, n_slabs_for(opts));
   PipeOpts po{};
   if (opts) { po.track_group = opts->track_group; po.track_teams = opts->track_teams; po.fit_teams = opts->fit_teams;
               po.sort_teams = opts->sort_teams; po.pool_units = opts->pool_units; }
   const int err = launch_reconstruct(a, (cudaStream_t)stream, opts ? opts->stage_events : nullptr, path, po);
   return err == 0 ? VELO_OK : VELO_ERR_CUDA;
+}
+
+}  // namespace
+
+int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
+                     velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
+                     const velo_launch_options_t* opts, uint32_t hit_base) {
+  if (!g || !hits || !params || !out || !workspace || !hits->event_offsets) return VELO_ERR_ARG;
+  if (hits->n_hits && (!hits->x || !hits->y || !hits->z || !hits->module)) return VELO_ERR_ARG;
+  KernelArgs a{};
+  a.x = hits->x; a.y = hits->y; a.z = hits->z; a.module = hits->module;
+  a.event_offsets = hits->event_offsets; a.hit_base = hit_base;
+  return run_batch(g, a, hits->n_events, hits->n_hits, params, out, workspace, workspace_bytes, stream, opts);
+}
+
+int reconstruct_pixels_impl(const velo_geometry_t* g, const velo_pixel_hits_t* hits, const velo_pixel_format_t* fmt,
+                            const velo_params_t* params, velo_tracks_t* out, void* workspace, size_t workspace_bytes,
+                            void* stream, const velo_launch_options_t* opts, uint32_t hit_base) {
+  if (!g || !hits || !fmt || !params || !out || !workspace || !hits->event_offsets) return VELO_ERR_ARG;
+  if (!hits->pixel) return VELO_ERR_ARG;          // also for an empty batch: it marks the packed path
+  if (!(fmt->pitch > 0.0)) return VELO_ERR_ARG;
+  KernelArgs a{};
+  a.pixel = hits->pixel; a.pitch = fmt->pitch; a.half_shift_x = fmt->half_shift_x;
+  a.event_offsets = hits->event_offsets; a.hit_base = hit_base;
+  return run_batch(g, a, hits->n_events, hits->n_hits, params, out, workspace, workspace_bytes, stream, opts);
 }
 
 }  // namespace velo
@@ -114,6 +133,12 @@ int velo_reconstruct_opts(const velo_geometry_t* g, const velo_hits_t* hits, con
 int velo_reconstruct(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
                      velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream) {
   return velo_reconstruct_opts(g, hits, params, out, workspace, workspace_bytes, stream, nullptr);
+}
+
+int velo_reconstruct_pixels(const velo_geometry_t* g, const velo_pixel_hits_t* hits, const velo_pixel_format_t* fmt,
+                            const velo_params_t* params, velo_tracks_t* out, void* workspace, size_t workspace_bytes,
+                            void* stream, const velo_launch_options_t* opts) {
+  return velo::reconstruct_pixels_impl(g, hits, fmt, params, out, workspace, workspace_bytes, stream, opts, 0u);
 }
 
 }  // extern "C"

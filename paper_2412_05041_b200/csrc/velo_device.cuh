@@ -42,6 +42,16 @@ __device__ __forceinline__ int phi16(float x, float y) {
   return ((k + 32768) & 65535) - 32768;
 }
 
+// ---- F-1, F-2 packed pixel address -> module, x, y (include/velo.h velo_pixel_hits_t) ----
+// Double precision with one final rounding, as the format defines it.
+__device__ __forceinline__ void pixel_decode(uint32_t w, double pitch, double half_shift_x, uint32_t& m, float& x, float& y) {
+  const int col = (int)(w & 2047u) - 1024, row = (int)((w >> 11) & 2047u) - 1024;
+  const double h = ((w >> 22) & 1u) ? 1.0 : -1.0;
+  m = w >> 23;
+  x = __double2float_rn(__dadd_rn(__dmul_rn(__dadd_rn((double)col, 0.5), pitch), __dmul_rn(h, half_shift_x)));
+  y = __double2float_rn(__dmul_rn(__dadd_rn((double)row, 0.5), pitch));
+}
+
 // ---- O-4 scatter: squared miss distance of the line h0->h1 extrapolated to z of h2 ------------
 // The part that depends only on (h0, h1) is hoisted by the callers: dx = x1-x0, dy = y1-y0,
 // dz10 = z1-z0. Operation order is exactly O-4's.

@@ -93,6 +93,8 @@ struct Workspace {
   uint32_t* ev_hit_base;  // n_events+1: exclusive scan of n_track_hits over events
   uint32_t* large_list;   // n_events: events deferred to the slab path
   uint32_t* order;        // n_events: event ids by ascending size class (velo_order_kernel)
+  float *ux, *uy, *uz;    // n_hits: fp32 coordinates of deferred events when the input is packed pixels
+  uint8_t* umod;          //   (index = absolute hit index - event_offsets[0])
   uint32_t* tmp_loff;     // cap_tracks: hit offset of a track inside its event's hit block
   uint32_t* tmp_hits;     // cap_track_hits
   float* tmp_states;      // VELO_N_STATE * cap_tracks
@@ -109,6 +111,8 @@ struct KernelArgs {
   // input
   const float *x, *y, *z;
   const uint8_t* module;
+  const uint32_t* pixel;             // packed pixel addresses instead of x, y, z, module (velo_pixel_hits_t), or NULL
+  double pitch, half_shift_x;        //   their format (velo_pixel_format_t)
   const uint32_t* event_offsets;
   uint32_t n_events, n_modules;
   uint32_t n_hits;                   // host knowledge of the batch size: sizes the scratch, steers launch heuristics
@@ -126,6 +130,27 @@ struct KernelArgs {
   uint32_t* summary;
   Workspace ws;
 };
+
+#ifdef __CUDACC__
+}  // namespace velo
+#include "velo_device.cuh"
+namespace velo {
+// Packed input: an event that leaves the pipeline for the general kernel is first decoded into the
+// workspace's fp32 planes by the team that gives it up (G threads, thread `tid`).
+template <int G>
+__device__ inline void unpack_event(const KernelArgs& a, uint32_t e, uint32_t tid) {
+  const uint32_t base = a.event_offsets[0], o0 = a.event_offsets[e], n = a.event_offsets[e + 1] - o0;
+  const uint32_t* src = a.pixel + (size_t)(o0 - a.hit_base);
+  const size_t d0 = (size_t)(o0 - base);
+  for (uint32_t i = tid; i < n; i += G) {
+    uint32_t m; float x, y;
+    pixel_decode(src[i], a.pitch, a.half_shift_x, m, x, y);
+    a.ws.ux[d0 + i] = x; a.ws.uy[d0 + i] = y;
+    a.ws.uz[d0 + i] = m < a.n_modules ? a.module_z[m] : 0.0f;
+    a.ws.umod[d0 + i] = (uint8_t)(m < 256u ? m : 255u);
+  }
+}
+#endif
 
 // Which event kernel(s) a batch runs through (velo_launch_options_t.path).
 enum { kPathDefault = 0,     // three-stage pipeline, slab kernel for the events it defers
@@ -155,5 +180,9 @@ namespace velo {
 int reconstruct_impl(const velo_geometry_t* g, const velo_hits_t* hits, const velo_params_t* params,
                      velo_tracks_t* out, void* workspace, size_t workspace_bytes, void* stream,
                      const velo_launch_options_t* opts, uint32_t hit_base);
+// The same over packed pixel addresses (hits->pixel points at absolute hit index `hit_base`).
+int reconstruct_pixels_impl(const velo_geometry_t* g, const velo_pixel_hits_t* hits, const velo_pixel_format_t* fmt,
+                            const velo_params_t* params, velo_tracks_t* out, void* workspace, size_t workspace_bytes,
+                            void* stream, const velo_launch_options_t* opts, uint32_t hit_base);
 
 }  // namespace velo

@@ -137,9 +137,11 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
     return;
   }
   const uint32_t n = o1 - o0;
-  const size_t g0 = (size_t)(o0 - a.hit_base);
-  const float* gx = a.x + g0; const float* gy = a.y + g0; const float* gz = a.z + g0;
-  const uint8_t* gm = a.module + g0;
+  // packed input: the team that deferred the event left its fp32 coordinates in the workspace
+  const size_t g0 = a.pixel ? (size_t)(o0 - obase) : (size_t)(o0 - a.hit_base);
+  const float* gx = (a.pixel ? a.ws.ux : a.x) + g0; const float* gy = (a.pixel ? a.ws.uy : a.y) + g0;
+  const float* gz = (a.pixel ? a.ws.uz : a.z) + g0;
+  const uint8_t* gm = (a.pixel ? a.ws.umod : a.module) + g0;
 
   // ---- S0 decode: phi16 and bucket histogram (O-1) ---------------------------------------------
   for (uint32_t b = tid; b <= nbins; b += nthr) binoff[b] = 0;
@@ -434,6 +436,15 @@ __global__ void __launch_bounds__(256) velo_offsets_kernel(const KernelArgs a) {
   }
 }
 
+// Packed input on the slab-only path: every event is decoded into the workspace planes first.
+__global__ void __launch_bounds__(256) velo_unpack_kernel(const KernelArgs a) {
+  for (uint32_t e = blockIdx.x; e < a.n_events; e += gridDim.x) {
+    const uint32_t base = a.event_offsets[0], o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
+    if (o1 < o0 || o0 < base || o1 - base > a.n_hits) continue;       // reported by the event kernel
+    unpack_event<256>(a, e, threadIdx.x);
+  }
+}
+
 }  // namespace
 
 // ---- host side -----------------------------------------------------------------------------------
@@ -473,6 +484,8 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t n_hits, uint32
   w.cmeta = (uint2*)take(8 * w.cand_total);
   w.cfit = (float*)take(4 * 9 * w.cand_total);
   w.cstate = (uint8_t*)take(w.cand_total);
+  w.ux = (float*)take(4 * ((size_t)n_hits + 1)); w.uy = (float*)take(4 * ((size_t)n_hits + 1));
+  w.uz = (float*)take(4 * ((size_t)n_hits + 1)); w.umod = (uint8_t*)take((size_t)n_hits + 1);
   w.tmp_loff = (uint32_t*)take(4 * ((size_t)cap_tracks + 1));
   w.tmp_hits = (uint32_t*)take(4 * ((size_t)cap_track_hits + 1));
   w.tmp_states = (float*)take(4 * (size_t)VELO_N_STATE * ((size_t)cap_tracks + 1));
@@ -497,6 +510,7 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const*
   const bool large_events = a.n_events && a.n_hits / a.n_events >= 4096u;
   if (a.n_events > 0) {
     if (path == kPathSlabOnly) {
+      if (a.pixel) velo_unpack_kernel<<<num_sms() * 8u, 256, 0, stream>>>(a);
       mark(1);
       velo_event_slab_kernel<kThreads, false, kBinShift><<<grid, kThreads, 0, stream>>>(a, 0);
     } else {

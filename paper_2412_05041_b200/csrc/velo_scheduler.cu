@@ -16,6 +16,7 @@ struct Lane {                 // one stream with its device buffers
   cudaStream_t stream = nullptr;
   float *x = nullptr, *y = nullptr, *z = nullptr;
   uint8_t* module = nullptr;
+  uint32_t* pixel = nullptr;  // packed input (velo_scheduler_run_host_pixels), allocated on first use
   uint32_t* offsets = nullptr;
   velo_tracks_t out{};        // device output buffers
   void* workspace = nullptr;
@@ -40,7 +41,7 @@ bool ok(cudaError_t e) { return e == cudaSuccess; }
 
 void free_lane(Lane& l) {
   if (l.stream) cudaStreamDestroy(l.stream);
-  cudaFree(l.x); cudaFree(l.y); cudaFree(l.z); cudaFree(l.module); cudaFree(l.offsets);
+  cudaFree(l.x); cudaFree(l.y); cudaFree(l.z); cudaFree(l.module); cudaFree(l.pixel); cudaFree(l.offsets);
   cudaFree(l.out.event_track_offsets); cudaFree(l.out.track_hit_offsets); cudaFree(l.out.track_hits);
   cudaFree(l.out.states); cudaFree(l.out.summary); cudaFree(l.workspace);
   if (l.summary_host) cudaFreeHost(l.summary_host);
@@ -116,10 +117,16 @@ int velo_scheduler_create(const velo_geometry_t* g, uint32_t n_streams, uint32_t
   return VELO_OK;
 }
 
-int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, const velo_hits_t* hits,
-                            const uint32_t* batch_begin, uint32_t n_batches, velo_tracks_t* out) {
-  if (!s || !params || !hits || !batch_begin || !out || !hits->event_offsets) return VELO_ERR_ARG;
-  if (batch_begin[0] != 0 || batch_begin[n_batches] != hits->n_events) return VELO_ERR_ARG;
+}  // extern "C"
+
+namespace {
+
+// One pass over the batches: `upload(lane, h0, nh)` copies the batch's hits, `launch(lane, ne, nh, h0)`
+// enqueues its reconstruction.
+template <class Upload, class Launch>
+int run_batches(velo_scheduler_t* s, const uint32_t* event_offsets, uint32_t n_events, const uint32_t* batch_begin,
+                uint32_t n_batches, velo_tracks_t* out, Upload&& upload, Launch&& launch) {
+  if (batch_begin[0] != 0 || batch_begin[n_batches] != n_events) return VELO_ERR_ARG;
   int rc = VELO_OK;
   for (uint32_t b = 0; b < n_batches && rc == VELO_OK; ++b) {
     Lane& l = s->lanes[b % s->lanes.size()];
@@ -131,29 +138,19 @@ int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, co
       rc = VELO_ERR_ARG; break;
     }
     const uint32_t ne = e1 - e0;
-    const uint32_t h0 = hits->event_offsets[e0], h1 = hits->event_offsets[e1];
+    const uint32_t h0 = event_offsets[e0], h1 = event_offsets[e1];
     if (h1 < h0 || ne > s->max_events || h1 - h0 > s->max_hits) {
       for (int k = 0; k < VELO_N_SUMMARY; ++k) o.summary[k] = 0;
       o.summary[2] = (uint32_t)VELO_ERR_CAPACITY;
       continue;
     }
     const uint32_t nh = h1 - h0;
-    bool good = true;
-    if (nh) {
-      good &= ok(cudaMemcpyAsync(l.x, hits->x + h0, 4 * (size_t)nh, cudaMemcpyHostToDevice, l.stream));
-      good &= ok(cudaMemcpyAsync(l.y, hits->y + h0, 4 * (size_t)nh, cudaMemcpyHostToDevice, l.stream));
-      good &= ok(cudaMemcpyAsync(l.z, hits->z + h0, 4 * (size_t)nh, cudaMemcpyHostToDevice, l.stream));
-      good &= ok(cudaMemcpyAsync(l.module, hits->module + h0, (size_t)nh, cudaMemcpyHostToDevice, l.stream));
-    }
-    good &= ok(cudaMemcpyAsync(l.offsets, hits->event_offsets + e0, 4 * ((size_t)ne + 1), cudaMemcpyHostToDevice,
-                               l.stream));
+    bool good = upload(l, h0, nh);
+    good &= ok(cudaMemcpyAsync(l.offsets, event_offsets + e0, 4 * ((size_t)ne + 1), cudaMemcpyHostToDevice, l.stream));
     if (!good) { rc = VELO_ERR_CUDA; break; }
     // the device copy holds hits [h0, h1) at index 0; the batch keeps its absolute offsets, so the
     // emitted track_hits stay absolute hit indices
-    velo_hits_t dh{};
-    dh.x = l.x; dh.y = l.y; dh.z = l.z; dh.module = l.module;
-    dh.event_offsets = l.offsets; dh.n_events = ne; dh.n_hits = nh;
-    rc = velo::reconstruct_impl(s->g, &dh, params, &l.out, l.workspace, l.workspace_bytes, (void*)l.stream, nullptr, h0);
+    rc = launch(l, ne, nh, h0);
     if (rc != VELO_OK) break;
     good &= ok(cudaMemcpyAsync(l.summary_host, l.out.summary, 4 * VELO_N_SUMMARY, cudaMemcpyDeviceToHost, l.stream));
     good &= ok(cudaMemcpyAsync(o.event_track_offsets, l.out.event_track_offsets, 4 * ((size_t)ne + 1),
@@ -166,6 +163,53 @@ int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, co
     if (rc == VELO_OK) rc = r;
   }
   return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int velo_scheduler_run_host(velo_scheduler_t* s, const velo_params_t* params, const velo_hits_t* hits,
+                            const uint32_t* batch_begin, uint32_t n_batches, velo_tracks_t* out) {
+  if (!s || !params || !hits || !batch_begin || !out || !hits->event_offsets) return VELO_ERR_ARG;
+  return run_batches(
+      s, hits->event_offsets, hits->n_events, batch_begin, n_batches, out,
+      [&](Lane& l, uint32_t h0, uint32_t nh) {
+        bool good = true;
+        if (nh) {
+          good &= ok(cudaMemcpyAsync(l.x, hits->x + h0, 4 * (size_t)nh, cudaMemcpyHostToDevice, l.stream));
+          good &= ok(cudaMemcpyAsync(l.y, hits->y + h0, 4 * (size_t)nh, cudaMemcpyHostToDevice, l.stream));
+          good &= ok(cudaMemcpyAsync(l.z, hits->z + h0, 4 * (size_t)nh, cudaMemcpyHostToDevice, l.stream));
+          good &= ok(cudaMemcpyAsync(l.module, hits->module + h0, (size_t)nh, cudaMemcpyHostToDevice, l.stream));
+        }
+        return good;
+      },
+      [&](Lane& l, uint32_t ne, uint32_t nh, uint32_t h0) {
+        velo_hits_t dh{};
+        dh.x = l.x; dh.y = l.y; dh.z = l.z; dh.module = l.module;
+        dh.event_offsets = l.offsets; dh.n_events = ne; dh.n_hits = nh;
+        return velo::reconstruct_impl(s->g, &dh, params, &l.out, l.workspace, l.workspace_bytes, (void*)l.stream, nullptr, h0);
+      });
+}
+
+int velo_scheduler_run_host_pixels(velo_scheduler_t* s, const velo_params_t* params, const velo_pixel_hits_t* hits,
+                                   const velo_pixel_format_t* fmt, const uint32_t* batch_begin, uint32_t n_batches,
+                                   velo_tracks_t* out) {
+  if (!s || !params || !hits || !fmt || !batch_begin || !out || !hits->event_offsets) return VELO_ERR_ARG;
+  if (hits->n_hits && !hits->pixel) return VELO_ERR_ARG;
+  for (Lane& l : s->lanes)
+    if (!l.pixel && !ok(cudaMalloc(&l.pixel, 4 * ((size_t)s->max_hits + 4)))) { cudaGetLastError(); return VELO_ERR_CUDA; }
+  return run_batches(
+      s, hits->event_offsets, hits->n_events, batch_begin, n_batches, out,
+      [&](Lane& l, uint32_t h0, uint32_t nh) {
+        return nh == 0 || ok(cudaMemcpyAsync(l.pixel, hits->pixel + h0, 4 * (size_t)nh, cudaMemcpyHostToDevice, l.stream));
+      },
+      [&](Lane& l, uint32_t ne, uint32_t nh, uint32_t h0) {
+        velo_pixel_hits_t dh{};
+        dh.pixel = l.pixel; dh.event_offsets = l.offsets; dh.n_events = ne; dh.n_hits = nh;
+        return velo::reconstruct_pixels_impl(s->g, &dh, fmt, params, &l.out, l.workspace, l.workspace_bytes,
+                                             (void*)l.stream, nullptr, h0);
+      });
 }
 
 }  // extern "C"

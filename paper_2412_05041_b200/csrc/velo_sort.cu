@@ -31,6 +31,7 @@ struct SortTeam {
   uint32_t event, n, o0, ol;         // event index, hits, first hit (absolute), first hit relative to the batch
   uint32_t units, first_unit, pool_off;
   uint32_t skip;                     // nothing to sort (empty / bad / deferred before the sort)
+  uint32_t unpack;                   // packed input: decode the deferred event for the general kernel
   uint32_t trouble;                  // bit 0: defer to the general kernel, bit 31: bad input
   unsigned long long ph_last;        // phase clocks (-DVELO_TIMELINE builds)
 };
@@ -64,7 +65,7 @@ __device__ __forceinline__ void set_status(uint32_t* counters, int code) {
 template <int G>
 __device__ void sort_fetch(const KernelArgs& a, PoolCtl& pool, SortTeam<G>& ts) {
   const uint32_t e = atomicAdd(&a.ws.counters[kCtrSortTicket], 1u);
-  ts.event = e; ts.units = 0; ts.skip = 1; ts.n = 0; ts.trouble = 0;
+  ts.event = e; ts.units = 0; ts.skip = 1; ts.n = 0; ts.trouble = 0; ts.unpack = 0;
   if (e >= a.n_events) return;
   const uint32_t base = a.event_offsets[0];
   const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
@@ -83,6 +84,7 @@ __device__ void sort_fetch(const KernelArgs& a, PoolCtl& pool, SortTeam<G>& ts) 
   if (n > a.team_max_hits || units > pool.units || fit_smem_bound(n) > pool.units * kUnitBytes) {
     info.state = kEvDeferred; a.ws.ev_info[e] = info;
     a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+    ts.unpack = a.pixel != nullptr;
     return;
   }
   const uint32_t first = pool_alloc(pool, units);
@@ -105,6 +107,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
   const size_t g0 = (size_t)(ts.o0 - a.hit_base);
   const float* gx = a.x + g0; const float* gy = a.y + g0; const float* gz = a.z + g0;
   const uint8_t* gm = a.module + g0;
+  const uint32_t* gp = a.pixel + g0;
 
   // ---- S0 decode: phi16 (O-1), bucket histogram; the plane check of the pipeline path -------------
   const uint32_t nwords = nbins / 2u;
@@ -123,6 +126,26 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
       stash[i] = (m << 27) | (pu << 11) | (slot & kMaxBinSlot);
       xyo[i] = make_float2(x, y);
     };
+    if (a.pixel) {
+      // F-1, F-2: packed pixel addresses, four per 128-bit load on the aligned interior; z is the
+      // module's plane by construction
+      auto decode_px = [&](uint32_t i, uint32_t wd) {
+        uint32_t m; float x, y;
+        pixel_decode(wd, a.pitch, a.half_shift_x, m, x, y);
+        decode(i, x, y, m < M ? mz[m] : 0.0f, m);
+      };
+      uint32_t head = (4u - (uint32_t)(((uintptr_t)gp >> 2) & 3u)) & 3u;
+      if (head > n) head = n;
+      const uint32_t nq = (n - head) / 4u;
+      for (uint32_t i = tid; i < head; i += G) decode_px(i, gp[i]);
+      const uint4* vp = (const uint4*)(gp + head);
+      for (uint32_t q = tid; q < nq; q += G) {
+        const uint4 W4 = vp[q];
+        const uint32_t i = head + 4u * q;
+        decode_px(i, W4.x); decode_px(i + 1, W4.y); decode_px(i + 2, W4.z); decode_px(i + 3, W4.w);
+      }
+      for (uint32_t i = head + 4u * nq + tid; i < n; i += G) decode_px(i, gp[i]);
+    } else {
     // 128-bit loads where the planes allow them. The three float planes and the byte plane are
     // indexed by the same hit index, so with the usual allocations they reach 16-byte (4-byte for
     // the modules) alignment after the same number of leading hits; otherwise everything is scalar.
@@ -147,6 +170,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
       }
     }
     for (uint32_t i = head + 4u * nq + tid; i < n; i += G) decode(i, gx[i], gy[i], gz[i], gm[i]);
+    }
     if (trouble) atomicOr(&ts.trouble, trouble);
   }
   team_sync<G>(team);
@@ -158,6 +182,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
       else a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
       a.ws.ev_info[e] = info;
     }
+    if (a.pixel && !(ts.trouble & 0x80000000u)) unpack_event<G>(a, e, tid);
     return;
   }
   // exclusive scan of the packed histogram -> bucket offsets; bo[nbins] = n
@@ -270,6 +295,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_sort_kernel(const KernelAr
     if (ts.event >= a.n_events) break;
     VELO_PH(a.ws.phase_clk, ts, 9);      // ticket, offsets, pool
     if (!ts.skip) sort_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity);
+    else if (ts.unpack) unpack_event<G>(a, ts.event, tid);
     team_sync<G>(team);
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
     VELO_PH(a.ws.phase_clk, ts, 15);

@@ -37,6 +37,7 @@ struct TrackTeam {
   uint32_t units, first_unit, pool_off, skip;
   uint32_t maxmod, cbase, tcap, acap;
   uint32_t defer;                    // set by any thread: the event continues in the general kernel
+  uint32_t unpack;                   // packed input: decode the deferred event for the general kernel
   unsigned long long ph_last;        // phase clocks (-DVELO_TIMELINE builds)
   uint16_t mod_off[kModOffStride];
 };
@@ -66,7 +67,7 @@ __device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod,
 template <int G>
 __device__ void track_fetch(const KernelArgs& a, PoolCtl& pool, TrackTeam<G>& ts) {
   const uint32_t k = atomicAdd(&a.ws.counters[kCtrTrackTicket], 1u);
-  ts.event = k; ts.units = 0; ts.skip = 1; ts.defer = 0;
+  ts.event = k; ts.units = 0; ts.skip = 1; ts.defer = 0; ts.unpack = 0;
   if (k >= a.n_events) return;
   // tickets walk the size-sorted list from both ends in turn: largest, smallest, second largest, ...
   const uint32_t e = a.ws.order[(k & 1u) ? (k >> 1) : a.n_events - 1u - (k >> 1)];
@@ -81,6 +82,7 @@ __device__ void track_fetch(const KernelArgs& a, PoolCtl& pool, TrackTeam<G>& ts
   if (units > pool.units) {
     a.ws.ev_info[e].state = kEvDeferred;
     a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+    ts.unpack = a.pixel != nullptr;
     return;
   }
   ts.cbase = atomicAdd(&a.ws.counters[kCtrCandAlloc], tcap);
@@ -393,6 +395,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
     if (ts.event >= a.n_events) break;
     VELO_PH(a.ws.phase_clk, ts, 17);     // ticket, descriptors, pool
     if (!ts.skip) track_event<G, kSameW>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity, phases);
+    if (a.pixel && (ts.unpack || (!ts.skip && ts.defer))) unpack_event<G>(a, ts.event, tid);
     team_sync<G>(team);   // every thread is done with the block and with ts before the leader reuses them
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
     VELO_PH(a.ws.phase_clk, ts, 23);     // tail: remaining loads, masks, flag bits

@@ -29,7 +29,8 @@ EXPORTS = ("velo_version", "velo_geometry_load", "velo_geometry_free", "velo_geo
            "velo_params_default", "velo_workspace_bytes", "velo_workspace_bytes_opts", "velo_reconstruct",
            "velo_reconstruct_opts", "velo_scheduler_create",
            "velo_scheduler_free", "velo_scheduler_run_host",
-           "velo_kalman_fit", "velo_pv_params_default", "velo_pv_workspace_bytes", "velo_pv_find")
+           "velo_kalman_fit", "velo_pv_params_default", "velo_pv_workspace_bytes", "velo_pv_find",
+           "velo_reconstruct_pixels", "velo_scheduler_run_host_pixels")
 
 
 class VeloError(RuntimeError):
@@ -53,6 +54,14 @@ class Params(ctypes.Structure):
 class Hits(ctypes.Structure):
     _fields_ = [("x", c_void_p), ("y", c_void_p), ("z", c_void_p), ("module", c_void_p),
                 ("event_offsets", c_void_p), ("n_events", c_uint32), ("n_hits", c_uint32)]
+
+
+class PixelHits(ctypes.Structure):
+    _fields_ = [("pixel", c_void_p), ("event_offsets", c_void_p), ("n_events", c_uint32), ("n_hits", c_uint32)]
+
+
+class PixelFormat(ctypes.Structure):
+    _fields_ = [("pitch", ctypes.c_double), ("half_shift_x", ctypes.c_double)]
 
 
 class Tracks(ctypes.Structure):
@@ -121,6 +130,12 @@ def lib():
         L.velo_scheduler_run_host.argtypes = [c_void_p, POINTER(Params), POINTER(Hits), c_void_p, c_uint32,
                                               POINTER(Tracks)]
         L.velo_scheduler_run_host.restype = c_int
+        L.velo_reconstruct_pixels.argtypes = [c_void_p, POINTER(PixelHits), POINTER(PixelFormat), POINTER(Params),
+                                              POINTER(Tracks), c_void_p, c_size_t, c_void_p, POINTER(LaunchOptions)]
+        L.velo_reconstruct_pixels.restype = c_int
+        L.velo_scheduler_run_host_pixels.argtypes = [c_void_p, POINTER(Params), POINTER(PixelHits), POINTER(PixelFormat),
+                                                     c_void_p, c_uint32, POINTER(Tracks)]
+        L.velo_scheduler_run_host_pixels.restype = c_int
         L.velo_kalman_fit.argtypes = [POINTER(Hits), POINTER(Tracks), c_float, c_float, c_void_p, c_void_p]
         L.velo_kalman_fit.restype = c_int
         L.velo_pv_params_default.argtypes = [POINTER(PvParams)]
@@ -269,6 +284,57 @@ def velo_reconstruct(geometry: Geometry, hits: Hits, params: Params, out: Device
 
 
 velo_reconstruct_opts = velo_reconstruct
+
+
+# ---- packed pixel input: the decode is fused into stage 1 ------------------------
+class DevicePixelHits:
+    """Packed pixel addresses of a batch resident in HBM (velo_pixel_hits_t): 4 bytes per hit."""
+
+    def __init__(self, pixel, event_offsets, device="cuda"):
+        torch = _torch()
+        px = np.ascontiguousarray(pixel, dtype=np.uint32)
+        self.pixel = torch.as_tensor(px.view(np.int32)).to(device)
+        off = np.ascontiguousarray(event_offsets, dtype=np.uint32)
+        self.event_offsets = torch.as_tensor(off.view(np.int32)).to(device)
+        self.n_events = off.shape[0] - 1
+        self.n_hits = int(off[-1]) - int(off[0]) if off.shape[0] else 0
+
+    def slice_struct(self, e0: int = 0, e1: int | None = None, n_hits: int | None = None) -> PixelHits:
+        e1 = self.n_events if e1 is None else e1
+        return PixelHits(pixel=self.pixel.data_ptr(), event_offsets=self.event_offsets.data_ptr() + 4 * e0,
+                         n_events=e1 - e0, n_hits=self.n_hits if n_hits is None else n_hits)
+
+
+def velo_reconstruct_pixels(geometry: Geometry, hits: PixelHits, fmt: PixelFormat, params: Params, out: DeviceTracks,
+                            stream=None, opts: LaunchOptions | None = None) -> None:
+    torch = _torch()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    tr = out.struct()
+    rc = lib().velo_reconstruct_pixels(geometry.handle, byref(hits), byref(fmt), byref(params), byref(tr),
+                                       c_void_p(out.workspace_ptr), c_size_t(out.workspace_bytes),
+                                       c_void_p(st.cuda_stream), byref(opts) if opts is not None else None)
+    if rc != VELO_OK:
+        raise VeloError(rc, "velo_reconstruct_pixels")
+
+
+def reconstruct_pixels(pixel, event_offsets, module_z, pitch: float = 0.055, half_shift_x: float = 0.0,
+                       params: Params | None = None, n_batches: int = 1, opts: LaunchOptions | None = None) -> dict:
+    """Convenience for tests: as reconstruct(), from packed pixel addresses."""
+    torch = _torch()
+    g = Geometry(module_z, pitch=pitch, half_shift_x=half_shift_x)
+    P = params if params is not None else velo_params_default(g)
+    fmt = PixelFormat(pitch=pitch, half_shift_x=half_shift_x)
+    dh = DevicePixelHits(pixel, event_offsets)
+    off = np.ascontiguousarray(event_offsets, dtype=np.uint32).astype(np.int64)
+    cuts = [dh.n_events * b // n_batches for b in range(n_batches + 1)]
+    streams = [torch.cuda.Stream() for _ in range(n_batches)]
+    sizes = [(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]] - off[cuts[b]])) for b in range(n_batches)]
+    outs = [DeviceTracks(ne, nh, opts=opts) for ne, nh in sizes]
+    torch.cuda.synchronize()
+    for b in range(n_batches):
+        velo_reconstruct_pixels(g, dh.slice_struct(cuts[b], cuts[b + 1], sizes[b][1]), fmt, P, outs[b], streams[b], opts)
+    torch.cuda.synchronize()
+    return stitch([o.to_host() for o in outs])
 
 
 # ---- after the hot path: Kalman filter on the VELO segment, primary vertices (SURVEY.md §8(f) f2, f3) ----
@@ -435,6 +501,20 @@ class Scheduler:
                                            len(outs), arr)
         if rc != VELO_OK:
             raise VeloError(rc, "velo_scheduler_run_host")
+
+    def run_host_pixels(self, params: Params, pixel, event_offsets, fmt: PixelFormat, batch_begin, outs: list) -> None:
+        """As run_host, from packed pixel addresses (HOST u32 array or CPU tensor): 4 bytes per hit cross the bus."""
+        ptr = lambda a: a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+        n_events = int(event_offsets.shape[0]) - 1
+        bb = np.ascontiguousarray(batch_begin, dtype=np.uint32)
+        first, last = int(event_offsets[0]), int(event_offsets[n_events])
+        hits = PixelHits(pixel=ptr(pixel), event_offsets=ptr(event_offsets), n_events=n_events,
+                         n_hits=(last - first) & 0xffffffff)
+        arr = (Tracks * len(outs))(*[o.struct() for o in outs])
+        rc = lib().velo_scheduler_run_host_pixels(self.handle, byref(params), byref(hits), byref(fmt),
+                                                  c_void_p(bb.ctypes.data), len(outs), arr)
+        if rc != VELO_OK:
+            raise VeloError(rc, "velo_scheduler_run_host_pixels")
 
     def close(self):
         h, self.handle = getattr(self, "handle", None), None
