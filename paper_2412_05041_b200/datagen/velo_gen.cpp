@@ -35,6 +35,7 @@ typedef struct {
   double hit_eff, noise_frac, ms_sigma;
   int32_t quantise;       // 1: snap to pixel centres and merge same-pixel hits (A19)
   int32_t shuffle;        // 1: Fisher-Yates shuffle of the event's hits (A16)
+  double backward_frac;   // fraction of tracks that leave the vertex towards -z (eta -> -eta; A23); 0 in BASELINE's configs
 } velogen_config_t;
 
 }  // extern "C"
@@ -148,8 +149,12 @@ void gen_event(const velogen_config_t& c, const double* mz, uint64_t e, EventBuf
       int32_t tid = (int32_t)b.trks.size();
       b.trks.push_back(Trk{xv, yv, zv, tx, ty});
       double x = xv, y = yv, zp = zv;
-      for (uint32_t m = 0; m < M; ++m) {
-        if (!(mz[m] > zv)) continue;
+      // a backward track crosses the modules below the vertex, nearest first (no extra random number
+      // is drawn when backward_frac is 0, so BASELINE's configs are unchanged)
+      const bool back = c.backward_frac > 0.0 && rng.uniform() < c.backward_frac;
+      for (uint32_t mm = 0; mm < M; ++mm) {
+        const uint32_t m = back ? M - 1 - mm : mm;
+        if (back ? !(mz[m] < zv) : !(mz[m] > zv)) continue;
         x += tx * (mz[m] - zp);
         y += ty * (mz[m] - zp);
         zp = mz[m];
