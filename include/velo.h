@@ -8,7 +8,7 @@
  * (per-module phi sort, search-by-triplet seeding, forwarding, ghost/clone filter, straight-line
  * least-squares fit to the state at closest approach to the beamline) are named by
  * BASELINE.json:north_star and made precise in SURVEY.md §8(c) items O-1 ... O-17, restated in
- * DESIGN.md §3. Coordinates: origin at the nominal interaction point, z along the beam, y up
+ * DESIGN.md §2. Coordinates: origin at the nominal interaction point, z along the beam, y up
  * (§2); lengths in mm.
  *
  * Conventions.

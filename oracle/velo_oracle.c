@@ -11,7 +11,7 @@
  * HLT1 uses "a more simplified pattern recognition algorithm" and "simplified track fitting"
  * (§5); it gives no step, constant or formula. Every step below therefore follows
  * the reading fixed in SURVEY.md §8(c) (items O-1 ... O-17, ambiguity log A1 ... A23), restated
- * in DESIGN.md §3. The method is a heuristic, so the oracle IS the algorithm, written step by
+ * in DESIGN.md §2. The method is a heuristic, so the oracle IS the algorithm, written step by
  * step in that order and notation: no blocking, no fusion, windows by linear scan.
  *
  * Arithmetic: IEEE-754 binary32, round-to-nearest-even, one rounding per written operator, no

@@ -5,7 +5,7 @@
 // straight-line fit, S6 clone filter, then writes its surviving tracks into a temp block
 // allocated with one atomic per event. A scan kernel turns the per-event counts into
 // offsets and a copy kernel moves the temp blocks into event order (S7).
-// Step semantics: SURVEY.md §8(c) O-1 ... O-14 (restated in DESIGN.md §3); the paper itself
+// Step semantics: SURVEY.md §8(c) O-1 ... O-14 (restated in DESIGN.md §2); the paper itself
 // (§5) names the objects but gives no step.
 #include "velo_device.cuh"
 #include "velo_internal.h"
