@@ -41,9 +41,17 @@ def default_params(pitch: float = 0.055) -> Params:
                   clone_num=1, clone_den=3)
 
 
+def _compile(src: str, lib: str) -> None:
+    """gcc into a temporary file, then an atomic rename: forked test workers may all find the library
+    stale at the same moment."""
+    tmp = f"{lib}.{os.getpid()}.tmp"
+    subprocess.run(["gcc", *CFLAGS, "-o", tmp, src, "-lm"], check=True)
+    os.replace(tmp, lib)
+
+
 def build(force: bool = False) -> str:
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.run(["gcc", *CFLAGS, "-o", _LIB, _SRC, "-lm"], check=True)
+        _compile(_SRC, _LIB)
     return _LIB
 
 
@@ -189,7 +197,7 @@ def default_pv_params() -> PvParams:
 
 def build_next(force: bool = False) -> str:
     if force or not os.path.exists(_LIB_NEXT) or os.path.getmtime(_LIB_NEXT) < os.path.getmtime(_SRC_NEXT):
-        subprocess.run(["gcc", *CFLAGS, "-o", _LIB_NEXT, _SRC_NEXT, "-lm"], check=True)
+        _compile(_SRC_NEXT, _LIB_NEXT)
     return _LIB_NEXT
 
 

@@ -157,6 +157,7 @@ __device__ void fit_fetch(const KernelArgs& a, PoolCtl& pool, FitTeam<G>& ts) {
   ts.event = e;
   const EvInfo info = a.ws.ev_info[e];
   if (info.state == kEvDeferred) return;           // the slab kernel has written this event's counts
+  if (info.state == kEvBig) return;                // velo_fit_big_kernel takes it
   if (info.state != kEvReady || info.ncand == 0) { a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); return; }
   const FitLayout L = fit_layout(info.n, info.ncand);
   const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;   // fits the pool: stage 1 checked fit_smem_bound
@@ -298,6 +299,42 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArg
   VELO_STAGE_END(a.ws.phase_clk, 2);
 }
 
+// ---- the same stage for the events of ws.big_list: one CTA of G threads per event, the per-event
+// arrays (owner per hit, keys, masks) in the CTA's global slab (L2-resident) -------------------------
+template <int G>
+__global__ void __launch_bounds__(G, 1) velo_fit_big_kernel(const KernelArgs a) {
+  __shared__ FitTeam<G> ts;
+  __shared__ float module_z[VELO_MAX_MODULES];
+  const uint32_t tid = threadIdx.x;
+  if (tid < VELO_MAX_MODULES) module_z[tid] = a.module_z[tid];
+  unsigned char* blk = a.ws.slabs + (size_t)blockIdx.x * slab_layout().bytes;
+  uint32_t parity = 0;
+  const uint32_t base = a.event_offsets[0];
+  for (;;) {
+    __syncthreads();
+    if (tid == 0) {
+      const uint32_t k = atomicAdd(&a.ws.counters[kCtrBigFitTicket], 1u);
+      ts.units = k >= a.ws.counters[kCtrBigN];      // 1 = no more events
+      ts.skip = 1;
+      if (!ts.units) {
+        const uint32_t e = a.ws.big_list[k];
+        const EvInfo info = a.ws.ev_info[e];
+        ts.event = e;
+        if (info.state == kEvBig) {                  // else: the general kernel has written its counts
+          if (info.ncand == 0) a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0);
+          else {
+            ts.n = info.n; ts.cbase = info.cbase; ts.ncand = info.ncand;
+            ts.o0 = a.event_offsets[e]; ts.sb = sorted_base(ts.o0 - base, e); ts.skip = 0;
+          }
+        }
+      }
+    }
+    __syncthreads();
+    if (ts.units) break;
+    if (!ts.skip) fit_event<G>(a, module_z, ts, blk, 0u, tid, parity);
+  }
+}
+
 // ---- S7 write: one warp per event places its surviving tracks in the final arrays ----------------
 // Offsets come from velo_offsets_kernel (event_track_offsets, ws.ev_hit_base). Candidates are in
 // creation order, so a running count over them is the track's place inside the event.
@@ -398,6 +435,14 @@ int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
     case 254: return launch_fit_t<256, 4>(a, stream, pu);
     default: return launch_fit_t<128, 8>(a, stream, pu);
   }
+}
+
+int launch_fit_big(const KernelArgs& a, cudaStream_t stream) {
+  const uint32_t sms = num_sms();
+  const uint32_t grid = a.ws.n_slabs < sms ? a.ws.n_slabs : sms;
+  if (grid == 0) return 0;
+  velo_fit_big_kernel<1024><<<grid, 1024, 0, stream>>>(a);
+  return (int)cudaGetLastError();
 }
 
 int launch_write(const KernelArgs& a, cudaStream_t stream) {

@@ -44,6 +44,7 @@ __host__ __device__ inline SlabLayout slab_layout() {
 //           4 event ticket, 5 large-event list length, 6 large-event ticket
 enum { kCtrTracks = 0, kCtrHits = 1, kCtrStatus = 2, kCtrCand = 3, kCtrTicket = 4, kCtrLargeN = 5,
        kCtrLargeTicket = 6, kCtrSortTicket = 7, kCtrTrackTicket = 8, kCtrFitTicket = 9, kCtrCandAlloc = 10,
+       kCtrBigN = 11, kCtrBigSortTicket = 12, kCtrBigTrackTicket = 13, kCtrBigFitTicket = 14,
        kNumCounters = 16, kNumPhaseClocks = 64 };
 
 // ---- the three-stage pipeline (velo_sort.cu -> velo_track.cu -> velo_fit.cu) ---------------------
@@ -72,7 +73,10 @@ __host__ __device__ inline uint32_t fit_smem_bound(uint32_t n) { return 4u * n +
 // fits from these rows and needs no gather. kXyStride float2 per candidate (16-byte aligned rows).
 constexpr uint32_t kXyStride = VELO_MAX_MODULES;
 // per-event state written by stage 1, updated by stage 2
-enum { kEvEmpty = 0, kEvReady = 1, kEvDeferred = 2, kEvBad = 3 };
+// kEvBig: an event of more than kPipeMaxHits hits. It runs through the same three stages in their
+// one-event-per-CTA form (velo_*_big_kernel: the sort's and the fit's per-event arrays in a global
+// slab instead of shared memory, the module loop reading the sorted records from L2 instead of a ring).
+enum { kEvEmpty = 0, kEvReady = 1, kEvDeferred = 2, kEvBad = 3, kEvBig = 4 };
 struct EvInfo { uint32_t n, state, cbase, ncand; };   // cbase: first candidate slot; ncand: candidates created
 
 struct Workspace {
@@ -92,6 +96,7 @@ struct Workspace {
   uint4* ev_rec;          // n_events: {temp track base, temp hit base, n_tracks, n_track_hits}
   uint32_t* ev_hit_base;  // n_events+1: exclusive scan of n_track_hits over events
   uint32_t* large_list;   // n_events: events deferred to the slab path
+  uint32_t* big_list;     // n_events: events of more than kPipeMaxHits hits (the one-event-per-CTA pipeline)
   uint32_t* order;        // n_events: event ids by ascending size class (velo_order_kernel)
   float *ux, *uy, *uz;    // n_hits: fp32 coordinates of deferred events when the input is packed pixels
   uint8_t* umod;          //   (index = absolute hit index - event_offsets[0])
@@ -119,6 +124,7 @@ struct KernelArgs {
   uint32_t hit_base;                 // x, y, z, module point at absolute hit index hit_base (0 for velo_reconstruct)
   uint32_t team_max_hits;            // events with more hits go to the general kernel
   uint32_t all_deferred;             // slab-only path: every event was reconstructed by the general kernel
+  uint32_t big_path;                 // events above team_max_hits take the one-event-per-CTA pipeline (else the general kernel)
   float module_z[VELO_MAX_MODULES];  // geometry: the shared-memory path requires z[i] == module_z[module[i]]
   velo_params_t P;
   // output
@@ -162,6 +168,10 @@ int launch_sort(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o);
 int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o);
 int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o);
 int launch_write(const KernelArgs& a, cudaStream_t stream);
+// The same stages for the events on ws.big_list: one event per CTA.
+int launch_sort_big(const KernelArgs& a, cudaStream_t stream);
+int launch_track_big(const KernelArgs& a, cudaStream_t stream);
+int launch_fit_big(const KernelArgs& a, cudaStream_t stream);
 
 // Enqueues the whole path for one batch on `stream`. Returns a cudaError_t as int.
 int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, void* const* stage_events, uint32_t path,

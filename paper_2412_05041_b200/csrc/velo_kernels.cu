@@ -432,7 +432,8 @@ __global__ void __launch_bounds__(256) velo_offsets_kernel(const KernelArgs a) {
     a.summary[0] = n_tracks; a.summary[1] = n_hits; a.summary[2] = status;
     a.summary[3] = a.ws.counters[kCtrCand];
     a.summary[4] = a.ws.counters[kCtrLargeN];
-    a.summary[5] = a.summary[6] = a.summary[7] = 0;
+    a.summary[5] = a.ws.counters[kCtrBigN];
+    a.summary[6] = a.summary[7] = 0;
   }
 }
 
@@ -472,6 +473,7 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t n_hits, uint32
   w.ev_rec = (uint4*)take(sizeof(uint4) * ((size_t)n_events + 1));
   w.ev_hit_base = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.large_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
+  w.big_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.order = (uint32_t*)take(4 * ((size_t)n_events + 1));
   const size_t sc = sorted_capacity(n_events, n_hits);
   w.rec16 = (uint4*)take(16 * sc);
@@ -499,6 +501,10 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const*
                        const PipeOpts& po) {
   KernelArgs a = a_in;
   a.all_deferred = path == kPathSlabOnly ? 1u : 0u;
+  // The one-event-per-CTA kernels are launched only for batches that can hold events above the pool's
+  // reach (a mean event above a quarter of kPipeMaxHits): three launches that a mu = 5 batch would only
+  // pay for. Without them such events take the general kernel, with the same results.
+  a.big_path = path != kPathSlabOnly && a.n_events > 0 && (unsigned long long)a.n_hits * 4ull > (unsigned long long)kPipeMaxHits * a.n_events ? 1u : 0u;
   auto mark = [&](int k) { if (stage_events && stage_events[k]) cudaEventRecord((cudaEvent_t)stage_events[k], stream); };
   cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);
   if (err != cudaSuccess) return (int)err;
@@ -518,10 +524,12 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const*
       // for whatever the pipeline deferred (usually nothing: its CTAs come and go); stage 3 below
       int rc = launch_sort(a, stream, po);
       if (rc != 0) return rc;
+      if (a.big_path && (rc = launch_sort_big(a, stream)) != 0) return rc;
       velo_order_kernel<<<1, 512, 0, stream>>>(a);
       mark(1);
       rc = launch_track(a, stream, po);
       if (rc != 0) return rc;
+      if (a.big_path && (rc = launch_track_big(a, stream)) != 0) return rc;
       if (large_events) velo_event_slab_kernel<kThreadsLarge, false, 8><<<grid, kThreadsLarge, 0, stream>>>(a, 1);
       else velo_event_slab_kernel<kThreads, true, kBinShift><<<grid, kThreads, 0, stream>>>(a, 1);
     }
@@ -530,8 +538,9 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const*
   }
   mark(2);
   if (path != kPathSlabOnly) {
-    const int rc = launch_fit(a, stream, po);   // fit and filters: per-candidate results, per-event counts
+    int rc = launch_fit(a, stream, po);   // fit and filters: per-candidate results, per-event counts
     if (rc != 0) return rc;
+    if (a.big_path && a.n_events > 0 && (rc = launch_fit_big(a, stream)) != 0) return rc;
   }
   mark(3);
   velo_offsets_kernel<<<1, 256, 0, stream>>>(a);   // counts -> event_track_offsets, summary

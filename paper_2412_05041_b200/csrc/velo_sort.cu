@@ -81,6 +81,11 @@ __device__ void sort_fetch(const KernelArgs& a, PoolCtl& pool, SortTeam<G>& ts) 
   if (n == 0) { a.ws.ev_info[e] = info; return; }
   const SortLayout L = sort_layout(n, a.n_modules);
   const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;
+  if (n > a.team_max_hits && a.big_path) {       // too large for an SM's pool: the one-event-per-CTA pipeline
+    info.state = kEvBig; a.ws.ev_info[e] = info;
+    a.ws.big_list[atomicAdd(&a.ws.counters[kCtrBigN], 1u)] = e;
+    return;
+  }
   if (n > a.team_max_hits || units > pool.units || fit_smem_bound(n) > pool.units * kUnitBytes) {
     info.state = kEvDeferred; a.ws.ev_info[e] = info;
     a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
@@ -94,7 +99,7 @@ __device__ void sort_fetch(const KernelArgs& a, PoolCtl& pool, SortTeam<G>& ts) 
 
 template <int G>
 __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts, unsigned char* blk, uint32_t team,
-                           uint32_t tid, uint32_t& parity) {
+                           uint32_t tid, uint32_t& parity, uint32_t done_state = kEvReady) {
   const uint32_t M = a.n_modules, nbins = M * kBinsPerModule;
   const uint32_t e = ts.event, n = ts.n;
   const SortLayout L = sort_layout(n, M);
@@ -269,7 +274,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
     mo[tid] = (uint16_t)lo;
     if (tid == 0) { mo[32] = (uint16_t)n; mo[kModOffStride - 1] = (uint16_t)sz; }
   }
-  if (tid == 0) a.ws.ev_info[e] = EvInfo{n, kEvReady, 0u, 0u};
+  if (tid == 0) a.ws.ev_info[e] = EvInfo{n, done_state, 0u, 0u};
   VELO_PH(a.ws.phase_clk, ts, 14);
 }
 
@@ -304,6 +309,41 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_sort_kernel(const KernelAr
   VELO_STAGE_END(a.ws.phase_clk, 0);
 }
 
+// ---- the same stage for the events of ws.big_list: one CTA of G threads per event, the per-event
+// arrays in the CTA's global slab (L2-resident) instead of shared memory --------------------------
+template <int G>
+__global__ void __launch_bounds__(G, 1) velo_sort_big_kernel(const KernelArgs a) {
+  __shared__ SortTeam<G> ts;
+  __shared__ float module_z[VELO_MAX_MODULES];
+  const uint32_t tid = threadIdx.x;
+  if (tid < VELO_MAX_MODULES) module_z[tid] = a.module_z[tid];
+  unsigned char* blk = a.ws.slabs + (size_t)blockIdx.x * slab_layout().bytes;
+  uint32_t parity = 0;
+  const uint32_t base = a.event_offsets[0];
+  for (;;) {
+    __syncthreads();
+    if (tid == 0) {
+      const uint32_t k = atomicAdd(&a.ws.counters[kCtrBigSortTicket], 1u);
+      ts.skip = k >= a.ws.counters[kCtrBigN];
+      if (!ts.skip) {
+        const uint32_t e = a.ws.big_list[k], o0 = a.event_offsets[e];
+        ts.event = e; ts.n = a.event_offsets[e + 1] - o0; ts.o0 = o0; ts.ol = o0 - base; ts.trouble = 0; ts.unpack = 0;
+      }
+    }
+    __syncthreads();
+    if (ts.skip) break;
+    sort_event<G>(a, module_z, ts, blk, 0u, tid, parity, kEvBig);
+  }
+}
+
+int launch_sort_big_impl(const KernelArgs& a, cudaStream_t stream) {
+  const uint32_t sms = num_sms();
+  const uint32_t grid = a.ws.n_slabs < sms ? a.ws.n_slabs : sms;
+  if (grid == 0) return 0;
+  velo_sort_big_kernel<1024><<<grid, 1024, 0, stream>>>(a);
+  return (int)cudaGetLastError();
+}
+
 template <int G, int kTeams>
 int launch_sort_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
   using Ctl = SortCtl<G, kTeams>;
@@ -319,6 +359,8 @@ int launch_sort_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units)
 }
 
 }  // namespace
+
+int launch_sort_big(const KernelArgs& a, cudaStream_t stream) { return launch_sort_big_impl(a, stream); }
 
 int launch_sort(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;

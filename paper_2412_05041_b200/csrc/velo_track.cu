@@ -52,10 +52,11 @@ struct TrackCtl {
 __device__ __forceinline__ uint32_t al16(uint32_t v) { return (v + 15u) & ~15u; }
 
 struct TrackLayout { uint32_t ring, act, flags, th0, cl, bytes; };
-__device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod, uint32_t tcap, uint32_t acap) {
+__device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod, uint32_t tcap, uint32_t acap,
+                                                    bool with_ring = true) {
   TrackLayout L;
   uint32_t o = 0;
-  L.ring = o; o += 4u * 16u * maxmod;
+  L.ring = o; o += with_ring ? 4u * 16u * maxmod : 0u;
   L.act = o; o += 32u * acap;
   L.flags = o; o += al16(4u * ((n + 31u) >> 5));
   L.th0 = o; o += al16(2u * tcap);
@@ -119,13 +120,16 @@ __device__ __forceinline__ Win make_win(uint32_t c, int W) {
 }
 
 // ---- one event, by one team ---------------------------------------------------------------------
-template <int G, bool kSameW>
+// kGlobal: the one-event-per-CTA form for events too large for a ring in shared memory: the module
+// slots ARE the sorted records in global scratch (L2), nothing is copied; the event ends in state
+// kEvBig so that the per-event kernels of stage 3 leave it to velo_fit_big_kernel.
+template <int G, bool kSameW, bool kGlobal = false>
 __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& ts, unsigned char* blk, uint32_t team,
                             uint32_t tid, uint32_t& parity, uint32_t& phases) {
   const uint32_t M = a.n_modules, n = ts.n, e = ts.event;
   const velo_params_t& P = a.P;
   const uint32_t slotcap = ts.maxmod, tcap = ts.tcap, acap = ts.acap;
-  const TrackLayout L = track_layout(n, slotcap, tcap, acap);
+  const TrackLayout L = track_layout(n, slotcap, tcap, acap, !kGlobal);
   uint4* ring = (uint4*)(blk + L.ring);
   uint4* act = (uint4*)(blk + L.act);
   uint32_t* flags = (uint32_t*)(blk + L.flags);   // one bit per sorted hit
@@ -159,13 +163,14 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
 
   // ring: module m lives in slot m & 3; loads are issued and waited for in descending module order
   auto issue = [&](uint32_t m) {
-    if (tid == 0) {
+    if (!kGlobal && tid == 0) {
       const uint32_t bytes = 16u * ((uint32_t)mo[m + 1] - (uint32_t)mo[m]);
       mbar_arrive_expect_tx(&ts.mbar[m & 3u], bytes);
       if (bytes) tma_load_1d(ring + (m & 3u) * slotcap, grec + mo[m], bytes, &ts.mbar[m & 3u]);
     }
   };
   auto wait = [&](uint32_t m) {
+    if (kGlobal) return;
     mbar_wait(&ts.mbar[m & 3u], (phases >> (m & 3u)) & 1u);
     phases ^= 1u << (m & 3u);
   };
@@ -186,9 +191,9 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     const uint32_t off_u = mo[u], nu = (uint32_t)mo[u + 1] - off_u;
     const uint32_t off_s = mo[s], ns = (uint32_t)mo[s + 1] - off_s;
     const uint32_t off_p = mo[s + 1], np = (uint32_t)mo[s + 2] - off_p;
-    const uint4* ring_u = ring + (u & 3u) * slotcap;
-    const uint4* ring_s = ring + (s & 3u) * slotcap;
-    const uint4* ring_p = ring + ((s + 1u) & 3u) * slotcap;
+    const uint4* ring_u = kGlobal ? grec + off_u : ring + (u & 3u) * slotcap;
+    const uint4* ring_s = kGlobal ? grec + off_s : ring + (s & 3u) * slotcap;
+    const uint4* ring_p = kGlobal ? grec + off_p : ring + ((s + 1u) & 3u) * slotcap;
     const float z2 = mz[u];
 
     // ---- (A) O-7 forwarding into module u of every track active at the start of the step ----------
@@ -363,7 +368,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) fb[i] = flags[i];
   }
   if (tid == 0) {
-    a.ws.ev_info[e] = EvInfo{n, kEvReady, ts.cbase, ncand};
+    a.ws.ev_info[e] = EvInfo{n, kGlobal ? kEvBig : kEvReady, ts.cbase, ncand};
     atomicAdd(&a.ws.counters[kCtrCand], ncand);
   }
 }
@@ -404,6 +409,69 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
   VELO_STAGE_END(a.ws.phase_clk, 1);
 }
 
+// ---- the same stage for the events of ws.big_list: one CTA of G threads per event ------------------
+template <int G, bool kSameW>
+__global__ void __launch_bounds__(G, 1) velo_track_big_kernel(const KernelArgs a, const uint32_t smem_bytes) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  using Ctl = TrackCtl<G, 1>;
+  constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
+  Ctl& ctl = *reinterpret_cast<Ctl*>(smem);
+  unsigned char* blk = smem + kCtl;
+  const uint32_t tid = threadIdx.x;
+  if (tid < VELO_MAX_MODULES) ctl.module_z[tid] = a.module_z[tid];
+  TrackTeam<G>& ts = ctl.team[0];
+  uint32_t parity = 0, phases = 0;
+  const uint32_t base = a.event_offsets[0];
+  for (;;) {
+    __syncthreads();
+    if (tid == 0) {
+      const uint32_t k = atomicAdd(&a.ws.counters[kCtrBigTrackTicket], 1u);
+      ts.units = k >= a.ws.counters[kCtrBigN];      // 1 = no more events
+      ts.skip = 1; ts.defer = 0; ts.unpack = 0;
+      if (!ts.units) {
+        const uint32_t e = a.ws.big_list[k];
+        const EvInfo info = a.ws.ev_info[e];
+        ts.event = e;
+        if (info.state == kEvBig) {                  // else: stage 1 gave it to the general kernel
+          const uint32_t n = info.n, maxmod = a.ws.mod_off[(size_t)e * kModOffStride + kModOffStride - 1];
+          const uint32_t tcap = cand_capacity(n), acap = active_capacity(n);
+          if (track_layout(n, maxmod, tcap, acap, false).bytes > smem_bytes - kCtl) {
+            a.ws.ev_info[e].state = kEvDeferred;
+            a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+            ts.unpack = a.pixel != nullptr;
+          } else {
+            ts.cbase = atomicAdd(&a.ws.counters[kCtrCandAlloc], tcap);
+            ts.n = n; ts.sb = sorted_base(a.event_offsets[e] - base, e);
+            ts.maxmod = maxmod; ts.tcap = tcap; ts.acap = acap; ts.skip = 0;
+          }
+        }
+      }
+    }
+    __syncthreads();
+    if (ts.units) break;
+    if (!ts.skip) track_event<G, kSameW, true>(a, ctl.module_z, ts, blk, 0u, tid, parity, phases);
+    if (a.pixel && (ts.unpack || (!ts.skip && ts.defer))) unpack_event<G>(a, ts.event, tid);
+  }
+}
+
+template <int G>
+int launch_track_big_t(const KernelArgs& a, cudaStream_t stream) {
+  const uint32_t smem = 227u * 1024u;
+  const bool same = a.P.phi_window_seed == a.P.phi_window_fwd;
+  const uint32_t grid = num_sms();
+  cudaError_t err;
+  if (same) {
+    err = cudaFuncSetAttribute(velo_track_big_kernel<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return (int)err;
+    velo_track_big_kernel<G, true><<<grid, G, smem, stream>>>(a, smem);
+  } else {
+    err = cudaFuncSetAttribute(velo_track_big_kernel<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return (int)err;
+    velo_track_big_kernel<G, false><<<grid, G, smem, stream>>>(a, smem);
+  }
+  return (int)cudaGetLastError();
+}
+
 template <int G, int kTeams>
 int launch_track_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
   static_assert(G == 32 || kTeams <= 15, "named barriers 1..15");
@@ -428,6 +496,8 @@ int launch_track_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units
 }
 
 }  // namespace
+
+int launch_track_big(const KernelArgs& a, cudaStream_t stream) { return launch_track_big_t<512>(a, stream); }
 
 int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;

@@ -266,7 +266,8 @@ class DeviceTracks:
         u = lambda t: t.cpu().numpy().view(np.uint32)
         return {"event_track_offsets": u(self.event_track_offsets), "track_hit_offsets": u(self.track_hit_offsets[:nt + 1]),
                 "track_hits": u(self.track_hits[:nh]), "states": self.states[:, :nt].cpu().numpy(),
-                "n_tracks": nt, "n_track_hits": nh, "status": status, "n_candidates": int(s[3]), "n_deferred": int(s[4])}
+                "n_tracks": nt, "n_track_hits": nh, "status": status, "n_candidates": int(s[3]), "n_deferred": int(s[4]),
+                "n_big": int(s[5])}
 
 
 def velo_reconstruct(geometry: Geometry, hits: Hits, params: Params, out: DeviceTracks, stream=None,
@@ -430,9 +431,9 @@ def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None 
 def stitch(parts: list[dict]) -> dict:
     """Concatenates per-batch results (batch-local offsets) into one result."""
     eto, tho, th, st = [np.zeros(1, np.uint32)], [np.zeros(1, np.uint32)], [], []
-    nt = nh = nc = nd = 0
+    nt = nh = nc = nd = nbig = 0
     for p in parts:
-        nd += p.get("n_deferred", 0)
+        nd += p.get("n_deferred", 0); nbig += p.get("n_big", 0)
         eto.append(p["event_track_offsets"][1:] + np.uint32(nt))
         tho.append(p["track_hit_offsets"][1:] + np.uint32(nh))
         th.append(p["track_hits"]); st.append(p["states"])
@@ -440,7 +441,7 @@ def stitch(parts: list[dict]) -> dict:
     return {"event_track_offsets": np.concatenate(eto), "track_hit_offsets": np.concatenate(tho),
             "track_hits": np.concatenate(th) if th else np.zeros(0, np.uint32),
             "states": np.concatenate(st, axis=1) if st else np.zeros((VELO_N_STATE, 0), np.float32),
-            "n_tracks": nt, "n_track_hits": nh, "status": 0, "n_candidates": nc, "n_deferred": nd}
+            "n_tracks": nt, "n_track_hits": nh, "status": 0, "n_candidates": nc, "n_deferred": nd, "n_big": nbig}
 
 
 # ---- end-to-end path over host buffers: the event-batch scheduler -------------------------------

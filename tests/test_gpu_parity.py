@@ -213,8 +213,10 @@ def test_config4_ion_like(velo):
     nh = np.diff(d["event_offsets"].astype(np.int64))
     assert nh.max() > 20000                  # the large-event path is exercised
     got = gpu(velo, d)
-    assert 0 < got["n_deferred"] < 160       # both kernels took part
+    assert 0 < got["n_big"] + got["n_deferred"] < 160      # the per-SM pipeline and the one-event-per-CTA pipeline took part
     check(got, cpu(d))
+    # the same batch through the general kernel alone, and with the large events in the general kernel (mu-like batch rule)
+    check(gpu(velo, d, opts=velo.LaunchOptions(path=1)), cpu(d))
 
 
 # ---- hand-made and degenerate inputs (SURVEY.md §8(c) whole-path pins, A14, A15) -----------------
@@ -393,10 +395,10 @@ def test_scheduler_reports_an_oversized_batch(velo):
 
 def test_config4_full_size_every_event(velo):
     """BASELINE.json:configs[4] at full size (2 000 ion-like events, one call): every event against the
-    oracle; the largest run in the general kernel, the others in the pipeline."""
+    oracle; events above 12 000 hits run in the one-event-per-CTA pipeline, the others in the per-SM pipeline."""
     d = datagen.generate_config(4)
     got = gpu(velo, d)
-    assert 0 < got["n_deferred"] < d["n_events"]
+    assert 0 < got["n_big"] < d["n_events"] and got["n_deferred"] < 20
     assert _compare_in_chunks(got, d, 500)
 
 
