@@ -317,7 +317,7 @@ __global__ void __launch_bounds__(G, 1) velo_fit_big_kernel(const KernelArgs a) 
       ts.units = k >= a.ws.counters[kCtrBigN];      // 1 = no more events
       ts.skip = 1;
       if (!ts.units) {
-        const uint32_t e = a.ws.big_list[k];
+        const uint32_t e = a.ws.big_sorted[k];
         const EvInfo info = a.ws.ev_info[e];
         ts.event = e;
         if (info.state == kEvBig) {                  // else: the general kernel has written its counts
@@ -374,6 +374,7 @@ __global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const Kerne
       }
       continue;
     }
+    if (info.state == kEvBig) continue;                 // velo_write_big_kernel: a CTA per such event
     const uint32_t o0 = a.event_offsets[e];
     const uint16_t* orig = a.ws.sorig + sorted_base(o0 - obase, e);
     const uint16_t* rows = a.ws.rows + (size_t)info.cbase * 32u;
@@ -395,6 +396,52 @@ __global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const Kerne
       float s9[9];
 #pragma unroll
       for (uint32_t k = 0; k < 9; ++k) s9[k] = cfit[k * cc + t];
+      float* dst_s = a.states + dst_t + lt;
+      dst_s[0] = s9[0]; dst_s[cs] = s9[1]; dst_s[2 * cs] = s9[2]; dst_s[3 * cs] = s9[3]; dst_s[4 * cs] = s9[4];
+      dst_s[5 * cs] = s9[5]; dst_s[6 * cs] = s9[6]; dst_s[7 * cs] = s9[7];
+      dst_s[8 * cs] = s9[5]; dst_s[9 * cs] = s9[6]; dst_s[10 * cs] = s9[7];
+      dst_s[11 * cs] = s9[8]; dst_s[12 * cs] = __uint_as_float(nh);
+      a.track_hit_offsets[dst_t + lt] = dst_h + lh;
+      uint32_t* dst = a.track_hits + dst_h + lh;
+      for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) { dst[i] = o0 + orig[h]; });
+    }
+  }
+}
+
+// The same for the events of the one-event-per-CTA pipeline (thousands of tracks each): a CTA per
+// event, a block-wide scan over its candidates instead of a warp's.
+__global__ void __launch_bounds__(1024) velo_write_big_kernel(const KernelArgs a) {
+  __shared__ unsigned long long warp_sums[33];
+  const uint32_t tid = threadIdx.x;
+  const uint32_t tot_t = a.event_track_offsets[a.n_events], tot_h = a.ws.ev_hit_base[a.n_events];
+  if (tot_t > a.cap_tracks || tot_h > a.cap_track_hits) return;  // VELO_ERR_CAPACITY: nothing valid
+  const size_t cs = a.cap_tracks, cc = a.ws.cand_total;
+  const uint32_t obase = a.event_offsets[0], nb = a.ws.counters[kCtrBigN];
+  for (uint32_t k = blockIdx.x; k < nb; k += gridDim.x) {
+    const uint32_t e = a.ws.big_sorted[k];
+    const EvInfo info = a.ws.ev_info[e];
+    const uint4 r = a.ws.ev_rec[e];
+    if (info.state != kEvBig || r.z == 0) continue;       // deferred on the way: the warp-per-event kernel copies its temp block
+    const uint32_t dst_t = a.event_track_offsets[e], dst_h = a.ws.ev_hit_base[e];
+    const uint32_t o0 = a.event_offsets[e];
+    const uint16_t* orig = a.ws.sorig + sorted_base(o0 - obase, e);
+    const uint16_t* rows = a.ws.rows + (size_t)info.cbase * 32u;
+    const uint2* cmeta = a.ws.cmeta + info.cbase;
+    const uint8_t* cstate = a.ws.cstate + info.cbase;
+    const float* cfit = a.ws.cfit + info.cbase;
+    uint32_t run_t = 0, run_h = 0;
+    for (uint32_t t0 = 0; t0 < info.ncand; t0 += blockDim.x) {
+      const uint32_t t = t0 + tid;
+      const bool surv = t < info.ncand && cstate[t] != 0;
+      const uint32_t nh = surv ? (uint32_t)__popc(cmeta[t].x) : 0u;
+      unsigned long long tot;
+      const unsigned long long pre = block_scan_excl(((unsigned long long)nh << 32) | (surv ? 1ull : 0ull), warp_sums, &tot);
+      const uint32_t lt = run_t + (uint32_t)(pre & 0xffffffffu), lh = run_h + (uint32_t)(pre >> 32);
+      run_t += (uint32_t)(tot & 0xffffffffu); run_h += (uint32_t)(tot >> 32);
+      if (!surv) continue;
+      float s9[9];
+#pragma unroll
+      for (uint32_t q = 0; q < 9; ++q) s9[q] = cfit[q * cc + t];
       float* dst_s = a.states + dst_t + lt;
       dst_s[0] = s9[0]; dst_s[cs] = s9[1]; dst_s[2 * cs] = s9[2]; dst_s[3 * cs] = s9[3]; dst_s[4 * cs] = s9[4];
       dst_s[5 * cs] = s9[5]; dst_s[6 * cs] = s9[6]; dst_s[7 * cs] = s9[7];
@@ -449,6 +496,7 @@ int launch_write(const KernelArgs& a, cudaStream_t stream) {
   if (a.n_events == 0) return 0;
   const uint32_t grid = (a.n_events + 3u) / 4u;     // a warp per event
   velo_write_kernel<8><<<grid, 128, 0, stream>>>(a);
+  if (a.big_path) velo_write_big_kernel<<<num_sms() * 2u, 1024, 0, stream>>>(a);
   return (int)cudaGetLastError();
 }
 

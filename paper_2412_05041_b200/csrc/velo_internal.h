@@ -97,6 +97,7 @@ struct Workspace {
   uint32_t* ev_hit_base;  // n_events+1: exclusive scan of n_track_hits over events
   uint32_t* large_list;   // n_events: events deferred to the slab path
   uint32_t* big_list;     // n_events: events of more than kPipeMaxHits hits (the one-event-per-CTA pipeline)
+  uint32_t* big_sorted;   // n_events: the same, largest first (stages 2 and 3 take them in this order)
   uint32_t* order;        // n_events: event ids by ascending size class (velo_order_kernel)
   float *ux, *uy, *uz;    // n_hits: fp32 coordinates of deferred events when the input is packed pixels
   uint8_t* umod;          //   (index = absolute hit index - event_offsets[0])

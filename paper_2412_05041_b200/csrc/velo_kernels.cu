@@ -437,6 +437,21 @@ __global__ void __launch_bounds__(256) velo_offsets_kernel(const KernelArgs a) {
   }
 }
 
+// The events of the one-event-per-CTA pipeline, largest first: an event's time grows faster than its
+// size, so the longest must start first. Rank by counting (a few hundred events; one CTA).
+__global__ void __launch_bounds__(1024) velo_big_order_kernel(const KernelArgs a) {
+  const uint32_t nb = a.ws.counters[kCtrBigN];
+  for (uint32_t i = threadIdx.x; i < nb; i += blockDim.x) {
+    const uint32_t e = a.ws.big_list[i], n = a.event_offsets[e + 1] - a.event_offsets[e];
+    uint32_t rank = 0;
+    for (uint32_t j = 0; j < nb; ++j) {
+      const uint32_t ej = a.ws.big_list[j], nj = a.event_offsets[ej + 1] - a.event_offsets[ej];
+      rank += (nj > n || (nj == n && j < i)) ? 1u : 0u;
+    }
+    a.ws.big_sorted[rank] = e;
+  }
+}
+
 // Packed input on the slab-only path: every event is decoded into the workspace planes first.
 __global__ void __launch_bounds__(256) velo_unpack_kernel(const KernelArgs a) {
   for (uint32_t e = blockIdx.x; e < a.n_events; e += gridDim.x) {
@@ -474,6 +489,7 @@ Workspace carve_workspace(void* base, uint32_t n_events, uint32_t n_hits, uint32
   w.ev_hit_base = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.large_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.big_list = (uint32_t*)take(4 * ((size_t)n_events + 1));
+  w.big_sorted = (uint32_t*)take(4 * ((size_t)n_events + 1));
   w.order = (uint32_t*)take(4 * ((size_t)n_events + 1));
   const size_t sc = sorted_capacity(n_events, n_hits);
   w.rec16 = (uint4*)take(16 * sc);
@@ -524,7 +540,10 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const*
       // for whatever the pipeline deferred (usually nothing: its CTAs come and go); stage 3 below
       int rc = launch_sort(a, stream, po);
       if (rc != 0) return rc;
-      if (a.big_path && (rc = launch_sort_big(a, stream)) != 0) return rc;
+      if (a.big_path) {
+        if ((rc = launch_sort_big(a, stream)) != 0) return rc;
+        velo_big_order_kernel<<<1, 1024, 0, stream>>>(a);
+      }
       velo_order_kernel<<<1, 512, 0, stream>>>(a);
       mark(1);
       rc = launch_track(a, stream, po);

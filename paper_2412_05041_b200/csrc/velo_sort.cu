@@ -46,12 +46,12 @@ struct SortCtl {
 __device__ __forceinline__ uint32_t align16u(uint32_t v) { return (v + 15u) & ~15u; }
 
 struct SortLayout { uint32_t xy, w, bins, stash, mod8, bytes; };
-__device__ __forceinline__ SortLayout sort_layout(uint32_t n, uint32_t M) {
+__device__ __forceinline__ SortLayout sort_layout(uint32_t n, uint32_t M, uint32_t bins_per_module = kBinsPerModule) {
   SortLayout L;
   uint32_t o = 0;
   L.xy = o; o += align16u(8u * n);
   L.w = o; o += align16u(4u * n);
-  L.bins = o; o += align16u(2u * (M * kBinsPerModule + 2u));
+  L.bins = o; o += align16u(2u * (M * bins_per_module + 2u));
   L.stash = o; o += align16u(4u * n);
   L.mod8 = o; o += align16u(n);
   L.bytes = o;
@@ -97,12 +97,16 @@ __device__ void sort_fetch(const KernelArgs& a, PoolCtl& pool, SortTeam<G>& ts) 
   ts.skip = 0;
 }
 
-template <int G>
+// kShift: phi units per bucket = 1 << kShift (the one-event-per-CTA form uses finer buckets: its events
+// have tens of hits per 1024-unit bucket, and the rank inside a bucket is a loop over the bucket).
+template <int G, int kShift = kBinShift>
 __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts, unsigned char* blk, uint32_t team,
                            uint32_t tid, uint32_t& parity, uint32_t done_state = kEvReady) {
+  constexpr uint32_t kBinsPerModule = 65536u >> kShift;
+  constexpr uint32_t kBinShift = kShift;
   const uint32_t M = a.n_modules, nbins = M * kBinsPerModule;
   const uint32_t e = ts.event, n = ts.n;
-  const SortLayout L = sort_layout(n, M);
+  const SortLayout L = sort_layout(n, M, kBinsPerModule);
   float2* xyo = (float2*)(blk + L.xy);          // (x, y) by ORIGINAL index
   uint32_t* w = (uint32_t*)(blk + L.w);
   uint32_t* binsw = (uint32_t*)(blk + L.bins);
@@ -332,7 +336,7 @@ __global__ void __launch_bounds__(G, 1) velo_sort_big_kernel(const KernelArgs a)
     }
     __syncthreads();
     if (ts.skip) break;
-    sort_event<G>(a, module_z, ts, blk, 0u, tid, parity, kEvBig);
+    sort_event<G, 8>(a, module_z, ts, blk, 0u, tid, parity, kEvBig);
   }
 }
 

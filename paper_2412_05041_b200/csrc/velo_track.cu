@@ -37,6 +37,7 @@ struct TrackTeam {
   uint32_t units, first_unit, pool_off, skip;
   uint32_t maxmod, cbase, tcap, acap;
   uint32_t defer;                    // set by any thread: the event continues in the general kernel
+  uint32_t npairs;                   // one-event-per-CTA seeding: (centre, h0) pairs listed in this round
   uint32_t unpack;                   // packed input: decode the deferred event for the general kernel
   unsigned long long ph_last;        // phase clocks (-DVELO_TIMELINE builds)
   uint16_t mod_off[kModOffStride];
@@ -51,7 +52,8 @@ struct TrackCtl {
 
 __device__ __forceinline__ uint32_t al16(uint32_t v) { return (v + 15u) & ~15u; }
 
-struct TrackLayout { uint32_t ring, act, flags, th0, cl, bytes; };
+constexpr uint32_t kPairCap = 8192;   // (centre, h0) pairs per round of the one-event-per-CTA seeding
+struct TrackLayout { uint32_t ring, act, flags, th0, cl, keys, plist, bytes; };
 __device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod, uint32_t tcap, uint32_t acap,
                                                     bool with_ring = true) {
   TrackLayout L;
@@ -61,6 +63,10 @@ __device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod,
   L.flags = o; o += al16(4u * ((n + 31u) >> 5));
   L.th0 = o; o += al16(2u * tcap);
   L.cl = o; o += al16(2u * maxmod);
+  // one-event-per-CTA form only: the best (scatter, h0, h2) of every centre of a round as a 64-bit
+  // key, and the round's list of (centre, h0) pairs
+  L.keys = o; o += with_ring ? 0u : 8u * 1024u;
+  L.plist = o; o += with_ring ? 0u : 4u * kPairCap;
   L.bytes = o;
   return L;
 }
@@ -130,6 +136,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
   const velo_params_t& P = a.P;
   const uint32_t slotcap = ts.maxmod, tcap = ts.tcap, acap = ts.acap;
   const TrackLayout L = track_layout(n, slotcap, tcap, acap, !kGlobal);
+  const TrackLayout& L_ = L;
   uint4* ring = (uint4*)(blk + L.ring);
   uint4* act = (uint4*)(blk + L.act);
   uint32_t* flags = (uint32_t*)(blk + L.flags);   // one bit per sorted hit
@@ -280,13 +287,72 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
     if (ncl) {
       const float zc0 = mz[s + 1], zc1 = mz[s];
       const float tz = __fdiv_rn(__fsub_rn(z2, zc1), __fsub_rn(zc1, zc0));
-      const uint32_t lsh = (4u * ncl <= (uint32_t)G) ? 2u : (2u * ncl <= (uint32_t)G) ? 1u : 0u;
+      const uint32_t lsh = kGlobal ? 0u : (4u * ncl <= (uint32_t)G) ? 2u : (2u * ncl <= (uint32_t)G) ? 1u : 0u;
       const uint32_t L = 1u << lsh;
       for (uint32_t k0 = 0; k0 < ncl; k0 += (uint32_t)G >> lsh) {
         const uint32_t k = k0 + (tid >> lsh), q = tid & (L - 1u);
         bool found = false; uint32_t b0 = 0, b2 = 0, j1 = 0; float best_sc = 0.0f;
         uint4 r1 = make_uint4(0, 0, 0, 0);
-        if (k < ncl) {
+        bool by_pairs = false;
+        if constexpr (kGlobal) {
+          // Large events: a centre has tens of h0 candidates and each means a long scan of the h2
+          // window, very unevenly over the centres. The round's (centre, h0) pairs are listed in shared
+          // memory and dealt out one per lane; a centre's best triplet is the minimum of a 64-bit key
+          // (scatter bits, h0, h2): the same lexicographic order, reached in any order.
+          unsigned long long* keys = (unsigned long long*)(blk + L_.keys);
+          uint32_t* plist = (uint32_t*)(blk + L_.plist);
+          uint32_t* npairs = &ts.npairs;
+          keys[tid] = ~0ull;
+          if (tid == 0) *npairs = 0u;
+          team_sync<G>(team);
+          if (k < ncl) {
+            j1 = cl[k];
+            r1 = ring_s[j1];
+            const uint32_t c = r1.z >> 16;
+            const Win wx = make_win(c, Wseed);
+            const Win ww = kSameW ? wx : make_win(c, Wwide);
+            for (uint32_t run0 = ww.wrapped ? 0u : 1u; run0 < 2u; ++run0) {
+              for (uint32_t j0 = run0 ? (r1.z & 0xffffu) : 0u; j0 < np; ++j0) {
+                const uint4 r0 = ring_p[j0];
+                if (!(r0.z - ww.lo16 <= ww.lim)) break;
+                if (!kSameW && !(r0.z - wx.lo16 <= wx.lim)) continue;
+                if (flagged(off_p + j0)) continue;
+                const uint32_t slot = atomicAdd(npairs, 1u);
+                if (slot < kPairCap) plist[slot] = (tid << 16) | j0;
+              }
+            }
+          }
+          team_sync<G>(team);
+          const uint32_t T = *npairs;
+          by_pairs = T <= kPairCap;        // else: the lane-per-centre search below
+          if (by_pairs) {
+            for (uint32_t p = tid; p < T; p += G) {
+              const uint32_t pr = plist[p], kl = pr >> 16, j0 = pr & 0xffffu;
+              const uint4 rc = ring_s[cl[k0 + kl]], r0 = ring_p[j0];
+              const float x1 = __uint_as_float(rc.x), y1 = __uint_as_float(rc.y);
+              const Win wx = make_win(rc.z >> 16, Wseed);
+              const Win ww = kSameW ? wx : make_win(rc.z >> 16, Wwide);
+              const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tz));
+              const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tz));
+              bool fnd = false; uint32_t bb2 = 0; float bsc = 0.0f;
+              auto visit2 = [&](uint32_t jj, const uint4& r, bool in) {
+                const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+                const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+                bool ok = in & !flagged(off_u + jj) & (sc <= max_seed) & (!fnd | (sc < bsc));
+                if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
+                fnd |= ok; bb2 = ok ? jj : bb2; bsc = ok ? sc : bsc;
+              };
+              if (ww.wrapped) scan_run(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
+              scan_run(ring_u, rc.w >> 16, nu, ww.lo16, ww.lim, visit2);
+              if (fnd) atomicMin(&keys[kl], ((unsigned long long)__float_as_uint(bsc) << 32) | ((unsigned long long)j0 << 16) | bb2);
+            }
+            team_sync<G>(team);
+            const unsigned long long key = keys[tid];
+            found = k < ncl && key != ~0ull;
+            b0 = (uint32_t)(key >> 16) & 0xffffu; b2 = (uint32_t)key & 0xffffu; best_sc = __uint_as_float((uint32_t)(key >> 32));
+          }
+        }
+        if (!by_pairs && k < ncl) {
           j1 = cl[k];
           r1 = ring_s[j1];
           const float x1 = __uint_as_float(r1.x), y1 = __uint_as_float(r1.y);
@@ -429,7 +495,7 @@ __global__ void __launch_bounds__(G, 1) velo_track_big_kernel(const KernelArgs a
       ts.units = k >= a.ws.counters[kCtrBigN];      // 1 = no more events
       ts.skip = 1; ts.defer = 0; ts.unpack = 0;
       if (!ts.units) {
-        const uint32_t e = a.ws.big_list[k];
+        const uint32_t e = a.ws.big_sorted[k];
         const EvInfo info = a.ws.ev_info[e];
         ts.event = e;
         if (info.state == kEvBig) {                  // else: stage 1 gave it to the general kernel
@@ -497,7 +563,7 @@ int launch_track_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units
 
 }  // namespace
 
-int launch_track_big(const KernelArgs& a, cudaStream_t stream) { return launch_track_big_t<512>(a, stream); }
+int launch_track_big(const KernelArgs& a, cudaStream_t stream) { return launch_track_big_t<768>(a, stream); }
 
 int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
