@@ -474,7 +474,8 @@ int launch_fit_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) 
 int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   if (a.n_events == 0) return 0;
   const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
-  switch (o.fit_teams) {
+  const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
+  switch (o.fit_teams ? o.fit_teams : (mean < 768u ? 15u : 0u)) {   // small events: 15 teams of 64 threads
     case 4: return launch_fit_t<128, 4>(a, stream, pu);
     case 6: return launch_fit_t<128, 6>(a, stream, pu);
     case 12: return launch_fit_t<64, 12>(a, stream, pu);

@@ -368,7 +368,11 @@ int launch_sort_big(const KernelArgs& a, cudaStream_t stream) { return launch_so
 
 int launch_sort(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
-  switch (o.sort_teams) {
+  // small events (open VELO: 320 hits) keep more teams busy with 128 threads each; from mu = 5 sizes on
+  // 256 threads finish an event in half the time and four of them fill the pool (measured: profiles/r02e)
+  const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
+  const uint32_t teams = o.sort_teams ? o.sort_teams : (mean < 768u ? 8u : 0u);
+  switch (teams) {
     case 4: return launch_sort_t<128, 4>(a, stream, pu);
     case 6: return launch_sort_t<128, 6>(a, stream, pu);
     case 7: return launch_sort_t<128, 7>(a, stream, pu);

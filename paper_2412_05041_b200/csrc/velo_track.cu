@@ -571,7 +571,8 @@ int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   if (g == 0) {
     // two warps per event for mu = 5 sized events; more threads per event when the events are large
     const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
-    g = mean >= 6144u ? 128u : 64u;
+    g = mean >= 6144u ? 128u : mean < 768u ? 32u : 64u;
+    if (g == 32u && t == 0) t = 24;            // small events (open VELO): a warp per event, 24 in flight
   }
   if (g == 128) {
     if (t == 0) t = 6;
