@@ -149,46 +149,52 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
     __syncwarp();
     uint32_t nout = 0;
     if (ns > 0) {
-      // Once the seeds are known the histogram is dead: its shared memory takes the event's tracks
-      // (six words and the seed index each), so that the fit iterations touch no global memory. An
-      // event with more tracks than fit there reads them from global memory instead, in the same order.
-      const uint32_t stage_cap = (4u * nbw + 4u * nb) / 25u;
-      const bool resident = nt <= stage_cap;
-      float* sx = reinterpret_cast<float*>(hw);
-      float* sy = sx + stage_cap; float* stx = sy + stage_cap; float* sty = stx + stage_cap;
-      float* sz = sty + stage_cap; float* sw0 = sz + stage_cap;
-      uint8_t* sasg = reinterpret_cast<uint8_t*>(sw0 + stage_cap);
-      // P-3 every track to its nearest seed (ties to the lower seed)
-      for (uint32_t i = lane; i < nt; i += 32u) {
-        const float z = Z[t0 + i];
-        uint32_t best = 0; float bd = fabsf(__fsub_rn(z, zs[0]));
-        for (uint32_t v = 1; v < ns; ++v) { const float dd = fabsf(__fsub_rn(z, zs[v])); if (dd < bd) { bd = dd; best = v; } }
-        if (resident) {
+      // Once the seeds are known the histogram is dead. Fast path (the usual event): its shared memory
+      // takes, per seed, 8 x 32 partial sums (lane l's column is its own: no conflicts) and the vertex
+      // table, and the event's tracks (six words and the seed index each). One pass over the tracks
+      // per iteration then serves every vertex of the event: a track adds to the sums of its own seed,
+      // in the oracle's order (lane = track index mod 32, increasing index), and the fit iterations
+      // touch no global memory.
+      // With many tracks the sums of only R < ns seeds fit beside them: the seeds then go in rounds of R
+      // (they are independent of each other).
+      const uint32_t hist_bytes = 4u * nbw + 4u * nb;
+      const uint32_t room = hist_bytes > 25u * nt + 512u ? (hist_bytes - 25u * nt - 512u) / 1024u : 0u;
+      const uint32_t R = room < ns ? room : ns;                 // seeds per round
+      const bool fast = R >= 1u;
+      if (fast) {
+        float* acc = reinterpret_cast<float*>(hw);            // [seed of the round][sum][lane]
+        float* vt = acc + R * 256u;                             // [seed]{x, y, z, alive}
+        const uint32_t cap2 = (hist_bytes - R * 1024u - 512u) / 25u;
+        float* sx = vt + 128u;
+        float* sy = sx + cap2; float* stx = sy + cap2; float* sty = stx + cap2; float* sz = sty + cap2; float* sw0 = sz + cap2;
+        uint8_t* sasg = reinterpret_cast<uint8_t*>(sw0 + cap2);
+        float zs_mine = lane < ns ? zs[lane] : 0.0f;
+        __syncwarp();                                           // zs is read before the table below may overwrite nothing: zs lies beyond the histogram
+        for (uint32_t i = lane; i < nt; i += 32u) {             // P-3
+          const float z = Z[t0 + i];
+          uint32_t best = 0; float bd = fabsf(__fsub_rn(z, zs[0]));
+          for (uint32_t v = 1; v < ns; ++v) { const float dd = fabsf(__fsub_rn(z, zs[v])); if (dd < bd) { bd = dd; best = v; } }
           sasg[i] = (uint8_t)best;
           sx[i] = X[t0 + i]; sy[i] = Y[t0 + i]; stx[i] = TX[t0 + i]; sty[i] = TY[t0 + i]; sz[i] = z;
           sw0[i] = __fdiv_rn(1.0f, CXX[t0 + i]);
-        } else {
-          a.asg[t0 + i] = (uint8_t)best;
         }
-      }
-      __syncwarp();
-      const float* PX = resident ? sx : X + t0; const float* PY = resident ? sy : Y + t0;
-      const float* PTX = resident ? stx : TX + t0; const float* PTY = resident ? sty : TY + t0;
-      const float* PZ = resident ? sz : Z + t0; const float* PW = resident ? sw0 : CXX + t0;
-      const uint8_t* PA = resident ? sasg : a.asg + t0;
-      // P-4, P-5, P-6: lane l sums the tracks with i mod 32 == l in increasing i, butterfly combine
-      for (uint32_t v = 0; v < ns; ++v) {
-        float xv = 0.0f, yv = 0.0f, zv = zs[v], S0 = 0.0f;
-        uint32_t ntrk = 0; bool alive = true;
-        for (uint32_t it = 0; it < a.P.n_iterations && alive; ++it) {
-          float l0 = 0.0f, lx = 0.0f, ly = 0.0f, lxx = 0.0f, la = 0.0f, lb = 0.0f, lc = 0.0f, ln = 0.0f;
-          for (uint32_t i = lane; i < nt; i += 32u) {
-            if (PA[i] != v) continue;
-            const float x = PX[i], y = PY[i], tx = PTX[i], ty = PTY[i], z = PZ[i];
-            const float w0 = resident ? PW[i] : __fdiv_rn(1.0f, PW[i]);
-            const float dz = __fsub_rn(zv, z);
-            const float rx = __fsub_rn(__fadd_rn(x, __fmul_rn(tx, dz)), xv);
-            const float ry = __fsub_rn(__fadd_rn(y, __fmul_rn(ty, dz)), yv);
+        if (lane < ns) { vt[4u * lane] = 0.0f; vt[4u * lane + 1u] = 0.0f; vt[4u * lane + 2u] = zs_mine; vt[4u * lane + 3u] = 1.0f; }
+        float my_s0 = 0.0f; uint32_t my_n = 0;                  // lane v keeps seed v's last sums
+        __syncwarp();
+        for (uint32_t v0 = 0; v0 < ns; v0 += R) {
+        const uint32_t v1 = min(v0 + R, ns);
+        for (uint32_t it = 0; it < a.P.n_iterations; ++it) {
+          for (uint32_t j = lane; j < (v1 - v0) * 256u; j += 32u) acc[j] = 0.0f;
+          __syncwarp();
+          for (uint32_t i = lane; i < nt; i += 32u) {           // P-4 and the sums of P-5
+            const uint32_t v = sasg[i];
+            if (v < v0 || v >= v1) continue;
+            const float4 vx = *reinterpret_cast<const float4*>(vt + 4u * v);
+            if (vx.w == 0.0f) continue;
+            const float x = sx[i], y = sy[i], tx = stx[i], ty = sty[i], z = sz[i], w0 = sw0[i];
+            const float dz = __fsub_rn(vx.z, z);
+            const float rx = __fsub_rn(__fadd_rn(x, __fmul_rn(tx, dz)), vx.x);
+            const float ry = __fsub_rn(__fadd_rn(y, __fmul_rn(ty, dz)), vx.y);
             const float c = __fmul_rn(w0, __fadd_rn(__fmul_rn(rx, rx), __fmul_rn(ry, ry)));
             float wt = 0.0f;
             if (c < a.P.chi2_max) { const float u = __fsub_rn(1.0f, __fdiv_rn(c, a.P.chi2_max)); wt = __fmul_rn(u, u); }
@@ -196,30 +202,122 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
             const float aa = __fsub_rn(x, __fmul_rn(tx, z)), bb = __fsub_rn(y, __fmul_rn(ty, z));
             const float t2 = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
             const float ab = __fadd_rn(__fmul_rn(tx, aa), __fmul_rn(ty, bb));
-            l0 = __fadd_rn(l0, w);
-            lx = __fadd_rn(lx, __fmul_rn(w, tx)); ly = __fadd_rn(ly, __fmul_rn(w, ty));
-            lxx = __fadd_rn(lxx, __fmul_rn(w, t2));
-            la = __fadd_rn(la, __fmul_rn(w, aa)); lb = __fadd_rn(lb, __fmul_rn(w, bb));
-            lc = __fadd_rn(lc, __fmul_rn(w, ab));
-            if (wt > 0.0f) ln = __fadd_rn(ln, 1.0f);
+            float* q = acc + (v - v0) * 256u + lane;
+            q[0] = __fadd_rn(q[0], w);
+            q[32] = __fadd_rn(q[32], __fmul_rn(w, tx)); q[64] = __fadd_rn(q[64], __fmul_rn(w, ty));
+            q[96] = __fadd_rn(q[96], __fmul_rn(w, t2));
+            q[128] = __fadd_rn(q[128], __fmul_rn(w, aa)); q[160] = __fadd_rn(q[160], __fmul_rn(w, bb));
+            q[192] = __fadd_rn(q[192], __fmul_rn(w, ab));
+            if (wt > 0.0f) q[224] = __fadd_rn(q[224], 1.0f);
           }
-          S0 = warp_butterfly(l0);
-          const float Sx = warp_butterfly(lx), Sy = warp_butterfly(ly), Sxx = warp_butterfly(lxx);
-          const float A = warp_butterfly(la), B = warp_butterfly(lb), C = warp_butterfly(lc);
-          ntrk = (uint32_t)warp_butterfly(ln);
-          if (!(S0 > 0.0f)) { alive = false; break; }
-          const float den = __fsub_rn(Sxx, __fdiv_rn(__fadd_rn(__fmul_rn(Sx, Sx), __fmul_rn(Sy, Sy)), S0));
-          if (!(den > 0.0f)) { alive = false; break; }
-          zv = __fdiv_rn(__fsub_rn(__fdiv_rn(__fadd_rn(__fmul_rn(Sx, A), __fmul_rn(Sy, B)), S0), C), den);
-          xv = __fdiv_rn(__fadd_rn(A, __fmul_rn(Sx, zv)), S0);
-          yv = __fdiv_rn(__fadd_rn(B, __fmul_rn(Sy, zv)), S0);
+          __syncwarp();
+          for (uint32_t v = v0; v < v1; ++v) {                  // the rest of P-5, vertex by vertex
+            if (vt[4u * v + 3u] == 0.0f) continue;
+            const float* q = acc + (v - v0) * 256u + lane;
+            const float S0 = warp_butterfly(q[0]);
+            const float Sx = warp_butterfly(q[32]), Sy = warp_butterfly(q[64]), Sxx = warp_butterfly(q[96]);
+            const float A = warp_butterfly(q[128]), B = warp_butterfly(q[160]), C = warp_butterfly(q[192]);
+            const uint32_t ntrk = (uint32_t)warp_butterfly(q[224]);
+            if (lane == v) { my_s0 = S0; my_n = ntrk; }
+            bool alive = S0 > 0.0f;
+            float den = 0.0f;
+            if (alive) { den = __fsub_rn(Sxx, __fdiv_rn(__fadd_rn(__fmul_rn(Sx, Sx), __fmul_rn(Sy, Sy)), S0)); alive = den > 0.0f; }
+            __syncwarp();
+            if (!alive) { if (lane == 0) vt[4u * v + 3u] = 0.0f; }
+            else {
+              const float zv = __fdiv_rn(__fsub_rn(__fdiv_rn(__fadd_rn(__fmul_rn(Sx, A), __fmul_rn(Sy, B)), S0), C), den);
+              const float xv = __fdiv_rn(__fadd_rn(A, __fmul_rn(Sx, zv)), S0);
+              const float yv = __fdiv_rn(__fadd_rn(B, __fmul_rn(Sy, zv)), S0);
+              if (lane == 0) { vt[4u * v] = xv; vt[4u * v + 1u] = yv; vt[4u * v + 2u] = zv; }
+            }
+          }
+          __syncwarp();
         }
-        if (alive && ntrk >= a.P.min_tracks) {
-          if (lane == 0) {
-            float* o = a.tmp_pv + ((size_t)e * kPvMax + nout) * 5u;
-            o[0] = xv; o[1] = yv; o[2] = zv; o[3] = S0; o[4] = __uint_as_float(ntrk);
+        }
+        for (uint32_t v = 0; v < ns; ++v) {                     // P-6
+          const float s0v = __shfl_sync(0xffffffffu, my_s0, v);
+          const uint32_t nv = __shfl_sync(0xffffffffu, my_n, v);
+          if (vt[4u * v + 3u] != 0.0f && nv >= a.P.min_tracks) {
+            if (lane == 0) {
+              float* o = a.tmp_pv + ((size_t)e * kPvMax + nout) * 5u;
+              o[0] = vt[4u * v]; o[1] = vt[4u * v + 1u]; o[2] = vt[4u * v + 2u]; o[3] = s0v; o[4] = __uint_as_float(nv);
+            }
+            ++nout;
           }
-          ++nout;
+        }
+      } else {
+      // Once the seeds are known the histogram is dead: its shared memory takes the event's tracks
+        // (six words and the seed index each), so that the fit iterations touch no global memory. An
+        // event with more tracks than fit there reads them from global memory instead, in the same order.
+        const uint32_t stage_cap = (4u * nbw + 4u * nb) / 25u;
+        const bool resident = nt <= stage_cap;
+        float* sx = reinterpret_cast<float*>(hw);
+        float* sy = sx + stage_cap; float* stx = sy + stage_cap; float* sty = stx + stage_cap;
+        float* sz = sty + stage_cap; float* sw0 = sz + stage_cap;
+        uint8_t* sasg = reinterpret_cast<uint8_t*>(sw0 + stage_cap);
+        // P-3 every track to its nearest seed (ties to the lower seed)
+        for (uint32_t i = lane; i < nt; i += 32u) {
+          const float z = Z[t0 + i];
+          uint32_t best = 0; float bd = fabsf(__fsub_rn(z, zs[0]));
+          for (uint32_t v = 1; v < ns; ++v) { const float dd = fabsf(__fsub_rn(z, zs[v])); if (dd < bd) { bd = dd; best = v; } }
+          if (resident) {
+            sasg[i] = (uint8_t)best;
+            sx[i] = X[t0 + i]; sy[i] = Y[t0 + i]; stx[i] = TX[t0 + i]; sty[i] = TY[t0 + i]; sz[i] = z;
+            sw0[i] = __fdiv_rn(1.0f, CXX[t0 + i]);
+          } else {
+            a.asg[t0 + i] = (uint8_t)best;
+          }
+        }
+        __syncwarp();
+        const float* PX = resident ? sx : X + t0; const float* PY = resident ? sy : Y + t0;
+        const float* PTX = resident ? stx : TX + t0; const float* PTY = resident ? sty : TY + t0;
+        const float* PZ = resident ? sz : Z + t0; const float* PW = resident ? sw0 : CXX + t0;
+        const uint8_t* PA = resident ? sasg : a.asg + t0;
+        // P-4, P-5, P-6: lane l sums the tracks with i mod 32 == l in increasing i, butterfly combine
+        for (uint32_t v = 0; v < ns; ++v) {
+          float xv = 0.0f, yv = 0.0f, zv = zs[v], S0 = 0.0f;
+          uint32_t ntrk = 0; bool alive = true;
+          for (uint32_t it = 0; it < a.P.n_iterations && alive; ++it) {
+            float l0 = 0.0f, lx = 0.0f, ly = 0.0f, lxx = 0.0f, la = 0.0f, lb = 0.0f, lc = 0.0f, ln = 0.0f;
+            for (uint32_t i = lane; i < nt; i += 32u) {
+              if (PA[i] != v) continue;
+              const float x = PX[i], y = PY[i], tx = PTX[i], ty = PTY[i], z = PZ[i];
+              const float w0 = resident ? PW[i] : __fdiv_rn(1.0f, PW[i]);
+              const float dz = __fsub_rn(zv, z);
+              const float rx = __fsub_rn(__fadd_rn(x, __fmul_rn(tx, dz)), xv);
+              const float ry = __fsub_rn(__fadd_rn(y, __fmul_rn(ty, dz)), yv);
+              const float c = __fmul_rn(w0, __fadd_rn(__fmul_rn(rx, rx), __fmul_rn(ry, ry)));
+              float wt = 0.0f;
+              if (c < a.P.chi2_max) { const float u = __fsub_rn(1.0f, __fdiv_rn(c, a.P.chi2_max)); wt = __fmul_rn(u, u); }
+              const float w = __fmul_rn(w0, wt);
+              const float aa = __fsub_rn(x, __fmul_rn(tx, z)), bb = __fsub_rn(y, __fmul_rn(ty, z));
+              const float t2 = __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty));
+              const float ab = __fadd_rn(__fmul_rn(tx, aa), __fmul_rn(ty, bb));
+              l0 = __fadd_rn(l0, w);
+              lx = __fadd_rn(lx, __fmul_rn(w, tx)); ly = __fadd_rn(ly, __fmul_rn(w, ty));
+              lxx = __fadd_rn(lxx, __fmul_rn(w, t2));
+              la = __fadd_rn(la, __fmul_rn(w, aa)); lb = __fadd_rn(lb, __fmul_rn(w, bb));
+              lc = __fadd_rn(lc, __fmul_rn(w, ab));
+              if (wt > 0.0f) ln = __fadd_rn(ln, 1.0f);
+            }
+            S0 = warp_butterfly(l0);
+            const float Sx = warp_butterfly(lx), Sy = warp_butterfly(ly), Sxx = warp_butterfly(lxx);
+            const float A = warp_butterfly(la), B = warp_butterfly(lb), C = warp_butterfly(lc);
+            ntrk = (uint32_t)warp_butterfly(ln);
+            if (!(S0 > 0.0f)) { alive = false; break; }
+            const float den = __fsub_rn(Sxx, __fdiv_rn(__fadd_rn(__fmul_rn(Sx, Sx), __fmul_rn(Sy, Sy)), S0));
+            if (!(den > 0.0f)) { alive = false; break; }
+            zv = __fdiv_rn(__fsub_rn(__fdiv_rn(__fadd_rn(__fmul_rn(Sx, A), __fmul_rn(Sy, B)), S0), C), den);
+            xv = __fdiv_rn(__fadd_rn(A, __fmul_rn(Sx, zv)), S0);
+            yv = __fdiv_rn(__fadd_rn(B, __fmul_rn(Sy, zv)), S0);
+          }
+          if (alive && ntrk >= a.P.min_tracks) {
+            if (lane == 0) {
+              float* o = a.tmp_pv + ((size_t)e * kPvMax + nout) * 5u;
+              o[0] = xv; o[1] = yv; o[2] = zv; o[3] = S0; o[4] = __uint_as_float(ntrk);
+            }
+            ++nout;
+          }
         }
       }
     }
