@@ -112,8 +112,9 @@ typedef struct {
   uint32_t cap_tracks, cap_track_hits;
   uint32_t* summary;             /* u32[VELO_N_SUMMARY]: n_tracks, n_track_hits, status (VELO_OK  */
                                  /* or a negative code as two's complement), n_candidates (before */
-                                 /* the filters), n_deferred (events the team kernel handed to    */
-                                 /* the general slab kernel), then three reserved zeros           */
+                                 /* the filters), n_deferred (events the pipeline handed to the   */
+                                 /* general slab kernel), n_big (events above 12 000 hits, run in  */
+                                 /* the one-event-per-CTA pipeline), then two reserved zeros      */
 } velo_tracks_t;
 /* If the batch needs more than cap_tracks tracks or cap_track_hits track-hits, summary[2] =
  * VELO_ERR_CAPACITY, summary[0..1] hold the REQUIRED sizes and the other output arrays are
