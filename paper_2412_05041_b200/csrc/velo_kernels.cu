@@ -1,10 +1,14 @@
-// velo_kernels.cu — sm_100a kernels of the VELO hot path (SURVEY.md §8(a) S0 ... S7).
+// velo_kernels.cu — the general kernel of the VELO hot path and the small kernels between the stages
+// of the pipeline (sm_100a; SURVEY.md §8(a) S0 ... S7).
 //
-// One CTA reconstructs one event at a time: S0 decode (phi16, bucket key), S1 phi sort, the
-// 24-step module loop with S3 forwarding and S2 search-by-triplet seeding, S4 ghost filter, S5
-// straight-line fit, S6 clone filter, then writes its surviving tracks into a temp block
-// allocated with one atomic per event. A scan kernel turns the per-event counts into
-// offsets and a copy kernel moves the temp blocks into event order (S7).
+// velo_event_slab_kernel: one CTA reconstructs one event at a time with every per-event array in a
+// slab in global memory: S0 decode (phi16, bucket key), S1 phi sort, the 24-step module loop with S3
+// forwarding and S2 search-by-triplet seeding, S4 ghost filter, S5 straight-line fit, S6 clone filter,
+// then writes its surviving tracks into a temp block allocated with one atomic per event (the write
+// kernel of velo_fit.cu moves it into place). It takes any legal input and the events the three-stage
+// pipeline (velo_sort.cu, velo_track.cu, velo_fit.cu) gives up. Also here: velo_order_kernel (the
+// order in which stages 2 and 3 take the events), velo_big_order_kernel, velo_offsets_kernel (S7:
+// counts -> offsets), the workspace layout and the launch sequence of a batch.
 // Step semantics: SURVEY.md §8(c) O-1 ... O-14 (restated in DESIGN.md §2); the paper itself
 // (§5) names the objects but gives no step.
 #include "velo_device.cuh"
@@ -15,7 +19,7 @@ namespace velo {
 namespace {
 
 constexpr int kThreads = 256;            // CTA size of the slab kernel when it takes every event of a batch
-constexpr int kThreadsLarge = 1024;      // ... and when it takes the events the team kernel deferred: those are
+constexpr int kThreadsLarge = 1024;      // ... and when it takes the events the pipeline deferred: those are
                                          // the large ones, and a batch waits for the latency of its largest event
 constexpr unsigned kInactive = 255u;     // tmiss value of a track that stopped forwarding
 
@@ -334,7 +338,7 @@ __device__ void process_event(const KernelArgs& a, const Ev& ev, Shared& sh, uin
 // ---- event kernel, slab variant: persistent CTAs pull events from a ticket counter -------------
 // from_list = 0: every event of the batch; 1: the events the shared-memory kernel deferred (ws.large_list).
 // kBinsInSlab: the bucket table lives in the slab too, so that the CTA needs almost no shared memory
-// and fits beside the team kernel of the next batch (the usual case: nothing was deferred).
+// and fits beside the pipeline kernels of the next batch (the usual case: nothing was deferred).
 template <int kCta, bool kBinsInSlab, int kShift>
 __global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs a, const int from_list) {
   static_assert(!kBinsInSlab || kShift == kBinShift, "the slab's bucket table is sized for the default buckets");
@@ -362,13 +366,13 @@ __global__ void __launch_bounds__(kCta) velo_event_slab_kernel(const KernelArgs 
   }
 }
 
-// ---- processing order for the team kernel: event ids by ascending size class --------------------
-// Events of a batch differ in size by more than 10x. The team kernel hands out the sorted list
+// ---- processing order for stages 2 and 3: event ids by ascending size class ------------------------
+// Events of a batch differ in size by more than 10x. Stages 2 and 3 hand out the sorted list
 // from both ends in turn (largest, smallest, second largest, ...), so the handful of events that
 // share an SM's shared memory at any time add up to about the same bytes and the pool neither
 // overflows (teams waiting for memory) nor sits half empty. Counting sort by n_hits / 64, one CTA.
 // The order only schedules: results and their placement do not depend on it.
-constexpr uint32_t kSizeClasses = 256;   // with the scan scratch: 1.2 KB of shared memory, it fits beside the team kernel
+constexpr uint32_t kSizeClasses = 256;   // with the scan scratch: 1.2 KB of shared memory
 __global__ void __launch_bounds__(512) velo_order_kernel(const KernelArgs a) {
   __shared__ uint32_t hist[kSizeClasses];
   __shared__ uint32_t wsum[32];
@@ -403,7 +407,7 @@ __global__ void __launch_bounds__(512) velo_order_kernel(const KernelArgs a) {
 }
 
 // ---- S7 part 2: exclusive scans of the per-event counts (one CTA) ------------------------------
-// 256 threads and few registers: it fits beside the team kernel of the next batch.
+// 256 threads and few registers: it fits beside the pipeline kernels of the next batch.
 __global__ void __launch_bounds__(256) velo_offsets_kernel(const KernelArgs a) {
   __shared__ unsigned long long warp_sums[33];
   const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;

@@ -78,7 +78,7 @@ def test_run_to_run_determinism(velo):
 
 
 # ---- the event kernels: the three-stage pipeline (default) in several launch geometries, the general
-# slab kernel on its own, and the round-1 team kernel --------------------------------------------------
+# slab kernel on its own ------------------------------------------------------------------------------
 @pytest.mark.parametrize("kw", [
     {"path": 1},                                                  # general slab kernel only
     {"track_group": 32, "track_teams": 8}, {"track_group": 32, "track_teams": 24},
@@ -122,7 +122,7 @@ def test_hand_made_pin_events(velo):
 
 
 def test_hits_off_their_module_plane_are_deferred_to_the_general_kernel(velo):
-    """The team kernel requires z == module_z[module]; events that break it take the slab kernel
+    """The pipeline requires z == module_z[module]; events that break it take the slab kernel
     inside the same call, and the batch result is still the oracle's."""
     d = datagen.generate_config(0, n_events=40)
     z = d["z"].copy()
