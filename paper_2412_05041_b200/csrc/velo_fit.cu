@@ -340,6 +340,10 @@ __global__ void __launch_bounds__(G, 1) velo_fit_big_kernel(const KernelArgs a) 
 // creation order, so a running count over them is the track's place inside the event.
 template <int kMinBlocks>
 __global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const KernelArgs a) {
+  // the hit lists of 32 candidates at a time go through shared memory, so that the warp writes
+  // track_hits as whole sectors instead of 32 scattered words per store
+  __shared__ uint32_t stage_all[4][32 * VELO_MAX_MODULES];
+  uint32_t* stage = stage_all[threadIdx.x >> 5];
   const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t tot_t = a.event_track_offsets[a.n_events], tot_h = a.ws.ev_hit_base[a.n_events];
@@ -391,19 +395,25 @@ __global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const Kerne
 #pragma unroll
       for (int d = 1; d < 32; d <<= 1) { const uint32_t o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= (uint32_t)d) inc += o; }
       const uint32_t lt = run_t + (uint32_t)__popc(b & ((1u << lane) - 1u)), lh = run_h + inc - nh;
-      run_t += (uint32_t)__popc(b); run_h += __shfl_sync(0xffffffffu, inc, 31);
-      if (!surv) continue;
-      float s9[9];
+      const uint32_t pass_h = __shfl_sync(0xffffffffu, inc, 31), pass_base = run_h;
+      run_t += (uint32_t)__popc(b); run_h += pass_h;
+      if (surv) {
+        float s9[9];
 #pragma unroll
-      for (uint32_t k = 0; k < 9; ++k) s9[k] = cfit[k * cc + t];
-      float* dst_s = a.states + dst_t + lt;
-      dst_s[0] = s9[0]; dst_s[cs] = s9[1]; dst_s[2 * cs] = s9[2]; dst_s[3 * cs] = s9[3]; dst_s[4 * cs] = s9[4];
-      dst_s[5 * cs] = s9[5]; dst_s[6 * cs] = s9[6]; dst_s[7 * cs] = s9[7];
-      dst_s[8 * cs] = s9[5]; dst_s[9 * cs] = s9[6]; dst_s[10 * cs] = s9[7];
-      dst_s[11 * cs] = s9[8]; dst_s[12 * cs] = __uint_as_float(nh);
-      a.track_hit_offsets[dst_t + lt] = dst_h + lh;
-      uint32_t* dst = a.track_hits + dst_h + lh;
-      for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) { dst[i] = o0 + orig[h]; });
+        for (uint32_t k = 0; k < 9; ++k) s9[k] = cfit[k * cc + t];
+        float* dst_s = a.states + dst_t + lt;
+        dst_s[0] = s9[0]; dst_s[cs] = s9[1]; dst_s[2 * cs] = s9[2]; dst_s[3 * cs] = s9[3]; dst_s[4 * cs] = s9[4];
+        dst_s[5 * cs] = s9[5]; dst_s[6 * cs] = s9[6]; dst_s[7 * cs] = s9[7];
+        dst_s[8 * cs] = s9[5]; dst_s[9 * cs] = s9[6]; dst_s[10 * cs] = s9[7];
+        dst_s[11 * cs] = s9[8]; dst_s[12 * cs] = __uint_as_float(nh);
+        a.track_hit_offsets[dst_t + lt] = dst_h + lh;
+        uint32_t* st = stage + (lh - pass_base);
+        for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) { st[i] = o0 + orig[h]; });
+      }
+      __syncwarp();
+      uint32_t* dst = a.track_hits + dst_h + pass_base;
+      for (uint32_t k = lane; k < pass_h; k += 32u) dst[k] = stage[k];
+      __syncwarp();
     }
   }
 }
