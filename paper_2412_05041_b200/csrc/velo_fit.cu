@@ -220,24 +220,26 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
               (unsigned long long)centre;
 #pragma unroll
     for (uint32_t k = 0; k < 9; ++k) cfit[k * cs + t] = s9[k];
+    // O-13 owners, step 1: every passing candidate writes its id on its hits (plain stores: where
+    // several share a hit, any one of them lands)
+    for_hits(rows + t * 32u, nh, [&](uint32_t, uint32_t h) { own[h] = t; });
   }
   team_sync<G>(team);
   VELO_PH(a.ws.phase_clk, ts, 35);
   // ---- O-13 owners: owner[h] = the candidate with the smallest key among those that contain h ----
-  // Step 1: every passing candidate writes its id on its hits (plain stores: where several share a
-  // hit, any one of them lands). Step 2: a candidate that finds another id on one of its hits
-  // settles it with a compare-and-swap on the 64-bit keys. Hits are shared rarely, so the common
-  // path has no atomics.
-  for (uint32_t t = tid; t < nt; t += G) {
-    if (!tstate[t]) continue;
-    for_hits(rows + t * 32u, (uint32_t)__popc(tmask[t]), [&](uint32_t, uint32_t h) { own[h] = t; });
-  }
-  team_sync<G>(team);
+  // Step 2: a candidate that finds another id on one of its hits settles it with a compare-and-swap
+  // on the 64-bit keys. Hits are shared rarely, so the common path has no atomics.
   VELO_PH(a.ws.phase_clk, ts, 36);
   for (uint32_t t = tid; t < nt; t += G) {
     if (!tstate[t]) continue;
+    // first look at all hits at once (independent loads): most candidates own every hit of theirs
+    const uint32_t nh = (uint32_t)__popc(tmask[t]);
+    uint32_t contested = 0;
+    for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) { contested |= (own[h] != t) ? (1u << i) : 0u; });
+    if (!contested) continue;
     const unsigned long long key = tkey[t];
-    for_hits(rows + t * 32u, (uint32_t)__popc(tmask[t]), [&](uint32_t, uint32_t h) {
+    for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) {
+      if (!((contested >> i) & 1u)) return;
       uint32_t old = *(volatile uint32_t*)&own[h];
       while (old != t && key < tkey[old]) {
         const uint32_t seen = atomicCAS(&own[h], old, t);
