@@ -88,6 +88,24 @@ def test_kalman_equals_generalised_least_squares_with_scattering():
     assert abs(k[0] - want[0]) < 5e-2 * abs(dzb) * 1e-3 + 1e-2 and abs(k[1] - want[1]) < 5e-2 * abs(dzb) * 1e-3 + 1e-2
 
 
+def test_kalman_noise_scales_with_the_path_length_through_a_plane():
+    """K-1: theta2 = ms_theta2 * (1 + tx^2 + ty^2). A steep track (tx = 0.3, ty = 0.2: factor 1.13) against
+    the same generalised-least-squares solve with the scaled kick variance; the unscaled one is 13 % off."""
+    rng = np.random.default_rng(12)
+    th2 = 4.0e-6
+    mods = [18, 17, 16, 15, 14, 13, 12]
+    hz = np.array([Z[m] for m in mods], np.float64)
+    hx = (1.0 + 0.3 * hz + rng.normal(0, 0.05, len(mods))).astype(np.float32)
+    hy = (-2.0 + 0.2 * hz + rng.normal(0, 0.05, len(mods))).astype(np.float32)
+    k = oracle.kalman(hx, hy, hz.astype(np.float32), SIG, th2)
+    s2 = float(np.float32(SIG) * np.float32(SIG))
+    scaled = th2 * (1 + 0.3 ** 2 + 0.2 ** 2)
+    _, C = _gls(hx.astype(np.float64), hz, s2, scaled)
+    _, C0 = _gls(hx.astype(np.float64), hz, s2, th2)
+    assert k[7] == pytest.approx(C[1, 1] + scaled, rel=5e-3)          # ctxtx with the last plane's noise (K-5)
+    assert abs(k[7] - (C0[1, 1] + th2)) > 0.05 * k[7]                  # ... and not the unscaled model
+
+
 def test_kalman_one_scatterer_hand_case():
     """Three hits at z = 50, 25, 0 on x = 0, 0, 1 (y = 0), sigma^2 = s2, kick variance q at the middle
     plane. By hand: two-point start at z = 25: x = 0, t = 0, P = s2 [[1, -1/25], [-1/25, 2/625]];
@@ -207,6 +225,22 @@ def test_pv_two_vertices_and_too_few_tracks():
     # an empty event and an event without tracks near each other
     r = oracle.pv_find(np.array([0, 0, 22, 22], np.uint32), st)
     np.testing.assert_array_equal(r["event_pv_offsets"], [0, 0, 2, 2])
+
+
+def test_pv_track_midway_between_two_seeds_goes_to_the_lower_one():
+    """P-3 tie: seeds at z = 10.125 and 12.125 (bin centres, 8 bins apart); a shallow track whose closest
+    approach is at z = 11.125 exactly is 1.0 from both and joins the LOWER seed: 7 and 6 tracks."""
+    rng = np.random.default_rng(6)
+    sl = lambda n: np.stack([rng.uniform(0.05, 0.2, n) * rng.choice([-1, 1], n), rng.uniform(0.05, 0.2, n)], axis=1)
+    st = _states_from_lines([(0.0, 0.0, 10.125)] * 6 + [(0.0, 0.0, 12.125)] * 6, sl(12))
+    mid = np.zeros((13, 1), np.float32)
+    mid[:6, 0] = [0.0, 0.0, 0.005, 0.003, 11.125, 4e-4]             # x, y, tx, ty, z, cxx: 6 um from either vertex
+    st = np.concatenate([st, mid], axis=1)
+    assert abs(np.float32(11.125) - np.float32(10.125)) == abs(np.float32(11.125) - np.float32(12.125))
+    r = oracle.pv_find(np.array([0, 13], np.uint32), st)
+    assert r["n_pvs"] == 2
+    np.testing.assert_allclose(r["pvs"][2], [10.125, 12.125], atol=2e-2)
+    np.testing.assert_array_equal(r["pvs"][4].view(np.uint32), [7, 6])
 
 
 def test_pv_one_iteration_is_a_weighted_least_squares_solve():
