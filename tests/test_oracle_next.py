@@ -105,6 +105,25 @@ def test_kalman_noise_scales_with_the_path_length_through_a_plane():
     assert k[7] == pytest.approx(C[1, 1] + scaled, rel=5e-3)          # ctxtx with the last plane's noise (K-5)
     assert abs(k[7] - (C0[1, 1] + th2)) > 0.05 * k[7]                  # ... and not the unscaled model
 
+    # the kicks inside the filter (K-4) carry the factor too: chi2 = the generalised-least-squares
+    # residual form (y - H b)^T V^-1 (y - H b) summed over x and y, which scales with 1 / theta2 here
+    def gls_chi2(t2):
+        tot = 0.0
+        for h in (hx, hy):
+            y = h.astype(np.float64); n = len(y); L = n - 1
+            H = np.stack([np.ones(n), hz - hz[L]], axis=1)
+            V = np.eye(n) * s2
+            for a_ in range(n):
+                for b_ in range(n):
+                    V[a_, b_] += t2 * sum((hz[j] - hz[a_]) * (hz[j] - hz[b_]) for j in range(max(a_, b_) + 1, L))
+            Vi = np.linalg.inv(V)
+            beta = np.linalg.inv(H.T @ Vi @ H) @ H.T @ Vi @ y
+            r = y - H @ beta
+            tot += float(r @ Vi @ r)
+        return tot
+    assert k[11] == pytest.approx(gls_chi2(scaled), rel=5e-3)
+    assert abs(k[11] - gls_chi2(th2)) > 0.05 * k[11]
+
 
 def test_kalman_one_scatterer_hand_case():
     """Three hits at z = 50, 25, 0 on x = 0, 0, 1 (y = 0), sigma^2 = s2, kick variance q at the middle
