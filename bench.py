@@ -158,7 +158,22 @@ def time_oracle(d: dict, n_events: int) -> tuple[float, int]:
     r = oracle.reconstruct(d["x"][:h1], d["y"][:h1], d["z"][:h1], d["module"][:h1], off[:n_events + 1], N_MODULES)
     dt = time.perf_counter() - t0
     assert r["status"] == 0
+    time_oracle.last_result = r
     return dt, h1 - int(off[0])
+
+
+def time_oracle_after_path(d: dict, n_events: int) -> dict:
+    """The oracle's Kalman filter and vertex finder (oracle/velo_next_oracle.c) on the tracks of the last
+    time_oracle() call: seconds for the sample, one thread."""
+    import oracle
+    r = time_oracle.last_result
+    h1 = int(d["event_offsets"][n_events])
+    t0 = time.perf_counter()
+    oracle.kalman_tracks(r, d["x"][:h1], d["y"][:h1], d["z"][:h1], oracle.default_params().sigma_hit)
+    t1 = time.perf_counter()
+    pv = oracle.pv_find(r["event_track_offsets"], r["states"])
+    t2 = time.perf_counter()
+    return {"kalman_s": t1 - t0, "pv_s": t2 - t1, "n_pvs": pv["n_pvs"], "events": n_events}
 
 
 def run_reference(args):
@@ -529,6 +544,12 @@ def run_velo(args):
         line["cpu_baseline"] = {"value": sample / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "hits_per_s": nh / dt, "host_cores_available": os.cpu_count(),
                                 "sample": f"first {sample} events of the workload, median of 3 passes, {dt:.1f} s each"}
+        ap = time_oracle_after_path(d, sample)
+        line["after_path"]["cpu_oracle"] = {"kalman_events_per_s": sample / ap["kalman_s"], "pv_events_per_s": sample / ap["pv_s"],
+                                            "cores": 1, "sample": f"the same {sample} events"}
+        per_batch = n_events / n_batches
+        line["after_path"]["kalman_events_per_s"] = per_batch / (line["after_path"]["kalman_ms_per_launch"] * 1e-3)
+        line["after_path"]["pv_events_per_s"] = per_batch / (line["after_path"]["pv_ms_per_launch"] * 1e-3)
 
     # -- the small- and large-event regimes: short legs on configs[3] and configs[4] (device-resident) --
     if args.config == 2 and not args.events and not args.no_other_workloads and world == 1:
