@@ -38,7 +38,7 @@ class _CConfig(ctypes.Structure):
         ("sigma_vxy", ctypes.c_double), ("sigma_vz", ctypes.c_double),
         ("hit_eff", ctypes.c_double), ("noise_frac", ctypes.c_double), ("ms_sigma", ctypes.c_double),
         ("quantise", ctypes.c_int32), ("shuffle", ctypes.c_int32),
-        ("backward_frac", ctypes.c_double),
+        ("backward_frac", ctypes.c_double), ("stagger_z", ctypes.c_double), ("overlap_x", ctypes.c_double),
     ]
 
 
@@ -62,6 +62,8 @@ class GenConfig:
     quantise: bool = True
     shuffle: bool = True
     backward_frac: float = 0.0   # tracks towards -z (none in BASELINE's configs)
+    stagger_z: float = 0.0       # §8(f) f4, 52-sensor layout: the two sensors of a station at z -+ stagger_z/2 ...
+    overlap_x: float = 0.0       # ... both reaching this far over x = 0 (0, 0 in BASELINE's configs)
     r_in: float = R_IN
     r_out: float = R_OUT
     pitch: float = PITCH
@@ -115,7 +117,8 @@ def _cconfig(cfg: GenConfig) -> _CConfig:
         mu=cfg.mu, trk_mean=cfg.trk_mean, mult_lo=cfg.mult_lo, mult_hi=cfg.mult_hi,
         eta_lo=cfg.eta_lo, eta_hi=cfg.eta_hi, sigma_vxy=cfg.sigma_vxy, sigma_vz=cfg.sigma_vz,
         hit_eff=cfg.hit_eff, noise_frac=cfg.noise_frac, ms_sigma=cfg.ms_sigma,
-        quantise=int(cfg.quantise), shuffle=int(cfg.shuffle), backward_frac=cfg.backward_frac)
+        quantise=int(cfg.quantise), shuffle=int(cfg.shuffle), backward_frac=cfg.backward_frac,
+        stagger_z=cfg.stagger_z, overlap_x=cfg.overlap_x)
 
 
 def _ptr(a):

@@ -36,6 +36,8 @@ typedef struct {
   int32_t quantise;       // 1: snap to pixel centres and merge same-pixel hits (A19)
   int32_t shuffle;        // 1: Fisher-Yates shuffle of the event's hits (A16)
   double backward_frac;   // fraction of tracks that leave the vertex towards -z (eta -> -eta; A23); 0 in BASELINE's configs
+  double stagger_z;       // 52-sensor layout: the -x sensor of a station sits at z - stagger_z/2, the +x one at z + stagger_z/2
+  double overlap_x;       // ... and both reach this far over the x = 0 line (a track in the strip crosses both); 0, 0 in BASELINE's configs
 } velogen_config_t;
 
 }  // extern "C"
@@ -96,7 +98,7 @@ inline uint64_t pixel_key(uint32_t m, int h, long ix, long iy) {
 // Record one crossing (local coordinates xl, y in half h of module m). Returns true if a new
 // hit was stored (false: pixel already hit, A19).
 bool record(const velogen_config_t& c, const double* mz, EventBuf& b, uint32_t m, int h, double xl, double y,
-            int32_t track) {
+            int32_t track, double z_sensor = 1e300) {
   double xo = xl, yo = y;
   if (c.quantise) {
     long ix = (long)std::floor(xl / c.pitch), iy = (long)std::floor(y / c.pitch);
@@ -115,7 +117,7 @@ bool record(const velogen_config_t& c, const double* mz, EventBuf& b, uint32_t m
   }
   hit.x = (float)(xo + (double)h * c.half_shift_x);
   hit.y = (float)yo;
-  hit.z = (float)mz[m];
+  hit.z = (float)(z_sensor < 1e299 ? z_sensor : mz[m]);
   hit.module = (uint8_t)m;
   hit.track = track;
   b.hits.push_back(hit);
@@ -152,7 +154,33 @@ void gen_event(const velogen_config_t& c, const double* mz, uint64_t e, EventBuf
       // a backward track crosses the modules below the vertex, nearest first (no extra random number
       // is drawn when backward_frac is 0, so BASELINE's configs are unchanged)
       const bool back = c.backward_frac > 0.0 && rng.uniform() < c.backward_frac;
-      for (uint32_t mm = 0; mm < M; ++mm) {
+      const bool sensors52 = c.stagger_z != 0.0 || c.overlap_x != 0.0;
+      for (uint32_t mm = 0; sensors52 && mm < M; ++mm) {
+        // 52-sensor layout: the two sensors of a station are planes of their own, crossed in z order;
+        // a track inside the overlap strip leaves a hit on both
+        const uint32_t m = back ? M - 1 - mm : mm;
+        for (int hh = 0; hh < 2; ++hh) {
+          const int h = (back ? (hh == 0) : (hh != 0)) ? 1 : -1;       // forward: -x sensor (lower z) first
+          const double zs = mz[m] + 0.5 * (double)h * c.stagger_z;
+          if (back ? !(zs < zv) : !(zs > zv)) continue;
+          x += tx * (zs - zp);
+          y += ty * (zs - zp);
+          zp = zs;
+          const double xl = x - (double)h * c.half_shift_x;
+          const bool in_half = (h < 0) ? (xl < c.overlap_x) : (xl >= -c.overlap_x);
+          if (!in_half) continue;
+          const double r = std::sqrt(xl * xl + y * y);
+          if (r < c.r_in || r > c.r_out) continue;
+          if (rng.uniform() < c.hit_eff) {
+            if (record(c, mz, b, m, h, xl, y, tid, zs)) signal_on_module[m]++;
+          }
+          if (c.ms_sigma > 0.0) {
+            tx += c.ms_sigma * rng.normal();
+            ty += c.ms_sigma * rng.normal();
+          }
+        }
+      }
+      for (uint32_t mm = 0; !sensors52 && mm < M; ++mm) {
         const uint32_t m = back ? M - 1 - mm : mm;
         if (back ? !(mz[m] < zv) : !(mz[m] > zv)) continue;
         x += tx * (mz[m] - zp);
@@ -184,7 +212,7 @@ void gen_event(const velogen_config_t& c, const double* mz, uint64_t e, EventBuf
         double a = 6.283185307179586476925 * rng.uniform();
         double xl = r * std::cos(a), y = r * std::sin(a);
         int h = (xl < 0.0) ? -1 : 1;
-        record(c, mz, b, m, h, xl, y, -1);
+        record(c, mz, b, m, h, xl, y, -1, (c.stagger_z != 0.0) ? mz[m] + 0.5 * (double)h * c.stagger_z : 1e300);
       }
     }
   }
