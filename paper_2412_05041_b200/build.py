@@ -6,6 +6,7 @@ is no JIT cache and no other architecture.
 from __future__ import annotations
 
 import os
+import shutil
 import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -42,8 +43,11 @@ def _compile(lib: str, extra: list[str], tag: str, verbose: bool = False) -> str
     """nvcc -c every source (in parallel: they are independent translation units), then link."""
     from concurrent.futures import ThreadPoolExecutor
 
-    os.makedirs(OBJ_DIR, exist_ok=True)
-    objs = [os.path.join(OBJ_DIR, f"{tag}_{f[:-3]}.o") for f in SOURCES]
+    # objects and the linked library are private to this process until an atomic rename: several ranks
+    # (torchrun) or forked test workers may find the library stale at the same moment
+    obj_dir = os.path.join(OBJ_DIR, f"{tag}_{os.getpid()}")
+    os.makedirs(obj_dir, exist_ok=True)
+    objs = [os.path.join(obj_dir, f"{f[:-3]}.o") for f in SOURCES]
 
     def one(src, obj):
         cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-I", INCLUDE, "-c", "-o", obj, os.path.join(CSRC, src)]
@@ -53,7 +57,10 @@ def _compile(lib: str, extra: list[str], tag: str, verbose: bool = False) -> str
 
     with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as ex:
         list(ex.map(one, SOURCES, objs))
-    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", lib, *objs], check=True)
+    tmp = f"{lib}.{os.getpid()}.tmp"
+    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs], check=True)
+    os.replace(tmp, lib)
+    shutil.rmtree(obj_dir, ignore_errors=True)
     return lib
 
 

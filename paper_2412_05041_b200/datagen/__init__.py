@@ -83,8 +83,10 @@ CONFIGS = {
 def build(force: bool = False) -> str:
     """Compile the generator with g++ (host only)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", _LIB, _SRC]
+        tmp = f"{_LIB}.{os.getpid()}.tmp"      # atomic: several ranks or test workers may build at once
+        cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", tmp, _SRC]
         subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
     return _LIB
 
 
