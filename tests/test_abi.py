@@ -88,3 +88,27 @@ def test_product_never_imports_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text and "velo_oracle" not in text, f
+
+
+def test_entry_points_around_the_path_check_their_arguments(lib):
+    """velo_pv_params_default holds the readings P-1 ... P-6 (and equals the oracle's own defaults, which
+    are written independently); null or inconsistent arguments come back as VELO_ERR_ARG before any CUDA
+    call (so this runs without a GPU)."""
+    import oracle
+    p = velo.velo_pv_params_default()
+    q = oracle.default_pv_params()
+    for name, _ in velo.PvParams._fields_:
+        assert getattr(p, name) == getattr(q, name), name
+    assert (p.n_bins, p.seed_min_sum, p.seed_half_window, p.n_iterations, p.min_tracks, p.max_pv_per_event) == (2400, 5, 6, 4, 4, 32)
+    assert velo.velo_pv_workspace_bytes(1000, 50000) > 1000 * 32 * 5 * 4
+    assert np.float32(velo.MS_THETA2_DEFAULT) == np.float32(oracle.MS_THETA2_DEFAULT)
+    L = lib
+    assert L.velo_kalman_fit(None, None, 0.016, 9e-8, None, None) == velo.VELO_ERR_ARG
+    assert L.velo_pv_find(None, 0, None, None, None, 0, None) == velo.VELO_ERR_ARG
+    assert L.velo_reconstruct_pixels(None, None, None, None, None, None, 0, None, None) == velo.VELO_ERR_ARG
+    assert L.velo_scheduler_run_host_pixels(None, None, None, None, None, 0, None) == velo.VELO_ERR_ARG
+    # a histogram larger than the kernel's shared memory is refused
+    tr = velo.Tracks(event_track_offsets=8, track_hit_offsets=8, track_hits=8, states=8, cap_tracks=4, cap_track_hits=4, summary=8)
+    pv = velo.Pvs(event_pv_offsets=8, pvs=8, cap_pvs=4, summary=8)
+    bad = velo.velo_pv_params_default(); bad.n_bins = 5000
+    assert L.velo_pv_find(ctypes.byref(tr), 1, ctypes.byref(bad), ctypes.byref(pv), ctypes.c_void_p(256), 1 << 20, None) == velo.VELO_ERR_ARG
