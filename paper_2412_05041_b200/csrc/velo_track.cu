@@ -47,20 +47,23 @@ template <int G, int kTeams>
 struct TrackCtl {
   PoolCtl pool;
   float module_z[VELO_MAX_MODULES];
+  float tz[VELO_MAX_MODULES * 4];    // O-4's z ratio for a track whose latest hits are on modules mb and mb + 1 + gap,
+                                     // forwarded to module mb - 1 - pend: [mb][gap][pend], gap and pend 0 or 1
   TrackTeam<G> team[kTeams];
 };
 
 __device__ __forceinline__ uint32_t al16(uint32_t v) { return (v + 15u) & ~15u; }
 
+constexpr uint32_t kSlotPad = 3;      // sentinel records behind every module slot of the ring (scan_run)
 constexpr uint32_t kPairCap = 8192;   // (centre, h0) pairs per round of the one-event-per-CTA seeding
 struct TrackLayout { uint32_t ring, act, flags, th0, cl, keys, plist, bytes; };
 __device__ __forceinline__ TrackLayout track_layout(uint32_t n, uint32_t maxmod, uint32_t tcap, uint32_t acap,
                                                     bool with_ring = true) {
   TrackLayout L;
   uint32_t o = 0;
-  L.ring = o; o += with_ring ? 4u * 16u * maxmod : 0u;
+  L.ring = o; o += with_ring ? 4u * 16u * (maxmod + kSlotPad) : 0u;
   L.act = o; o += 32u * acap;
-  L.flags = o; o += al16(4u * ((n + 31u) >> 5));
+  L.flags = o; o += al16(4u * ((n + 31u + kSlotPad) >> 5));      // a padded trip may test a bit or two past the event
   L.th0 = o; o += al16(2u * tcap);
   L.cl = o; o += al16(2u * maxmod);
   // one-event-per-CTA form only: the best (scatter, h0, h2) of every centre of a round as a 64-bit
@@ -101,16 +104,21 @@ __device__ void track_fetch(const KernelArgs& a, PoolCtl& pool, TrackTeam<G>& ts
 
 // Visits positions j0, j0 + 1, ... of a module slot (nm hits) while they lie inside the wide window
 // (lo16w, limw), four per trip: the four 16-byte loads of a trip are issued before its arithmetic.
-// f(jj, rec, in) must be branch-free; for padding lanes `in` is false and jj repeats nm - 1.
-template <class F>
+// f(jj, rec, in) must be branch-free. kPad: the slot ends with three sentinel records (x = +inf: their
+// scatter is +inf, no cut accepts them), so a trip reads past the module without clamping its indices;
+// otherwise padding lanes repeat position nm - 1 with `in` false.
+template <bool kPad, class F>
 __device__ __forceinline__ void scan_run(const uint4* slot, uint32_t j0, uint32_t nm, uint32_t lo16w, uint32_t limw, F&& f) {
   for (uint32_t j = j0; j < nm; j += 4u) {
     uint4 r[4]; uint32_t jj[4];
 #pragma unroll
-    for (uint32_t k = 0; k < 4; ++k) { jj[k] = min(j + k, nm - 1u); r[k] = slot[jj[k]]; }
+    for (uint32_t k = 0; k < 4; ++k) { jj[k] = kPad ? j + k : min(j + k, nm - 1u); r[k] = slot[jj[k]]; }
     bool in = false;
 #pragma unroll
-    for (uint32_t k = 0; k < 4; ++k) { in = (j + k < nm) & (r[k].z - lo16w <= limw); f(jj[k], r[k], in); }
+    for (uint32_t k = 0; k < 4; ++k) {
+      in = kPad ? (r[k].z - lo16w <= limw) : ((j + k < nm) & (r[k].z - lo16w <= limw));
+      f(jj[k], r[k], in);
+    }
     if (!in) break;     // the last of the four is outside (or past the module): so is everything after it
   }
 }
@@ -130,12 +138,13 @@ __device__ __forceinline__ Win make_win(uint32_t c, int W) {
 // slots ARE the sorted records in global scratch (L2), nothing is copied; the event ends in state
 // kEvBig so that the per-event kernels of stage 3 leave it to velo_fit_big_kernel.
 template <int G, bool kSameW, bool kGlobal = false>
-__device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& ts, unsigned char* blk, uint32_t team,
-                            uint32_t tid, uint32_t& parity, uint32_t& phases) {
+__device__ void track_event(const KernelArgs& a, const float* mz, const float* tzt, TrackTeam<G>& ts, unsigned char* blk,
+                            uint32_t team, uint32_t tid, uint32_t& parity, uint32_t& phases) {
   const uint32_t M = a.n_modules, n = ts.n, e = ts.event;
   const velo_params_t& P = a.P;
-  const uint32_t slotcap = ts.maxmod, tcap = ts.tcap, acap = ts.acap;
-  const TrackLayout L = track_layout(n, slotcap, tcap, acap, !kGlobal);
+  const uint32_t tcap = ts.tcap, acap = ts.acap;
+  const TrackLayout L = track_layout(n, ts.maxmod, tcap, acap, !kGlobal);
+  const uint32_t slotcap = ts.maxmod + kSlotPad;
   const TrackLayout& L_ = L;
   uint4* ring = (uint4*)(blk + L.ring);
   uint4* act = (uint4*)(blk + L.act);
@@ -165,7 +174,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
   const int Wwide = Wseed > Wfwd ? Wseed : Wfwd;
 
   for (uint32_t i = tid; i < kModOffStride; i += G) ts.mod_off[i] = a.ws.mod_off[(size_t)e * kModOffStride + i];
-  for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) flags[i] = 0;
+  for (uint32_t i = tid; i < ((n + 31u + kSlotPad) >> 5); i += G) flags[i] = 0;
   team_sync<G>(team);
 
   // ring: module m lives in slot m & 3; loads are issued and waited for in descending module order
@@ -174,6 +183,10 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
       const uint32_t bytes = 16u * ((uint32_t)mo[m + 1] - (uint32_t)mo[m]);
       mbar_arrive_expect_tx(&ts.mbar[m & 3u], bytes);
       if (bytes) tma_load_1d(ring + (m & 3u) * slotcap, grec + mo[m], bytes, &ts.mbar[m & 3u]);
+      // the sentinels behind the module's records (see scan_run): nobody reads the slot's old tenant any more
+      uint4* pad = ring + (m & 3u) * slotcap + (bytes >> 4);
+#pragma unroll
+      for (uint32_t k = 0; k < kSlotPad; ++k) pad[k] = make_uint4(0x7f800000u, 0u, 0u, 0u);
     }
   };
   auto wait = [&](uint32_t m) {
@@ -215,8 +228,10 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
         const float x1 = __uint_as_float(q0.z), y1 = __uint_as_float(q0.w);
         const uint32_t c = q1.x >> 16, id = q1.x & 0xffffu, w3 = q1.y, hab = q1.z, mask = q1.w;
         const uint32_t mb = __ffs(mask) - 1u, ma = __ffs(mask & (mask - 1u)) - 1u;
-        const float z1 = mz[mb], z0 = mz[ma];
-        const float tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0));
+        const uint32_t gap = ma - mb - 1u, pend0 = mb - s;
+        float tz;
+        if ((gap | pend0) <= 1u) tz = tzt[mb * 4u + gap * 2u + pend0];        // the same quotient, taken once per CTA
+        else { const float z1 = mz[mb], z0 = mz[ma]; tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0)); }
         const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, x0), tz));
         const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, y0), tz));
         const Win wx = make_win(c, Wfwd);
@@ -231,8 +246,8 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
         const uint32_t pend = mb - s;      // modules already missed since the latest hit
         if (pend <= 1u) {
           const Win ww = kSameW ? wx : make_win(c, Wwide);
-          if (ww.wrapped) scan_run(ring_u, 0u, nu, ww.lo16, ww.lim, visit);          // low-phi run of a window across +-pi
-          scan_run(ring_u, pend ? (w3 & 0xffffu) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
+          if (ww.wrapped) scan_run<!kGlobal>(ring_u, 0u, nu, ww.lo16, ww.lim, visit);          // low-phi run of a window across +-pi
+          scan_run<!kGlobal>(ring_u, pend ? (w3 & 0xffffu) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
         } else {
           // no stored start for a target this far from the latest hit (max_skipped >= 2): whole module
           for (uint32_t j = 0; j < nu; ++j) {
@@ -342,8 +357,8 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
                 fnd |= ok; bb2 = ok ? jj : bb2; bsc = ok ? sc : bsc;
               };
-              if (ww.wrapped) scan_run(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
-              scan_run(ring_u, rc.w >> 16, nu, ww.lo16, ww.lim, visit2);
+              if (ww.wrapped) scan_run<!kGlobal>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
+              scan_run<!kGlobal>(ring_u, rc.w >> 16, nu, ww.lo16, ww.lim, visit2);
               if (fnd) atomicMin(&keys[kl], ((unsigned long long)__float_as_uint(bsc) << 32) | ((unsigned long long)j0 << 16) | bb2);
             }
             team_sync<G>(team);
@@ -375,8 +390,8 @@ __device__ void track_event(const KernelArgs& a, const float* mz, TrackTeam<G>& 
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
                 found |= ok; b0 = ok ? j0 : b0; b2 = ok ? jj : b2; best_sc = ok ? sc : best_sc;
               };
-              if (ww.wrapped) scan_run(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
-              scan_run(ring_u, r1.w >> 16, nu, ww.lo16, ww.lim, visit2);
+              if (ww.wrapped) scan_run<!kGlobal>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
+              scan_run<!kGlobal>(ring_u, r1.w >> 16, nu, ww.lo16, ww.lim, visit2);
             }
           }
         }
@@ -450,6 +465,13 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
   const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
   if (threadIdx.x == 0) pool_init(ctl.pool, pool_units);
   if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
+  if (threadIdx.x < VELO_MAX_MODULES * 4u) {
+    const uint32_t mb = threadIdx.x >> 2, gap = (threadIdx.x >> 1) & 1u, pend = threadIdx.x & 1u, ma = mb + 1u + gap;
+    float v = 0.0f;
+    if (ma < a.n_modules && mb >= 1u + pend)
+      v = __fdiv_rn(__fsub_rn(a.module_z[mb - 1u - pend], a.module_z[mb]), __fsub_rn(a.module_z[mb], a.module_z[ma]));
+    ctl.tz[threadIdx.x] = v;
+  }
   TrackTeam<G>& ts = ctl.team[team];
   if (tid == 0) {
 #pragma unroll
@@ -465,7 +487,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
     VELO_PH(a.ws.phase_clk, ts, 17);     // ticket, descriptors, pool
-    if (!ts.skip) track_event<G, kSameW>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity, phases);
+    if (!ts.skip) track_event<G, kSameW>(a, ctl.module_z, ctl.tz, ts, pool + ts.pool_off, team, tid, parity, phases);
     if (a.pixel && (ts.unpack || (!ts.skip && ts.defer))) unpack_event<G>(a, ts.event, tid);
     team_sync<G>(team);   // every thread is done with the block and with ts before the leader reuses them
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
@@ -485,6 +507,13 @@ __global__ void __launch_bounds__(G, 1) velo_track_big_kernel(const KernelArgs a
   unsigned char* blk = smem + kCtl;
   const uint32_t tid = threadIdx.x;
   if (tid < VELO_MAX_MODULES) ctl.module_z[tid] = a.module_z[tid];
+  if (threadIdx.x < VELO_MAX_MODULES * 4u) {
+    const uint32_t mb = threadIdx.x >> 2, gap = (threadIdx.x >> 1) & 1u, pend = threadIdx.x & 1u, ma = mb + 1u + gap;
+    float v = 0.0f;
+    if (ma < a.n_modules && mb >= 1u + pend)
+      v = __fdiv_rn(__fsub_rn(a.module_z[mb - 1u - pend], a.module_z[mb]), __fsub_rn(a.module_z[mb], a.module_z[ma]));
+    ctl.tz[threadIdx.x] = v;
+  }
   TrackTeam<G>& ts = ctl.team[0];
   uint32_t parity = 0, phases = 0;
   const uint32_t base = a.event_offsets[0];
@@ -515,7 +544,7 @@ __global__ void __launch_bounds__(G, 1) velo_track_big_kernel(const KernelArgs a
     }
     __syncthreads();
     if (ts.units) break;
-    if (!ts.skip) track_event<G, kSameW, true>(a, ctl.module_z, ts, blk, 0u, tid, parity, phases);
+    if (!ts.skip) track_event<G, kSameW, true>(a, ctl.module_z, ctl.tz, ts, blk, 0u, tid, parity, phases);
     if (a.pixel && (ts.unpack || (!ts.skip && ts.defer))) unpack_event<G>(a, ts.event, tid);
   }
 }
