@@ -224,6 +224,10 @@ int velo_scheduler_run_host_pixels(velo_scheduler_t* s, const velo_params_t* par
  * batch reported an error). Asynchronous on `stream`; returns VELO_ERR_ARG / VELO_ERR_CUDA. */
 int velo_kalman_fit(const velo_hits_t* hits, const velo_tracks_t* tracks, float sigma_hit, float ms_theta2,
                     float* kalman_states, void* stream);
+/* The same on the packed pixel addresses that velo_reconstruct_pixels was given (decoded per hit as F-2). */
+int velo_kalman_fit_pixels(const velo_geometry_t* g, const velo_pixel_hits_t* hits, const velo_pixel_format_t* fmt,
+                           const velo_tracks_t* tracks, float sigma_hit, float ms_theta2, float* kalman_states,
+                           void* stream);
 
 /* f3. Primary vertices from the beamline states (§5: VELO tracks are straight
  * lines; displaced-vertex lines need primary vertices; the paper gives no algorithm: readings

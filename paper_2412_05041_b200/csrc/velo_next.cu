@@ -17,8 +17,19 @@ namespace {
 // ---- f2: one thread per track -----------------------------------------------------------------------
 // The hits of a track are gathered through track_hits (absolute hit indices, discovery order =
 // decreasing z). The next hit's index and coordinates are loaded while the current one is filtered.
-__global__ void __launch_bounds__(256) velo_kalman_kernel(const float* __restrict__ hx, const float* __restrict__ hy,
-                                                          const float* __restrict__ hz, const uint32_t* __restrict__ tho,
+// Where the hits come from: fp32 planes, or packed pixel addresses decoded on the fly (F-2).
+struct KalmanHits {
+  const float *x, *y, *z;
+  const uint32_t* pixel;               // or NULL
+  double pitch, half_shift_x;
+  float module_z[VELO_MAX_MODULES];
+  __device__ __forceinline__ void get(uint32_t i, float& hx, float& hy, float& hz) const {
+    if (pixel) { uint32_t m; pixel_decode(pixel[i], pitch, half_shift_x, m, hx, hy); hz = module_z[m & (VELO_MAX_MODULES - 1)]; }
+    else { hx = x[i]; hy = y[i]; hz = z[i]; }
+  }
+};
+
+__global__ void __launch_bounds__(256) velo_kalman_kernel(const KalmanHits H, const uint32_t* __restrict__ tho,
                                                           const uint32_t* __restrict__ th, const uint32_t* __restrict__ summary,
                                                           float sigma_hit, float ms_theta2, float* __restrict__ out,
                                                           uint32_t cap_tracks) {
@@ -28,19 +39,19 @@ __global__ void __launch_bounds__(256) velo_kalman_kernel(const float* __restric
   const uint32_t a = tho[t], n = tho[t + 1] - a;
   const float s2 = __fmul_rn(sigma_hit, sigma_hit);
   uint32_t i0 = th[a], i1 = th[a + 1];
-  const float x0 = hx[i0], y0 = hy[i0], z0 = hz[i0];
-  float zp = hz[i1];
-  float x = hx[i1], y = hy[i1];
+  float x0, y0, z0, x, y, zp;
+  H.get(i0, x0, y0, z0);
+  H.get(i1, x, y, zp);
   float dz = __fsub_rn(zp, z0);
   float tx = __fdiv_rn(__fsub_rn(x, x0), dz), ty = __fdiv_rn(__fsub_rn(y, y0), dz);
   float cxx = s2, cxtx = __fdiv_rn(s2, dz), ctxtx = __fdiv_rn(__fadd_rn(s2, s2), __fmul_rn(dz, dz));
   float chi2 = 0.0f;
   // software pipeline: hit i+1 is in flight while hit i is processed
   float nx = 0.0f, ny = 0.0f, nz = 0.0f;
-  if (n > 2) { const uint32_t j = th[a + 2]; nx = hx[j]; ny = hy[j]; nz = hz[j]; }
+  if (n > 2) H.get(th[a + 2], nx, ny, nz);
   for (uint32_t i = 2; i < n; ++i) {
     const float mx = nx, my = ny, mzz = nz;
-    if (i + 1 < n) { const uint32_t j = th[a + i + 1]; nx = hx[j]; ny = hy[j]; nz = hz[j]; }
+    if (i + 1 < n) H.get(th[a + i + 1], nx, ny, nz);
     const float sl = __fadd_rn(1.0f, __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty)));
     ctxtx = __fadd_rn(ctxtx, __fmul_rn(ms_theta2, sl));
     dz = __fsub_rn(mzz, zp);
@@ -379,17 +390,33 @@ PvWorkspace carve_pv(void* base, uint32_t n_events, uint32_t cap_tracks) {
 
 extern "C" {
 
-int velo_kalman_fit(const velo_hits_t* hits, const velo_tracks_t* tracks, float sigma_hit, float ms_theta2,
-                    float* kalman_states, void* stream) {
-  if (!hits || !tracks || !kalman_states) return VELO_ERR_ARG;
+static int kalman_launch(const velo::KalmanHits& H, const velo_tracks_t* tracks, float sigma_hit, float ms_theta2,
+                         float* kalman_states, void* stream) {
+  if (!tracks || !kalman_states) return VELO_ERR_ARG;
   if (!tracks->track_hit_offsets || !tracks->track_hits || !tracks->summary || tracks->cap_tracks == 0) return VELO_ERR_ARG;
-  if (hits->n_hits && (!hits->x || !hits->y || !hits->z)) return VELO_ERR_ARG;
   if (!(sigma_hit > 0.0f) || !(ms_theta2 >= 0.0f)) return VELO_ERR_ARG;
   const uint32_t threads = 256, grid = (tracks->cap_tracks + threads - 1) / threads;
   velo::velo_kalman_kernel<<<grid, threads, 0, (cudaStream_t)stream>>>(
-      hits->x, hits->y, hits->z, tracks->track_hit_offsets, tracks->track_hits, tracks->summary, sigma_hit, ms_theta2,
-      kalman_states, tracks->cap_tracks);
+      H, tracks->track_hit_offsets, tracks->track_hits, tracks->summary, sigma_hit, ms_theta2, kalman_states, tracks->cap_tracks);
   return cudaGetLastError() == cudaSuccess ? VELO_OK : VELO_ERR_CUDA;
+}
+
+int velo_kalman_fit(const velo_hits_t* hits, const velo_tracks_t* tracks, float sigma_hit, float ms_theta2,
+                    float* kalman_states, void* stream) {
+  if (!hits) return VELO_ERR_ARG;
+  if (hits->n_hits && (!hits->x || !hits->y || !hits->z)) return VELO_ERR_ARG;
+  velo::KalmanHits H{};
+  H.x = hits->x; H.y = hits->y; H.z = hits->z;
+  return kalman_launch(H, tracks, sigma_hit, ms_theta2, kalman_states, stream);
+}
+
+int velo_kalman_fit_pixels(const velo_geometry_t* g, const velo_pixel_hits_t* hits, const velo_pixel_format_t* fmt,
+                           const velo_tracks_t* tracks, float sigma_hit, float ms_theta2, float* kalman_states, void* stream) {
+  if (!g || !hits || !fmt || !hits->pixel || !(fmt->pitch > 0.0)) return VELO_ERR_ARG;
+  velo::KalmanHits H{};
+  H.pixel = hits->pixel; H.pitch = fmt->pitch; H.half_shift_x = fmt->half_shift_x;
+  for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) H.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
+  return kalman_launch(H, tracks, sigma_hit, ms_theta2, kalman_states, stream);
 }
 
 void velo_pv_params_default(velo_pv_params_t* p) {

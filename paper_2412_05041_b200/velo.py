@@ -30,7 +30,7 @@ EXPORTS = ("velo_version", "velo_geometry_load", "velo_geometry_free", "velo_geo
            "velo_reconstruct_opts", "velo_scheduler_create",
            "velo_scheduler_free", "velo_scheduler_run_host",
            "velo_kalman_fit", "velo_pv_params_default", "velo_pv_workspace_bytes", "velo_pv_find",
-           "velo_reconstruct_pixels", "velo_scheduler_run_host_pixels")
+           "velo_reconstruct_pixels", "velo_scheduler_run_host_pixels", "velo_kalman_fit_pixels")
 
 
 class VeloError(RuntimeError):
@@ -136,6 +136,9 @@ def lib():
         L.velo_scheduler_run_host_pixels.argtypes = [c_void_p, POINTER(Params), POINTER(PixelHits), POINTER(PixelFormat),
                                                      c_void_p, c_uint32, POINTER(Tracks)]
         L.velo_scheduler_run_host_pixels.restype = c_int
+        L.velo_kalman_fit_pixels.argtypes = [c_void_p, POINTER(PixelHits), POINTER(PixelFormat), POINTER(Tracks), c_float,
+                                             c_float, c_void_p, c_void_p]
+        L.velo_kalman_fit_pixels.restype = c_int
         L.velo_kalman_fit.argtypes = [POINTER(Hits), POINTER(Tracks), c_float, c_float, c_void_p, c_void_p]
         L.velo_kalman_fit.restype = c_int
         L.velo_pv_params_default.argtypes = [POINTER(PvParams)]
@@ -354,6 +357,20 @@ def velo_kalman_fit(hits: Hits, tracks: DeviceTracks, sigma_hit: float, ms_theta
                                c_void_p(st.cuda_stream))
     if rc != VELO_OK:
         raise VeloError(rc, "velo_kalman_fit")
+    return out
+
+
+def velo_kalman_fit_pixels(geometry: Geometry, hits: PixelHits, fmt: PixelFormat, tracks: DeviceTracks, sigma_hit: float,
+                           ms_theta2: float = MS_THETA2_DEFAULT, stream=None):
+    """velo_kalman_fit for the packed-pixel path. Returns a device tensor of 13 planes x cap_tracks."""
+    torch = _torch()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    out = torch.empty((VELO_N_STATE, tracks.cap_tracks), dtype=torch.float32, device=tracks.states.device)
+    tr = tracks.struct()
+    rc = lib().velo_kalman_fit_pixels(geometry.handle, byref(hits), byref(fmt), byref(tr), c_float(sigma_hit), c_float(ms_theta2),
+                                      c_void_p(out.data_ptr()), c_void_p(st.cuda_stream))
+    if rc != VELO_OK:
+        raise VeloError(rc, "velo_kalman_fit_pixels")
     return out
 
 

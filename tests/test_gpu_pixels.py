@@ -74,3 +74,24 @@ def test_scheduler_with_packed_host_buffers(velo):
     want = T.oracle_parallel(d, M, None, None)
     same(got, want)
     sched.close()
+
+
+def test_kalman_filter_on_the_packed_path(velo):
+    """velo_reconstruct_pixels -> velo_kalman_fit_pixels: the states equal the oracle's filter on the oracle's decode."""
+    import torch
+    d = datagen.generate_config(3, n_events=1500, pixels=True)
+    shift = d["cfg"].half_shift_x
+    g = velo.velo_geometry_load(datagen.MODULE_Z, half_shift_x=shift)
+    P = velo.velo_params_default(g)
+    fmt = velo.PixelFormat(pitch=0.055, half_shift_x=shift)
+    dh = velo.DevicePixelHits(d["pixel"], d["event_offsets"])
+    out = velo.DeviceTracks(dh.n_events, dh.n_hits)
+    hs = dh.slice_struct()
+    velo.velo_reconstruct_pixels(g, hs, fmt, P, out)
+    ks = velo.velo_kalman_fit_pixels(g, hs, fmt, out, P.sigma_hit)
+    torch.cuda.synchronize()
+    res = out.to_host()
+    dec = oracle.pixel_decode(d["pixel"], datagen.MODULE_Z, half_shift_x=shift)
+    want = oracle.kalman_tracks(res, dec["x"], dec["y"], dec["z"], P.sigma_hit)
+    np.testing.assert_array_equal(ks[:, :res["n_tracks"]].cpu().numpy().view(np.uint32), want.view(np.uint32))
+    assert res["n_tracks"] > 50000
