@@ -1,16 +1,17 @@
 // velo_track.cu — stage 2 of the pipeline: the O-6 module loop (S3 forwarding, S2 search-by-triplet
 // seeding, hit flags) over the phi-sorted blocks that stage 1 left in global scratch (sm_100a).
 //
-// One persistent CTA per SM owns the SM's shared memory as a pool; a team of G threads (a warp by
-// default: every phase boundary of the loop is then a __syncwarp, not a barrier) takes an event and
-// holds, instead of the whole event, only what a step touches at random:
+// One persistent CTA per SM owns the SM's shared memory as a pool; a team of G threads (two warps for
+// mu = 5 events, one for open-VELO events, four for events of several thousand hits) takes an event;
+// its warps work side by side and meet twice per step (track_event_w). It holds, instead of the whole
+// event, only what a step touches at random:
 //   * a ring of four module slots fed by 1-D TMA bulk copies (cp.async.bulk + mbarrier): step s
 //     reads modules s+1, s, s-1 while module s-2 is in flight, a full step ahead of its use;
 //   * the list of ACTIVE tracks as self-contained 32-byte records (last two hits' coordinates,
 //     phi and window starts of the latest hit, hit indices, module mask, candidate id), compacted
 //     in place every step, so the lanes of the forwarding pass are always dense;
-//   * one flag byte per hit, the first hit of every candidate, the list of unflagged centre hits.
-// About 19 KB for a mu = 5 event of 1.9 k hits instead of the 34 KB of the whole sorted event, and
+//   * one flag bit per hit, the first hit of every candidate, the list of unflagged centre hits.
+// About 15 KB for a mu = 5 event of 1.9 k hits instead of the 34 KB of the whole sorted event, and
 // only for the duration of the loop: the sort (stage 1) and the fit/filters/output (stage 3) run
 // in their own kernels. Candidates leave as 64-byte rows of sorted hit indices plus {module mask,
 // seed scatter}; the final flags leave as one bit per hit.
@@ -133,20 +134,19 @@ __device__ __forceinline__ Win make_win(uint32_t c, int W) {
   return q;
 }
 
-// ---- one event, by one team ---------------------------------------------------------------------
-// kGlobal: the one-event-per-CTA form for events too large for a ring in shared memory: the module
-// slots ARE the sorted records in global scratch (L2), nothing is copied; the event ends in state
-// kEvBig so that the per-event kernels of stage 3 leave it to velo_fit_big_kernel.
-template <int G, bool kSameW, bool kGlobal = false>
-__device__ void track_event(const KernelArgs& a, const float* mz, const float* tzt, TrackTeam<G>& ts, unsigned char* blk,
-                            uint32_t team, uint32_t tid, uint32_t& parity, uint32_t& phases) {
+// ---- one event, by one CTA ----------------------------------------------------------------------
+// The one-event-per-CTA form for events too large for a ring in shared memory: the module slots ARE
+// the sorted records in global scratch (L2), nothing is copied; one list of active tracks, compacted
+// over the whole team after every pass; the event ends in state kEvBig so that the per-event kernels
+// of stage 3 leave it to velo_fit_big_kernel. (Events that fit a team: track_event_w below.)
+template <int G, bool kSameW>
+__device__ void track_event_big(const KernelArgs& a, const float* mz, const float* tzt, TrackTeam<G>& ts, unsigned char* blk,
+                                uint32_t team, uint32_t tid, uint32_t& parity) {
   const uint32_t M = a.n_modules, n = ts.n, e = ts.event;
   const velo_params_t& P = a.P;
   const uint32_t tcap = ts.tcap, acap = ts.acap;
-  const TrackLayout L = track_layout(n, ts.maxmod, tcap, acap, !kGlobal);
-  const uint32_t slotcap = ts.maxmod + kSlotPad;
+  const TrackLayout L = track_layout(n, ts.maxmod, tcap, acap, false);
   const TrackLayout& L_ = L;
-  uint4* ring = (uint4*)(blk + L.ring);
   uint4* act = (uint4*)(blk + L.act);
   uint32_t* flags = (uint32_t*)(blk + L.flags);   // one bit per sorted hit
   auto flagged = [&](uint32_t h) -> bool { return (flags[h >> 5] >> (h & 31u)) & 1u; };
@@ -177,26 +177,6 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
   for (uint32_t i = tid; i < ((n + 31u + kSlotPad) >> 5); i += G) flags[i] = 0;
   team_sync<G>(team);
 
-  // ring: module m lives in slot m & 3; loads are issued and waited for in descending module order
-  auto issue = [&](uint32_t m) {
-    if (!kGlobal && tid == 0) {
-      const uint32_t bytes = 16u * ((uint32_t)mo[m + 1] - (uint32_t)mo[m]);
-      mbar_arrive_expect_tx(&ts.mbar[m & 3u], bytes);
-      if (bytes) tma_load_1d(ring + (m & 3u) * slotcap, grec + mo[m], bytes, &ts.mbar[m & 3u]);
-      // the sentinels behind the module's records (see scan_run): nobody reads the slot's old tenant any more
-      uint4* pad = ring + (m & 3u) * slotcap + (bytes >> 4);
-#pragma unroll
-      for (uint32_t k = 0; k < kSlotPad; ++k) pad[k] = make_uint4(0x7f800000u, 0u, 0u, 0u);
-    }
-  };
-  auto wait = [&](uint32_t m) {
-    if (kGlobal) return;
-    mbar_wait(&ts.mbar[m & 3u], (phases >> (m & 3u)) & 1u);
-    phases ^= 1u << (m & 3u);
-  };
-  uint32_t issued = M, waited = M;       // lowest module issued / waited for so far
-  for (uint32_t k = 0; k < 4 && issued > 0; ++k) issue(--issued);
-  wait(--waited); wait(--waited);        // modules M-1 and M-2
   VELO_PH(a.ws.phase_clk, ts, 18);       // descriptors, flags, first loads
 
   uint32_t nact = 0, ncand = 0;
@@ -206,14 +186,13 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
     // No hit in modules 0 .. u: forwarding can only miss and seeding finds no third hit, in this step
     // and in all that follow, and what a miss changes (the miss count) is not read after the loop.
     if (mo[u + 1] == 0) break;
-    wait(--waited);                      // module u has landed
     VELO_PH(a.ws.phase_clk, ts, 19);
     const uint32_t off_u = mo[u], nu = (uint32_t)mo[u + 1] - off_u;
     const uint32_t off_s = mo[s], ns = (uint32_t)mo[s + 1] - off_s;
     const uint32_t off_p = mo[s + 1], np = (uint32_t)mo[s + 2] - off_p;
-    const uint4* ring_u = kGlobal ? grec + off_u : ring + (u & 3u) * slotcap;
-    const uint4* ring_s = kGlobal ? grec + off_s : ring + (s & 3u) * slotcap;
-    const uint4* ring_p = kGlobal ? grec + off_p : ring + ((s + 1u) & 3u) * slotcap;
+    const uint4* ring_u = grec + off_u;
+    const uint4* ring_s = grec + off_s;
+    const uint4* ring_p = grec + off_p;
     const float z2 = mz[u];
 
     // ---- (A) O-7 forwarding into module u of every track active at the start of the step ----------
@@ -246,8 +225,8 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
         const uint32_t pend = mb - s;      // modules already missed since the latest hit
         if (pend <= 1u) {
           const Win ww = kSameW ? wx : make_win(c, Wwide);
-          if (ww.wrapped) scan_run<!kGlobal>(ring_u, 0u, nu, ww.lo16, ww.lim, visit);          // low-phi run of a window across +-pi
-          scan_run<!kGlobal>(ring_u, pend ? (w3 & 0xffffu) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
+          if (ww.wrapped) scan_run<false>(ring_u, 0u, nu, ww.lo16, ww.lim, visit);          // low-phi run of a window across +-pi
+          scan_run<false>(ring_u, pend ? (w3 & 0xffffu) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
         } else {
           // no stored start for a target this far from the latest hit (max_skipped >= 2): whole module
           for (uint32_t j = 0; j < nu; ++j) {
@@ -296,20 +275,16 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
     }
     team_sync<G>(team);
     VELO_PH(a.ws.phase_clk, ts, 21);
-    // (C2) L = 1, 2 or 4 adjacent lanes per unflagged centre hit (as many as the team can seat at once),
-    // lane q taking every L-th h0 of the window: best (h0, h2) under (scatter, h0, h2), reduced over
-    // the L lanes with shuffles under the same lexicographic order
+    // (C2) rounds of G unflagged centre hits: best (h0, h2) of a centre under (scatter, h0, h2)
     if (ncl) {
       const float zc0 = mz[s + 1], zc1 = mz[s];
       const float tz = __fdiv_rn(__fsub_rn(z2, zc1), __fsub_rn(zc1, zc0));
-      const uint32_t lsh = kGlobal ? 0u : (4u * ncl <= (uint32_t)G) ? 2u : (2u * ncl <= (uint32_t)G) ? 1u : 0u;
-      const uint32_t L = 1u << lsh;
-      for (uint32_t k0 = 0; k0 < ncl; k0 += (uint32_t)G >> lsh) {
-        const uint32_t k = k0 + (tid >> lsh), q = tid & (L - 1u);
+      for (uint32_t k0 = 0; k0 < ncl; k0 += (uint32_t)G) {
+        const uint32_t k = k0 + tid;
         bool found = false; uint32_t b0 = 0, b2 = 0, j1 = 0; float best_sc = 0.0f;
         uint4 r1 = make_uint4(0, 0, 0, 0);
         bool by_pairs = false;
-        if constexpr (kGlobal) {
+        {
           // Large events: a centre has tens of h0 candidates and each means a long scan of the h2
           // window, very unevenly over the centres. The round's (centre, h0) pairs are listed in shared
           // memory and dealt out one per lane; a centre's best triplet is the minimum of a 64-bit key
@@ -357,8 +332,8 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
                 fnd |= ok; bb2 = ok ? jj : bb2; bsc = ok ? sc : bsc;
               };
-              if (ww.wrapped) scan_run<!kGlobal>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
-              scan_run<!kGlobal>(ring_u, rc.w >> 16, nu, ww.lo16, ww.lim, visit2);
+              if (ww.wrapped) scan_run<false>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
+              scan_run<false>(ring_u, rc.w >> 16, nu, ww.lo16, ww.lim, visit2);
               if (fnd) atomicMin(&keys[kl], ((unsigned long long)__float_as_uint(bsc) << 32) | ((unsigned long long)j0 << 16) | bb2);
             }
             team_sync<G>(team);
@@ -375,7 +350,7 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
           const Win wx = make_win(c, Wseed);
           const Win ww = kSameW ? wx : make_win(c, Wwide);
           for (uint32_t run0 = ww.wrapped ? 0u : 1u; run0 < 2u; ++run0) {
-            for (uint32_t j0 = (run0 ? (r1.z & 0xffffu) : 0u) + q; j0 < np; j0 += L) {
+            for (uint32_t j0 = run0 ? (r1.z & 0xffffu) : 0u; j0 < np; ++j0) {
               const uint4 r0 = ring_p[j0];
               if (!(r0.z - ww.lo16 <= ww.lim)) break;
               if (!kSameW && !(r0.z - wx.lo16 <= wx.lim)) continue;
@@ -390,20 +365,11 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
                 found |= ok; b0 = ok ? j0 : b0; b2 = ok ? jj : b2; best_sc = ok ? sc : best_sc;
               };
-              if (ww.wrapped) scan_run<!kGlobal>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
-              scan_run<!kGlobal>(ring_u, r1.w >> 16, nu, ww.lo16, ww.lim, visit2);
+              if (ww.wrapped) scan_run<false>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
+              scan_run<false>(ring_u, r1.w >> 16, nu, ww.lo16, ww.lim, visit2);
             }
           }
         }
-        for (uint32_t d = 1; d < L; d <<= 1) {
-          const bool o_found = __shfl_xor_sync(0xffffffffu, (int)found, d) != 0;
-          const float o_sc = __shfl_xor_sync(0xffffffffu, best_sc, d);
-          const uint32_t o_b0 = __shfl_xor_sync(0xffffffffu, b0, d), o_b2 = __shfl_xor_sync(0xffffffffu, b2, d);
-          const bool better = o_found & (!found | (o_sc < best_sc) |
-                                         ((o_sc == best_sc) & ((o_b0 < b0) | ((o_b0 == b0) & (o_b2 < b2)))));
-          found |= o_found; b0 = better ? o_b0 : b0; b2 = better ? o_b2 : b2; best_sc = better ? o_sc : best_sc;
-        }
-        found &= (q == 0u);                // one lane speaks for the centre
         uint32_t total;
         const uint32_t pos = team_scan_pred<G>(found, ts.wsum, team, parity, &total);
         if (found && ncand + pos < tcap) {
@@ -424,13 +390,10 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
       }
     }
     if (ncand > tcap) { if (tid == 0) ts.defer = 1; }
-    team_sync<G>(team);                  // the new tracks are visible; module s+1 has been read for the last time
+    team_sync<G>(team);                  // the new tracks are visible
     VELO_PH(a.ws.phase_clk, ts, 22);
     if (ts.defer) break;
-    if (issued > 0) issue(--issued);     // module s-3 into the slot of module s+1
   }
-  // every load that was issued must land before the block can be freed
-  while (waited > issued) wait(--waited);
   if (ts.defer) {
     if (tid == 0) {
       a.ws.ev_info[e].state = kEvDeferred;
@@ -449,7 +412,292 @@ __device__ void track_event(const KernelArgs& a, const float* mz, const float* t
     for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) fb[i] = flags[i];
   }
   if (tid == 0) {
-    a.ws.ev_info[e] = EvInfo{n, kGlobal ? kEvBig : kEvReady, ts.cbase, ncand};
+    a.ws.ev_info[e] = EvInfo{n, kEvBig, ts.cbase, ncand};
+    atomicAdd(&a.ws.counters[kCtrCand], ncand);
+  }
+}
+
+// ---- one event, by one team whose warps work side by side ------------------------------------------
+// The same step semantics as track_event (the form the one-event-per-CTA kernel keeps), dealt out so
+// that the warps of a team meet twice per step instead of after every pass:
+//   * every warp owns a share of the active-track list (the tracks it seeded): forwarding, the
+//     compaction of its share (ballot) and the appends never leave the warp;
+//   * every warp owns a contiguous share of the centre module's positions: it lists its unflagged
+//     centres and searches their triplets on its own, parking what it finds where the new tracks'
+//     records will be (the tail of its share of the list);
+//   * barrier 1 follows forwarding (the flags of the step are final), barrier 2 follows the search:
+//     the warps exchange how many seeds each found, which fixes the candidate ids in the order B1
+//     (centre position ascending: warp 0's share precedes warp 1's), then each warp writes its own.
+template <int G, bool kSameW>
+__device__ void track_event_w(const KernelArgs& a, const float* mz, const float* tzt, TrackTeam<G>& ts, unsigned char* blk,
+                              uint32_t team, uint32_t tid, uint32_t& phases) {
+  constexpr uint32_t W = G / 32;
+  const uint32_t lane = tid & 31u, w = tid >> 5, lt = (1u << lane) - 1u;
+  const uint32_t M = a.n_modules, n = ts.n, e = ts.event;
+  const velo_params_t& P = a.P;
+  const uint32_t tcap = ts.tcap, acap_w = ts.acap / W, ovf_w = tcap / W;
+  const TrackLayout L = track_layout(n, ts.maxmod, tcap, ts.acap);
+  const uint32_t slotcap = ts.maxmod + kSlotPad;
+  uint4* ring = (uint4*)(blk + L.ring);
+  uint4* act = (uint4*)(blk + L.act) + 2u * w * acap_w;       // this warp's share
+  uint32_t* flags = (uint32_t*)(blk + L.flags);               // one bit per sorted hit
+  auto flagged = [&](uint32_t h) -> bool { return (flags[h >> 5] >> (h & 31u)) & 1u; };
+  auto set_flag = [&](uint32_t h) { atomicOr(&flags[h >> 5], 1u << (h & 31u)); };
+  // beyond the shared-memory share: global scratch (stage 3's state planes, unused until stage 3)
+  uint4* act_ovf = reinterpret_cast<uint4*>(a.ws.cfit) + 2u * ((size_t)ts.cbase + (size_t)w * ovf_w);
+  auto act_load = [&](uint32_t k, uint4& q0, uint4& q1) {
+    if (k < acap_w) { q0 = act[2u * k]; q1 = act[2u * k + 1u]; }
+    else if (k - acap_w < ovf_w) { q0 = __ldcg(act_ovf + 2u * (k - acap_w)); q1 = __ldcg(act_ovf + 2u * (k - acap_w) + 1u); }
+    else { q0 = make_uint4(0, 0, 0, 0); q1 = q0; }      // never stored (act_store): the event is being given up
+  };
+  auto act_store = [&](uint32_t k, const uint4& q0, const uint4& q1) {
+    if (k < acap_w) { act[2u * k] = q0; act[2u * k + 1u] = q1; }
+    else if (k - acap_w < ovf_w) { act_ovf[2u * (k - acap_w)] = q0; act_ovf[2u * (k - acap_w) + 1u] = q1; }
+    else ts.defer = 1;                 // a share this lopsided: the general kernel takes the event
+  };
+  uint16_t* th0 = (uint16_t*)(blk + L.th0);
+  uint16_t* cl = (uint16_t*)(blk + L.cl);
+  const uint16_t* mo = ts.mod_off;
+  const uint4* grec = a.ws.rec16 + ts.sb;
+  uint16_t* rows = a.ws.rows + (size_t)ts.cbase * 32u;
+  uint2* cmeta = a.ws.cmeta + ts.cbase;
+  float2* rows_xy = a.ws.rows_xy + (size_t)ts.cbase * kXyStride;
+  const int Wseed = P.phi_window_seed, Wfwd = P.phi_window_fwd;
+  const int Wwide = Wseed > Wfwd ? Wseed : Wfwd;
+
+  for (uint32_t i = tid; i < kModOffStride; i += G) ts.mod_off[i] = a.ws.mod_off[(size_t)e * kModOffStride + i];
+  for (uint32_t i = tid; i < ((n + 31u + kSlotPad) >> 5); i += G) flags[i] = 0;
+  team_sync<G>(team);
+
+  // ring: module m lives in slot m & 3; loads are issued and waited for in descending module order
+  auto issue = [&](uint32_t m) {
+    if (tid == 0) {
+      const uint32_t bytes = 16u * ((uint32_t)mo[m + 1] - (uint32_t)mo[m]);
+      mbar_arrive_expect_tx(&ts.mbar[m & 3u], bytes);
+      if (bytes) tma_load_1d(ring + (m & 3u) * slotcap, grec + mo[m], bytes, &ts.mbar[m & 3u]);
+      uint4* pad = ring + (m & 3u) * slotcap + (bytes >> 4);    // the sentinels behind the records (scan_run)
+#pragma unroll
+      for (uint32_t k = 0; k < kSlotPad; ++k) pad[k] = make_uint4(0x7f800000u, 0u, 0u, 0u);
+    }
+  };
+  auto wait = [&](uint32_t m) {
+    mbar_wait(&ts.mbar[m & 3u], (phases >> (m & 3u)) & 1u);
+    phases ^= 1u << (m & 3u);
+  };
+  uint32_t issued = M, waited = M;       // lowest module issued / waited for so far
+  for (uint32_t k = 0; k < 4 && issued > 0; ++k) issue(--issued);
+  wait(--waited); wait(--waited);        // modules M-1 and M-2
+  VELO_PH(a.ws.phase_clk, ts, 18);       // descriptors, flags, first loads
+
+  uint32_t nact = 0, ncand = 0;          // nact: this warp's share
+  const float max_fwd = P.max_scatter_fwd, max_seed = P.max_scatter_seed;
+  for (uint32_t s = M - 2; s >= 1; --s) {
+    const uint32_t u = s - 1;
+    if (mo[u + 1] == 0) break;           // no hit in modules 0 .. u: nothing can change any more (see track_event)
+    wait(--waited);                      // module u has landed
+    VELO_PH(a.ws.phase_clk, ts, 19);
+    const uint32_t off_u = mo[u], nu = (uint32_t)mo[u + 1] - off_u;
+    const uint32_t off_s = mo[s], ns = (uint32_t)mo[s + 1] - off_s;
+    const uint32_t off_p = mo[s + 1], np = (uint32_t)mo[s + 2] - off_p;
+    const uint4* ring_u = ring + (u & 3u) * slotcap;
+    const uint4* ring_s = ring + (s & 3u) * slotcap;
+    const uint4* ring_p = ring + ((s + 1u) & 3u) * slotcap;
+    const float z2 = mz[u];
+
+    // ---- (A) O-7 forwarding into module u of this warp's share of the active tracks ----------------
+    uint32_t wbase = 0;
+    for (uint32_t p0 = 0; p0 < nact; p0 += 32u) {
+      const uint32_t k = p0 + lane;
+      bool alive = false;
+      uint4 q0 = make_uint4(0, 0, 0, 0), q1 = q0;
+      if (k < nact) {
+        act_load(k, q0, q1);
+        const float x0 = __uint_as_float(q0.x), y0 = __uint_as_float(q0.y);
+        const float x1 = __uint_as_float(q0.z), y1 = __uint_as_float(q0.w);
+        const uint32_t c = q1.x >> 16, id = q1.x & 0xffffu, w3 = q1.y, hab = q1.z, mask = q1.w;
+        const uint32_t mb = __ffs(mask) - 1u, ma = __ffs(mask & (mask - 1u)) - 1u;
+        const uint32_t gap = ma - mb - 1u, pend = mb - s;     // pend: modules already missed since the latest hit
+        float tz;
+        if ((gap | pend) <= 1u) tz = tzt[mb * 4u + gap * 2u + pend];        // the same quotient, taken once per CTA
+        else { const float z1 = mz[mb], z0 = mz[ma]; tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0)); }
+        const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, x0), tz));
+        const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, y0), tz));
+        const Win wx = make_win(c, Wfwd);
+        bool found = false; uint32_t best = 0; float best_sc = 0.0f;
+        auto visit = [&](uint32_t jj, const uint4& r, bool in) {
+          const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+          const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+          bool ok = in & (sc <= max_fwd) & (!found | (sc < best_sc));
+          if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
+          found |= ok; best = ok ? jj : best; best_sc = ok ? sc : best_sc;
+        };
+        if (pend <= 1u) {
+          const Win ww = kSameW ? wx : make_win(c, Wwide);
+          if (ww.wrapped) scan_run<true>(ring_u, 0u, nu, ww.lo16, ww.lim, visit);          // low-phi run of a window across +-pi
+          scan_run<true>(ring_u, pend ? (w3 & 0xffffu) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
+        } else {
+          // no stored start for a target this far from the latest hit (max_skipped >= 2): whole module
+          for (uint32_t j = 0; j < nu; ++j) {
+            const uint4 r = ring_u[j];
+            const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+            const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+            const bool ok = (r.z - wx.lo16 <= wx.lim) & (sc <= max_fwd) & (!found | (sc < best_sc));
+            found |= ok; best = ok ? j : best; best_sc = ok ? sc : best_sc;
+          }
+        }
+        if (found) {
+          const uint4 r2 = ring_u[best];
+          const uint32_t h2 = off_u + best, nh = (uint32_t)__popc(mask);
+          rows[id * 32u + nh] = (uint16_t)h2;
+          rows_xy[id * kXyStride + nh] = make_float2(__uint_as_float(r2.x), __uint_as_float(r2.y));
+          // (B): forwarding never reads flags, so they can be set right away
+          if (nh + 1u == 4u) { set_flag(th0[id]); set_flag(hab >> 16); set_flag(hab & 0xffffu); }
+          if (nh + 1u >= 4u) set_flag(h2);
+          q0 = make_uint4(q0.z, q0.w, r2.x, r2.y);
+          q1 = make_uint4((r2.z & 0xffff0000u) | id, r2.w, (hab << 16) | h2, mask | (1u << u));
+          alive = true;
+        } else {
+          alive = (mb - u) <= P.max_skipped;       // consecutive misses so far, this one included
+          if (!alive && __popc(mask) > 3) cmeta[id].x = mask;
+        }
+      }
+      const uint32_t b = __ballot_sync(0xffffffffu, alive);      // (also: every read of this pass is done)
+      if (alive) act_store(wbase + (uint32_t)__popc(b & lt), q0, q1);
+      wbase += (uint32_t)__popc(b);
+    }
+    nact = wbase;
+    team_sync<G>(team);                  // barrier 1: the flags of this step are final
+    VELO_PH(a.ws.phase_clk, ts, 20);
+    if (ts.defer) break;                 // set before the barrier by a warp whose share overflowed: every warp sees it here
+
+    // ---- (C) O-8 seeding with centre module s: this warp's share of the module's positions ----------
+    const uint32_t c_lo = (w * ns) / W, c_hi = ((w + 1u) * ns) / W;
+    uint16_t* clw = cl + c_lo;           // at most c_hi - c_lo entries: the share's unflagged centres
+    // (C1) the unflagged centre hits, in ascending order
+    uint32_t ncl = 0;
+    for (uint32_t c0 = c_lo; c0 < c_hi; c0 += 32u) {
+      const uint32_t j = c0 + lane;
+      const bool open = j < c_hi && !flagged(off_s + j);
+      const uint32_t b = __ballot_sync(0xffffffffu, open);
+      if (open) clw[ncl + (uint32_t)__popc(b & lt)] = (uint16_t)j;
+      ncl += (uint32_t)__popc(b);
+    }
+    __syncwarp();
+    VELO_PH(a.ws.phase_clk, ts, 21);
+    // (C2) L = 1, 2 or 4 adjacent lanes per centre (as many as the warp can seat at once), lane q taking
+    // every L-th h0 of the window: best (h0, h2) under (scatter, h0, h2), reduced over the L lanes with
+    // shuffles under the same lexicographic order
+    uint32_t nfound = 0;
+    if (ncl) {
+      const float zc0 = mz[s + 1], zc1 = mz[s];
+      const float tz = __fdiv_rn(__fsub_rn(z2, zc1), __fsub_rn(zc1, zc0));
+      const uint32_t lsh = (4u * ncl <= 32u) ? 2u : (2u * ncl <= 32u) ? 1u : 0u;
+      const uint32_t Ls = 1u << lsh;
+      for (uint32_t k0 = 0; k0 < ncl; k0 += 32u >> lsh) {
+        const uint32_t k = k0 + (lane >> lsh), q = lane & (Ls - 1u);
+        bool found = false; uint32_t b0 = 0, b2 = 0, j1 = 0; float best_sc = 0.0f;
+        if (k < ncl) {
+          j1 = clw[k];
+          const uint4 r1 = ring_s[j1];
+          const float x1 = __uint_as_float(r1.x), y1 = __uint_as_float(r1.y);
+          const uint32_t c = r1.z >> 16;
+          const Win wx = make_win(c, Wseed);
+          const Win ww = kSameW ? wx : make_win(c, Wwide);
+          for (uint32_t run0 = ww.wrapped ? 0u : 1u; run0 < 2u; ++run0) {
+            for (uint32_t j0 = (run0 ? (r1.z & 0xffffu) : 0u) + q; j0 < np; j0 += Ls) {
+              const uint4 r0 = ring_p[j0];
+              if (!(r0.z - ww.lo16 <= ww.lim)) break;
+              if (!kSameW && !(r0.z - wx.lo16 <= wx.lim)) continue;
+              if (flagged(off_p + j0)) continue;
+              const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tz));
+              const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tz));
+              // h0 and h2 ascending: strict < keeps the lexicographic minimum; branch-free body
+              auto visit2 = [&](uint32_t jj, const uint4& r, bool in) {
+                const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+                const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
+                bool ok = in & !flagged(off_u + jj) & (sc <= max_seed) & (!found | (sc < best_sc));
+                if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
+                found |= ok; b0 = ok ? j0 : b0; b2 = ok ? jj : b2; best_sc = ok ? sc : best_sc;
+              };
+              if (ww.wrapped) scan_run<true>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
+              scan_run<true>(ring_u, r1.w >> 16, nu, ww.lo16, ww.lim, visit2);
+            }
+          }
+        }
+        for (uint32_t d = 1; d < Ls; d <<= 1) {
+          const bool o_found = __shfl_xor_sync(0xffffffffu, (int)found, d) != 0;
+          const float o_sc = __shfl_xor_sync(0xffffffffu, best_sc, d);
+          const uint32_t o_b0 = __shfl_xor_sync(0xffffffffu, b0, d), o_b2 = __shfl_xor_sync(0xffffffffu, b2, d);
+          const bool better = o_found & (!found | (o_sc < best_sc) |
+                                         ((o_sc == best_sc) & ((o_b0 < b0) | ((o_b0 == b0) & (o_b2 < b2)))));
+          found |= o_found; b0 = better ? o_b0 : b0; b2 = better ? o_b2 : b2; best_sc = better ? o_sc : best_sc;
+        }
+        found &= (q == 0u);                // one lane speaks for the centre
+        const uint32_t b = __ballot_sync(0xffffffffu, found);
+        if (found) {
+          // parked where the new track's record will be: {x, y of h0, h0 << 16 | h2 (positions), scatter | centre}
+          const uint4 r0 = ring_p[b0];
+          act_store(nact + nfound + (uint32_t)__popc(b & lt), make_uint4(r0.x, r0.y, (b0 << 16) | b2, __float_as_uint(best_sc)),
+                    make_uint4(j1, 0u, 0u, 0u));
+        }
+        nfound += (uint32_t)__popc(b);
+      }
+    }
+    if (W > 1 && lane == 0) ts.wsum[w] = nfound;
+    team_sync<G>(team);                  // barrier 2: every search is done (module s+1 has been read for the last
+                                         // time); how many seeds each warp found fixes the candidate ids
+    uint32_t base = ncand, total = nfound;
+    if (W > 1) {
+      total = 0;
+#pragma unroll
+      for (uint32_t k = 0; k < W; ++k) { const uint32_t c = ts.wsum[k]; if (k < w) base += c; total += c; }
+    }
+    if (issued > 0) issue(--issued);     // module s-3 into the slot of module s+1
+    for (uint32_t f = lane; f < nfound; f += 32u) {
+      const uint32_t id = base + f;
+      if (id < tcap) {
+        uint4 sb4, sb1;
+        act_load(nact + f, sb4, sb1);
+        const uint32_t j1 = sb1.x, b0 = sb4.z >> 16, b2 = sb4.z & 0xffffu;
+        const uint32_t h0 = off_p + b0, h1 = off_s + j1, h2 = off_u + b2;
+        const uint4 r1 = ring_s[j1], r2 = ring_u[b2];
+        *reinterpret_cast<uint2*>(rows + id * 32u) = make_uint2(h0 | (h1 << 16), h2);
+        float4* rxy = reinterpret_cast<float4*>(rows_xy + id * kXyStride);
+        rxy[0] = make_float4(__uint_as_float(sb4.x), __uint_as_float(sb4.y), __uint_as_float(r1.x), __uint_as_float(r1.y));
+        rows_xy[id * kXyStride + 2u] = make_float2(__uint_as_float(r2.x), __uint_as_float(r2.y));
+        cmeta[id] = make_uint2(7u << u, sb4.w);
+        th0[id] = (uint16_t)h0;
+        act_store(nact + f, make_uint4(r1.x, r1.y, r2.x, r2.y),
+                  make_uint4((r2.z & 0xffff0000u) | id, r2.w, (h1 << 16) | h2, 7u << u));
+      }
+    }
+    nact += nfound; ncand += total;
+    __syncwarp();                        // the appended records and th0 are visible to the warp's other lanes
+    VELO_PH(a.ws.phase_clk, ts, 22);
+    if (ncand > tcap) { if (tid == 0) ts.defer = 1; break; }     // the same for every warp
+  }
+  // every load that was issued must land before the block can be freed
+  while (waited > issued) wait(--waited);
+  team_sync<G>(team);                    // a share that overflowed in the last step's appends is seen by every warp
+  if (ts.defer) {
+    if (tid == 0) {
+      a.ws.ev_info[e].state = kEvDeferred;
+      a.ws.large_list[atomicAdd(&a.ws.counters[kCtrLargeN], 1u)] = e;
+    }
+    return;
+  }
+  // tracks still active take their final module mask; the final flags leave as bits
+  for (uint32_t k = lane; k < nact; k += 32u) {
+    uint4 q0, q1;
+    act_load(k, q0, q1);
+    if (__popc(q1.w) > 3) cmeta[q1.x & 0xffffu].x = q1.w;
+  }
+  {
+    uint32_t* fb = a.ws.flag_bits + ((a.event_offsets[e] - a.event_offsets[0]) >> 5) + e;
+    for (uint32_t i = tid; i < ((n + 31u) >> 5); i += G) fb[i] = flags[i];
+  }
+  if (tid == 0) {
+    a.ws.ev_info[e] = EvInfo{n, kEvReady, ts.cbase, ncand};
     atomicAdd(&a.ws.counters[kCtrCand], ncand);
   }
 }
@@ -480,14 +728,14 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
   }
   __syncthreads();
   VELO_STAGE_BEGIN(a.ws.phase_clk, 1);
-  uint32_t parity = 0, phases = 0;
+  uint32_t phases = 0;
   VELO_PH_START(ts);
   for (;;) {
     if (tid == 0) track_fetch<G>(a, ctl.pool, ts);
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
     VELO_PH(a.ws.phase_clk, ts, 17);     // ticket, descriptors, pool
-    if (!ts.skip) track_event<G, kSameW>(a, ctl.module_z, ctl.tz, ts, pool + ts.pool_off, team, tid, parity, phases);
+    if (!ts.skip) track_event_w<G, kSameW>(a, ctl.module_z, ctl.tz, ts, pool + ts.pool_off, team, tid, phases);
     if (a.pixel && (ts.unpack || (!ts.skip && ts.defer))) unpack_event<G>(a, ts.event, tid);
     team_sync<G>(team);   // every thread is done with the block and with ts before the leader reuses them
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
@@ -515,7 +763,7 @@ __global__ void __launch_bounds__(G, 1) velo_track_big_kernel(const KernelArgs a
     ctl.tz[threadIdx.x] = v;
   }
   TrackTeam<G>& ts = ctl.team[0];
-  uint32_t parity = 0, phases = 0;
+  uint32_t parity = 0;
   const uint32_t base = a.event_offsets[0];
   for (;;) {
     __syncthreads();
@@ -544,7 +792,7 @@ __global__ void __launch_bounds__(G, 1) velo_track_big_kernel(const KernelArgs a
     }
     __syncthreads();
     if (ts.units) break;
-    if (!ts.skip) track_event<G, kSameW, true>(a, ctl.module_z, ctl.tz, ts, blk, 0u, tid, parity, phases);
+    if (!ts.skip) track_event_big<G, kSameW>(a, ctl.module_z, ctl.tz, ts, blk, 0u, tid, parity);
     if (a.pixel && (ts.unpack || (!ts.skip && ts.defer))) unpack_event<G>(a, ts.event, tid);
   }
 }
