@@ -212,10 +212,12 @@ def run_reference(args):
 class Workload:
     """One BASELINE.json config resident in HBM: pinned host arrays, device hits, per-batch outputs."""
 
-    def __init__(self, velo, datagen, sharding, torch, cfg_index, n_events_override, rank, opts_kw, want_pixels=False):
+    def __init__(self, velo, datagen, sharding, torch, cfg_index, n_events_override, rank, opts_kw, want_pixels=False,
+                 custom=None):
         self.torch, self.velo = torch, velo
         self.cfg_index = cfg_index
-        cfg, n_events, n_batches = datagen.CONFIGS[cfg_index]
+        # custom: (GenConfig, n_events, n_batches) of a workload that is not one of BASELINE.json's configs
+        cfg, n_events, n_batches = custom if custom is not None else datagen.CONFIGS[cfg_index]
         if n_events_override:
             n_events = n_events_override
         self.n_events, self.n_batches, self.cfg = n_events, n_batches, cfg
@@ -583,6 +585,24 @@ def run_velo(args):
                            "events_deferred_to_slab_kernel": sum(r["n_deferred"] for r in r2),
                            "roofline": {"bound": "hbm", "step_achieved": gbs2, "peak": peak, "unit": "GB/s", "step_frac": gbs2 / peak,
                                         "stage_ms_per_launch": st2}})
+            w2.free()
+        # SURVEY.md §8(f) f4's layout variants (DESIGN.md §2 A23, L-1), mu = 5 like configs[1]: half of the tracks
+        # backward (same kernels), and the 52-sensor layout (two staggered, overlapping sensors per station: every
+        # event goes through the general kernel, the pipeline keeps one z per module)
+        from dataclasses import replace
+        base_cfg = datagen.CONFIGS[1][0]
+        for name, cfg_v, n_v in (("mu=5, backward_frac 0.5", replace(base_cfg, backward_frac=0.5), 25000),
+                                 ("mu=5, 52-sensor layout (stagger_z 12.5 mm, overlap_x 0.5 mm)",
+                                  replace(base_cfg, stagger_z=12.5, overlap_x=0.5), 5000)):
+            w2 = Workload(velo, datagen, sharding, torch, 1, None, rank, opts_kw, custom=(cfg_v, n_v, 1))
+            _, ps = timed_steps(torch, dist, world, w2, 3, 3)
+            r2 = w2.results()
+            ms2 = float(np.median(ps))
+            launches += kernels_per_batch * (3 + 3)
+            others.append({"workload": f"{name}: {n_v} events in 1 batch, seed 1", "value": n_v / (ms2 * 1e-3), "unit": UNIT,
+                           "hits_per_s": w2.n_hits / (ms2 * 1e-3), "ms_per_step": ms2, "steps": 3, "hits": w2.n_hits,
+                           "tracks": sum(r["n_tracks"] for r in r2),
+                           "events_deferred_to_slab_kernel": sum(r["n_deferred"] for r in r2)})
             w2.free()
         line["other_workloads"] = others
     line["gpu_launches"] = launches
