@@ -235,7 +235,11 @@ class Workload:
         self.off = off = d["event_offsets"]
         self.n_hits = d["n_hits"]
         self.cuts = cuts = [n_events * b // n_batches for b in range(n_batches + 1)]
-        self.g = velo.velo_geometry_load(datagen.MODULE_Z, half_shift_x=cfg.half_shift_x)
+        if cfg.stagger_z != 0.0:      # 52-sensor layout: both sensor planes of every station (include/velo.h module_z_b)
+            za, zb = datagen.sensor_planes(cfg)
+            self.g = velo.velo_geometry_load(za, half_shift_x=cfg.half_shift_x, module_z_b=zb)
+        else:
+            self.g = velo.velo_geometry_load(datagen.MODULE_Z, half_shift_x=cfg.half_shift_x)
         self.P = velo.velo_params_default(self.g)
         self.dh = velo.DeviceHits(d["x"], d["y"], d["z"], d["module"], off)
         self.opts_kw = opts_kw
@@ -587,13 +591,13 @@ def run_velo(args):
                                         "stage_ms_per_launch": st2}})
             w2.free()
         # SURVEY.md §8(f) f4's layout variants (DESIGN.md §2 A23, L-1), mu = 5 like configs[1]: half of the tracks
-        # backward (same kernels), and the 52-sensor layout (two staggered, overlapping sensors per station: every
-        # event goes through the general kernel, the pipeline keeps one z per module)
+        # backward (same kernels), and the 52-sensor layout (two staggered, overlapping sensors per station, both
+        # planes declared in the geometry: the two-plane instantiation of the pipeline's kernels)
         from dataclasses import replace
         base_cfg = datagen.CONFIGS[1][0]
         for name, cfg_v, n_v in (("mu=5, backward_frac 0.5", replace(base_cfg, backward_frac=0.5), 25000),
                                  ("mu=5, 52-sensor layout (stagger_z 12.5 mm, overlap_x 0.5 mm)",
-                                  replace(base_cfg, stagger_z=12.5, overlap_x=0.5), 5000)):
+                                  replace(base_cfg, stagger_z=12.5, overlap_x=0.5), 25000)):
             w2 = Workload(velo, datagen, sharding, torch, 1, None, rank, opts_kw, custom=(cfg_v, n_v, 1))
             _, ps = timed_steps(torch, dist, world, w2, 3, 3)
             r2 = w2.results()

@@ -60,6 +60,11 @@ typedef struct {           /* HOST POD, copied by velo_geometry_load            
   float r_in, r_out;       /* active annulus 5.1 .. 42.0 mm (informational)                      */
   float pitch;             /* pixel pitch 0.055 mm; sets the default sigma_hit = pitch/sqrt(12)  */
   float half_shift_x;      /* 0 closed; 24.5 = the 2023 49 mm opening (§2)           */
+  const float* module_z_b; /* HOST, n_modules, or NULL. The 52-sensor layout (DESIGN.md §2 L-1): */
+                           /* a station's second sensor plane; module_z is then the first one's. */
+                           /* Every plane of module m must lie below every plane of module m+1;  */
+                           /* needs n_modules <= 30. A hit on either plane takes the pipeline;   */
+                           /* any other z is legal and takes the general kernel (as with NULL).  */
 } velo_geometry_desc_t;
 
 /* Validates and copies the description. *out is set to a new handle (free it with

@@ -21,10 +21,23 @@ int velo_geometry_load(const velo_geometry_desc_t* desc, velo_geometry_t** out) 
     if (m && !(desc->module_z[m] > desc->module_z[m - 1])) return VELO_ERR_GEOMETRY;
   }
   if (!(desc->pitch > 0.0f) || !isfinite(desc->pitch)) return VELO_ERR_GEOMETRY;
+  if (desc->module_z_b) {
+    if (desc->n_modules > velo::kTwoPlaneMaxModules) return VELO_ERR_GEOMETRY;
+    for (uint32_t m = 0; m < desc->n_modules; ++m) {
+      const float a = desc->module_z[m], b = desc->module_z_b[m];
+      if (!isfinite(b)) return VELO_ERR_GEOMETRY;
+      if (m) {
+        const float pa = desc->module_z[m - 1], pb = desc->module_z_b[m - 1];
+        if (!((a < b ? a : b) > (pa > pb ? pa : pb))) return VELO_ERR_GEOMETRY;
+      }
+    }
+  }
   velo_geometry* g = new (std::nothrow) velo_geometry();
   if (!g) return VELO_ERR_ARG;
   g->n_modules = desc->n_modules;
   memcpy(g->module_z, desc->module_z, sizeof(float) * desc->n_modules);
+  g->two_plane = desc->module_z_b ? 1u : 0u;
+  if (desc->module_z_b) memcpy(g->module_z_b, desc->module_z_b, sizeof(float) * desc->n_modules);
   g->r_in = desc->r_in; g->r_out = desc->r_out; g->pitch = desc->pitch; g->half_shift_x = desc->half_shift_x;
   *out = g;
   return VELO_OK;
@@ -78,6 +91,8 @@ int run_batch(const velo_geometry_t* g, KernelArgs& a, uint32_t n_events, uint32
   const uint32_t path = opts ? opts->path : 0u;
   a.team_max_hits = kPipeMaxHits;
   for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
+  a.two_plane = g->two_plane;
+  for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z_b[m] = (g->two_plane && m < g->n_modules) ? g->module_z_b[m] : 0.0f;
   a.P = *params;
   if (a.P.max_skipped > 200u) a.P.max_skipped = 200u;  // more misses than modules is all the same
   // A negative window holds no hit (O-3). The kernels take windows >= 0; the same result follows

@@ -38,6 +38,7 @@ template <int G, int kTeams>
 struct FitCtl {
   PoolCtl pool;
   float module_z[VELO_MAX_MODULES];
+  float module_z_b[VELO_MAX_MODULES];  // two-plane geometries (L-1)
   FitTeam<G> team[kTeams];
 };
 
@@ -100,15 +101,19 @@ __device__ __forceinline__ void for_xy(const XyRow& r, uint32_t n, F&& f) {
   }
 }
 
-__device__ __forceinline__ void fit_track(const float2* rxy_g, const float* mz, uint32_t n, uint32_t mask,
+// kTwoPlane (L-1): bit m of the row's kSideSlot entry says on which of module m's two planes the hit lies.
+template <bool kTwoPlane>
+__device__ __forceinline__ void fit_track(const float2* rxy_g, const float* mz, const float* mzb, uint32_t n, uint32_t mask,
                                           float sig2, float inv_s2, float* s9) {
   XyRow rxy;
   rxy.load(rxy_g, n);
+  const uint32_t sides = kTwoPlane ? __float_as_uint(__ldcs(reinterpret_cast<const float*>(rxy_g + kSideSlot))) : 0u;
+  auto zof = [&](uint32_t m) -> float { return (kTwoPlane && ((sides >> m) & 1u)) ? mzb[m] : mz[m]; };
   float sz = 0.0f, sx = 0.0f, sy = 0.0f;
   uint32_t mk = mask;
   for_xy(rxy, n, [&](const float2 p) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    sz = __fadd_rn(sz, mz[m]); sx = __fadd_rn(sx, p.x); sy = __fadd_rn(sy, p.y);
+    sz = __fadd_rn(sz, zof(m)); sx = __fadd_rn(sx, p.x); sy = __fadd_rn(sy, p.y);
   });
   const float nf = (float)n;
   const float zb = __fdiv_rn(sz, nf), xb = __fdiv_rn(sx, nf), yb = __fdiv_rn(sy, nf);
@@ -116,7 +121,7 @@ __device__ __forceinline__ void fit_track(const float2* rxy_g, const float* mz, 
   mk = mask;
   for_xy(rxy, n, [&](const float2 p) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float d = __fsub_rn(mz[m], zb);
+    const float d = __fsub_rn(zof(m), zb);
     sdd = __fadd_rn(sdd, __fmul_rn(d, d));
     sdx = __fadd_rn(sdx, __fmul_rn(d, __fsub_rn(p.x, xb)));
     sdy = __fadd_rn(sdy, __fmul_rn(d, __fsub_rn(p.y, yb)));
@@ -126,7 +131,7 @@ __device__ __forceinline__ void fit_track(const float2* rxy_g, const float* mz, 
   mk = mask;
   for_xy(rxy, n, [&](const float2 p) {
     const uint32_t m = 31u - __clz(mk); mk &= ~(1u << m);
-    const float d = __fsub_rn(mz[m], zb);
+    const float d = __fsub_rn(zof(m), zb);
     const float rx = __fsub_rn(__fsub_rn(p.x, xb), __fmul_rn(tx, d));
     const float ry = __fsub_rn(__fsub_rn(p.y, yb), __fmul_rn(ty, d));
     c = __fadd_rn(c, __fmul_rn(rx, rx));
@@ -169,9 +174,9 @@ __device__ void fit_fetch(const KernelArgs& a, PoolCtl& pool, FitTeam<G>& ts) {
 }
 
 // ---- one pipeline event, by one team ------------------------------------------------------------
-template <int G>
-__device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, unsigned char* blk, uint32_t team,
-                          uint32_t tid, uint32_t& parity) {
+template <int G, bool kTwoPlane = false>
+__device__ void fit_event(const KernelArgs& a, const float* mz, const float* mzb, FitTeam<G>& ts, unsigned char* blk,
+                          uint32_t team, uint32_t tid, uint32_t& parity) {
   const velo_params_t& P = a.P;
   const uint32_t e = ts.event, n = ts.n, nt = ts.ncand, o0 = ts.o0;
   const FitLayout L = fit_layout(n, nt);
@@ -212,7 +217,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
     if (!tstate[t]) continue;
     const uint32_t mask = tmask[t], nh = (uint32_t)__popc(mask);
     float s9[9];
-    fit_track(rows_xy + t * kXyStride, mz, nh, mask, sig2, inv_s2, s9);
+    fit_track<kTwoPlane>(rows_xy + t * kXyStride, mz, mzb, nh, mask, sig2, inv_s2, s9);
     const float lim = __fmul_rn(P.max_chi2_ndof, (float)(2 * (int)nh - 4));
     if (s9[8] > lim) { tstate[t] = 0; continue; }
     const uint32_t centre = rows[t * 32u + 1u];
@@ -272,7 +277,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, FitTeam<G>& ts, 
 }
 
 // ---- the fit kernel: one CTA per SM, kTeams teams of G threads ------------------------------------
-template <int G, int kTeams>
+template <int G, int kTeams, bool kTwoPlane>
 __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArgs a, const uint32_t pool_units) {
   extern __shared__ __align__(16) unsigned char smem[];
   using Ctl = FitCtl<G, kTeams>;
@@ -281,7 +286,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArg
   unsigned char* pool = smem + kCtl;
   const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
   if (threadIdx.x == 0) pool_init(ctl.pool, pool_units);
-  if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
+  if (threadIdx.x < VELO_MAX_MODULES) { ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x]; ctl.module_z_b[threadIdx.x] = a.module_z_b[threadIdx.x]; }
   FitTeam<G>& ts = ctl.team[team];
   __syncthreads();
   VELO_STAGE_BEGIN(a.ws.phase_clk, 2);
@@ -292,7 +297,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArg
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
     VELO_PH(a.ws.phase_clk, ts, 33);     // ticket, descriptors, pool
-    if (!ts.skip) fit_event<G>(a, ctl.module_z, ts, pool + ts.pool_off, team, tid, parity);
+    if (!ts.skip) fit_event<G, kTwoPlane>(a, ctl.module_z, ctl.module_z_b, ts, pool + ts.pool_off, team, tid, parity);
     team_sync<G>(team);
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
     VELO_PH(a.ws.phase_clk, ts, 38);     // clone filter, counts
@@ -333,7 +338,7 @@ __global__ void __launch_bounds__(G, 1) velo_fit_big_kernel(const KernelArgs a) 
     }
     __syncthreads();
     if (ts.units) break;
-    if (!ts.skip) fit_event<G>(a, module_z, ts, blk, 0u, tid, parity);
+    if (!ts.skip) fit_event<G>(a, module_z, module_z, ts, blk, 0u, tid, parity);
   }
 }
 
@@ -466,18 +471,18 @@ __global__ void __launch_bounds__(1024) velo_write_big_kernel(const KernelArgs a
   }
 }
 
-template <int G, int kTeams>
+template <int G, int kTeams, bool kTwoPlane = false>
 int launch_fit_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
   static_assert(G == 32 || kTeams <= 15, "named barriers 1..15");
   using Ctl = FitCtl<G, kTeams>;
   constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
   const uint32_t smem = kCtl + pool_units * kUnitBytes;
-  cudaError_t err = cudaFuncSetAttribute(velo_fit_kernel<G, kTeams>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t err = cudaFuncSetAttribute(velo_fit_kernel<G, kTeams, kTwoPlane>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return (int)err;
   const uint32_t sms = num_sms();
   const uint32_t want = (a.n_events + kTeams - 1) / kTeams;
   const uint32_t grid = want < sms ? (want ? want : 1u) : sms;
-  velo_fit_kernel<G, kTeams><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
+  velo_fit_kernel<G, kTeams, kTwoPlane><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
   return (int)cudaGetLastError();
 }
 
@@ -487,6 +492,8 @@ int launch_fit(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
   if (a.n_events == 0) return 0;
   const uint32_t pu = o.pool_units ? (o.pool_units > kPoolUnitsMax ? kPoolUnitsMax : o.pool_units) : kPoolUnitsMax;
   const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
+  if (a.two_plane)                     // two sensor planes per module (L-1): the default team shapes only
+    return mean < 768u ? launch_fit_t<64, 15, true>(a, stream, pu) : launch_fit_t<128, 8, true>(a, stream, pu);
   switch (o.fit_teams ? o.fit_teams : (mean < 768u ? 15u : 0u)) {   // small events: 15 teams of 64 threads
     case 4: return launch_fit_t<128, 4>(a, stream, pu);
     case 6: return launch_fit_t<128, 6>(a, stream, pu);

@@ -72,6 +72,10 @@ __host__ __device__ inline uint32_t fit_smem_bound(uint32_t n) { return 4u * n +
 // (x, y) of a candidate's hits in discovery order, written by stage 2 as it appends them: stage 3
 // fits from these rows and needs no gather. kXyStride float2 per candidate (16-byte aligned rows).
 constexpr uint32_t kXyStride = VELO_MAX_MODULES;
+// Two-plane geometries (at most 30 modules, so at most 30 hits per candidate): the row's last entry holds,
+// as a bit pattern, which of its module's two planes each hit lies on (bit m = side of the hit in module m).
+constexpr uint32_t kSideSlot = kXyStride - 1u;
+constexpr uint32_t kTwoPlaneMaxModules = 30;
 // per-event state written by stage 1, updated by stage 2
 // kEvBig: an event of more than kPipeMaxHits hits. It runs through the same three stages in their
 // one-event-per-CTA form (velo_*_big_kernel: the sort's and the fit's per-event arrays in a global
@@ -127,6 +131,8 @@ struct KernelArgs {
   uint32_t all_deferred;             // slab-only path: every event was reconstructed by the general kernel
   uint32_t big_path;                 // events above team_max_hits take the one-event-per-CTA pipeline (else the general kernel)
   float module_z[VELO_MAX_MODULES];  // geometry: the shared-memory path requires z[i] == module_z[module[i]]
+  float module_z_b[VELO_MAX_MODULES];// ... or, with two_plane, == module_z_b[module[i]] (the station's second sensor: side 1)
+  uint32_t two_plane;
   velo_params_t P;
   // output
   uint32_t* event_track_offsets;
@@ -182,6 +188,8 @@ int launch_reconstruct(const KernelArgs& a, cudaStream_t stream, void* const* st
 struct velo_geometry {
   uint32_t n_modules;
   float module_z[VELO_MAX_MODULES];
+  float module_z_b[VELO_MAX_MODULES];
+  uint32_t two_plane;
   float r_in, r_out, pitch, half_shift_x;
 };
 namespace velo {

@@ -524,7 +524,9 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const*
   // The one-event-per-CTA kernels are launched only for batches that can hold events above the pool's
   // reach (a mean event above a quarter of kPipeMaxHits): three launches that a mu = 5 batch would only
   // pay for. Without them such events take the general kernel, with the same results.
-  a.big_path = path != kPathSlabOnly && a.n_events > 0 && (unsigned long long)a.n_hits * 4ull > (unsigned long long)kPipeMaxHits * a.n_events ? 1u : 0u;
+  // (not with two sensor planes per module: the records' plane bit needs modules of fewer than 32768 hits)
+  a.big_path = path != kPathSlabOnly && !a.two_plane && a.n_events > 0 &&
+               (unsigned long long)a.n_hits * 4ull > (unsigned long long)kPipeMaxHits * a.n_events ? 1u : 0u;
   auto mark = [&](int k) { if (stage_events && stage_events[k]) cudaEventRecord((cudaEvent_t)stage_events[k], stream); };
   cudaError_t err = cudaMemsetAsync(a.ws.counters, 0, sizeof(uint32_t) * kNumCounters, stream);
   if (err != cudaSuccess) return (int)err;

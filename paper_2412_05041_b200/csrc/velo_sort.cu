@@ -45,7 +45,7 @@ struct SortCtl {
 
 __device__ __forceinline__ uint32_t align16u(uint32_t v) { return (v + 15u) & ~15u; }
 
-struct SortLayout { uint32_t xy, w, bins, stash, mod8, bytes; };
+struct SortLayout { uint32_t xy, w, bins, stash, mod8, side, bytes; };
 __device__ __forceinline__ SortLayout sort_layout(uint32_t n, uint32_t M, uint32_t bins_per_module = kBinsPerModule) {
   SortLayout L;
   uint32_t o = 0;
@@ -54,6 +54,7 @@ __device__ __forceinline__ SortLayout sort_layout(uint32_t n, uint32_t M, uint32
   L.bins = o; o += align16u(2u * (M * bins_per_module + 2u));
   L.stash = o; o += align16u(4u * n);
   L.mod8 = o; o += align16u(n);
+  L.side = o; o += align16u(4u * ((n + 31u) >> 5));   // two-plane geometries: one bit per ORIGINAL index
   L.bytes = o;
   return L;
 }
@@ -112,7 +113,10 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
   uint32_t* binsw = (uint32_t*)(blk + L.bins);
   uint16_t* bo = (uint16_t*)binsw;
   uint32_t* stash = (uint32_t*)(blk + L.stash);
-  uint8_t* mod8 = blk + L.mod8;                 // module by SORTED position
+  uint8_t* mod8 = blk + L.mod8;                 // module by SORTED position (bit 7: the hit's plane, two-plane geometries)
+  uint32_t* sideb = (uint32_t*)(blk + L.side);
+  const float* mzb = a.module_z_b;              // (constant bank: read once per hit, two-plane geometries only)
+  const bool two_plane = a.two_plane != 0u;
   const size_t g0 = (size_t)(ts.o0 - a.hit_base);
   const float* gx = a.x + g0; const float* gy = a.y + g0; const float* gz = a.z + g0;
   const uint8_t* gm = a.module + g0;
@@ -121,12 +125,17 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
   // ---- S0 decode: phi16 (O-1), bucket histogram; the plane check of the pipeline path -------------
   const uint32_t nwords = nbins / 2u;
   for (uint32_t b = tid; b <= nwords; b += G) binsw[b] = 0;
+  if (two_plane) for (uint32_t b = tid; b < ((n + 31u) >> 5); b += G) sideb[b] = 0;
   team_sync<G>(team);
   {
     uint32_t trouble = 0;
     auto decode = [&](uint32_t i, float x, float y, float z, uint32_t m) {
       if (m >= M) { trouble |= 0x80000000u; return; }
-      if (__float_as_uint(z) != __float_as_uint(mz[m])) trouble |= 1u;
+      if (__float_as_uint(z) != __float_as_uint(mz[m])) {
+        // L-1: the station's second sensor plane, else the event is the general kernel's
+        if (two_plane && __float_as_uint(z) == __float_as_uint(mzb[m])) atomicOr(&sideb[i >> 5], 1u << (i & 31u));
+        else trouble |= 1u;
+      }
       const uint32_t pu = (uint32_t)(phi16(x, y) + 32768);
       const uint32_t bin = m * kBinsPerModule + (pu >> kBinShift);
       const uint32_t sh = (bin & 1u) * 16u;
@@ -233,7 +242,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
     const uint32_t st = stash[i], pu = (st >> 11) & 0xffffu, m = st >> 27;
     const uint32_t r = (uint32_t)bo[m * kBinsPerModule + (pu >> kBinShift)] + (st & kMaxBinSlot);
     w[r] = (pu << 16) | i;
-    mod8[r] = (uint8_t)m;
+    mod8[r] = (uint8_t)(two_plane ? m | (((sideb[i >> 5] >> (i & 31u)) & 1u) << 7) : m);
   }
   team_sync<G>(team);
   VELO_PH(a.ws.phase_clk, ts, 13);
@@ -255,7 +264,7 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
   uint4* rec = a.ws.rec16 + sb;
   uint16_t* sorig = a.ws.sorig + sb;
   for (uint32_t h = tid; h < n; h += G) {
-    const uint32_t item = w[h], pu = item >> 16, i = item & 0xffffu, m = mod8[h];
+    const uint32_t item = w[h], pu = item >> 16, i = item & 0xffffu, m8 = mod8[h], m = m8 & 31u;
     const float2 p = xyo[i];
     uint32_t sp1 = 0, sm1 = 0, sm2 = 0;
     if (!whole) {
@@ -264,7 +273,9 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
       if (m >= 1u) sm1 = start_in(m - 1u, lo);
       if (m >= 2u) sm2 = start_in(m - 2u, lo);
     }
-    rec[h] = make_uint4(__float_as_uint(p.x), __float_as_uint(p.y), (pu << 16) | sp1, (sm1 << 16) | sm2);
+    // two-plane geometries: bit 15 of the last word is the hit's plane (a module of a pipeline event has
+    // fewer than 32768 hits, so start(m-2) leaves it free)
+    rec[h] = make_uint4(__float_as_uint(p.x), __float_as_uint(p.y), (pu << 16) | sp1, (sm1 << 16) | sm2 | ((m8 >> 7) << 15));
     sorig[h] = (uint16_t)i;
   }
   // module offsets and the largest module

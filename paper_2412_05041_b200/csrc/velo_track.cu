@@ -48,6 +48,7 @@ template <int G, int kTeams>
 struct TrackCtl {
   PoolCtl pool;
   float module_z[VELO_MAX_MODULES];
+  float module_z_b[VELO_MAX_MODULES];  // two-plane geometries (L-1): the modules' second sensor planes
   float tz[VELO_MAX_MODULES * 4];    // O-4's z ratio for a track whose latest hits are on modules mb and mb + 1 + gap,
                                      // forwarded to module mb - 1 - pend: [mb][gap][pend], gap and pend 0 or 1
   TrackTeam<G> team[kTeams];
@@ -428,9 +429,16 @@ __device__ void track_event_big(const KernelArgs& a, const float* mz, const floa
 //   * barrier 1 follows forwarding (the flags of the step are final), barrier 2 follows the search:
 //     the warps exchange how many seeds each found, which fixes the candidate ids in the order B1
 //     (centre position ascending: warp 0's share precedes warp 1's), then each warp writes its own.
-template <int G, bool kSameW>
-__device__ void track_event_w(const KernelArgs& a, const float* mz, const float* tzt, TrackTeam<G>& ts, unsigned char* blk,
-                              uint32_t team, uint32_t tid, uint32_t& phases) {
+// kTwoPlane (DESIGN.md §2 L-1: two sensor planes per module): bit 15 of a record's last word says which
+// plane the hit lies on, O-4's z ratio is taken per candidate plane, bits 31 and 30 of an active track's
+// module mask hold the planes of its latest and previous hit, and the planes of all its hits leave in
+// the last entry of its coordinate row (kSideSlot) for the fit.
+template <int G, bool kSameW, bool kTwoPlane>
+__device__ void track_event_w(const KernelArgs& a, const float* mz, const float* mzb, const float* tzt, TrackTeam<G>& ts,
+                              unsigned char* blk, uint32_t team, uint32_t tid, uint32_t& phases) {
+  constexpr uint32_t kMaskBits = kTwoPlane ? 0x3fffffffu : 0xffffffffu;
+  constexpr uint32_t kStartBits = kTwoPlane ? 0x7fffu : 0xffffu;
+  auto plane_of = [](const uint4& r) -> uint32_t { return (r.w >> 15) & 1u; };
   constexpr uint32_t W = G / 32;
   const uint32_t lane = tid & 31u, w = tid >> 5, lt = (1u << lane) - 1u;
   const uint32_t M = a.n_modules, n = ts.n, e = ts.event;
@@ -514,18 +522,26 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
         act_load(k, q0, q1);
         const float x0 = __uint_as_float(q0.x), y0 = __uint_as_float(q0.y);
         const float x1 = __uint_as_float(q0.z), y1 = __uint_as_float(q0.w);
-        const uint32_t c = q1.x >> 16, id = q1.x & 0xffffu, w3 = q1.y, hab = q1.z, mask = q1.w;
+        const uint32_t c = q1.x >> 16, id = q1.x & 0xffffu, w3 = q1.y, hab = q1.z, mask = q1.w & kMaskBits;
         const uint32_t mb = __ffs(mask) - 1u, ma = __ffs(mask & (mask - 1u)) - 1u;
         const uint32_t gap = ma - mb - 1u, pend = mb - s;     // pend: modules already missed since the latest hit
-        float tz;
-        if ((gap | pend) <= 1u) tz = tzt[mb * 4u + gap * 2u + pend];        // the same quotient, taken once per CTA
+        float tz, px_b = 0.0f, py_b = 0.0f;                   // (px_b, py_b): the prediction on the module's second plane
+        if constexpr (kTwoPlane) {
+          const float z1 = (q1.w >> 31) ? mzb[mb] : mz[mb], z0 = ((q1.w >> 30) & 1u) ? mzb[ma] : mz[ma];
+          const float den = __fsub_rn(z1, z0);
+          tz = __fdiv_rn(__fsub_rn(z2, z1), den);
+          const float tzb = __fdiv_rn(__fsub_rn(mzb[u], z1), den);
+          px_b = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, x0), tzb));
+          py_b = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, y0), tzb));
+        } else if ((gap | pend) <= 1u) tz = tzt[mb * 4u + gap * 2u + pend];        // the same quotient, taken once per CTA
         else { const float z1 = mz[mb], z0 = mz[ma]; tz = __fdiv_rn(__fsub_rn(z2, z1), __fsub_rn(z1, z0)); }
         const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, x0), tz));
         const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, y0), tz));
         const Win wx = make_win(c, Wfwd);
         bool found = false; uint32_t best = 0; float best_sc = 0.0f;
         auto visit = [&](uint32_t jj, const uint4& r, bool in) {
-          const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+          const bool pb = kTwoPlane && plane_of(r) != 0u;
+          const float ex = __fsub_rn(pb ? px_b : px, __uint_as_float(r.x)), ey = __fsub_rn(pb ? py_b : py, __uint_as_float(r.y));
           const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
           bool ok = in & (sc <= max_fwd) & (!found | (sc < best_sc));
           if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
@@ -534,12 +550,13 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
         if (pend <= 1u) {
           const Win ww = kSameW ? wx : make_win(c, Wwide);
           if (ww.wrapped) scan_run<true>(ring_u, 0u, nu, ww.lo16, ww.lim, visit);          // low-phi run of a window across +-pi
-          scan_run<true>(ring_u, pend ? (w3 & 0xffffu) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
+          scan_run<true>(ring_u, pend ? (w3 & kStartBits) : (w3 >> 16), nu, ww.lo16, ww.lim, visit);
         } else {
           // no stored start for a target this far from the latest hit (max_skipped >= 2): whole module
           for (uint32_t j = 0; j < nu; ++j) {
             const uint4 r = ring_u[j];
-            const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+            const bool pb = kTwoPlane && plane_of(r) != 0u;
+            const float ex = __fsub_rn(pb ? px_b : px, __uint_as_float(r.x)), ey = __fsub_rn(pb ? py_b : py, __uint_as_float(r.y));
             const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
             const bool ok = (r.z - wx.lo16 <= wx.lim) & (sc <= max_fwd) & (!found | (sc < best_sc));
             found |= ok; best = ok ? j : best; best_sc = ok ? sc : best_sc;
@@ -554,7 +571,13 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
           if (nh + 1u == 4u) { set_flag(th0[id]); set_flag(hab >> 16); set_flag(hab & 0xffffu); }
           if (nh + 1u >= 4u) set_flag(h2);
           q0 = make_uint4(q0.z, q0.w, r2.x, r2.y);
-          q1 = make_uint4((r2.z & 0xffff0000u) | id, r2.w, (hab << 16) | h2, mask | (1u << u));
+          uint32_t nmask = mask | (1u << u);
+          if constexpr (kTwoPlane) {
+            const uint32_t p2 = plane_of(r2);
+            nmask |= (p2 << 31) | ((q1.w >> 31) << 30);
+            if (p2) atomicOr(reinterpret_cast<uint32_t*>(rows_xy + id * kXyStride + kSideSlot), 1u << u);
+          }
+          q1 = make_uint4((r2.z & 0xffff0000u) | id, r2.w, (hab << 16) | h2, nmask);
           alive = true;
         } else {
           alive = (mb - u) <= P.max_skipped;       // consecutive misses so far, this one included
@@ -600,6 +623,7 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
           j1 = clw[k];
           const uint4 r1 = ring_s[j1];
           const float x1 = __uint_as_float(r1.x), y1 = __uint_as_float(r1.y);
+          const float z1c = (kTwoPlane && plane_of(r1)) ? mzb[s] : zc1;
           const uint32_t c = r1.z >> 16;
           const Win wx = make_win(c, Wseed);
           const Win ww = kSameW ? wx : make_win(c, Wwide);
@@ -609,11 +633,19 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
               if (!(r0.z - ww.lo16 <= ww.lim)) break;
               if (!kSameW && !(r0.z - wx.lo16 <= wx.lim)) continue;
               if (flagged(off_p + j0)) continue;
-              const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tz));
-              const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tz));
+              float tza = tz, tzb = 0.0f;
+              if constexpr (kTwoPlane) {
+                const float den = __fsub_rn(z1c, plane_of(r0) ? mzb[s + 1] : zc0);
+                tza = __fdiv_rn(__fsub_rn(z2, z1c), den); tzb = __fdiv_rn(__fsub_rn(mzb[u], z1c), den);
+              }
+              const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tza));
+              const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tza));
+              const float px_b = kTwoPlane ? __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tzb)) : 0.0f;
+              const float py_b = kTwoPlane ? __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tzb)) : 0.0f;
               // h0 and h2 ascending: strict < keeps the lexicographic minimum; branch-free body
               auto visit2 = [&](uint32_t jj, const uint4& r, bool in) {
-                const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
+                const bool pb = kTwoPlane && plane_of(r) != 0u;
+                const float ex = __fsub_rn(pb ? px_b : px, __uint_as_float(r.x)), ey = __fsub_rn(pb ? py_b : py, __uint_as_float(r.y));
                 const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
                 bool ok = in & !flagged(off_u + jj) & (sc <= max_seed) & (!found | (sc < best_sc));
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
@@ -638,7 +670,7 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
           // parked where the new track's record will be: {x, y of h0, h0 << 16 | h2 (positions), scatter | centre}
           const uint4 r0 = ring_p[b0];
           act_store(nact + nfound + (uint32_t)__popc(b & lt), make_uint4(r0.x, r0.y, (b0 << 16) | b2, __float_as_uint(best_sc)),
-                    make_uint4(j1, 0u, 0u, 0u));
+                    make_uint4(j1, plane_of(r0), 0u, 0u));
         }
         nfound += (uint32_t)__popc(b);
       }
@@ -667,8 +699,14 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
         rows_xy[id * kXyStride + 2u] = make_float2(__uint_as_float(r2.x), __uint_as_float(r2.y));
         cmeta[id] = make_uint2(7u << u, sb4.w);
         th0[id] = (uint16_t)h0;
+        uint32_t nmask = 7u << u;
+        if constexpr (kTwoPlane) {
+          const uint32_t p0 = sb1.y, p1 = plane_of(r1), p2 = plane_of(r2);
+          nmask |= (p2 << 31) | (p1 << 30);
+          rows_xy[id * kXyStride + kSideSlot] = make_float2(__uint_as_float((p0 << (s + 1u)) | (p1 << s) | (p2 << u)), 0.0f);
+        }
         act_store(nact + f, make_uint4(r1.x, r1.y, r2.x, r2.y),
-                  make_uint4((r2.z & 0xffff0000u) | id, r2.w, (h1 << 16) | h2, 7u << u));
+                  make_uint4((r2.z & 0xffff0000u) | id, r2.w, (h1 << 16) | h2, nmask));
       }
     }
     nact += nfound; ncand += total;
@@ -690,7 +728,7 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
   for (uint32_t k = lane; k < nact; k += 32u) {
     uint4 q0, q1;
     act_load(k, q0, q1);
-    if (__popc(q1.w) > 3) cmeta[q1.x & 0xffffu].x = q1.w;
+    if (__popc(q1.w & kMaskBits) > 3) cmeta[q1.x & 0xffffu].x = q1.w & kMaskBits;
   }
   {
     uint32_t* fb = a.ws.flag_bits + ((a.event_offsets[e] - a.event_offsets[0]) >> 5) + e;
@@ -703,7 +741,7 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
 }
 
 // ---- the kernel: one CTA per SM, kTeams teams of G threads ---------------------------------------
-template <int G, int kTeams, bool kSameW>
+template <int G, int kTeams, bool kSameW, bool kTwoPlane>
 __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelArgs a, const uint32_t pool_units) {
   extern __shared__ __align__(16) unsigned char smem[];
   using Ctl = TrackCtl<G, kTeams>;
@@ -712,7 +750,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
   unsigned char* pool = smem + kCtl;
   const uint32_t team = threadIdx.x / G, tid = threadIdx.x % G;
   if (threadIdx.x == 0) pool_init(ctl.pool, pool_units);
-  if (threadIdx.x < VELO_MAX_MODULES) ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x];
+  if (threadIdx.x < VELO_MAX_MODULES) { ctl.module_z[threadIdx.x] = a.module_z[threadIdx.x]; ctl.module_z_b[threadIdx.x] = a.module_z_b[threadIdx.x]; }
   if (threadIdx.x < VELO_MAX_MODULES * 4u) {
     const uint32_t mb = threadIdx.x >> 2, gap = (threadIdx.x >> 1) & 1u, pend = threadIdx.x & 1u, ma = mb + 1u + gap;
     float v = 0.0f;
@@ -735,7 +773,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_track_kernel(const KernelA
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
     VELO_PH(a.ws.phase_clk, ts, 17);     // ticket, descriptors, pool
-    if (!ts.skip) track_event_w<G, kSameW>(a, ctl.module_z, ctl.tz, ts, pool + ts.pool_off, team, tid, phases);
+    if (!ts.skip) track_event_w<G, kSameW, kTwoPlane>(a, ctl.module_z, ctl.module_z_b, ctl.tz, ts, pool + ts.pool_off, team, tid, phases);
     if (a.pixel && (ts.unpack || (!ts.skip && ts.defer))) unpack_event<G>(a, ts.event, tid);
     team_sync<G>(team);   // every thread is done with the block and with ts before the leader reuses them
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
@@ -815,27 +853,35 @@ int launch_track_big_t(const KernelArgs& a, cudaStream_t stream) {
   return (int)cudaGetLastError();
 }
 
-template <int G, int kTeams>
-int launch_track_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
+template <int G, int kTeams, bool kSameW, bool kTwoPlane>
+int launch_track_k(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
   static_assert(G == 32 || kTeams <= 15, "named barriers 1..15");
   using Ctl = TrackCtl<G, kTeams>;
   constexpr uint32_t kCtl = (sizeof(Ctl) + 127u) & ~127u;
   const uint32_t smem = kCtl + pool_units * kUnitBytes;
-  const bool same = a.P.phi_window_seed == a.P.phi_window_fwd;
   const uint32_t sms = num_sms();
   const uint32_t want = (a.n_events + kTeams - 1) / kTeams;
   const uint32_t grid = want < sms ? (want ? want : 1u) : sms;
-  cudaError_t err;
-  if (same) {
-    err = cudaFuncSetAttribute(velo_track_kernel<G, kTeams, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return (int)err;
-    velo_track_kernel<G, kTeams, true><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
-  } else {
-    err = cudaFuncSetAttribute(velo_track_kernel<G, kTeams, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return (int)err;
-    velo_track_kernel<G, kTeams, false><<<grid, G * kTeams, smem, stream>>>(a, pool_units);
-  }
+  auto* kern = velo_track_kernel<G, kTeams, kSameW, kTwoPlane>;
+  const cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (err != cudaSuccess) return (int)err;
+  kern<<<grid, G * kTeams, smem, stream>>>(a, pool_units);
   return (int)cudaGetLastError();
+}
+
+template <int G, int kTeams>
+int launch_track_t(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
+  const bool same = a.P.phi_window_seed == a.P.phi_window_fwd;
+  return same ? launch_track_k<G, kTeams, true, false>(a, stream, pool_units)
+              : launch_track_k<G, kTeams, false, false>(a, stream, pool_units);
+}
+
+// Two sensor planes per module (L-1): the default team shapes only.
+template <int G, int kTeams>
+int launch_track_2p(const KernelArgs& a, cudaStream_t stream, uint32_t pool_units) {
+  const bool same = a.P.phi_window_seed == a.P.phi_window_fwd;
+  return same ? launch_track_k<G, kTeams, true, true>(a, stream, pool_units)
+              : launch_track_k<G, kTeams, false, true>(a, stream, pool_units);
 }
 
 }  // namespace
@@ -850,6 +896,11 @@ int launch_track(const KernelArgs& a, cudaStream_t stream, const PipeOpts& o) {
     const uint32_t mean = a.n_events ? a.n_hits / a.n_events : 0u;
     g = mean >= 6144u ? 128u : mean < 768u ? 32u : 64u;
     if (g == 32u && t == 0) t = 24;            // small events (open VELO): a warp per event, 24 in flight
+  }
+  if (a.two_plane) {
+    if (g == 128) return launch_track_2p<128, 6>(a, stream, pu);
+    if (g == 64) return launch_track_2p<64, 12>(a, stream, pu);
+    return launch_track_2p<32, 24>(a, stream, pu);
   }
   if (g == 128) {
     if (t == 0) t = 6;

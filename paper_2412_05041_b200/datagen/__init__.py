@@ -182,6 +182,13 @@ def generate_config(i: int, n_events: int | None = None, e0: int = 0, **kw) -> d
     return generate(cfg, e0, n if n_events is None else n_events, **kw)
 
 
+def sensor_planes(cfg: GenConfig) -> tuple[np.ndarray, np.ndarray]:
+    """z of the two sensor planes of every station in the 52-sensor layout (stagger_z): the -x sensor's and
+    the +x sensor's, as the fp32 values the generated hits carry (include/velo.h: module_z, module_z_b)."""
+    z = np.asarray(cfg.module_z, dtype=np.float64)
+    return (z - 0.5 * cfg.stagger_z).astype(np.float32), (z + 0.5 * cfg.stagger_z).astype(np.float32)
+
+
 def ideal_config(**kw) -> GenConfig:
     """Noise-free, 100 % efficient, unquantised, unscattered straight tracks (SURVEY.md §8(c)
     whole-path pin (ii))."""

@@ -41,7 +41,7 @@ class VeloError(RuntimeError):
 
 class GeometryDesc(ctypes.Structure):
     _fields_ = [("n_modules", c_uint32), ("module_z", POINTER(c_float)), ("r_in", c_float),
-                ("r_out", c_float), ("pitch", c_float), ("half_shift_x", c_float)]
+                ("r_out", c_float), ("pitch", c_float), ("half_shift_x", c_float), ("module_z_b", POINTER(c_float))]
 
 
 class Params(ctypes.Structure):
@@ -159,10 +159,14 @@ def velo_version() -> str:
 class Geometry:
     """Owns a velo_geometry_t handle."""
 
-    def __init__(self, module_z, r_in=5.1, r_out=42.0, pitch=0.055, half_shift_x=0.0):
+    def __init__(self, module_z, r_in=5.1, r_out=42.0, pitch=0.055, half_shift_x=0.0, module_z_b=None):
         z = np.ascontiguousarray(module_z, dtype=np.float32)
+        zb = None if module_z_b is None else np.ascontiguousarray(module_z_b, dtype=np.float32)
+        if zb is not None and zb.shape != z.shape:
+            raise ValueError("module_z_b: one plane per module")
         desc = GeometryDesc(n_modules=z.shape[0], module_z=z.ctypes.data_as(POINTER(c_float)),
-                            r_in=r_in, r_out=r_out, pitch=pitch, half_shift_x=half_shift_x)
+                            r_in=r_in, r_out=r_out, pitch=pitch, half_shift_x=half_shift_x,
+                            module_z_b=None if zb is None else zb.ctypes.data_as(POINTER(c_float)))
         h = c_void_p()
         rc = lib().velo_geometry_load(byref(desc), byref(h))
         if rc != VELO_OK:

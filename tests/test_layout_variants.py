@@ -150,8 +150,8 @@ def test_efficiency_in_the_52_sensor_layout_with_overlap():
 
 @pytest.mark.gpu
 def test_gpu_parity_in_the_52_sensor_layout():
-    """The pipeline's fast path takes one z per module; hits on the staggered sensors are off that plane, so
-    every event goes to the general kernel: same tracks as the oracle, bit for bit."""
+    """With one plane per module declared, hits on the staggered sensors are off that plane, so every event
+    goes to the general kernel: same tracks as the oracle, bit for bit."""
     import torch
     assert torch.cuda.is_available()
     from paper_2412_05041_b200 import build as vbuild
@@ -164,3 +164,84 @@ def test_gpu_parity_in_the_52_sensor_layout():
     info = T.assert_same_result(got, want)
     assert info["bit_identical_states"] and got["n_deferred"] > 1900
     np.testing.assert_array_equal(got["track_hits"], want["track_hits"])
+
+
+def test_sensor_planes_are_the_z_of_the_generated_hits():
+    """datagen.sensor_planes gives, bit for bit, the two z values the hits of a station carry (the planes the
+    library's geometry takes as module_z and module_z_b): -x sensor below, +x sensor above."""
+    cfg = replace(datagen.GenConfig(), stagger_z=12.5, overlap_x=0.5)
+    d = datagen.generate(cfg, 0, 50)
+    za, zb = datagen.sensor_planes(cfg)
+    m = d["module"].astype(np.int64)
+    on_a, on_b = d["z"] == za[m], d["z"] == zb[m]
+    assert np.all(on_a | on_b) and on_a.any() and on_b.any()
+    assert np.all(za < zb) and np.all(zb[:-1] < za[1:])
+    # hits of the -x sensor sit at x below the overlap strip's upper edge, those of the +x one above its lower edge
+    assert d["x"][on_a].max() < 0.5 + 0.06 and d["x"][on_b].min() > -0.5 - 0.06
+
+
+def test_geometry_with_two_planes_is_validated():
+    """include/velo.h velo_geometry_desc_t.module_z_b: every plane of module m below every plane of m+1,
+    at most 30 modules."""
+    from paper_2412_05041_b200 import build as vbuild
+    from paper_2412_05041_b200 import velo
+    vbuild.build()
+    cfg = replace(datagen.GenConfig(), stagger_z=12.5)
+    za, zb = datagen.sensor_planes(cfg)
+    assert velo.Geometry(za, module_z_b=zb).n_modules == 26
+    bad = zb.copy(); bad[3] = za[4] + 1.0                       # reaches beyond the next station's first plane
+    with pytest.raises(velo.VeloError):
+        velo.Geometry(za, module_z_b=bad)
+    z31 = np.arange(31, dtype=np.float32) * 30.0
+    velo.Geometry(z31)                                          # one plane: up to 32 modules
+    with pytest.raises(velo.VeloError):
+        velo.Geometry(z31, module_z_b=z31 + 10.0)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", ["mu5", "open", "dense"])
+def test_gpu_parity_in_the_52_sensor_layout_with_both_planes_declared(case):
+    """With both sensor planes in the geometry the events stay in the three-stage pipeline (hits carry their
+    plane through the sorted records, O-4 and O-11 take z per plane): same tracks as the oracle, bit for
+    bit, nothing deferred; and the same again through the general kernel alone."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2412_05041_b200 import build as vbuild
+    from paper_2412_05041_b200 import velo
+    vbuild.build()
+    base = {"mu5": datagen.GenConfig(), "open": datagen.CONFIGS[3][0], "dense": replace(datagen.GenConfig(), mu=20.0)}[case]
+    cfg = replace(base, stagger_z=12.5, overlap_x=0.5, backward_frac=0.2)
+    d = datagen.generate(cfg, 0, {"mu5": 1500, "open": 3000, "dense": 300}[case])
+    za, zb = datagen.sensor_planes(cfg)
+    want = T.oracle_parallel(d, 26, None, None)
+    got = velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], za, n_batches=2, module_z_b=zb,
+                           half_shift_x=cfg.half_shift_x)
+    info = T.assert_same_result(got, want)
+    # (a dense event may still overflow its candidate table and go to the general kernel, as in any layout)
+    assert info["bit_identical_states"] and got["n_deferred"] <= (3 if case == "dense" else 0)
+    np.testing.assert_array_equal(got["track_hits"], want["track_hits"])
+    slab = velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], za, n_batches=1, module_z_b=zb,
+                            half_shift_x=cfg.half_shift_x, opts=velo.LaunchOptions(path=1))
+    assert T.assert_same_result(slab, want)["bit_identical_states"]
+
+
+@pytest.mark.gpu
+def test_gpu_a_hit_off_both_planes_sends_its_event_to_the_general_kernel():
+    """Two planes declared, one hit of a few events moved off them: those events (only) are deferred, results
+    stay equal to the oracle."""
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2412_05041_b200 import build as vbuild
+    from paper_2412_05041_b200 import velo
+    vbuild.build()
+    cfg = replace(datagen.GenConfig(), stagger_z=12.5, overlap_x=0.5)
+    d = datagen.generate(cfg, 0, 400)
+    za, zb = datagen.sensor_planes(cfg)
+    z = d["z"].copy(); off = d["event_offsets"].astype(np.int64)
+    moved = [e for e in (3, 77, 250) if off[e + 1] > off[e]]
+    for e in moved:
+        z[off[e]] += 0.25
+    d2 = dict(d); d2["z"] = z
+    want = T.oracle_parallel(d2, 26, None, None)
+    got = velo.reconstruct(d2["x"], d2["y"], z, d2["module"], d2["event_offsets"], za, n_batches=1, module_z_b=zb)
+    assert T.assert_same_result(got, want)["bit_identical_states"] and got["n_deferred"] == len(moved)
