@@ -42,8 +42,9 @@ enum {
   VELO_ERR_WORKSPACE = -3, /* workspace_bytes < velo_workspace_bytes(...)                        */
   VELO_ERR_CUDA = -4,      /* a CUDA runtime call or a kernel launch failed                      */
   VELO_ERR_CAPACITY = -5,  /* (device status) tracks or track-hits exceed the output capacities  */
-  VELO_ERR_INPUT = -6      /* (device status) module id >= n_modules, non-monotone offsets, or   */
+  VELO_ERR_INPUT = -6,     /* (device status) module id >= n_modules, non-monotone offsets, or   */
                            /* an event with more than VELO_MAX_EVENT_HITS hits                   */
+  VELO_ERR_STATIC_LIMIT = -7 /* sizes beyond the fixed maximum of a *_static entry point         */
 };
 
 #define VELO_MAX_MODULES 32
@@ -269,6 +270,23 @@ size_t velo_pv_workspace_bytes(uint32_t n_events, uint32_t cap_tracks);
  * summary[0] = the required capacity; a failed velo_reconstruct status is passed on. */
 int velo_pv_find(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_params_t* params, velo_pvs_t* out,
                  void* workspace, size_t workspace_bytes, void* stream);
+
+/* The same operation for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the workspace is a fixed array inside the
+ * library (a file-scope `static __device__` array of 4 736 256 bytes, which every GPU that loads the
+ * library holds until the process exits), so the call takes no workspace and performs no cudaMalloc,
+ * cudaFree or allocating library call. Inputs, outputs, results and error behaviour are those of
+ * velo_pv_find, with two fixed limits: n_events <= VELO_PV_STATIC_MAX_EVENTS and tracks->cap_tracks <=
+ * VELO_PV_STATIC_MAX_TRACKS; larger sizes return VELO_ERR_STATIC_LIMIT and enqueue nothing.
+ * The array is shared by every call on the device and keeps the last call's contents; the kernels
+ * write every word of it before they read it, so nothing needs clearing between calls. Calls that
+ * overlap on the GPU (different streams, or graphs replayed concurrently) RACE on it: serialise them
+ * (one stream, or events), or use velo_pv_find with one workspace per stream. The array's device
+ * address is looked up once per device (cudaGetSymbolAddress, with that device current). */
+#define VELO_PV_STATIC_MAX_EVENTS 4096u
+#define VELO_PV_STATIC_MAX_TRACKS 2097152u
+int velo_pv_find_static(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_params_t* params, velo_pvs_t* out,
+                        void* stream);
 
 /* Library version string, e.g. "velo-b200 0.1 (sm_100a)". */
 const char* velo_version(void);

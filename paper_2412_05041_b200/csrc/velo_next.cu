@@ -7,6 +7,8 @@
 // Both consume the device outputs of velo_reconstruct. Every float operation is a round-to-nearest
 // intrinsic in the order DESIGN.md §2 fixes (no FMA contraction): the filter's chi2 and the fitted
 // vertex decide integers (track weights > 0, vertices kept), so the order is part of the method.
+#include <mutex>
+
 #include "velo_device.cuh"
 #include "velo_internal.h"
 
@@ -384,6 +386,34 @@ PvWorkspace carve_pv(void* base, uint32_t n_events, uint32_t cap_tracks) {
   return w;
 }
 
+// ---- velo_pv_find_static: the finder's scratch as a fixed array inside the library ------------------
+// For callers that cannot allocate (include/velo.h). In HOST code the name g_pv_static is a host-side
+// stand-in, not a device address: the address the kernels get comes from cudaGetSymbolAddress, once per
+// device, with that device current. Every call on a device shares the array (calls that overlap race).
+constexpr size_t r256(size_t b) { return (b + 255) / 256 * 256; }
+constexpr size_t kPvStaticBytes = r256(sizeof(float) * 5u * kPvMax * ((size_t)VELO_PV_STATIC_MAX_EVENTS + 1)) +
+                                  r256(4 * ((size_t)VELO_PV_STATIC_MAX_EVENTS + 1)) +
+                                  r256((size_t)VELO_PV_STATIC_MAX_TRACKS + 1);       // = carve_pv at the two maxima
+static_assert(kPvStaticBytes == 4736256, "include/velo.h states this size");
+static __device__ __align__(256) unsigned char g_pv_static[kPvStaticBytes];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_pv_static_mutex;
+void* g_pv_static_ptr[kMaxDevices] = {};     // device address of g_pv_static on device i, once looked up
+
+// Device address of the array on the current device; nullptr if a CUDA call fails.
+void* pv_static_address() {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+  std::lock_guard<std::mutex> lock(g_pv_static_mutex);
+  if (!g_pv_static_ptr[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_pv_static) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    g_pv_static_ptr[dev] = p;
+  }
+  return g_pv_static_ptr[dev];
+}
+
 }  // namespace
 
 }  // namespace velo
@@ -451,6 +481,44 @@ int velo_pv_find(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_p
   const uint32_t smem = kPvWarps * (4u * nbw + 4u * params->n_bins + 4u * kPvMax);
   cudaError_t err = cudaFuncSetAttribute(velo_pv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return VELO_ERR_CUDA;
+  if (n_events > 0) {
+    uint32_t grid = (n_events + kPvWarps - 1) / kPvWarps;
+    const uint32_t most = num_sms() * 8u;
+    if (grid > most) grid = most;
+    velo_pv_kernel<<<grid, 32 * kPvWarps, smem, st>>>(a);
+  }
+  velo_pv_offsets_kernel<<<1, 1024, 0, st>>>(a, out->event_pv_offsets, out->cap_pvs, out->summary);
+  if (n_events > 0) {
+    const size_t slots = (size_t)n_events * kPvMax;
+    velo_pv_place_kernel<<<(uint32_t)((slots + 255) / 256), 256, 0, st>>>(a, out->event_pv_offsets, out->pvs, out->cap_pvs);
+  }
+  return cudaGetLastError() == cudaSuccess ? VELO_OK : VELO_ERR_CUDA;
+}
+
+// The same launches as velo_pv_find over the library's own array: no allocation of any kind.
+int velo_pv_find_static(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_params_t* params, velo_pvs_t* out,
+                        void* stream) {
+  using namespace velo;
+  if (!tracks || !params || !out) return VELO_ERR_ARG;
+  if (!tracks->event_track_offsets || !tracks->states || !tracks->summary || tracks->cap_tracks == 0) return VELO_ERR_ARG;
+  if (!out->event_pv_offsets || !out->pvs || !out->summary || out->cap_pvs == 0) return VELO_ERR_ARG;
+  if (params->n_bins == 0 || params->n_bins > VELO_PV_MAX_BINS || !(params->bin_width > 0.0f) || !(params->chi2_max > 0.0f))
+    return VELO_ERR_ARG;
+  if (n_events > VELO_PV_STATIC_MAX_EVENTS || tracks->cap_tracks > VELO_PV_STATIC_MAX_TRACKS) return VELO_ERR_STATIC_LIMIT;
+  void* base = pv_static_address();
+  if (!base) return VELO_ERR_CUDA;
+  const PvWorkspace w = carve_pv(base, n_events, tracks->cap_tracks);
+  if (w.bytes > kPvStaticBytes) return VELO_ERR_STATIC_LIMIT;      // cannot happen below the two maxima
+  PvArgs a{};
+  a.eto = tracks->event_track_offsets; a.states = tracks->states; a.summary = tracks->summary;
+  a.stride = tracks->cap_tracks; a.n_events = n_events; a.P = *params;
+  a.inv_w = 1.0f / params->bin_width;
+  a.tmp_pv = w.tmp_pv; a.tmp_cnt = w.tmp_cnt; a.asg = w.asg;
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint32_t nbw = (params->n_bins + 1u) >> 1;
+  const uint32_t smem = kPvWarps * (4u * nbw + 4u * params->n_bins + 4u * kPvMax);
+  if (cudaFuncSetAttribute(velo_pv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return VELO_ERR_CUDA;
   if (n_events > 0) {
     uint32_t grid = (n_events + kPvWarps - 1) / kPvWarps;
     const uint32_t most = num_sms() * 8u;

@@ -16,13 +16,16 @@ from . import build as _build
 
 VELO_OK, VELO_ERR_ARG, VELO_ERR_GEOMETRY, VELO_ERR_WORKSPACE = 0, -1, -2, -3
 VELO_ERR_CUDA, VELO_ERR_CAPACITY, VELO_ERR_INPUT = -4, -5, -6
+VELO_ERR_STATIC_LIMIT = -7
+VELO_PV_STATIC_MAX_EVENTS, VELO_PV_STATIC_MAX_TRACKS = 4096, 2097152
 VELO_MAX_MODULES, VELO_MAX_EVENT_HITS, VELO_N_STATE = 32, 65535, 13
 VELO_PATH_DEFAULT, VELO_PATH_SLAB_ONLY = 0, 1
 VELO_N_STAGE_EVENTS = 6
 VELO_N_SUMMARY = 8
 STATE_NAMES = ("x", "y", "tx", "ty", "z", "cxx", "cxtx", "ctxtx", "cyy", "cyty", "ctyty", "chi2", "n_hits")
 ERROR_NAMES = {0: "VELO_OK", -1: "VELO_ERR_ARG", -2: "VELO_ERR_GEOMETRY", -3: "VELO_ERR_WORKSPACE",
-               -4: "VELO_ERR_CUDA", -5: "VELO_ERR_CAPACITY", -6: "VELO_ERR_INPUT"}
+               -4: "VELO_ERR_CUDA", -5: "VELO_ERR_CAPACITY", -6: "VELO_ERR_INPUT",
+               -7: "VELO_ERR_STATIC_LIMIT"}
 
 # every symbol include/velo.h declares
 EXPORTS = ("velo_version", "velo_geometry_load", "velo_geometry_free", "velo_geometry_n_modules",
@@ -30,7 +33,7 @@ EXPORTS = ("velo_version", "velo_geometry_load", "velo_geometry_free", "velo_geo
            "velo_reconstruct_opts", "velo_scheduler_create",
            "velo_scheduler_free", "velo_scheduler_run_host",
            "velo_kalman_fit", "velo_pv_params_default", "velo_pv_workspace_bytes", "velo_pv_find",
-           "velo_reconstruct_pixels", "velo_scheduler_run_host_pixels", "velo_kalman_fit_pixels")
+           "velo_reconstruct_pixels", "velo_scheduler_run_host_pixels", "velo_kalman_fit_pixels", "velo_pv_find_static")
 
 
 class VeloError(RuntimeError):
@@ -148,6 +151,8 @@ def lib():
         L.velo_pv_find.argtypes = [POINTER(Tracks), c_uint32, POINTER(PvParams), POINTER(Pvs), c_void_p, c_size_t,
                                    c_void_p]
         L.velo_pv_find.restype = c_int
+        L.velo_pv_find_static.argtypes = [POINTER(Tracks), c_uint32, POINTER(PvParams), POINTER(Pvs), c_void_p]
+        L.velo_pv_find_static.restype = c_int
         _lib = L
     return _lib
 
@@ -391,7 +396,9 @@ def velo_pv_workspace_bytes(n_events: int, cap_tracks: int) -> int:
 class DevicePvs:
     """Caller-allocated output buffers of velo_pv_find (velo_pvs_t) plus its workspace."""
 
-    def __init__(self, n_events: int, cap_tracks: int, cap_pvs: int | None = None, device="cuda"):
+    def __init__(self, n_events: int, cap_tracks: int, cap_pvs: int | None = None, device="cuda",
+                 with_workspace: bool = True):
+        """with_workspace=False: output buffers only, for velo_pv_find_static (the library's own scratch)."""
         torch = _torch()
         self.n_events = n_events
         self.cap_pvs = int(cap_pvs if cap_pvs is not None else 32 * n_events + 1)
@@ -399,6 +406,9 @@ class DevicePvs:
         self.event_pv_offsets = torch.empty(n_events + 1, **i32)
         self.pvs = torch.empty((VELO_N_PV_WORDS, self.cap_pvs), dtype=torch.float32, device=device)
         self.summary = torch.zeros(4, **i32)
+        if not with_workspace:
+            self.workspace_bytes, self.workspace, self.workspace_ptr = 0, None, 0
+            return
         self.workspace_bytes = velo_pv_workspace_bytes(n_events, cap_tracks)
         self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=device)
         self.workspace_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
@@ -425,6 +435,19 @@ def velo_pv_find(tracks: DeviceTracks, out: DevicePvs, params: PvParams | None =
                             c_size_t(out.workspace_bytes), c_void_p(st.cuda_stream))
     if rc != VELO_OK:
         raise VeloError(rc, "velo_pv_find")
+
+
+def velo_pv_find_static(tracks: DeviceTracks, out: DevicePvs, params: PvParams | None = None, stream=None) -> None:
+    """velo_pv_find over the library's fixed scratch array: the call allocates nothing (include/velo.h). At most
+    VELO_PV_STATIC_MAX_EVENTS events and VELO_PV_STATIC_MAX_TRACKS of track capacity; calls that overlap on the
+    GPU race on the shared array."""
+    torch = _torch()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    P = params if params is not None else velo_pv_params_default()
+    tr = tracks.struct(); pv = out.struct()
+    rc = lib().velo_pv_find_static(byref(tr), tracks.n_events, byref(P), byref(pv), c_void_p(st.cuda_stream))
+    if rc != VELO_OK:
+        raise VeloError(rc, "velo_pv_find_static")
 
 
 def reconstruct(x, y, z, module, event_offsets, module_z, params: Params | None = None, n_batches: int = 1,
