@@ -407,8 +407,9 @@ __global__ void __launch_bounds__(512) velo_order_kernel(const KernelArgs a) {
 }
 
 // ---- S7 part 2: exclusive scans of the per-event counts (one CTA) ------------------------------
-// 256 threads and few registers: it fits beside the pipeline kernels of the next batch.
-__global__ void __launch_bounds__(256) velo_offsets_kernel(const KernelArgs a) {
+// A thread takes a contiguous run of events (25 of a 25 000-event batch), read twice with the loads of a
+// run issued together: the kernel is one chain of global-memory latencies, so more threads = shorter chain.
+__global__ void __launch_bounds__(1024) velo_offsets_kernel(const KernelArgs a) {
   __shared__ unsigned long long warp_sums[33];
   const uint32_t tid = threadIdx.x, nthr = blockDim.x, ne = a.n_events;
   const uint32_t per = (ne + nthr - 1) / nthr;
@@ -568,7 +569,7 @@ int launch_reconstruct(const KernelArgs& a_in, cudaStream_t stream, void* const*
     if (a.big_path && a.n_events > 0 && (rc = launch_fit_big(a, stream)) != 0) return rc;
   }
   mark(3);
-  velo_offsets_kernel<<<1, 256, 0, stream>>>(a);   // counts -> event_track_offsets, summary
+  velo_offsets_kernel<<<1, 1024, 0, stream>>>(a);   // counts -> event_track_offsets, summary
   mark(4);
   const int rc = launch_write(a, stream);          // every final array, once
   mark(5);

@@ -17,7 +17,7 @@
 // seed scatter}; the final flags leave as one bit per hit.
 //
 // Window scans never search: stage 1 stored with every hit where its window starts in the three
-// modules a scan can target (records' words 2 and 3); a scan runs from there, four hits per trip
+// modules a scan can target (records' words 2 and 3); a scan runs from there, three hits per trip
 // with the loads issued first, until the window test fails. A window across +-pi first visits its
 // low-phi run from position 0, so hits are always met in ascending sorted index and ties resolve
 // to the lowest index by strict comparison (O-7, O-8). Step semantics: SURVEY.md §8(c) O-3 ... O-9;
@@ -105,23 +105,27 @@ __device__ void track_fetch(const KernelArgs& a, PoolCtl& pool, TrackTeam<G>& ts
 }
 
 // Visits positions j0, j0 + 1, ... of a module slot (nm hits) while they lie inside the wide window
-// (lo16w, limw), four per trip: the four 16-byte loads of a trip are issued before its arithmetic.
+// (lo16w, limw), a few per trip: the 16-byte loads of a trip are issued before its arithmetic.
 // f(jj, rec, in) must be branch-free. kPad: the slot ends with three sentinel records (x = +inf: their
 // scatter is +inf, no cut accepts them), so a trip reads past the module without clamping its indices;
 // otherwise padding lanes repeat position nm - 1 with `in` false.
 template <bool kPad, class F>
 __device__ __forceinline__ void scan_run(const uint4* slot, uint32_t j0, uint32_t nm, uint32_t lo16w, uint32_t limw, F&& f) {
-  for (uint32_t j = j0; j < nm; j += 4u) {
-    uint4 r[4]; uint32_t jj[4];
+  // records per trip: a window holds 0.7 hits on average (mu = 5), so most scans end in their first trip;
+  // three per trip from a ring slot (measured: 4 / 3 / 2 / 1 -> 1469 / 1448 / 1467 / 1514 us), four from L2
+  constexpr uint32_t T = kPad ? 3u : 4u;
+  static_assert(T - 1u <= kSlotPad, "a trip may read T - 1 records past the module");
+  for (uint32_t j = j0; j < nm; j += T) {
+    uint4 r[T]; uint32_t jj[T];
 #pragma unroll
-    for (uint32_t k = 0; k < 4; ++k) { jj[k] = kPad ? j + k : min(j + k, nm - 1u); r[k] = slot[jj[k]]; }
+    for (uint32_t k = 0; k < T; ++k) { jj[k] = kPad ? j + k : min(j + k, nm - 1u); r[k] = slot[jj[k]]; }
     bool in = false;
 #pragma unroll
-    for (uint32_t k = 0; k < 4; ++k) {
+    for (uint32_t k = 0; k < T; ++k) {
       in = kPad ? (r[k].z - lo16w <= limw) : ((j + k < nm) & (r[k].z - lo16w <= limw));
       f(jj[k], r[k], in);
     }
-    if (!in) break;     // the last of the four is outside (or past the module): so is everything after it
+    if (!in) break;     // the last of the trip is outside (or past the module): so is everything after it
   }
 }
 
@@ -157,11 +161,11 @@ __device__ void track_event_big(const KernelArgs& a, const float* mz, const floa
   // which nothing reads before stage 3 writes them.
   uint4* act_ovf = reinterpret_cast<uint4*>(a.ws.cfit) + 2u * (size_t)ts.cbase;
   auto act_load = [&](uint32_t k, uint4& q0, uint4& q1) {
-    if (k < acap) { q0 = act[2u * k]; q1 = act[2u * k + 1u]; }
+    if (k < acap) { q0 = act[k]; q1 = act[acap + k]; }
     else { q0 = __ldcg(act_ovf + 2u * (k - acap)); q1 = __ldcg(act_ovf + 2u * (k - acap) + 1u); }
   };
   auto act_store = [&](uint32_t k, const uint4& q0, const uint4& q1) {
-    if (k < acap) { act[2u * k] = q0; act[2u * k + 1u] = q1; }
+    if (k < acap) { act[k] = q0; act[acap + k] = q1; }
     else { act_ovf[2u * (k - acap)] = q0; act_ovf[2u * (k - acap) + 1u] = q1; }
   };
   uint16_t* th0 = (uint16_t*)(blk + L.th0);
@@ -454,12 +458,12 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
   // beyond the shared-memory share: global scratch (stage 3's state planes, unused until stage 3)
   uint4* act_ovf = reinterpret_cast<uint4*>(a.ws.cfit) + 2u * ((size_t)ts.cbase + (size_t)w * ovf_w);
   auto act_load = [&](uint32_t k, uint4& q0, uint4& q1) {
-    if (k < acap_w) { q0 = act[2u * k]; q1 = act[2u * k + 1u]; }
+    if (k < acap_w) { q0 = act[k]; q1 = act[acap_w + k]; }      // two planes of 16-byte halves: a warp's loads meet no bank twice
     else if (k - acap_w < ovf_w) { q0 = __ldcg(act_ovf + 2u * (k - acap_w)); q1 = __ldcg(act_ovf + 2u * (k - acap_w) + 1u); }
     else { q0 = make_uint4(0, 0, 0, 0); q1 = q0; }      // never stored (act_store): the event is being given up
   };
   auto act_store = [&](uint32_t k, const uint4& q0, const uint4& q1) {
-    if (k < acap_w) { act[2u * k] = q0; act[2u * k + 1u] = q1; }
+    if (k < acap_w) { act[k] = q0; act[acap_w + k] = q1; }
     else if (k - acap_w < ovf_w) { act_ovf[2u * (k - acap_w)] = q0; act_ovf[2u * (k - acap_w) + 1u] = q1; }
     else ts.defer = 1;                 // a share this lopsided: the general kernel takes the event
   };
