@@ -44,10 +44,11 @@ struct FitCtl {
 
 __device__ __forceinline__ uint32_t a16(uint32_t v) { return (v + 15u) & ~15u; }
 
-struct FitLayout { uint32_t own, fbits, key, mask, state, bytes; };
-__device__ __forceinline__ FitLayout fit_layout(uint32_t n, uint32_t nt) {
+struct FitLayout { uint32_t rowc, own, fbits, key, mask, state, bytes; };
+__device__ __forceinline__ FitLayout fit_layout(uint32_t n, uint32_t nt, bool cache_rows) {
   FitLayout L;
   uint32_t o = 0;
+  L.rowc = o; o += cache_rows ? 32u * nt : 0u;   // the first 16 hit indices of every candidate's row (teams in shared memory)
   L.own = o; o += a16(4u * n);           // O-13 owner (candidate id) per hit
   L.fbits = o; o += a16(4u * ((n + 31u) >> 5));
   L.key = o; o += a16(8u * nt);
@@ -63,6 +64,22 @@ __device__ __forceinline__ void for_hits(const uint16_t* row, uint32_t n, F&& f)
   const uint4* r4 = reinterpret_cast<const uint4*>(row);
   for (uint32_t g = 0; g * 8u < n; ++g) {
     const uint4 v = r4[g];
+    const uint32_t q[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (uint32_t j = 0; j < 8; ++j) {
+      if (g * 8u + j < n) f(g * 8u + j, (q[j >> 1] >> ((j & 1u) * 16u)) & 0xffffu);
+    }
+  }
+}
+
+// The same with the row's first 32 bytes (16 hits) taken from the event's copy `c` in shared memory: a
+// candidate's row is read in four passes of fit_event, and each read from global scratch is a round trip
+// to L2/HBM that the few warps of a team cannot hide. Longer tracks (rare) read their tail from the row.
+template <bool kCache, class F>
+__device__ __forceinline__ void for_hits_c(const uint4* c, const uint16_t* row, uint32_t n, F&& f) {
+  const uint4* r4 = reinterpret_cast<const uint4*>(row);
+  for (uint32_t g = 0; g * 8u < n; ++g) {
+    const uint4 v = (kCache && g < 2u) ? c[g] : r4[g];
     const uint32_t q[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
     for (uint32_t j = 0; j < 8; ++j) {
@@ -164,7 +181,7 @@ __device__ void fit_fetch(const KernelArgs& a, PoolCtl& pool, FitTeam<G>& ts) {
   if (info.state == kEvDeferred) return;           // the slab kernel has written this event's counts
   if (info.state == kEvBig) return;                // velo_fit_big_kernel takes it
   if (info.state != kEvReady || info.ncand == 0) { a.ws.ev_rec[e] = make_uint4(0, 0, 0, 0); return; }
-  const FitLayout L = fit_layout(info.n, info.ncand);
+  const FitLayout L = fit_layout(info.n, info.ncand, true);
   const uint32_t units = (L.bytes + kUnitBytes - 1u) / kUnitBytes;   // fits the pool: stage 1 checked fit_smem_bound
   const uint32_t first = pool_alloc(pool, units);
   ts.n = info.n; ts.cbase = info.cbase; ts.ncand = info.ncand;
@@ -174,12 +191,13 @@ __device__ void fit_fetch(const KernelArgs& a, PoolCtl& pool, FitTeam<G>& ts) {
 }
 
 // ---- one pipeline event, by one team ------------------------------------------------------------
-template <int G, bool kTwoPlane = false>
+template <int G, bool kTwoPlane = false, bool kCacheRows = false>
 __device__ void fit_event(const KernelArgs& a, const float* mz, const float* mzb, FitTeam<G>& ts, unsigned char* blk,
                           uint32_t team, uint32_t tid, uint32_t& parity) {
   const velo_params_t& P = a.P;
   const uint32_t e = ts.event, n = ts.n, nt = ts.ncand, o0 = ts.o0;
-  const FitLayout L = fit_layout(n, nt);
+  const FitLayout L = fit_layout(n, nt, kCacheRows);
+  uint4* rowc = (uint4*)(blk + L.rowc);  // kCacheRows: candidate t's first 16 hit indices at rowc[2t], rowc[2t + 1]
   uint32_t* own = (uint32_t*)(blk + L.own);
   uint32_t* fbits = (uint32_t*)(blk + L.fbits);
   unsigned long long* tkey = (unsigned long long*)(blk + L.key);
@@ -199,10 +217,18 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, const float* mzb
   // ---- O-10 ghost filter part 1 (reads the final flags) -------------------------------------------
   for (uint32_t t = tid; t < nt; t += G) {
     const uint2 cm = cmeta[t];
+    uint2 r = make_uint2(0u, 0u);
+    if (kCacheRows) {
+      // both halves lie in one 32-byte sector: loaded together with cmeta, whatever the track's length
+      const uint4* gr = reinterpret_cast<const uint4*>(rows + t * 32u);
+      const uint4 r0 = gr[0], r1 = gr[1];
+      rowc[2u * t] = r0; rowc[2u * t + 1u] = r1;
+      r = make_uint2(r0.x, r0.y);
+    }
     tmask[t] = cm.x;
     bool pass = true;
     if (__popc(cm.x) == 3) {
-      const uint2 r = *reinterpret_cast<const uint2*>(rows + t * 32u);
+      if (!kCacheRows) r = *reinterpret_cast<const uint2*>(rows + t * 32u);
       const uint32_t h0 = r.x & 0xffffu, h1 = r.x >> 16, h2 = r.y & 0xffffu;
       const uint32_t f = ((fbits[h0 >> 5] >> (h0 & 31u)) | (fbits[h1 >> 5] >> (h1 & 31u)) | (fbits[h2 >> 5] >> (h2 & 31u))) & 1u;
       if (f || !(__uint_as_float(cm.y) <= P.max_scatter_weak)) pass = false;
@@ -220,14 +246,14 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, const float* mzb
     fit_track<kTwoPlane>(rows_xy + t * kXyStride, mz, mzb, nh, mask, sig2, inv_s2, s9);
     const float lim = __fmul_rn(P.max_chi2_ndof, (float)(2 * (int)nh - 4));
     if (s9[8] > lim) { tstate[t] = 0; continue; }
-    const uint32_t centre = rows[t * 32u + 1u];
+    const uint32_t centre = kCacheRows ? rowc[2u * t].x >> 16 : (uint32_t)rows[t * 32u + 1u];
     tkey[t] = ((unsigned long long)(255u - nh) << 56) | ((unsigned long long)__float_as_uint(s9[8]) << 24) |
               (unsigned long long)centre;
 #pragma unroll
     for (uint32_t k = 0; k < 9; ++k) cfit[k * cs + t] = s9[k];
     // O-13 owners, step 1: every passing candidate writes its id on its hits (plain stores: where
     // several share a hit, any one of them lands)
-    for_hits(rows + t * 32u, nh, [&](uint32_t, uint32_t h) { own[h] = t; });
+    for_hits_c<kCacheRows>(rowc + 2u * t, rows + t * 32u, nh, [&](uint32_t, uint32_t h) { own[h] = t; });
   }
   team_sync<G>(team);
   VELO_PH(a.ws.phase_clk, ts, 35);
@@ -240,10 +266,10 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, const float* mzb
     // first look at all hits at once (independent loads): most candidates own every hit of theirs
     const uint32_t nh = (uint32_t)__popc(tmask[t]);
     uint32_t contested = 0;
-    for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) { contested |= (own[h] != t) ? (1u << i) : 0u; });
+    for_hits_c<kCacheRows>(rowc + 2u * t, rows + t * 32u, nh, [&](uint32_t i, uint32_t h) { contested |= (own[h] != t) ? (1u << i) : 0u; });
     if (!contested) continue;
     const unsigned long long key = tkey[t];
-    for_hits(rows + t * 32u, nh, [&](uint32_t i, uint32_t h) {
+    for_hits_c<kCacheRows>(rowc + 2u * t, rows + t * 32u, nh, [&](uint32_t i, uint32_t h) {
       if (!((contested >> i) & 1u)) return;
       uint32_t old = *(volatile uint32_t*)&own[h];
       while (old != t && key < tkey[old]) {
@@ -264,7 +290,7 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, const float* mzb
     if (t < nt && tstate[t]) {
       nh = (uint32_t)__popc(tmask[t]);
       uint32_t lost = 0;
-      for_hits(rows + t * 32u, nh, [&](uint32_t, uint32_t h) { lost += (own[h] != t) ? 1u : 0u; });
+      for_hits_c<kCacheRows>(rowc + 2u * t, rows + t * 32u, nh, [&](uint32_t, uint32_t h) { lost += (own[h] != t) ? 1u : 0u; });
       surv = !((unsigned long long)lost * P.clone_den > (unsigned long long)nh * P.clone_num) ? 1u : 0u;
       if (!surv) nh = 0;
     }
@@ -297,7 +323,7 @@ __global__ void __launch_bounds__(G * kTeams, 1) velo_fit_kernel(const KernelArg
     team_sync<G>(team);
     if (ts.event >= a.n_events) break;
     VELO_PH(a.ws.phase_clk, ts, 33);     // ticket, descriptors, pool
-    if (!ts.skip) fit_event<G, kTwoPlane>(a, ctl.module_z, ctl.module_z_b, ts, pool + ts.pool_off, team, tid, parity);
+    if (!ts.skip) fit_event<G, kTwoPlane, true>(a, ctl.module_z, ctl.module_z_b, ts, pool + ts.pool_off, team, tid, parity);
     team_sync<G>(team);
     if (tid == 0 && ts.units) pool_free(ctl.pool, ts.first_unit, ts.units);
     VELO_PH(a.ws.phase_clk, ts, 38);     // clone filter, counts
@@ -515,7 +541,7 @@ int launch_fit_big(const KernelArgs& a, cudaStream_t stream) {
 int launch_write(const KernelArgs& a, cudaStream_t stream) {
   if (a.n_events == 0) return 0;
   const uint32_t grid = (a.n_events + 3u) / 4u;     // a warp per event
-  velo_write_kernel<8><<<grid, 128, 0, stream>>>(a);
+  velo_write_kernel<12><<<grid, 128, 0, stream>>>(a);
   if (a.big_path) velo_write_big_kernel<<<num_sms() * 2u, 1024, 0, stream>>>(a);
   return (int)cudaGetLastError();
 }

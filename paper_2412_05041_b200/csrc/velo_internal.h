@@ -45,7 +45,8 @@ __host__ __device__ inline SlabLayout slab_layout() {
 enum { kCtrTracks = 0, kCtrHits = 1, kCtrStatus = 2, kCtrCand = 3, kCtrTicket = 4, kCtrLargeN = 5,
        kCtrLargeTicket = 6, kCtrSortTicket = 7, kCtrTrackTicket = 8, kCtrFitTicket = 9, kCtrCandAlloc = 10,
        kCtrBigN = 11, kCtrBigSortTicket = 12, kCtrBigTrackTicket = 13, kCtrBigFitTicket = 14,
-       kNumCounters = 16, kNumPhaseClocks = 64 };
+       kNumCounters = 16, kNumPhaseClocks = 64,
+       kSizeClasses = 256 };   // events by n_hits / 64 (velo_order_kernel); ws.size_hist: counts, then cursors
 
 // ---- the three-stage pipeline (velo_sort.cu -> velo_track.cu -> velo_fit.cu) ---------------------
 // Stage 1 writes every event's phi-sorted hits to global scratch; stage 2 streams them module by
@@ -64,11 +65,16 @@ __host__ __device__ inline uint32_t cand_capacity(uint32_t n) { return ((n >> 3)
 // of a mean mu = 5 event, 0.104/hit at most in 600 events of configs[1]): what does not fit spills
 // to global scratch (velo_track.cu), so this capacity trades shared memory against rare L2 trips.
 __host__ __device__ inline uint32_t active_capacity(uint32_t n) { return (((n * 7u) >> 7) + 24u + 7u) & ~7u; }
+// Size class of an event for the scheduling order of stages 2 and 3 (velo_order_kernel): n_hits / 64, capped.
+__host__ __device__ inline uint32_t size_class(uint32_t o0, uint32_t o1) {
+  const uint32_t c = (o1 >= o0 ? o1 - o0 : 0u) >> 6;
+  return c < (uint32_t)kSizeClasses - 1u ? c : (uint32_t)kSizeClasses - 1u;
+}
 constexpr uint32_t kModOffStride = 40;   // u16 per event: mod_off[0 .. M] (M <= 32), [39] = largest module
 constexpr uint32_t kPipeMaxHits = 12000; // largest event the pipeline path takes (stage 1: 17 B/hit, stage 3: ~18 B/hit of shared memory)
 // Upper bound of stage 3's shared-memory block for an event of n hits (velo_fit.cu: fit_layout with
 // every candidate slot used): stage 1 defers an event to the general kernel if this does not fit.
-__host__ __device__ inline uint32_t fit_smem_bound(uint32_t n) { return 4u * n + (n >> 3) + 13u * cand_capacity(n) + 256u; }
+__host__ __device__ inline uint32_t fit_smem_bound(uint32_t n) { return 4u * n + (n >> 3) + 45u * cand_capacity(n) + 256u; }
 // (x, y) of a candidate's hits in discovery order, written by stage 2 as it appends them: stage 3
 // fits from these rows and needs no gather. kXyStride float2 per candidate (16-byte aligned rows).
 constexpr uint32_t kXyStride = VELO_MAX_MODULES;
@@ -103,6 +109,7 @@ struct Workspace {
   uint32_t* big_list;     // n_events: events of more than kPipeMaxHits hits (the one-event-per-CTA pipeline)
   uint32_t* big_sorted;   // n_events: the same, largest first (stages 2 and 3 take them in this order)
   uint32_t* order;        // n_events: event ids by ascending size class (velo_order_kernel)
+  uint32_t* size_hist;    // 2 * kSizeClasses: events per size class (counted by stage 1's leaders), placement cursors
   float *ux, *uy, *uz;    // n_hits: fp32 coordinates of deferred events when the input is packed pixels
   uint8_t* umod;          //   (index = absolute hit index - event_offsets[0])
   uint32_t* tmp_loff;     // cap_tracks: hit offset of a track inside its event's hit block

@@ -70,6 +70,7 @@ __device__ void sort_fetch(const KernelArgs& a, PoolCtl& pool, SortTeam<G>& ts) 
   if (e >= a.n_events) return;
   const uint32_t base = a.event_offsets[0];
   const uint32_t o0 = a.event_offsets[e], o1 = a.event_offsets[e + 1];
+  atomicAdd(&a.ws.size_hist[size_class(o0, o1)], 1u);    // events per size class, for velo_order_kernel
   EvInfo info{0u, kEvEmpty, 0u, 0u};
   // every event must stay inside the batch, [base, base + n_hits]: nothing is read out of bounds
   if (o1 < o0 || o0 < base || o1 - base > a.n_hits || o1 - o0 > VELO_MAX_EVENT_HITS) {
