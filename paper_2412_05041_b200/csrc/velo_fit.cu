@@ -541,7 +541,7 @@ int launch_fit_big(const KernelArgs& a, cudaStream_t stream) {
 int launch_write(const KernelArgs& a, cudaStream_t stream) {
   if (a.n_events == 0) return 0;
   const uint32_t grid = (a.n_events + 3u) / 4u;     // a warp per event
-  velo_write_kernel<12><<<grid, 128, 0, stream>>>(a);
+  velo_write_kernel<8><<<grid, 128, 0, stream>>>(a);
   if (a.big_path) velo_write_big_kernel<<<num_sms() * 2u, 1024, 0, stream>>>(a);
   return (int)cudaGetLastError();
 }
