@@ -226,6 +226,9 @@ __device__ void fit_event(const KernelArgs& a, const float* mz, const float* mzb
       r = make_uint2(r0.x, r0.y);
     }
     tmask[t] = cm.x;
+    // the coordinate row this thread fits from in the next pass (64 bytes per 8 hits): on its way to L2 now
+    prefetch_l2(rows_xy + t * kXyStride);
+    if (__popc(cm.x) > 8) prefetch_l2(rows_xy + t * kXyStride + 8u);
     bool pass = true;
     if (__popc(cm.x) == 3) {
       if (!kCacheRows) r = *reinterpret_cast<const uint2*>(rows + t * 32u);
@@ -384,11 +387,13 @@ __global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const Kerne
   const size_t cs = a.cap_tracks, cc = a.ws.cand_total;
   const uint32_t obase = a.event_offsets[0];
   for (uint32_t e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; e < a.n_events; e += warps) {
+    // the event's four descriptors in one round trip (a warp has one event: every round trip counts)
     const uint4 r = a.ws.ev_rec[e];
-    if (r.z == 0) continue;
     const uint32_t dst_t = a.event_track_offsets[e], dst_h = a.ws.ev_hit_base[e];
     EvInfo info{0u, kEvDeferred, 0u, 0u};
     if (!a.all_deferred) info = a.ws.ev_info[e];
+    const uint32_t o0 = a.event_offsets[e];
+    if (r.z == 0) continue;
     if (info.state == kEvDeferred) {
       // tracks of the general kernel: temp block -> place (four independent loads per lane and trip)
       const uint32_t* src = a.ws.tmp_hits + r.y;
@@ -412,15 +417,24 @@ __global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const Kerne
       continue;
     }
     if (info.state == kEvBig) continue;                 // velo_write_big_kernel: a CTA per such event
-    const uint32_t o0 = a.event_offsets[e];
     const uint16_t* orig = a.ws.sorig + sorted_base(o0 - obase, e);
     const uint16_t* rows = a.ws.rows + (size_t)info.cbase * 32u;
     const uint2* cmeta = a.ws.cmeta + info.cbase;
     const uint8_t* cstate = a.ws.cstate + info.cbase;
     const float* cfit = a.ws.cfit + info.cbase;
     uint32_t run_t = 0, run_h = 0;
+    // the event's index map, candidate masks and fates, and the first pass's rows and fit planes: on their way to L2
+    for (uint32_t k = lane * 64u; k < info.n; k += 32u * 64u) prefetch_l2(orig + k);
+    for (uint32_t k = lane * 16u; k < info.ncand; k += 32u * 16u) prefetch_l2(cmeta + k);
+    if (lane * 128u < info.ncand) prefetch_l2(cstate + lane * 128u);
+    if (lane < info.ncand) prefetch_l2(rows + lane * 32u);
+    if (lane < 9u) prefetch_l2(cfit + lane * cc);
     for (uint32_t t0 = 0; t0 < info.ncand; t0 += 32u) {
       const uint32_t t = t0 + lane;
+      if (t + 32u < info.ncand) {        // the next pass's candidates: their rows and fit planes on the way to L2
+        prefetch_l2(rows + (t + 32u) * 32u);
+        if (lane < 9u) prefetch_l2(cfit + lane * cc + t0 + 32u);
+      }
       const bool surv = t < info.ncand && cstate[t] != 0;
       const uint32_t nh = surv ? (uint32_t)__popc(cmeta[t].x) : 0u;
       const uint32_t b = __ballot_sync(0xffffffffu, surv);

@@ -51,6 +51,9 @@ __device__ __forceinline__ unsigned long long velo_globaltimer() {
 #define VELO_STAGE_END(clk, k) do { } while (0)
 #endif
 
+// Asks L2 for the line at p (no register, no wait): what a thread will read a few microseconds later.
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // ---- team barrier: G threads; G == 32 is a warp -------------------------------------------------
 template <int G>
 __device__ __forceinline__ void team_sync(uint32_t team) {

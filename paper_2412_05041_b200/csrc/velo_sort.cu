@@ -123,6 +123,20 @@ __device__ void sort_event(const KernelArgs& a, const float* mz, SortTeam<G>& ts
   const uint8_t* gm = a.module + g0;
   const uint32_t* gp = a.pixel + g0;
 
+  // Tickets go out in event order and events lie one behind the other in the input planes: what this team
+  // asks L2 for now, its own length of input kPrefetchAhead hits further on, is what the teams of the events
+  // a few hundred tickets later will read (every line of the batch is asked for once, by some team).
+  {
+    constexpr uint32_t kPrefetchAhead = 1u << 20;      // hits: about the events in flight on the GPU at mu = 5
+    const uint32_t end = a.event_offsets[0] + a.n_hits - a.hit_base;   // first hit index (relative to the planes) behind the batch
+    const uint32_t p0 = ((uint32_t)g0 + kPrefetchAhead) & ~31u;
+    const uint32_t p1 = min((uint32_t)g0 + n + kPrefetchAhead, end);
+    if (a.pixel) { for (uint32_t i = p0 + 32u * tid; i < p1; i += 32u * G) prefetch_l2(a.pixel + i); }
+    else {
+      for (uint32_t i = p0 + 32u * tid; i < p1; i += 32u * G) { prefetch_l2(a.x + i); prefetch_l2(a.y + i); prefetch_l2(a.z + i); }
+      for (uint32_t i = (p0 & ~127u) + 128u * tid; i < p1; i += 128u * G) prefetch_l2(a.module + i);
+    }
+  }
   // ---- S0 decode: phi16 (O-1), bucket histogram; the plane check of the pipeline path -------------
   const uint32_t nwords = nbins / 2u;
   for (uint32_t b = tid; b <= nwords; b += G) binsw[b] = 0;
