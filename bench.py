@@ -308,8 +308,8 @@ class Workload:
                     e[2].record(st)
         torch.cuda.synchronize()
         n_pvs = sum(p.to_host()["n_pvs"] for p in pvs)
-        return {"kalman_ms_per_launch": float(np.mean([e[0].elapsed_time(e[1]) for e in ev])),
-                "pv_ms_per_launch": float(np.mean([e[1].elapsed_time(e[2]) for e in ev])), "n_pvs": n_pvs,
+        return {"kalman_ms_per_launch": float(np.median([e[0].elapsed_time(e[1]) for e in ev])),
+                "pv_ms_per_launch": float(np.median([e[1].elapsed_time(e[2]) for e in ev])), "n_pvs": n_pvs,
                 "what": "velo_kalman_fit (parameterised Kalman filter on the VELO segment) and velo_pv_find (primary "
                         "vertices) on each batch's device outputs; not part of `value`"}
 

@@ -91,6 +91,11 @@ __global__ void __launch_bounds__(256) velo_kalman_kernel(const KalmanHits H, co
 // ---- f3: one warp per event ---------------------------------------------------------------------------
 constexpr uint32_t kPvMax = VELO_PV_MAX_PER_EVENT;   // 32: a seed per lane
 constexpr uint32_t kPvWarps = 4;                      // events per CTA
+// Shared memory of a warp: packed histogram, smoothed counts, seed z, one word per block of 32 bins (16-byte multiple).
+__host__ __device__ inline uint32_t pv_smem_per_warp(uint32_t n_bins) {
+  const uint32_t nbw = (n_bins + 1u) >> 1;
+  return (4u * nbw + 4u * n_bins + 4u * kPvMax + 4u * ((n_bins + 31u) >> 5) + 15u) & ~15u;
+}
 
 struct PvArgs {
   const uint32_t* eto;        // event_track_offsets[n_events + 1]
@@ -115,18 +120,19 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
   extern __shared__ __align__(16) unsigned char smem[];
   const uint32_t wid = threadIdx.x >> 5, lane = threadIdx.x & 31u;
   const uint32_t nb = a.P.n_bins, nbw = (nb + 1u) >> 1;          // bins; packed-u16 words
-  const uint32_t per_warp = 4u * nbw + 4u * nb + 4u * kPvMax;
+  const uint32_t per_warp = pv_smem_per_warp(nb);
   uint32_t* hw = reinterpret_cast<uint32_t*>(smem + (size_t)wid * per_warp);   // P-1 histogram, two u16 counts per word
   uint32_t* s = hw + nbw;                                                       // P-2 smoothed counts
   float* zs = reinterpret_cast<float*>(s + nb);                                 // seed z
+  uint32_t* bm = reinterpret_cast<uint32_t*>(zs + kPvMax);                      // per 32 bins: does any reach seed_min_sum?
+  const uint32_t nblk = (nb + 31u) >> 5;
   const bool failed = a.summary[2] != 0u;
   const float* X = a.states; const float* Y = X + a.stride; const float* TX = Y + a.stride; const float* TY = TX + a.stride;
   const float* Z = TY + a.stride; const float* CXX = Z + a.stride;
-  auto hist = [&](uint32_t b) -> uint32_t { return (hw[b >> 1] >> ((b & 1u) * 16u)) & 0xffffu; };
   for (uint32_t e = blockIdx.x * kPvWarps + wid; e < a.n_events; e += gridDim.x * kPvWarps) {
     const uint32_t t0 = failed ? 0u : a.eto[e], nt = failed ? 0u : a.eto[e + 1] - t0;
     // P-1
-    for (uint32_t k = lane; k < nbw; k += 32u) hw[k] = 0u;
+    for (uint32_t k = lane; 4u * k < nbw; k += 32u) reinterpret_cast<uint4*>(hw)[k] = make_uint4(0u, 0u, 0u, 0u);   // (may run up to three words into s, which is written later)
     __syncwarp();
     for (uint32_t i = lane; i < nt; i += 32u) {
       const float t = __fmul_rn(__fsub_rn(Z[t0 + i], a.P.z_min), a.inv_w);
@@ -134,16 +140,27 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
     }
     __syncwarp();
     // P-2 smoothed counts, then seeds in ascending bin order (ballot keeps the order)
-    for (uint32_t b = lane; b < nb; b += 32u) {
-      uint32_t v = 2u * hist(b);
-      if (b > 0u) v += hist(b - 1u);
-      if (b + 1u < nb) v += hist(b + 1u);
-      s[b] = v;
+    // A lane takes a packed word (bins 2k, 2k + 1); a ballot notes which blocks of 32 bins hold a count that
+    // can seed: an event's 200 tracks touch a handful of the 75 blocks, and the seed scan skips the rest.
+    const uint32_t min_sum = a.P.seed_min_sum > 1u ? a.P.seed_min_sum : 1u;
+    for (uint32_t k0 = 0; k0 < nbw; k0 += 32u) {
+      const uint32_t k = k0 + lane;
+      uint32_t c0 = 0u, c1 = 0u;
+      if (k < nbw) {
+        const uint32_t wm = k > 0u ? hw[k - 1u] : 0u, wc = hw[k], wp = k + 1u < nbw ? hw[k + 1u] : 0u;
+        const uint32_t lo = wc & 0xffffu, hi = wc >> 16;
+        c0 = 2u * lo + (wm >> 16) + hi;
+        s[2u * k] = c0;
+        if (2u * k + 1u < nb) { c1 = 2u * hi + lo + (wp & 0xffffu); s[2u * k + 1u] = c1; }
+      }
+      const uint32_t m = __ballot_sync(0xffffffffu, c0 >= min_sum || c1 >= min_sum);
+      if (lane == 0) { bm[k0 >> 4] = m & 0xffffu; if ((k0 >> 4) + 1u < nblk) bm[(k0 >> 4) + 1u] = m >> 16; }
     }
     __syncwarp();
     uint32_t ns = 0;
     const uint32_t cap = a.P.max_pv_per_event < kPvMax ? a.P.max_pv_per_event : kPvMax;
     for (uint32_t b0 = 0; b0 < nb && ns < cap; b0 += 32u) {
+      if (bm[b0 >> 5] == 0u) continue;       // no bin of this block reaches seed_min_sum
       const uint32_t b = b0 + lane;
       bool ok = false;
       if (b < nb) {
@@ -477,8 +494,7 @@ int velo_pv_find(const velo_tracks_t* tracks, uint32_t n_events, const velo_pv_p
   a.inv_w = 1.0f / params->bin_width;
   a.tmp_pv = w.tmp_pv; a.tmp_cnt = w.tmp_cnt; a.asg = w.asg;
   cudaStream_t st = (cudaStream_t)stream;
-  const uint32_t nbw = (params->n_bins + 1u) >> 1;
-  const uint32_t smem = kPvWarps * (4u * nbw + 4u * params->n_bins + 4u * kPvMax);
+  const uint32_t smem = kPvWarps * pv_smem_per_warp(params->n_bins);
   cudaError_t err = cudaFuncSetAttribute(velo_pv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return VELO_ERR_CUDA;
   if (n_events > 0) {
@@ -515,8 +531,7 @@ int velo_pv_find_static(const velo_tracks_t* tracks, uint32_t n_events, const ve
   a.inv_w = 1.0f / params->bin_width;
   a.tmp_pv = w.tmp_pv; a.tmp_cnt = w.tmp_cnt; a.asg = w.asg;
   cudaStream_t st = (cudaStream_t)stream;
-  const uint32_t nbw = (params->n_bins + 1u) >> 1;
-  const uint32_t smem = kPvWarps * (4u * nbw + 4u * params->n_bins + 4u * kPvMax);
+  const uint32_t smem = kPvWarps * pv_smem_per_warp(params->n_bins);
   if (cudaFuncSetAttribute(velo_pv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return VELO_ERR_CUDA;
   if (n_events > 0) {
