@@ -241,24 +241,30 @@ __global__ void __launch_bounds__(32 * kPvWarps) velo_pv_kernel(const PvArgs a) 
             if (wt > 0.0f) q[224] = __fadd_rn(q[224], 1.0f);
           }
           __syncwarp();
-          for (uint32_t v = v0; v < v1; ++v) {                  // the rest of P-5, vertex by vertex
+          // the rest of P-5: the sums vertex by vertex (every lane gets them; lane v keeps vertex v's), then
+          // the closed form for all vertices of the round at once, lane v solving vertex v
+          float lS0 = 0.0f, lSx = 0.0f, lSy = 0.0f, lSxx = 0.0f, lA = 0.0f, lB = 0.0f, lC = 0.0f;
+          bool mine = false;
+          for (uint32_t v = v0; v < v1; ++v) {
             if (vt[4u * v + 3u] == 0.0f) continue;
             const float* q = acc + (v - v0) * 256u + lane;
             const float S0 = warp_butterfly(q[0]);
             const float Sx = warp_butterfly(q[32]), Sy = warp_butterfly(q[64]), Sxx = warp_butterfly(q[96]);
             const float A = warp_butterfly(q[128]), B = warp_butterfly(q[160]), C = warp_butterfly(q[192]);
             const uint32_t ntrk = (uint32_t)warp_butterfly(q[224]);
-            if (lane == v) { my_s0 = S0; my_n = ntrk; }
-            bool alive = S0 > 0.0f;
+            if (lane == v) { my_s0 = S0; my_n = ntrk; lS0 = S0; lSx = Sx; lSy = Sy; lSxx = Sxx; lA = A; lB = B; lC = C; mine = true; }
+          }
+          __syncwarp();
+          if (mine) {
+            bool alive = lS0 > 0.0f;
             float den = 0.0f;
-            if (alive) { den = __fsub_rn(Sxx, __fdiv_rn(__fadd_rn(__fmul_rn(Sx, Sx), __fmul_rn(Sy, Sy)), S0)); alive = den > 0.0f; }
-            __syncwarp();
-            if (!alive) { if (lane == 0) vt[4u * v + 3u] = 0.0f; }
+            if (alive) { den = __fsub_rn(lSxx, __fdiv_rn(__fadd_rn(__fmul_rn(lSx, lSx), __fmul_rn(lSy, lSy)), lS0)); alive = den > 0.0f; }
+            if (!alive) vt[4u * lane + 3u] = 0.0f;
             else {
-              const float zv = __fdiv_rn(__fsub_rn(__fdiv_rn(__fadd_rn(__fmul_rn(Sx, A), __fmul_rn(Sy, B)), S0), C), den);
-              const float xv = __fdiv_rn(__fadd_rn(A, __fmul_rn(Sx, zv)), S0);
-              const float yv = __fdiv_rn(__fadd_rn(B, __fmul_rn(Sy, zv)), S0);
-              if (lane == 0) { vt[4u * v] = xv; vt[4u * v + 1u] = yv; vt[4u * v + 2u] = zv; }
+              const float zv = __fdiv_rn(__fsub_rn(__fdiv_rn(__fadd_rn(__fmul_rn(lSx, lA), __fmul_rn(lSy, lB)), lS0), lC), den);
+              const float xv = __fdiv_rn(__fadd_rn(lA, __fmul_rn(lSx, zv)), lS0);
+              const float yv = __fdiv_rn(__fadd_rn(lB, __fmul_rn(lSy, zv)), lS0);
+              vt[4u * lane] = xv; vt[4u * lane + 1u] = yv; vt[4u * lane + 2u] = zv;
             }
           }
           __syncwarp();
