@@ -28,8 +28,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # ncu --set full counters of one 25 000-event launch of every kernel of the path (configs[2] batch size),
-# written from the capture summarised in profiles/r02h_pipeline.md; read by name, never pasted here
-STAGE_COUNTERS_CSV = os.path.join(ROOT, "profiles", "r02i_stage_counters.csv")
+# written from the capture summarised in profiles/r02j_pipeline.md; read by name, never pasted here
+STAGE_COUNTERS_CSV = os.path.join(ROOT, "profiles", "r02j_stage_counters.csv")
 STAGE_COUNTERS_EVENTS = 25_000
 # stage k runs between stage events k and k+1 of velo_launch_options_t (include/velo.h)
 STAGES = [("sort", ["velo_sort_kernel", "velo_order_kernel"]),
@@ -130,7 +130,7 @@ class ClockSampler:
 
 
 def stage_counters() -> dict:
-    """kernel name -> counters of one 25 000-event launch (profiles/r02i_stage_counters.csv); {} if absent."""
+    """kernel name -> counters of one 25 000-event launch (profiles/r02j_stage_counters.csv); {} if absent."""
     import csv
     try:
         with open(STAGE_COUNTERS_CSV) as f:
@@ -475,7 +475,7 @@ def run_velo(args):
         "roofline": {"bound": "hbm", "kernel": " + ".join(dom["kernels"][:1]), "stage": dom["stage"],
                      "achieved": dom["achieved"], "peak": peak, "unit": "GB/s", "frac": dom["achieved"] / peak,
                      "traffic": dom["traffic"],
-                     "traffic_source": "profiles/r02i_stage_counters.csv (ncu --set full, one 25 000-event launch of every kernel)"
+                     "traffic_source": "profiles/r02j_stage_counters.csv (ncu --set full, one 25 000-event launch of every kernel)"
                                        if counters else None,
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_launch,
                      "kernel_ms_per_launch": dom["ms_per_launch"], "kernel_share_of_step": dom["share_of_path"],
@@ -487,10 +487,10 @@ def run_velo(args):
                      "step_traffic_over_algorithmic": step_traffic * n_batches / float(sum(alg_batch)) if step_traffic else None,
                      "frac_of_nominal_8TBs": step_gbs / 8000.0, "target_frac": 0.40, "target_met": step_gbs / peak >= 0.40,
                      "limiter": "instruction issue and event latency, not HBM: every stage holds an event's shared memory "
-                                "for the length of its dependent instruction chains (profiles/r02h_pipeline.md)"},
+                                "for the length of its dependent instruction chains and waits at its team barriers (profiles/r02j_pipeline.md)"},
         "issue": ({"bound": "alu", "achieved": events_per_s / world * warp_inst / 1e9, "peak": issue_peak / 1e9,
                    "unit": "G warp instr/s", "frac": events_per_s / world * warp_inst / issue_peak,
-                   "warp_instructions_per_event": warp_inst, "source": "profiles/r02i_stage_counters.csv"}
+                   "warp_instructions_per_event": warp_inst, "source": "profiles/r02j_stage_counters.csv"}
                   if warp_inst else None),
         "after_path": after_path,
         "clocks": clocks,
