@@ -374,11 +374,11 @@ __global__ void __launch_bounds__(G, 1) velo_fit_big_kernel(const KernelArgs a) 
 // ---- S7 write: one warp per event places its surviving tracks in the final arrays ----------------
 // Offsets come from velo_offsets_kernel (event_track_offsets, ws.ev_hit_base). Candidates are in
 // creation order, so a running count over them is the track's place inside the event.
-template <int kMinBlocks>
-__global__ void __launch_bounds__(128, kMinBlocks) velo_write_kernel(const KernelArgs a) {
+template <int kWarps, int kMinBlocks>
+__global__ void __launch_bounds__(32 * kWarps, kMinBlocks) velo_write_kernel(const KernelArgs a) {
   // the hit lists of 32 candidates at a time go through shared memory, so that the warp writes
   // track_hits as whole sectors instead of 32 scattered words per store
-  __shared__ uint32_t stage_all[4][32 * VELO_MAX_MODULES];
+  __shared__ uint32_t stage_all[kWarps][32 * VELO_MAX_MODULES];
   uint32_t* stage = stage_all[threadIdx.x >> 5];
   const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
   const uint32_t lane = threadIdx.x & 31u;
@@ -554,8 +554,8 @@ int launch_fit_big(const KernelArgs& a, cudaStream_t stream) {
 
 int launch_write(const KernelArgs& a, cudaStream_t stream) {
   if (a.n_events == 0) return 0;
-  const uint32_t grid = (a.n_events + 3u) / 4u;     // a warp per event
-  velo_write_kernel<8><<<grid, 128, 0, stream>>>(a);
+  // a warp per event, four per CTA (1, 2 or 8 warps per CTA: 315, 309, 312 us against 305)
+  velo_write_kernel<4, 8><<<(a.n_events + 3u) / 4u, 128, 0, stream>>>(a);
   if (a.big_path) velo_write_big_kernel<<<num_sms() * 2u, 1024, 0, stream>>>(a);
   return (int)cudaGetLastError();
 }

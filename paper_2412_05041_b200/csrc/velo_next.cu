@@ -48,12 +48,15 @@ __global__ void __launch_bounds__(256) velo_kalman_kernel(const KalmanHits H, co
   float tx = __fdiv_rn(__fsub_rn(x, x0), dz), ty = __fdiv_rn(__fsub_rn(y, y0), dz);
   float cxx = s2, cxtx = __fdiv_rn(s2, dz), ctxtx = __fdiv_rn(__fadd_rn(s2, s2), __fmul_rn(dz, dz));
   float chi2 = 0.0f;
-  // software pipeline: hit i+1 is in flight while hit i is processed
+  // software pipeline, two deep: while hit i is processed the coordinates of hit i+1 are in flight (through the
+  // index loaded one trip earlier) and so is the index of hit i+2: a trip waits for one load, not for two in a row
   float nx = 0.0f, ny = 0.0f, nz = 0.0f;
   if (n > 2) H.get(th[a + 2], nx, ny, nz);
+  uint32_t nidx = n > 3 ? th[a + 3] : 0u;
   for (uint32_t i = 2; i < n; ++i) {
     const float mx = nx, my = ny, mzz = nz;
-    if (i + 1 < n) H.get(th[a + i + 1], nx, ny, nz);
+    if (i + 1 < n) H.get(nidx, nx, ny, nz);
+    if (i + 2 < n) nidx = th[a + i + 2];
     const float sl = __fadd_rn(1.0f, __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty)));
     ctxtx = __fadd_rn(ctxtx, __fmul_rn(ms_theta2, sl));
     dz = __fsub_rn(mzz, zp);
