@@ -346,6 +346,19 @@ def test_full_size_every_event(velo, config):
     assert (np.diff(mod)[same_track] < 0).all()                              # decreasing module order
 
 
+def test_one_launch_beyond_a_single_wave_of_the_scans(velo):
+    """More than 148 x 256 events in ONE launch: a thread of velo_offsets_kernel then takes several events
+    (its chunks no longer hold 256), velo_order_kernel runs a few hundred CTAs, and the offsets must still
+    be the exclusive scan over all events. Every event against the oracle, and against four streamed batches."""
+    d = datagen.generate_config(3, n_events=60000)
+    got = gpu(velo, d, n_batches=1)
+    assert got["n_deferred"] == 0
+    assert _compare_in_chunks(got, d, 20000)
+    four = gpu(velo, d, n_batches=4)
+    for k in ("event_track_offsets", "track_hit_offsets"):
+        np.testing.assert_array_equal(got[k], four[k])
+
+
 # ---- the end-to-end call over host buffers: velo_scheduler_run_host (S8) --------------------------
 def _run_scheduler(velo, d, cuts, n_streams, pinned=True):
     import torch
