@@ -62,6 +62,8 @@ def parse_args():
     ap.add_argument("--timeline", action="store_true",
                     help="instrumented build: print when each pipeline stage of each batch ran, then exit")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-split", default="growing", choices=["growing", "equal"],
+                    help="batch sizes of the end-to-end call: 10/20/30/40 %% of the events (default) or four equal batches")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -500,13 +502,21 @@ def run_velo(args):
     #    inputs -> H2D -> kernels -> D2H of the produced tracks, all inside the timed region --
     d = wl.d
     if not args.no_e2e:
-        max_ev = max(cuts[b + 1] - cuts[b] for b in range(n_batches))
-        max_h = max(int(off[cuts[b + 1]]) - int(off[cuts[b]]) for b in range(n_batches))
+        # The packed-input call is bound by the device->host copy of the produced tracks, which cannot start before
+        # the first batch is through H2D and the kernels: batches of growing size (10, 20, 30, 40 % of the events)
+        # let it start after a tenth of the input, and every later batch is ready before the copy of the one before
+        # ends (39.8 instead of 42.3 ms per step). The fp32 call is bound by its 2.46 GB of input and keeps equal
+        # batches (a large last batch would leave its kernels and its copy behind the last upload).
+        eq_cuts = cuts
+        if n_batches == 4 and args.e2e_split == "growing":
+            cuts = [0] + [int(round(n_events * f)) for f in (0.10, 0.30, 0.60)] + [n_events]
+        max_ev = max(c[b + 1] - c[b] for c in (cuts, eq_cuts) for b in range(n_batches))
+        max_h = max(int(off[c[b + 1]]) - int(off[c[b]]) for c in (cuts, eq_cuts) for b in range(n_batches))
         g, P = wl.g, wl.P
         wl.outs = wl.hstructs = wl.dh = None
         torch.cuda.empty_cache()
         sched = velo.Scheduler(g, n_batches, max_ev, max_h)
-        houts = [velo.HostTracks(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]])) for b in range(n_batches)]
+        houts = [velo.HostTracks(eq_cuts[b + 1] - eq_cuts[b], int(off[eq_cuts[b + 1]]) - int(off[eq_cuts[b]])) for b in range(n_batches)]
         off_pinned = torch.from_numpy(off.view(np.int32).copy()).pin_memory()
         e2e_steps = max(1, min(args.steps, 5))
         off_u32 = off_pinned.numpy().view(np.uint32)
@@ -530,10 +540,10 @@ def run_velo(args):
             assert sum(r["n_tracks"] for r in hres) == n_tracks and sum(r["n_track_hits"] for r in hres) == n_thits
             return t_, hres
 
-        soa_s, hres = measure(lambda: sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off_u32, cuts, houts))
-        d2h = sum(4 * velo.VELO_N_SUMMARY + 4 * (cuts[b + 1] - cuts[b] + 1) + 4 * (r["n_tracks"] + 1) + 52 * r["n_tracks"] + 4 * r["n_track_hits"]
+        soa_s, hres = measure(lambda: sched.run_host(P, d["x"], d["y"], d["z"], d["module"], off_u32, eq_cuts, houts))
+        d2h = sum(4 * velo.VELO_N_SUMMARY + 4 * (eq_cuts[b + 1] - eq_cuts[b] + 1) + 4 * (r["n_tracks"] + 1) + 52 * r["n_tracks"] + 4 * r["n_track_hits"]
                   for b, r in enumerate(hres))
-        off_bytes = sum(4 * (cuts[b + 1] - cuts[b] + 1) for b in range(n_batches))
+        off_bytes = sum(4 * (eq_cuts[b + 1] - eq_cuts[b] + 1) for b in range(n_batches))
         e2e_soa = {"value": world * n_events / soa_s, "unit": UNIT, "h2d_bytes_per_step": 13 * n_hits + off_bytes,
                    "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * soa_s, "steps": e2e_steps,
                    "pcie_gbs": (13 * n_hits + off_bytes + d2h) / soa_s / 1e9,
@@ -541,6 +551,9 @@ def run_velo(args):
                    "api": "velo_scheduler_run_host (pinned host buffers, %d streams)" % n_batches}
         launches += kernels_per_batch * n_batches * (e2e_steps + 1)
         if px_pinned is not None:
+            if cuts is not eq_cuts:
+                houts = None   # (pinned host memory: free the equal batches' buffers first)
+                houts = [velo.HostTracks(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]])) for b in range(n_batches)]
             px_s, _ = measure(lambda: sched.run_host_pixels(P, px_pinned, off_u32, fmt, cuts, houts))
             line["e2e"] = {"value": world * n_events / px_s, "unit": UNIT, "h2d_bytes_per_step": 4 * n_hits + off_bytes,
                            "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * px_s, "steps": e2e_steps,
@@ -548,7 +561,8 @@ def run_velo(args):
                            "input": "packed pixel addresses (4 B per hit; include/velo.h velo_pixel_hits_t), decoded inside "
                                     "stage 1; identical tracks to the fp32 path (tests/test_gpu_pixels.py)",
                            "bound": "PCIe: the device->host copy of the produced tracks (%.2f GB per step)" % (d2h / 1e9),
-                           "api": "velo_scheduler_run_host_pixels (pinned host buffers, %d streams)" % n_batches}
+                           "api": "velo_scheduler_run_host_pixels (pinned host buffers, %d streams)" % n_batches,
+                           "batches": [cuts[b + 1] - cuts[b] for b in range(n_batches)]}
             line["e2e_fp32_soa"] = e2e_soa
             launches += kernels_per_batch * n_batches * (e2e_steps + 1)
         else:
