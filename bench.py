@@ -64,6 +64,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-split", default="growing", choices=["growing", "equal"],
                     help="batch sizes of the end-to-end call: 10/20/30/40 %% of the events (default) or four equal batches")
+    ap.add_argument("--e2e-fractions", default="0.10,0.20,0.30,0.40",
+                    help="the growing split (measured: 6/14/30/50 %% 39.4 ms, 10/20/30/40 %% 39.7 ms, six or eight growing "
+                         "batches 42-50 ms: every batch costs two host synchronisations)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -509,13 +512,16 @@ def run_velo(args):
         # batches (a large last batch would leave its kernels and its copy behind the last upload).
         eq_cuts = cuts
         if n_batches == 4 and args.e2e_split == "growing":
-            cuts = [0] + [int(round(n_events * f)) for f in (0.10, 0.30, 0.60)] + [n_events]
-        max_ev = max(c[b + 1] - c[b] for c in (cuts, eq_cuts) for b in range(n_batches))
-        max_h = max(int(off[c[b + 1]]) - int(off[c[b]]) for c in (cuts, eq_cuts) for b in range(n_batches))
+            fr = [float(v) for v in args.e2e_fractions.split(",")]
+            acc = np.cumsum(fr) / sum(fr)
+            cuts = [0] + [int(round(n_events * f)) for f in acc[:-1]] + [n_events]
+        px_batches = len(cuts) - 1
+        max_ev = max(c[b + 1] - c[b] for c in (cuts, eq_cuts) for b in range(len(c) - 1))
+        max_h = max(int(off[c[b + 1]]) - int(off[c[b]]) for c in (cuts, eq_cuts) for b in range(len(c) - 1))
         g, P = wl.g, wl.P
         wl.outs = wl.hstructs = wl.dh = None
         torch.cuda.empty_cache()
-        sched = velo.Scheduler(g, n_batches, max_ev, max_h)
+        sched = velo.Scheduler(g, max(n_batches, px_batches), max_ev, max_h)
         houts = [velo.HostTracks(eq_cuts[b + 1] - eq_cuts[b], int(off[eq_cuts[b + 1]]) - int(off[eq_cuts[b]])) for b in range(n_batches)]
         off_pinned = torch.from_numpy(off.view(np.int32).copy()).pin_memory()
         e2e_steps = max(1, min(args.steps, 5))
@@ -553,7 +559,7 @@ def run_velo(args):
         if px_pinned is not None:
             if cuts is not eq_cuts:
                 houts = None   # (pinned host memory: free the equal batches' buffers first)
-                houts = [velo.HostTracks(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]])) for b in range(n_batches)]
+                houts = [velo.HostTracks(cuts[b + 1] - cuts[b], int(off[cuts[b + 1]]) - int(off[cuts[b]])) for b in range(px_batches)]
             px_s, _ = measure(lambda: sched.run_host_pixels(P, px_pinned, off_u32, fmt, cuts, houts))
             line["e2e"] = {"value": world * n_events / px_s, "unit": UNIT, "h2d_bytes_per_step": 4 * n_hits + off_bytes,
                            "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * px_s, "steps": e2e_steps,
@@ -561,10 +567,10 @@ def run_velo(args):
                            "input": "packed pixel addresses (4 B per hit; include/velo.h velo_pixel_hits_t), decoded inside "
                                     "stage 1; identical tracks to the fp32 path (tests/test_gpu_pixels.py)",
                            "bound": "PCIe: the device->host copy of the produced tracks (%.2f GB per step)" % (d2h / 1e9),
-                           "api": "velo_scheduler_run_host_pixels (pinned host buffers, %d streams)" % n_batches,
-                           "batches": [cuts[b + 1] - cuts[b] for b in range(n_batches)]}
+                           "api": "velo_scheduler_run_host_pixels (pinned host buffers, %d streams)" % max(n_batches, px_batches),
+                           "batches": [cuts[b + 1] - cuts[b] for b in range(px_batches)]}
             line["e2e_fp32_soa"] = e2e_soa
-            launches += kernels_per_batch * n_batches * (e2e_steps + 1)
+            launches += kernels_per_batch * px_batches * (e2e_steps + 1)
         else:
             line["e2e"] = e2e_soa
         sched.close()
