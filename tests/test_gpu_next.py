@@ -74,6 +74,18 @@ def test_parameter_variants_and_edge_cases(velo):
     got, want = pv.to_host(), oracle.pv_find(res["event_track_offsets"], res["states"], Po)
     np.testing.assert_array_equal(got["event_pv_offsets"], want["event_pv_offsets"])
     same_bits(got["pvs"], want["pvs"])
+    # an odd number of bins that is no multiple of 32 (the last packed word holds one bin, the last block of the
+    # seed scan is ragged), fine bins, a seed window wider than a block's halo
+    for nb, bw, hw in ((2399, 0.25, 6), (4095, 0.15, 9), (33, 20.0, 1)):
+        P3 = velo.velo_pv_params_default()
+        P3.n_bins = nb; P3.bin_width = bw; P3.seed_half_window = hw; P3.seed_min_sum = 1
+        _, _, pv3 = run_gpu(velo, d, pv_params=P3)
+        Po3 = oracle.default_pv_params()
+        Po3.n_bins = nb; Po3.bin_width = bw; Po3.seed_half_window = hw; Po3.seed_min_sum = 1
+        got3, want3 = pv3.to_host(), oracle.pv_find(res["event_track_offsets"], res["states"], Po3)
+        np.testing.assert_array_equal(got3["event_pv_offsets"], want3["event_pv_offsets"])
+        same_bits(got3["pvs"], want3["pvs"])
+        assert got3["n_pvs"] > 0
     # at most two vertices per event, lowest z first
     P2 = velo.velo_pv_params_default(); P2.max_pv_per_event = 2
     _, _, pv2 = run_gpu(velo, d, pv_params=P2)
