@@ -400,7 +400,8 @@ def run_velo(args):
                                                  for nm, (s, e) in zip(("sort", "track", "fit"), r)), flush=True)
         # SM clocks per event and phase, summed over the team leaders (batch 0)
         names = {"sort": (8, ["fetch", "decode", "scan", "scatter+rank", "place", "starts+write", "free"]),
-                 "track": (16, ["fetch", "setup", "wait module", "forwarding", "centre list", "seeding", "tail"]),
+                 "track": (16, ["fetch: pool wait and barrier", "setup", "wait module", "forwarding", "centre list", "seeding", "tail",
+                                "fetch: ticket and descriptors"]),
                  "fit": (32, ["fetch", "weak filter", "fit", "owners 1", "owners 2", "clone+counts"])}
         clk = phases[0]
         for nm, (base, labels) in names.items():

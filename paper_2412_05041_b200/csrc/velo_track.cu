@@ -98,6 +98,9 @@ __device__ void track_fetch(const KernelArgs& a, PoolCtl& pool, TrackTeam<G>& ts
     return;
   }
   ts.cbase = atomicAdd(&a.ws.counters[kCtrCandAlloc], tcap);
+#ifdef VELO_TIMELINE
+  { const uint32_t tid = 0; VELO_PH(a.ws.phase_clk, ts, 24); }     // ticket and descriptors; what follows in "fetch" is the pool
+#endif
   const uint32_t first = pool_alloc(pool, units);
   ts.n = n; ts.sb = sorted_base(a.event_offsets[e] - a.event_offsets[0], e);
   ts.maxmod = maxmod; ts.tcap = tcap; ts.acap = acap;
