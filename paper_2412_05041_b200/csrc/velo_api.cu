@@ -88,7 +88,7 @@ int run_batch(const velo_geometry_t* g, KernelArgs& a, uint32_t n_events, uint32
   const size_t need = velo_workspace_bytes_opts(n_events, n_hits, out->cap_tracks, out->cap_track_hits, opts);
   if (workspace_bytes < need) return VELO_ERR_WORKSPACE;
   a.n_events = n_events; a.n_modules = g->n_modules; a.n_hits = n_hits;
-  const uint32_t path = opts ? opts->path : 0u;
+  uint32_t path = opts ? opts->path : 0u;
   a.team_max_hits = kPipeMaxHits;
   for (uint32_t m = 0; m < VELO_MAX_MODULES; ++m) a.module_z[m] = m < g->n_modules ? g->module_z[m] : 0.0f;
   a.two_plane = g->two_plane;
@@ -99,6 +99,9 @@ int run_batch(const velo_geometry_t* g, KernelArgs& a, uint32_t n_events, uint32
   // from a scatter cut that nothing passes (scatter is a sum of squares, never below zero).
   if (a.P.phi_window_seed < 0) { a.P.phi_window_seed = 0; a.P.max_scatter_seed = -1.0f; }
   if (a.P.phi_window_fwd < 0) { a.P.phi_window_fwd = 0; a.P.max_scatter_fwd = -1.0f; }
+  // The module loop of the pipeline keeps "scatter <= cut" as "scatter < the next float above the cut", which
+  // needs a cut below +inf: any other cut (+inf, NaN) takes the general kernel and its plain comparison.
+  if (!(a.P.max_scatter_seed < INFINITY) || !(a.P.max_scatter_fwd < INFINITY)) path = kPathSlabOnly;
   a.event_track_offsets = out->event_track_offsets; a.track_hit_offsets = out->track_hit_offsets;
   a.track_hits = out->track_hits; a.states = out->states;
   a.cap_tracks = out->cap_tracks; a.cap_track_hits = out->cap_track_hits; a.summary = out->summary;

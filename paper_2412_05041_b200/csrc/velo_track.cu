@@ -505,7 +505,11 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
   VELO_PH(a.ws.phase_clk, ts, 18);       // descriptors, flags, first loads
 
   uint32_t nact = 0, ncand = 0;          // nact: this warp's share
-  const float max_fwd = P.max_scatter_fwd, max_seed = P.max_scatter_seed;
+  // "scatter <= max and below the best so far" is kept as one comparison, scatter < bound, with the bound starting
+  // at the next float above max (the cuts are finite here: velo_api.cu sends any other cut through the general
+  // kernel); a match is found iff an index was taken. Ties still go to the first record met (strict <).
+  const float fwd_bound = nextafterf(P.max_scatter_fwd, INFINITY), seed_bound = nextafterf(P.max_scatter_seed, INFINITY);
+  constexpr uint32_t kNone = 0xffffffffu;
   for (uint32_t s = M - 2; s >= 1; --s) {
     const uint32_t u = s - 1;
     if (mo[u + 1] == 0) break;           // no hit in modules 0 .. u: nothing can change any more (see track_event)
@@ -545,14 +549,14 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
         const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, x0), tz));
         const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, y0), tz));
         const Win wx = make_win(c, Wfwd);
-        bool found = false; uint32_t best = 0; float best_sc = 0.0f;
+        uint32_t best = kNone; float best_sc = fwd_bound;
         auto visit = [&](uint32_t jj, const uint4& r, bool in) {
           const bool pb = kTwoPlane && plane_of(r) != 0u;
           const float ex = __fsub_rn(pb ? px_b : px, __uint_as_float(r.x)), ey = __fsub_rn(pb ? py_b : py, __uint_as_float(r.y));
           const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-          bool ok = in & (sc <= max_fwd) & (!found | (sc < best_sc));
+          bool ok = in & (sc < best_sc);
           if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
-          found |= ok; best = ok ? jj : best; best_sc = ok ? sc : best_sc;
+          best = ok ? jj : best; best_sc = ok ? sc : best_sc;
         };
         if (pend <= 1u) {
           const Win ww = kSameW ? wx : make_win(c, Wwide);
@@ -565,11 +569,11 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
             const bool pb = kTwoPlane && plane_of(r) != 0u;
             const float ex = __fsub_rn(pb ? px_b : px, __uint_as_float(r.x)), ey = __fsub_rn(pb ? py_b : py, __uint_as_float(r.y));
             const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-            const bool ok = (r.z - wx.lo16 <= wx.lim) & (sc <= max_fwd) & (!found | (sc < best_sc));
-            found |= ok; best = ok ? j : best; best_sc = ok ? sc : best_sc;
+            const bool ok = (r.z - wx.lo16 <= wx.lim) & (sc < best_sc);
+            best = ok ? j : best; best_sc = ok ? sc : best_sc;
           }
         }
-        if (found) {
+        if (best != kNone) {
           const uint4 r2 = ring_u[best];
           const uint32_t h2 = off_u + best, nh = (uint32_t)__popc(mask);
           rows[id * 32u + nh] = (uint16_t)h2;
@@ -625,7 +629,7 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
       const uint32_t Ls = 1u << lsh;
       for (uint32_t k0 = 0; k0 < ncl; k0 += 32u >> lsh) {
         const uint32_t k = k0 + (lane >> lsh), q = lane & (Ls - 1u);
-        bool found = false; uint32_t b0 = 0, b2 = 0, j1 = 0; float best_sc = 0.0f;
+        uint32_t b0 = kNone, b2 = 0, j1 = 0; float best_sc = seed_bound;
         if (k < ncl) {
           j1 = clw[k];
           const uint4 r1 = ring_s[j1];
@@ -654,15 +658,16 @@ __device__ void track_event_w(const KernelArgs& a, const float* mz, const float*
                 const bool pb = kTwoPlane && plane_of(r) != 0u;
                 const float ex = __fsub_rn(pb ? px_b : px, __uint_as_float(r.x)), ey = __fsub_rn(pb ? py_b : py, __uint_as_float(r.y));
                 const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-                bool ok = in & !flagged(off_u + jj) & (sc <= max_seed) & (!found | (sc < best_sc));
+                bool ok = in & !flagged(off_u + jj) & (sc < best_sc);
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
-                found |= ok; b0 = ok ? j0 : b0; b2 = ok ? jj : b2; best_sc = ok ? sc : best_sc;
+                b0 = ok ? j0 : b0; b2 = ok ? jj : b2; best_sc = ok ? sc : best_sc;
               };
               if (ww.wrapped) scan_run<true>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
               scan_run<true>(ring_u, r1.w >> 16, nu, ww.lo16, ww.lim, visit2);
             }
           }
         }
+        bool found = b0 != kNone;
         for (uint32_t d = 1; d < Ls; d <<= 1) {
           const bool o_found = __shfl_xor_sync(0xffffffffu, (int)found, d) != 0;
           const float o_sc = __shfl_xor_sync(0xffffffffu, best_sc, d);
