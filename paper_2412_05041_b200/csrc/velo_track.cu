@@ -188,7 +188,11 @@ __device__ void track_event_big(const KernelArgs& a, const float* mz, const floa
   VELO_PH(a.ws.phase_clk, ts, 18);       // descriptors, flags, first loads
 
   uint32_t nact = 0, ncand = 0;
-  const float max_fwd = P.max_scatter_fwd, max_seed = P.max_scatter_seed;
+  const float max_seed = P.max_scatter_seed;
+  // one comparison per visited record, as in track_event_w: scatter < bound, the bound starting at the next float
+  // above the (finite: velo_api.cu) cut
+  const float fwd_bound = nextafterf(P.max_scatter_fwd, INFINITY), seed_bound = nextafterf(P.max_scatter_seed, INFINITY);
+  constexpr uint32_t kNone = 0xffffffffu;
   for (uint32_t s = M - 2; s >= 1; --s) {
     const uint32_t u = s - 1;
     // No hit in modules 0 .. u: forwarding can only miss and seeding finds no third hit, in this step
@@ -222,13 +226,13 @@ __device__ void track_event_big(const KernelArgs& a, const float* mz, const floa
         const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, x0), tz));
         const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, y0), tz));
         const Win wx = make_win(c, Wfwd);
-        bool found = false; uint32_t best = 0; float best_sc = 0.0f;
+        uint32_t best = kNone; float best_sc = fwd_bound;
         auto visit = [&](uint32_t jj, const uint4& r, bool in) {
           const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
           const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-          bool ok = in & (sc <= max_fwd) & (!found | (sc < best_sc));
+          bool ok = in & (sc < best_sc);
           if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
-          found |= ok; best = ok ? jj : best; best_sc = ok ? sc : best_sc;
+          best = ok ? jj : best; best_sc = ok ? sc : best_sc;
         };
         const uint32_t pend = mb - s;      // modules already missed since the latest hit
         if (pend <= 1u) {
@@ -241,11 +245,11 @@ __device__ void track_event_big(const KernelArgs& a, const float* mz, const floa
             const uint4 r = ring_u[j];
             const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
             const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-            const bool ok = (r.z - wx.lo16 <= wx.lim) & (sc <= max_fwd) & (!found | (sc < best_sc));
-            found |= ok; best = ok ? j : best; best_sc = ok ? sc : best_sc;
+            const bool ok = (r.z - wx.lo16 <= wx.lim) & (sc < best_sc);
+            best = ok ? j : best; best_sc = ok ? sc : best_sc;
           }
         }
-        if (found) {
+        if (best != kNone) {
           const uint4 r2 = ring_u[best];
           const uint32_t h2 = off_u + best, nh = (uint32_t)__popc(mask);
           rows[id * 32u + nh] = (uint16_t)h2;
@@ -332,17 +336,17 @@ __device__ void track_event_big(const KernelArgs& a, const float* mz, const floa
               const Win ww = kSameW ? wx : make_win(rc.z >> 16, Wwide);
               const float px = __fadd_rn(x1, __fmul_rn(__fsub_rn(x1, __uint_as_float(r0.x)), tz));
               const float py = __fadd_rn(y1, __fmul_rn(__fsub_rn(y1, __uint_as_float(r0.y)), tz));
-              bool fnd = false; uint32_t bb2 = 0; float bsc = 0.0f;
+              uint32_t bb2 = kNone; float bsc = seed_bound;
               auto visit2 = [&](uint32_t jj, const uint4& r, bool in) {
                 const float ex = __fsub_rn(px, __uint_as_float(r.x)), ey = __fsub_rn(py, __uint_as_float(r.y));
                 const float sc = __fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey));
-                bool ok = in & !flagged(off_u + jj) & (sc <= max_seed) & (!fnd | (sc < bsc));
+                bool ok = in & !flagged(off_u + jj) & (sc < bsc);
                 if (!kSameW) ok &= (r.z - wx.lo16 <= wx.lim);
-                fnd |= ok; bb2 = ok ? jj : bb2; bsc = ok ? sc : bsc;
+                bb2 = ok ? jj : bb2; bsc = ok ? sc : bsc;
               };
               if (ww.wrapped) scan_run<false>(ring_u, 0u, nu, ww.lo16, ww.lim, visit2);
               scan_run<false>(ring_u, rc.w >> 16, nu, ww.lo16, ww.lim, visit2);
-              if (fnd) atomicMin(&keys[kl], ((unsigned long long)__float_as_uint(bsc) << 32) | ((unsigned long long)j0 << 16) | bb2);
+              if (bb2 != kNone) atomicMin(&keys[kl], ((unsigned long long)__float_as_uint(bsc) << 32) | ((unsigned long long)j0 << 16) | bb2);
             }
             team_sync<G>(team);
             const unsigned long long key = keys[tid];
