@@ -283,11 +283,18 @@ def test_parameter_variants(velo):
                    {"phi_window_seed": 0, "phi_window_fwd": 5},
                    {"max_skipped": 0}, {"max_skipped": 3},
                    {"clone_num": 0, "clone_den": 1}, {"clone_num": 1, "clone_den": 1},
-                   {"max_chi2_ndof": 2.0}, {"max_scatter_seed": 0.5, "max_scatter_fwd": 0.02, "max_scatter_weak": 0.5}):
+                   {"max_chi2_ndof": 2.0}, {"max_scatter_seed": 0.5, "max_scatter_fwd": 0.02, "max_scatter_weak": 0.5},
+                   # cuts at the edges of the single-comparison form of the scans: nothing passes (negative), only an exact
+                   # match passes (zero), the largest finite cut, and cuts that are not finite (these take the general kernel)
+                   {"max_scatter_seed": -1.0, "max_scatter_fwd": 0.1}, {"max_scatter_seed": 0.1, "max_scatter_fwd": 0.0},
+                   {"max_scatter_seed": 3.4028234663852886e38, "max_scatter_fwd": 3.4028234663852886e38, "phi_window_seed": 60, "phi_window_fwd": 60},
+                   {"max_scatter_seed": float("inf"), "max_scatter_fwd": 0.1, "phi_window_seed": 60},
+                   {"max_scatter_seed": 0.1, "max_scatter_fwd": float("nan")}):
         p = velo.velo_params_default(g)
         for k, v in change.items():
             setattr(p, k, v)
-        got = velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], datagen.MODULE_Z, params=p)
+        got = velo.reconstruct(d["x"], d["y"], d["z"], d["module"], d["event_offsets"], datagen.MODULE_Z, params=p,
+                               cap_tracks=d["n_hits"], cap_track_hits=4 * d["n_hits"])     # (wide cuts make many tracks)
         check(got, cpu(d, _oracle_params(p), workers=4))
 
 
